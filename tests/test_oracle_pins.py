@@ -1,0 +1,279 @@
+"""Pins P1-P7, P11 for the CPU oracle (no GPU).  Each test pins the oracle to something
+other than itself: Fock-space brute force, closed forms, library routines, invariants.
+Citations: PAPER.md lines as in oracle/afqmc_oracle.py; pin numbers from DESIGN.md."""
+import numpy as np
+import pytest
+import scipy.linalg
+import scipy.sparse.linalg
+
+from oracle import afqmc_oracle as O
+from workloads import make_workload, random_walkers
+from tests.fockspace import Fock
+
+SMALL = dict(M=4, n_alpha=2, n_beta=1, n_chol=5, n_walkers=3)
+
+
+@pytest.fixture(scope="module")
+def small():
+    wl = make_workload(1, overrides=SMALL)
+    ini = O.o_init(wl.h, wl.L, wl.dt, wl.psi_a, wl.psi_b)
+    fk = Fock(wl.M)
+    return wl, ini, fk
+
+
+def _V(L):
+    return np.einsum("gik,gjl->ijkl", L, L)
+
+
+def _trial_vec(fk, wl):
+    return fk.determinant(wl.psi_a.astype(complex), wl.psi_b.astype(complex))
+
+
+def test_P1_hamiltonian_identity(small):
+    """Eq. (1) == sum h'_ij c+c + 1/2 sum_g Lhat_g^2 with h' = h - 1/2 sum L_g L_g."""
+    wl, ini, fk = small
+    H1 = fk.hamiltonian_eq1(wl.h, _V(wl.L))
+    H2 = fk.one_body(ini["hp"])
+    for g in range(wl.n_chol):
+        Lg = fk.one_body(wl.L[g])
+        H2 = H2 + 0.5 * (Lg @ Lg)
+    assert abs(H1 - H2).max() < 1e-12
+
+
+def test_P2_overlap_green_forcebias_fock(small):
+    """<Psi_T|phi>, <Psi_T|c+_i c_j|phi>/<Psi_T|phi>, <L_g> from explicit Fock vectors."""
+    wl, ini, fk = small
+    phi = random_walkers(wl, 3, seed=3, spread=0.8)
+    S, theta, G = O.o_green(wl.psi_a, wl.psi_b, phi, want_G=True)
+    f_a, f_b = O.o_force_bias(ini["R"], theta, wl.n_alpha)
+    bra = _trial_vec(fk, wl).conj()
+    for w in range(3):
+        ket = fk.determinant(phi[w][:, :wl.n_alpha], phi[w][:, wl.n_alpha:])
+        ov = bra @ ket
+        assert abs(ov - S[w]) < 1e-12 * abs(ov)
+        for s in range(2):
+            for i in range(wl.M):
+                for j in range(wl.M):
+                    g = bra @ (fk.cre(i, s) @ (fk.ann(j, s) @ ket)) / ov
+                    assert abs(g - G[w, s, i, j]) < 1e-12
+        for g_ in range(wl.n_chol):
+            ref = bra @ (fk.one_body(wl.L[g_]) @ ket) / ov
+            assert abs(ref - (f_a[w, g_] + f_b[w, g_])) < 1e-12
+
+
+def test_P2_gauge_invariance(small):
+    """Phi -> Phi X scales S by det X and leaves Theta-derived f, E_L unchanged."""
+    wl, ini, _ = small
+    rng = np.random.default_rng(5)
+    phi = random_walkers(wl, 3, seed=4)
+    Xa = rng.standard_normal((2, 2)) + 1j * rng.standard_normal((2, 2))
+    Xb = rng.standard_normal((1, 1)) + 1j * rng.standard_normal((1, 1))
+    phi2 = np.concatenate([phi[..., :2] @ Xa, phi[..., 2:] @ Xb], axis=2)
+    S1, th1 = O.o_green(wl.psi_a, wl.psi_b, phi)
+    S2, th2 = O.o_green(wl.psi_a, wl.psi_b, phi2)
+    assert np.allclose(S2, S1 * np.linalg.det(Xa) * np.linalg.det(Xb), rtol=1e-12)
+    G1 = O.o_green(wl.psi_a, wl.psi_b, phi, want_G=True)[2]
+    G2 = O.o_green(wl.psi_a, wl.psi_b, phi2, want_G=True)[2]
+    assert np.allclose(G1, G2, atol=1e-12)
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_P3_hartree_fock_energy(cfg):
+    """Walker == single-determinant trial => E_L == E_HF by independent einsum over h and V."""
+    ov = {3: dict(M=24, n_alpha=6, n_beta=5, n_chol=40)}.get(cfg)
+    wl = make_workload(cfg, overrides=ov)
+    ini = O.o_init(wl.h, wl.L, wl.dt, wl.psi_a, wl.psi_b)
+    st = O.o_seed_state(ini, wl.walkers(2), wl.n_alpha)
+    Pa, Pb = wl.psi_a @ wl.psi_a.T, wl.psi_b @ wl.psi_b.T
+    P = Pa + Pb
+    V = _V(wl.L)
+    e_hf = (np.einsum("ij,ji->", wl.h, P) + 0.5 * np.einsum("ijkl,ik,jl->", V, P, P)
+            - 0.5 * np.einsum("ijkl,il,jk->", V, Pa, Pa) - 0.5 * np.einsum("ijkl,il,jk->", V, Pb, Pb))
+    assert np.allclose(st.eloc, e_hf, rtol=1e-12, atol=1e-12)
+    assert np.allclose(st.S, 1.0, atol=1e-12)
+
+
+def test_P3_local_energy_fock_and_forms(small):
+    """E_L == <Psi_T|H|phi>/<Psi_T|phi> in Fock space; Y form == Cholesky form (Eq. 5)."""
+    wl, ini, fk = small
+    phi = random_walkers(wl, 3, seed=11, spread=0.8)
+    S, theta = O.o_green(wl.psi_a, wl.psi_b, phi)
+    f_a, f_b = O.o_force_bias(ini["R"], theta, wl.n_alpha)
+    e_y = O.o_local_energy(ini, theta, f_a, f_b, wl.n_alpha)
+    e_c = O.o_local_energy_chol(ini, theta, wl.n_alpha)
+    assert np.allclose(e_y, e_c, rtol=1e-12)
+    H = fk.hamiltonian_eq1(wl.h, _V(wl.L))
+    bra = _trial_vec(fk, wl).conj()
+    for w in range(3):
+        ket = fk.determinant(phi[w][:, :wl.n_alpha], phi[w][:, wl.n_alpha:])
+        ref = bra @ (H @ ket) / (bra @ ket)
+        assert abs(ref - e_y[w]) < 1e-11 * max(1.0, abs(ref))
+
+
+def test_P3_invariance_under_gamma_mixing(small):
+    """E_L depends on L only through V: L_g -> sum_d O_gd L_d with O orthogonal."""
+    wl, ini, _ = small
+    Q, _ = np.linalg.qr(np.random.default_rng(2).standard_normal((wl.n_chol, wl.n_chol)))
+    ini2 = O.o_init(wl.h, np.tensordot(Q, wl.L, axes=(1, 0)), wl.dt, wl.psi_a, wl.psi_b)
+    phi = random_walkers(wl, 3, seed=12)
+    e1 = O.o_seed_state(ini, phi, wl.n_alpha).eloc
+    e2 = O.o_seed_state(ini2, phi, wl.n_alpha).eloc
+    assert np.allclose(e1, e2, rtol=1e-11)
+
+
+def test_P4_thouless_and_taylor(small):
+    """exp(Ahat)|phi> == |expm(A) Phi> for complex symmetric A (Thouless);
+    Taylor-K differs from expm by <= ||A||^{K+1}/(K+1)! e^{||A||}; x real, xbar=0 => unitary."""
+    wl, ini, fk = small
+    rng = np.random.default_rng(8)
+    phi = random_walkers(wl, 1, seed=13)
+    xs = (rng.standard_normal((1, wl.n_chol)) + 0.3j * rng.standard_normal((1, wl.n_chol)))
+    A = O.o_assemble(wl.L, xs, 0.05)
+    assert np.allclose(A[0], A[0].T)
+    K = 6
+    I = np.eye(wl.M)
+    out = O.o_propagate(I, A, phi, K)[0]
+    exact = scipy.linalg.expm(A[0]) @ phi[0]
+    nA = np.linalg.norm(A[0], 2)
+    import math
+    bound = nA ** (K + 1) / math.factorial(K + 1) * math.exp(nA)
+    assert np.linalg.norm(out - exact, 2) <= bound * np.linalg.norm(phi[0], 2) + 1e-14
+    out30 = O.o_propagate(I, A, phi, 30)[0]
+    assert np.allclose(out30, exact, atol=1e-13)
+    ket = fk.determinant(phi[0][:, :2], phi[0][:, 2:])
+    ket2 = scipy.sparse.linalg.expm_multiply(fk.one_body(A[0]).tocsc(), ket)
+    ref = fk.determinant(exact[:, :2], exact[:, 2:])
+    assert np.allclose(ket2, ref, atol=1e-12)
+    # one-body half step: Eh == expm(-dt/2 h')
+    assert np.allclose(ini["Eh"], scipy.linalg.expm(-0.5 * wl.dt * ini["hp"]), atol=1e-13)
+    Areal = O.o_assemble(wl.L, rng.standard_normal((1, wl.n_chol)), 0.05)[0]
+    U = scipy.linalg.expm(Areal)
+    assert np.allclose(U.conj().T @ U, I, atol=1e-12)
+
+
+def test_P5_importance_function(small):
+    """(a) E_x[I(x)] == <Psi_T|e^{-dt H}|phi>/<Psi_T|phi> up to Trotter/Taylor error (Eq. 2, 3);
+    (b) force-bias sign: the odd-in-x part of log I is far smaller with the shift than without."""
+    wl, _, fk = small
+    dt = 0.01
+    ini = O.o_init(wl.h, wl.L, dt, wl.psi_a, wl.psi_b)
+    phi1 = random_walkers(wl, 1, seed=21, spread=0.3)
+    n = 40000
+    phi = np.ascontiguousarray(np.broadcast_to(phi1[0], (n,) + phi1[0].shape))
+    st = O.o_seed_state(ini, phi, wl.n_alpha)
+    x = np.random.default_rng(99).standard_normal((n // 2, wl.n_chol))
+    x = np.concatenate([x, -x])                                  # antithetic pairs
+    st2, rec = O.o_step(ini, st, x, wl.n_alpha, K=8)
+    I = (st2.S / st.S) * np.exp(rec["c"])
+    H = fk.hamiltonian_eq1(wl.h, _V(wl.L))
+    bra = _trial_vec(fk, wl).conj()
+    ket = fk.determinant(phi1[0][:, :2], phi1[0][:, 2:])
+    exact = bra @ scipy.sparse.linalg.expm_multiply(-dt * H.tocsc(), ket) / (bra @ ket)
+    err = abs(I.mean() - exact)
+    sem = I.std() / np.sqrt(n)
+    assert err < 5 * sem + 5e-5, (err, sem)
+    # and the first-order statement: (E[I]-1)/dt ~ -E_L
+    assert abs((I.mean() - 1) / dt + st.eloc[0]) < 0.05 * abs(st.eloc[0]) + 5 * sem / dt
+    # (b) odd part of log I with and without the shift
+    logI = np.log(I)
+    odd_with = 0.5 * (logI[: n // 2] - logI[n // 2:])
+    st0 = O.OracleState(st.phi, st.w, st.S, st.theta, 0 * st.f_a, 0 * st.f_b, st.eloc)
+    st3, rec3 = O.o_step(ini, st0, x, wl.n_alpha, K=8)
+    logI0 = np.log(st3.S / st.S)
+    odd_without = 0.5 * (logI0[: n // 2] - logI0[n // 2:])
+    assert np.abs(odd_with).mean() < 0.1 * np.abs(odd_without).mean()
+
+
+def test_P6_smw_identity():
+    """Eq. (4) == direct recomputation for rank 0, 1, 2."""
+    rng = np.random.default_rng(0)
+    n = 6
+    A = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
+    Ainv, detA = np.linalg.inv(A), np.linalg.det(A)
+    for E in (1, 2, 3):
+        U = np.zeros((n, E))
+        U[rng.permutation(n)[:E], np.arange(E)] = 1.0
+        Vt = rng.standard_normal((E, n)) + 1j * rng.standard_normal((E, n))
+        det, inv = O.o_smw_det_inverse(Ainv, detA, U, Vt)
+        B = A + U @ Vt
+        assert abs(det - np.linalg.det(B)) < 1e-12 * abs(det)
+        assert np.allclose(inv, np.linalg.inv(B), atol=1e-12)
+
+
+def test_P6_multidet_smw_equals_definition():
+    """Batched SMW path == per-determinant direct recomputation (S, f, E_L, mixed G)."""
+    wl = make_workload(4, overrides=dict(M=12, n_alpha=4, n_beta=3, n_chol=9, n_act=9, n_det=40))
+    ini = O.o_init(wl.h, wl.L, wl.dt, wl.psi_a, wl.psi_b)
+    tr = O.MultiDetTrial(wl.C_act, wl.det_coeff, wl.det_exc, wl.n_alpha, wl.n_beta)
+    phi = random_walkers(wl, 4, seed=5, spread=0.5)
+    S1, f1, E1, G1 = O.o_multidet_definition(ini, tr, phi, wl.n_alpha, want_G=True)
+    S2, th0, f2, E2, G2 = O.o_multidet_smw(ini, tr, phi, wl.n_alpha, want_G=True)
+    assert np.allclose(S1, S2, rtol=1e-11)
+    assert np.allclose(f1, f2, atol=1e-10)
+    assert np.allclose(E1, E2, rtol=1e-10)
+    assert np.allclose(G1, G2, atol=1e-10)
+    # ranks 0, 1 and 2 per spin are all present in the list
+    ranks = {(int((wl.det_exc[i, 0, :, 0] >= 0).sum()), int((wl.det_exc[i, 1, :, 0] >= 0).sum()))
+             for i in range(wl.n_det)}
+    assert {(0, 0), (1, 0), (0, 1), (2, 0), (0, 2), (1, 1)} <= ranks
+
+
+def _pivoted_cholesky(Vmat, tol):
+    """Library-free pivoted Cholesky of a PSD matrix; returns rows l_g with V ~ sum_g l_g l_g^T."""
+    d = np.diag(Vmat).copy()
+    vecs = []
+    while d.max() > tol:
+        p = int(np.argmax(d))
+        col = Vmat[:, p].copy()
+        for v in vecs:
+            col -= v * v[p]
+        v = col / np.sqrt(d[p])
+        vecs.append(v)
+        d -= v * v
+    return np.array(vecs)
+
+
+def test_P7_cholesky_vectors_reproduce_tensor(small):
+    """V_ijkl = sum_g L_ik L_jl: pivoted Cholesky of V gives <= N_g symmetric vectors
+    that reproduce V, E_HF and E_L."""
+    wl, ini, _ = small
+    M = wl.M
+    Vmat = _V(wl.L).transpose(0, 2, 1, 3).reshape(M * M, M * M)       # [(i,k)][(j,l)]
+    vecs = _pivoted_cholesky(Vmat, 1e-10)
+    assert vecs.shape[0] <= wl.n_chol
+    Lt = vecs.reshape(-1, M, M)
+    assert np.allclose(Lt, Lt.transpose(0, 2, 1), atol=1e-9)
+    assert abs(_V(Lt) - _V(wl.L)).max() < 1e-9
+    ini2 = O.o_init(wl.h, Lt, wl.dt, wl.psi_a, wl.psi_b)
+    phi = random_walkers(wl, 3, seed=14)
+    e1 = O.o_seed_state(ini, phi, wl.n_alpha).eloc
+    e2 = O.o_seed_state(ini2, phi, wl.n_alpha).eloc
+    assert np.allclose(e1, e2, rtol=1e-9)
+
+
+def test_P11_mean_field_variant(small):
+    """mf inputs: same Hamiltonian on the (N_a,N_b) sector up to e_const; E_L identical."""
+    wl, ini, fk = small
+    wm = make_workload(1, "mf", overrides=SMALL)
+    idx = fk.sector(wl.n_alpha, wl.n_beta)
+    H1 = fk.hamiltonian_eq1(wl.h, _V(wl.L))[idx][:, idx].toarray()
+    H2 = fk.hamiltonian_eq1(wm.h, _V(wm.L))[idx][:, idx].toarray() + wm.e_const * np.eye(idx.size)
+    assert abs(H1 - H2).max() < 1e-11
+    P = wl.psi_a @ wl.psi_a.T + wl.psi_b @ wl.psi_b.T
+    assert np.allclose(np.einsum("gij,ji->g", wm.L, P), 0, atol=1e-12)
+    inim = O.o_init(wm.h, wm.L, wm.dt, wm.psi_a, wm.psi_b)
+    phi = random_walkers(wl, 3, seed=15)
+    e1 = O.o_seed_state(ini, phi, wl.n_alpha).eloc
+    e2 = O.o_seed_state(inim, phi, wl.n_alpha).eloc + wm.e_const
+    assert np.allclose(e1, e2, rtol=1e-11)
+
+
+def test_closed_shell_invariant():
+    """R18: closed shell => Phi_alpha == Phi_beta at every step (cfg 1)."""
+    wl = make_workload(1)
+    ini = O.o_init(wl.h, wl.L, wl.dt, wl.psi_a, wl.psi_b)
+    st = O.o_seed_state(ini, wl.walkers(8), wl.n_alpha)
+    x = wl.fields(3, 8)
+    for n in range(3):
+        st, _ = O.o_step(ini, st, x[n], wl.n_alpha)
+        assert np.allclose(st.phi[..., :2], st.phi[..., 2:], atol=1e-14)
