@@ -1,0 +1,159 @@
+/* afqmc.h -- C ABI of the B200-native phaseless-AFQMC walker step.
+ *
+ * Source of every operation: Shee, Arthur, Zhang, Reichman, Friesner, "Phaseless Auxiliary-Field
+ * Quantum Monte Carlo on Graphical Processing Units" (arXiv:1804.03310).  Citations are
+ * PAPER.md:<line> (+ section / equation).  Where the paper is silent the reading is the one
+ * listed in DESIGN.md "Readings" (R1..R18).
+ *
+ * Conventions that hold for every entry point
+ *   - returns an afqmc_status; never throws, never prints, never allocates device memory;
+ *   - the device entry points enqueue work on the stream given to afqmc_init and do NOT
+ *     synchronise (the caller synchronises its stream); afqmc_init and afqmc_step_host do;
+ *   - "DEVICE" pointers are caller-owned device memory (the Python binding hands in
+ *     torch tensors' data_ptr()); "HOST" pointers are ordinary host memory;
+ *   - complex = interleaved (re, im) pairs of the stated real type;
+ *   - the real type T of walkers / Green's functions / force bias / fields follows
+ *     afqmc_params.precision (0: float, complex64 walkers; 1: double, complex128 walkers);
+ *     overlaps, weights, local energies are ALWAYS FP64 (R17: |S| reaches 1e209);
+ *   - numerical events never fail a call: they set bits in flags[w]
+ *       bit 0  overlap matrix singular / pivot below eps*max|A|
+ *       bit 1  non-finite overlap or weight
+ *       bit 2  walker killed by the phaseless rule cos(dtheta) <= 0 (weight := 0 exactly)
+ *   - argument errors (null pointers, sizes out of the supported range) return
+ *     AFQMC_EINVAL / AFQMC_EUNSUPPORTED before any launch.
+ *
+ * Layouts (w = walker, M = basis size, N_t = n_alpha + n_beta, alpha columns first)
+ *   phi   [N_w][M][N_t] complex T     walker determinants Phi_w
+ *   theta [N_w][M][N_t] complex T     Theta_s = Phi_s (Psi_s^T Phi_s)^-1
+ *                                     (multi-det: Theta of the reference determinant)
+ *   G     [N_w][2][M][M] complex T    G_s[i][j] = <Psi_T|c+_i c_j|phi>/<Psi_T|phi> (mixed for multi-det)
+ *   fb    [N_w][n_chol]  complex T    f_g = sum_s Tr(L_g G_s)
+ *   x     [N_w][n_chol]  T            auxiliary fields (host-drawn N(0,1)) PAPER.md:45 Eq.(2)
+ *   ovlp  [N_w] complex double        S = <Psi_T|phi_w>
+ *   weight[N_w] double ; eloc [N_w] complex double ; flags [N_w] int32
+ */
+#ifndef AFQMC_B200_H
+#define AFQMC_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define AFQMC_API __attribute__((visibility("default")))
+#else
+#define AFQMC_API
+#endif
+
+typedef struct afqmc_ctx afqmc_ctx; /* opaque; owns no memory the caller allocated */
+
+typedef enum {
+  AFQMC_OK = 0,
+  AFQMC_EINVAL = 1,
+  AFQMC_EUNSUPPORTED = 2,
+  AFQMC_ECUDA = 3,
+  AFQMC_ENOMEM = 4
+} afqmc_status;
+
+typedef struct {
+  int32_t M;            /* orbitals */
+  int32_t n_alpha;      /* spin-up electrons (<= 32) */
+  int32_t n_beta;       /* spin-down electrons (<= 32, may be 0) */
+  int32_t n_chol;       /* N_gamma Cholesky / DF vectors */
+  int32_t n_walkers;    /* N_w, batch handled by every call */
+  int32_t precision;    /* 0: complex64 walkers / FP32 operands; 1: complex128 / FP64 */
+  int32_t taylor_order; /* K of exp(A) ~ sum_{k<=K} A^k/k! (R9); 1..20 */
+  int32_t weight_mode;  /* 0: hybrid; 1: local-energy form */
+  int32_t n_det;        /* determinants in the trial, 1 = single determinant */
+  int32_t n_act;        /* active orbitals spanning all determinants (0 if n_det == 1) */
+  int32_t max_exc;      /* slots per spin in det_exc; excitation rank per spin <= 2 */
+  int32_t gemm_path;    /* 0: auto; 1: SIMT FP32/FP64 everywhere; 2: tcgen05 3xTF32 where available
+                           (precision 0 only).  DESIGN.md "Precision split". */
+  double dt;            /* time step */
+  double E0;            /* projector shift in e^{dt(E0-H)} (R7) */
+} afqmc_params;
+
+/* Bytes of DEVICE memory the caller must hand to afqmc_init: const_bytes holds the operands
+ * precomputed once (E_h, R, Y, transposed L, ... PAPER.md:80 "computed once at the start"),
+ * work_bytes holds per-step intermediates (one-body operators A_w, split planes, ...) and the
+ * FP64 staging used during init.  Both are multiples of 256. */
+AFQMC_API afqmc_status afqmc_query_bytes(const afqmc_params* p, size_t* const_bytes, size_t* work_bytes);
+
+/* Build a context.  HOST inputs, FP64, row-major, read only during this call:
+ *   h1      [M][M]          one-body matrix T_ij of Eq.(1), real symmetric
+ *   L_chol  [n_chol][M][M]  V_ijkl = sum_g L_g[i][k] L_g[j][l], each real symmetric
+ *   psiT_a  [M][n_alpha], psiT_b [M][n_beta]   trial orbitals, single determinant
+ *   multi-determinant trial (n_det > 1): C_act [M][n_act] orthonormal columns shared
+ *   by both spins, first n_sigma columns = reference determinant (psiT_a/psiT_b are then ignored
+ *   and may be NULL); det_coeff [n_det] real c_i; det_exc [n_det][2][max_exc][2] =
+ *   (hole < n_sigma, particle >= n_sigma) pairs, -1 padded: column `hole` of the reference is
+ *   replaced in place by column `particle` of C_act (no re-sorting, hence no sign).
+ * DEVICE: const_mem / work_mem of at least the sizes afqmc_query_bytes returned, 256-aligned,
+ * owned by the caller, must outlive the context.  stream = cudaStream_t (0 = legacy default).
+ * Precomputes on the device (hand-written FP64 kernels): h' = h - 1/2 sum_g L_g^2,
+ * E_h = exp(-dt/2 h') (R3), R^s_g = Psi_s^T L_g, Y^s of Eq.(5), Psi_s^T h.
+ * Synchronises the stream before returning.  Errors: EINVAL (null / non-symmetric h or L /
+ * bad excitation list), EUNSUPPORTED (sizes), ECUDA. */
+AFQMC_API afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1, const double* L_chol,
+                        const double* psiT_a, const double* psiT_b, const double* C_act,
+                        const double* det_coeff, const int32_t* det_exc, void* const_mem, void* work_mem,
+                        void* stream);
+AFQMC_API void afqmc_destroy(afqmc_ctx* ctx);
+/* Last error text of this context ("" if none); valid until the next call on ctx. ctx may be NULL
+ * (then the text of the last failed afqmc_init of this thread). */
+AFQMC_API const char* afqmc_last_error(const afqmc_ctx* ctx);
+
+/* H1-H3: per walker A_s = Psi_s^T Phi_s, S = det A_a det A_b (LU, partial
+ * pivoting), Theta_s = Phi_s A_s^-1; optional full G (DEVICE or NULL).  Multi-determinant trial:
+ * S = sum_i c_i S_i with S_i from Sherman-Morrison-Woodbury updates off the reference (Eq.(4),
+ * PAPER.md:63-66), theta = reference Theta_0, G = mixed Green's function. All DEVICE. */
+AFQMC_API afqmc_status afqmc_overlap_green(afqmc_ctx* ctx, const void* phi, void* ovlp, void* theta, void* G_or_null,
+                                 int32_t* flags);
+
+/* H4: f_g = sum_s sum_{a,k} R^s_g[a][k] Theta_s[k][a] = sum_s Tr(L_g G_s)
+ * (multi-det: mixed over determinants, needs the walker itself).  All DEVICE.  phi may be NULL for a
+ * single-determinant trial. */
+AFQMC_API afqmc_status afqmc_force_bias(afqmc_ctx* ctx, const void* phi, const void* theta, void* fb);
+
+/* H5-H8 (Eq.(2),(3); :97): xbar = -i sqrt(dt) f, xs = x - xbar,
+ * A = i sqrt(dt) sum_g xs_g L_g, Phi' = E_h [sum_{k<=K} A^k/k!] E_h Phi, then overlap / Theta of Phi',
+ * dtheta = arg(S'/S), hybrid weight w' = w e^{dt E0} |S'/S e^{c}| max(0, cos dtheta),
+ * c = x.xbar - xbar.xbar/2.  phi, ovlp, weight in/out; theta out; flags OR-ed.  All DEVICE.
+ * weight_mode 1 uses exp(-dt(Re E_L - E0)) with eloc_pre = E_L of the pre-step walker (DEVICE,
+ * complex double [N_w]); eloc_pre may be NULL in mode 0. */
+AFQMC_API afqmc_status afqmc_propagate(afqmc_ctx* ctx, void* phi, const void* x, const void* fb, void* ovlp, double* weight,
+                             void* theta, const void* eloc_pre, int32_t* flags);
+
+/* H9 / H10 (Eq.(5)): E_L = sum_s Tr(Psi_s^T h Theta_s) + 1/2 sum_s vec(Theta_s)^T Y^s
+ * vec(Theta_s) + sum_g f^a_g f^b_g  (complex).  Multi-det: mixed over determinants with rank-E updates
+ * (needs phi).  All DEVICE.  phi may be NULL for a single-determinant trial. */
+AFQMC_API afqmc_status afqmc_local_energy(afqmc_ctx* ctx, const void* phi, const void* theta, void* eloc);
+
+/* n_steps full walker steps (order R10): [shift -> assemble -> Taylor propagate -> overlap/Theta ->
+ * weight -> force bias -> local energy] per step.  State on entry/exit: phi, weight, ovlp, theta, fb of
+ * the current walkers (seed with afqmc_overlap_green + afqmc_force_bias).  x [n_steps][N_w][n_chol] T,
+ * eloc [n_steps][N_w] complex double (E_L of the post-step walker), flags OR-ed.  All DEVICE. */
+AFQMC_API afqmc_status afqmc_step(afqmc_ctx* ctx, void* phi, double* weight, void* ovlp, void* theta, void* fb,
+                        const void* x, int32_t n_steps, void* eloc, int32_t* flags);
+
+/* The same n_steps through HOST buffers (pinned or pageable): copies phi, weight, x to the device,
+ * seeds ovlp/theta/fb from phi, runs afqmc_step, copies phi, weight, ovlp, eloc, flags back, and
+ * synchronises.  Device staging lives in work_mem (sized by afqmc_query_bytes for one step of fields;
+ * x is streamed step by step).  h2d_bytes / d2h_bytes (may be NULL) receive the bytes moved. */
+AFQMC_API afqmc_status afqmc_step_host(afqmc_ctx* ctx, void* phi_h, double* weight_h, void* ovlp_h, const void* x_h,
+                             int32_t n_steps, void* eloc_h, int32_t* flags_h, size_t* h2d_bytes,
+                             size_t* d2h_bytes);
+
+/* Number of kernels this context has launched since init (bench.py's gpu_launches). */
+AFQMC_API int64_t afqmc_launch_count(const afqmc_ctx* ctx);
+
+/* Which contraction path the context resolved to: 1 = SIMT, 2 = tcgen05 3xTF32. */
+AFQMC_API int32_t afqmc_gemm_path(const afqmc_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AFQMC_B200_H */

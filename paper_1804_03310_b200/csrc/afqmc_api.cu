@@ -1,0 +1,606 @@
+// afqmc_api.cu -- C-ABI entry points (include/afqmc.h) of the B200-native ph-AFQMC walker step.
+// Host-side orchestration only: every arithmetic step of the path runs in the kernels of this directory.
+#include "../../include/afqmc.h"
+
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+#include "gemm_simt.cuh"
+#include "green.cuh"
+#include "misc.cuh"
+#include "taylor.cuh"
+
+using namespace afq;
+
+namespace {
+
+inline size_t rup(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct Carver {
+  size_t off = 0;
+  char* base = nullptr;
+  void* take(size_t bytes) {
+    void* p = base ? base + off : nullptr;
+    off += rup(bytes, 256);
+    return p;
+  }
+};
+
+thread_local char g_init_err[256] = "";
+
+}  // namespace
+
+struct afqmc_ctx {
+  afqmc_params p;
+  cudaStream_t stream;
+  int M, MP, na, nb, nt, ng, NGP, nw, KA, KB, KT, ts;  // ts = sizeof(T)
+  int split, path;
+  int tay_cw, tay_nch, tay_threads;
+  size_t tay_smem, green_smem;
+  // constants
+  void *psi_a, *psi_b, *Eh, *Lt, *Lt_lo, *Rall, *Rall_lo, *Y[2], *Y_lo[2], *hrot;
+  // per-step work
+  void *Z, *Z_lo, *Abuf, *thp, *thp_lo, *fs;
+  zcplx *cshift, *eloc_scratch;
+  // device staging for afqmc_step_host
+  void *h_phi, *h_theta, *h_fb, *h_x;
+  zcplx *h_ovlp, *h_eloc;
+  double* h_weight;
+  int32_t* h_flags;
+  // init staging (FP64)
+  double *Ld, *hd, *hpd, *Rd, *hrotd, *ex[4], *psid;
+  char err[256];
+  int64_t launches;
+};
+
+namespace {
+
+afqmc_status fail(afqmc_ctx* c, afqmc_status s, const char* fmt, const char* a = "") {
+  char* dst = c ? c->err : g_init_err;
+  snprintf(dst, 256, fmt, a);
+  return s;
+}
+
+#define CUDA_OK(c, call)                                                              \
+  do {                                                                                \
+    cudaError_t e_ = (call);                                                          \
+    if (e_ != cudaSuccess) return fail((c), AFQMC_ECUDA, "CUDA: %s", cudaGetErrorString(e_)); \
+  } while (0)
+
+#define LAUNCH(c, kern, grid, block, smem, ...)                                       \
+  do {                                                                                \
+    kern<<<(grid), (block), (smem), (c)->stream>>>(__VA_ARGS__);                      \
+    (c)->launches++;                                                                  \
+    cudaError_t e_ = cudaGetLastError();                                              \
+    if (e_ != cudaSuccess) return fail((c), AFQMC_ECUDA, #kern ": %s", cudaGetErrorString(e_)); \
+  } while (0)
+
+// Taylor kernel configuration: chunk width CW (compile-time), chunks, threads.
+template <typename T> int taylor_maxt(int cw) {
+  int cwp = (cw + 3) & ~3;
+  if (sizeof(T) == 4) return cwp >= 16 ? 448 : cwp >= 12 ? 576 : cwp >= 8 ? 768 : 1024;
+  return cwp >= 8 ? 448 : 768;
+}
+template <typename T> bool taylor_pick(int M, int nt, int& cw, int& nch) {
+  const int cwmax = sizeof(T) == 4 ? 16 : 8;
+  for (nch = 1; nch <= nt; ++nch) {
+    cw = (nt + nch - 1) / nch;
+    if (cw <= cwmax && M * nch <= taylor_maxt<T>(cw)) return true;
+  }
+  return false;
+}
+
+struct Layout {
+  int M, MP, na, nb, nt, ng, NGP, nw, KA, KB, KT, ts;
+  size_t const_bytes, work_bytes;
+};
+
+afqmc_status check_params(const afqmc_params* p, char* err) {
+  if (!p) { snprintf(err, 256, "params is NULL"); return AFQMC_EINVAL; }
+  if (p->M < 1 || p->n_alpha < 1 || p->n_beta < 0 || p->n_chol < 1 || p->n_walkers < 0 ||
+      p->n_alpha > p->M || p->n_beta > p->M) {
+    snprintf(err, 256, "bad sizes: need M>=1, 1<=n_alpha<=M, 0<=n_beta<=M, n_chol>=1, n_walkers>=0");
+    return AFQMC_EINVAL;
+  }
+  if (p->precision != 0 && p->precision != 1) { snprintf(err, 256, "precision must be 0 or 1"); return AFQMC_EINVAL; }
+  if (p->taylor_order < 1 || p->taylor_order > 20) { snprintf(err, 256, "taylor_order must be in 1..20"); return AFQMC_EINVAL; }
+  if (p->weight_mode != 0 && p->weight_mode != 1) { snprintf(err, 256, "weight_mode must be 0 or 1"); return AFQMC_EINVAL; }
+  if (!(p->dt > 0.0) || !isfinite(p->dt) || !isfinite(p->E0)) { snprintf(err, 256, "dt must be > 0 and finite"); return AFQMC_EINVAL; }
+  if (p->gemm_path < 0 || p->gemm_path > 2) { snprintf(err, 256, "gemm_path must be 0, 1 or 2"); return AFQMC_EINVAL; }
+  if (p->n_alpha > 32 || p->n_beta > 32) { snprintf(err, 256, "n_alpha, n_beta <= 32 supported"); return AFQMC_EUNSUPPORTED; }
+  if (p->n_det < 1) { snprintf(err, 256, "n_det must be >= 1"); return AFQMC_EINVAL; }
+  if (p->n_det > 1) { snprintf(err, 256, "multi-determinant trials not built yet"); return AFQMC_EUNSUPPORTED; }
+  if (p->gemm_path == 2) { snprintf(err, 256, "tcgen05 path not built yet"); return AFQMC_EUNSUPPORTED; }
+  int cw, nch;
+  bool ok = p->precision ? taylor_pick<double>(p->M, p->n_alpha + p->n_beta, cw, nch)
+                         : taylor_pick<float>(p->M, p->n_alpha + p->n_beta, cw, nch);
+  if (!ok) { snprintf(err, 256, "M * ceil(N_t / chunk) exceeds one CTA (M too large for the Taylor kernel)"); return AFQMC_EUNSUPPORTED; }
+  size_t gs = p->precision ? green_smem_bytes<double>(p->M, p->n_alpha, p->n_beta)
+                           : green_smem_bytes<float>(p->M, p->n_alpha, p->n_beta);
+  if (gs > 200 * 1024) { snprintf(err, 256, "walker does not fit one CTA's shared memory"); return AFQMC_EUNSUPPORTED; }
+  return AFQMC_OK;
+}
+
+// Carve (or just size, when base pointers are null) every buffer.
+void carve(const afqmc_params* p, afqmc_ctx* c, char* cbase, char* wbase, size_t* cb, size_t* wb) {
+  const int M = p->M, na = p->n_alpha, nb = p->n_beta, nt = na + nb, ng = p->n_chol, nw = p->n_walkers;
+  const int ts = p->precision ? 8 : 4;
+  const int MP = (M + 3) & ~3, NGP = (int)rup(ng, 32);
+  const int KA = (int)rup((size_t)M * na, 32), KB = (int)rup((size_t)M * nb, 32), KT = KA + KB;
+  c->M = M; c->MP = MP; c->na = na; c->nb = nb; c->nt = nt; c->ng = ng; c->NGP = NGP; c->nw = nw;
+  c->KA = KA; c->KB = KB; c->KT = KT; c->ts = ts;
+  const int split = c->split;
+  Carver cc; cc.base = cbase;
+  c->psi_a = cc.take((size_t)M * na * ts);
+  c->psi_b = cc.take((size_t)M * (nb ? nb : 1) * ts);
+  c->Eh = cc.take((size_t)M * MP * ts);
+  c->Lt = cc.take((size_t)M * M * NGP * ts);
+  c->Lt_lo = split ? cc.take((size_t)M * M * NGP * ts) : nullptr;
+  c->Rall = cc.take((size_t)rup(ng, 128) * KT * ts);
+  c->Rall_lo = split ? cc.take((size_t)rup(ng, 128) * KT * ts) : nullptr;
+  c->Y[0] = cc.take((size_t)KA * KA * ts);
+  c->Y[1] = cc.take((size_t)(KB ? KB : 32) * (KB ? KB : 32) * ts);
+  c->Y_lo[0] = split ? cc.take((size_t)KA * KA * ts) : nullptr;
+  c->Y_lo[1] = split ? cc.take((size_t)(KB ? KB : 32) * (KB ? KB : 32) * ts) : nullptr;
+  c->hrot = cc.take((size_t)KT * ts);
+  *cb = cc.off;
+
+  Carver w; w.base = wbase;
+  const size_t nw1 = nw ? nw : 1;
+  c->Z = w.take(2 * nw1 * NGP * ts);
+  c->Z_lo = split ? w.take(2 * nw1 * NGP * ts) : nullptr;
+  c->Abuf = w.take(nw1 * M * 2 * MP * ts);
+  c->thp = w.take(2 * nw1 * KT * ts);
+  c->thp_lo = split ? w.take(2 * nw1 * KT * ts) : nullptr;
+  c->fs = w.take(2 * 2 * nw1 * NGP * ts);
+  c->cshift = (zcplx*)w.take(nw1 * sizeof(zcplx));
+  c->eloc_scratch = (zcplx*)w.take(nw1 * sizeof(zcplx));
+  c->h_phi = w.take(nw1 * M * nt * 2 * ts);
+  c->h_theta = w.take(nw1 * M * nt * 2 * ts);
+  c->h_fb = w.take(nw1 * ng * 2 * ts);
+  c->h_x = w.take(nw1 * ng * ts);
+  c->h_ovlp = (zcplx*)w.take(nw1 * sizeof(zcplx));
+  c->h_eloc = (zcplx*)w.take(nw1 * sizeof(zcplx));
+  c->h_weight = (double*)w.take(nw1 * sizeof(double));
+  c->h_flags = (int32_t*)w.take(nw1 * sizeof(int32_t));
+  // FP64 init staging
+  c->Ld = (double*)w.take((size_t)ng * M * M * 8);
+  c->hd = (double*)w.take((size_t)M * M * 8);
+  c->hpd = (double*)w.take((size_t)M * M * 8);
+  c->Rd = (double*)w.take((size_t)ng * KT * 8);
+  c->hrotd = (double*)w.take((size_t)KT * 8);
+  for (int i = 0; i < 4; ++i) c->ex[i] = (double*)w.take((size_t)M * M * 8);
+  c->psid = (double*)w.take((size_t)M * nt * 8);
+  *wb = w.off;
+}
+
+template <typename T> afqmc_status init_device(afqmc_ctx* c, const double* h1, const double* L, const double* pa, const double* pb) {
+  const int M = c->M, MP = c->MP, na = c->na, nb = c->nb, ng = c->ng, NGP = c->NGP, KA = c->KA, KB = c->KB, KT = c->KT;
+  cudaStream_t st = c->stream;
+  size_t cb, wb;
+  {
+    afqmc_ctx tmp = *c;
+    carve(&c->p, &tmp, nullptr, nullptr, &cb, &wb);
+  }
+  CUDA_OK(c, cudaMemsetAsync(c->psi_a, 0, cb, st));           // const_mem starts at psi_a
+  CUDA_OK(c, cudaMemsetAsync(c->Z, 0, wb, st));               // work_mem starts at Z
+  CUDA_OK(c, cudaMemcpyAsync(c->hd, h1, (size_t)M * M * 8, cudaMemcpyHostToDevice, st));
+  CUDA_OK(c, cudaMemcpyAsync(c->Ld, L, (size_t)ng * M * M * 8, cudaMemcpyHostToDevice, st));
+  double* psid_a = c->psid;
+  double* psid_b = c->psid + (size_t)M * na;
+  CUDA_OK(c, cudaMemcpyAsync(psid_a, pa, (size_t)M * na * 8, cudaMemcpyHostToDevice, st));
+  if (nb) CUDA_OK(c, cudaMemcpyAsync(psid_b, pb, (size_t)M * nb * 8, cudaMemcpyHostToDevice, st));
+
+  const int mm = M * M;
+  LAUNCH(c, k_init_hprime, (mm + 127) / 128, 128, 0, M, ng, c->hd, c->Ld, c->hpd);
+  // E_h = expm(-(dt/2) h') by scaling and squaring of an order-18 Taylor (Horner) series, FP64
+  std::vector<double> hp((size_t)mm);
+  CUDA_OK(c, cudaMemcpyAsync(hp.data(), c->hpd, (size_t)mm * 8, cudaMemcpyDeviceToHost, st));
+  CUDA_OK(c, cudaStreamSynchronize(st));
+  double n1 = 0.0;
+  for (int j = 0; j < M; ++j) {
+    double s = 0.0;
+    for (int i = 0; i < M; ++i) s += fabs(hp[(size_t)i * M + j]);
+    n1 = fmax(n1, s);
+  }
+  if (!isfinite(n1)) return fail(c, AFQMC_EINVAL, "h1 / L_chol contain non-finite values");
+  n1 *= 0.5 * c->p.dt;
+  int sq = 0;
+  while (n1 > 0.5 && sq < 60) { n1 *= 0.5; ++sq; }
+  double* X = c->ex[0];
+  double* E = c->ex[1];
+  double* Tm = c->ex[2];
+  LAUNCH(c, k_dscale_eye, (mm + 127) / 128, 128, 0, M, -0.5 * c->p.dt / ldexp(1.0, sq), c->hpd, 0.0, X);
+  LAUNCH(c, k_dscale_eye, (mm + 127) / 128, 128, 0, M, 0.0, c->hpd, 1.0, E);
+  for (int k = 18; k >= 1; --k) {
+    LAUNCH(c, k_dgemm_small, (mm + 127) / 128, 128, 0, M, 1.0 / k, X, E, 0.0, (const double*)nullptr, Tm);
+    LAUNCH(c, k_dscale_eye, (mm + 127) / 128, 128, 0, M, 1.0, Tm, 1.0, E);
+  }
+  for (int s = 0; s < sq; ++s) {
+    LAUNCH(c, k_dgemm_small, (mm + 127) / 128, 128, 0, M, 1.0, E, E, 0.0, (const double*)nullptr, Tm);
+    double* t = E; E = Tm; Tm = t;
+  }
+  LAUNCH(c, k_cast2d<T>, (mm + 127) / 128, 128, 0, M, M, E, (size_t)M, (T*)c->Eh, (T*)nullptr, (size_t)MP, 0);
+  // trial orbitals in T
+  LAUNCH(c, k_cast2d<T>, (M * na + 127) / 128, 128, 0, M, na, psid_a, (size_t)na, (T*)c->psi_a, (T*)nullptr, (size_t)na, 0);
+  if (nb) LAUNCH(c, k_cast2d<T>, (M * nb + 127) / 128, 128, 0, M, nb, psid_b, (size_t)nb, (T*)c->psi_b, (T*)nullptr, (size_t)nb, 0);
+  // R^s_g = Psi_s^T L_g and Psi_s^T h, spin-blocked index (s_off + k*n_s + a)
+  for (int s = 0; s < 2; ++s) {
+    int n = s ? nb : na, soff = s ? KA : 0;
+    if (!n) continue;
+    const double* C = s ? psid_b : psid_a;
+    size_t tot = (size_t)ng * M * n;
+    LAUNCH(c, k_init_rot, (unsigned)((tot + 127) / 128), 128, 0, M, n, n, C, ng, c->Ld, soff, KT, c->Rd);
+    LAUNCH(c, k_init_rot, (M * n + 127) / 128, 128, 0, M, n, n, C, 1, c->hd, soff, KT, c->hrotd);
+    int Ks = s ? KB : KA;
+    LAUNCH(c, k_init_Y<T>, dim3((M * n + 127) / 128, M * n), 128, 0, M, n, ng, c->Rd, soff, KT, (T*)c->Y[s],
+           (T*)c->Y_lo[s], Ks, c->split);
+  }
+  {
+    size_t tot = (size_t)ng * KT;
+    LAUNCH(c, k_cast2d<T>, (unsigned)((tot + 127) / 128), 128, 0, ng, KT, c->Rd, (size_t)KT, (T*)c->Rall, (T*)c->Rall_lo,
+           (size_t)KT, c->split);
+    LAUNCH(c, k_cast2d<T>, (KT + 127) / 128, 128, 0, 1, KT, c->hrotd, (size_t)KT, (T*)c->hrot, (T*)nullptr, (size_t)KT, 0);
+  }
+  // Lt[ij][g] = L[g][ij]  (K-major operand of the assembly GEMM)
+  LAUNCH(c, k_transpose_cast<T>, dim3((ng + 31) / 32, (mm + 31) / 32), dim3(32, 8), 0, mm, ng, c->Ld, (size_t)mm,
+         (T*)c->Lt, (T*)c->Lt_lo, (size_t)NGP, c->split);
+  CUDA_OK(c, cudaStreamSynchronize(st));
+  return AFQMC_OK;
+}
+
+// ---- stage launchers -------------------------------------------------------------------------
+
+template <typename T>
+afqmc_status run_green(afqmc_ctx* c, const void* phi, void* ovlp, void* theta, int do_weight, double* weight,
+                       const void* eloc_pre, int32_t* flags) {
+  GreenArgs<T> g;
+  g.M = c->M; g.na = c->na; g.nb = c->nb; g.nw = c->nw;
+  g.phi = (const cplx<T>*)phi; g.psi_a = (const T*)c->psi_a; g.psi_b = (const T*)c->psi_b;
+  g.theta = (cplx<T>*)theta; g.thp = (T*)c->thp; g.thp_lo = (T*)c->thp_lo;
+  g.KA = c->KA; g.KT = c->KT; g.split = c->split;
+  g.ovlp = (zcplx*)ovlp; g.do_weight = do_weight; g.cshift = c->cshift; g.weight = weight;
+  g.eloc_pre = (const zcplx*)eloc_pre; g.weight_mode = c->p.weight_mode; g.dt = c->p.dt; g.E0 = c->p.E0;
+  g.flags = flags;
+  LAUNCH(c, k_green<T>, c->nw, 128, c->green_smem, g);
+  return AFQMC_OK;
+}
+
+template <typename T, class Epi>
+afqmc_status run_gemm(afqmc_ctx* c, const T* A, int lda, int m, const T* B, int ldb, int n, int K, Epi epi) {
+  typedef GemmCfg<T> G;
+  dim3 grid((n + G::BN - 1) / G::BN, (m + G::BM - 1) / G::BM);
+  auto kern = k_gemm_nt<T, Epi>;
+  LAUNCH(c, kern, grid, 256, 0, A, lda, m, B, ldb, n, K, epi);
+  return AFQMC_OK;
+}
+
+// per-spin traces f^s_g = sum R^s_g[a][k] Theta_s[k][a] from the planar Theta in ctx->thp
+template <typename T> afqmc_status run_fb_gemm(afqmc_ctx* c) {
+  for (int s = 0; s < 2; ++s) {
+    int n = s ? c->nb : c->na, soff = s ? c->KA : 0, Ks = s ? c->KB : c->KA;
+    if (!n) continue;
+    EpiStoreT<T> epi;
+    epi.out = (T*)c->fs + (size_t)s * 2 * c->nw * c->NGP; epi.ldo = c->NGP; epi.m_real = c->ng; epi.n_real = 2 * c->nw;
+    afqmc_status st = run_gemm<T>(c, (const T*)c->Rall + soff, c->KT, c->ng, (const T*)c->thp + soff, c->KT, 2 * c->nw, Ks, epi);
+    if (st) return st;
+  }
+  return AFQMC_OK;
+}
+
+template <typename T> afqmc_status run_energy_gemm(afqmc_ctx* c, zcplx* eloc) {
+  for (int s = 0; s < 2; ++s) {
+    int n = s ? c->nb : c->na, soff = s ? c->KA : 0, Ks = s ? c->KB : c->KA;
+    if (!n) continue;
+    EpiEnergy<T> epi;
+    epi.thp = (const T*)c->thp; epi.thp_lo = (const T*)c->thp_lo; epi.KT = c->KT; epi.soff = soff;
+    epi.hrot = (const T*)c->hrot + soff; epi.eloc = (double*)eloc; epi.m_real = c->M * n; epi.n_real = 2 * c->nw;
+    afqmc_status st = run_gemm<T>(c, (const T*)c->Y[s], Ks, c->M * n, (const T*)c->thp + soff, c->KT, 2 * c->nw, Ks, epi);
+    if (st) return st;
+  }
+  return AFQMC_OK;
+}
+
+template <typename T> afqmc_status run_taylor(afqmc_ctx* c, void* phi) {
+  TaylorArgs<T> g;
+  g.M = c->M; g.MP = c->MP; g.nt = c->nt; g.K = c->p.taylor_order; g.nchunks = c->tay_nch;
+  g.phi = (cplx<T>*)phi; g.A = (const T*)c->Abuf; g.Eh = (const T*)c->Eh;
+#define TAY_CASE(CW)                                                                                        \
+  case CW: {                                                                                                \
+    constexpr int MT = sizeof(T) == 4 ? (((CW + 3) & ~3) >= 16 ? 448 : ((CW + 3) & ~3) >= 12 ? 576 : ((CW + 3) & ~3) >= 8 ? 768 : 1024) \
+                                      : (((CW + 3) & ~3) >= 8 ? 448 : 768);                                 \
+    auto kern = k_taylor<T, CW, MT>;                                                                        \
+    if (c->tay_smem > 48 * 1024)                                                                            \
+      CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tay_smem)); \
+    LAUNCH(c, kern, c->nw, c->tay_threads, c->tay_smem, g);                                                 \
+  } break;
+  switch (c->tay_cw) {
+    TAY_CASE(1) TAY_CASE(2) TAY_CASE(3) TAY_CASE(4) TAY_CASE(5) TAY_CASE(6) TAY_CASE(7) TAY_CASE(8)
+    default:
+      if constexpr (sizeof(T) == 4) {
+        switch (c->tay_cw) {
+          TAY_CASE(9) TAY_CASE(10) TAY_CASE(11) TAY_CASE(12) TAY_CASE(13) TAY_CASE(14) TAY_CASE(15) TAY_CASE(16)
+          default: return fail(c, AFQMC_EUNSUPPORTED, "taylor chunk width");
+        }
+      } else {
+        return fail(c, AFQMC_EUNSUPPORTED, "taylor chunk width");
+      }
+  }
+#undef TAY_CASE
+  return AFQMC_OK;
+}
+
+template <typename T>
+afqmc_status do_propagate(afqmc_ctx* c, void* phi, const void* x, const void* fb, void* ovlp, double* weight, void* theta,
+                          const void* eloc_pre, int32_t* flags) {
+  LAUNCH(c, k_shift<T>, c->nw, 128, 0, c->ng, c->NGP, c->p.dt, (const cplx<T>*)fb, (const T*)x, (T*)c->Z, (T*)c->Z_lo,
+         c->split, c->cshift);
+  EpiAssemble<T> epi;
+  epi.out = (T*)c->Abuf; epi.M = c->M; epi.MP = c->MP; epi.m_real = c->M * c->M; epi.n_real = 2 * c->nw;
+  afqmc_status st = run_gemm<T>(c, (const T*)c->Lt, c->NGP, c->M * c->M, (const T*)c->Z, c->NGP, 2 * c->nw, c->NGP, epi);
+  if (st) return st;
+  st = run_taylor<T>(c, phi);
+  if (st) return st;
+  return run_green<T>(c, phi, ovlp, theta, 1, weight, eloc_pre, flags);
+}
+
+template <typename T> afqmc_status do_force_bias(afqmc_ctx* c, const void* theta, void* fb) {
+  LAUNCH(c, k_planarize<T>, c->nw, 128, 0, c->M, c->na, c->nb, c->KA, c->KT, c->split, (const cplx<T>*)theta, (T*)c->thp,
+         (T*)c->thp_lo);
+  afqmc_status st = run_fb_gemm<T>(c);
+  if (st) return st;
+  LAUNCH(c, k_fb_finish<T>, c->nw, 128, 0, c->ng, c->NGP, c->nw, (const T*)c->fs, (cplx<T>*)fb, (zcplx*)nullptr);
+  return AFQMC_OK;
+}
+
+// energy of the walkers whose planar Theta is in ctx->thp; runs the force-bias GEMM too (fb may be null)
+template <typename T> afqmc_status do_fb_energy_planar(afqmc_ctx* c, void* fb, zcplx* eloc) {
+  afqmc_status st = run_fb_gemm<T>(c);
+  if (st) return st;
+  LAUNCH(c, k_fb_finish<T>, c->nw, 128, 0, c->ng, c->NGP, c->nw, (const T*)c->fs, (cplx<T>*)fb, eloc);
+  return run_energy_gemm<T>(c, eloc);
+}
+
+template <typename T>
+afqmc_status do_step(afqmc_ctx* c, void* phi, double* weight, void* ovlp, void* theta, void* fb, const void* x, int n_steps,
+                     void* eloc, int32_t* flags) {
+  zcplx* el = (zcplx*)eloc;
+  const zcplx* epre = nullptr;
+  if (c->p.weight_mode == 1) {
+    // E_L of the walkers on entry (needs their planar Theta)
+    LAUNCH(c, k_planarize<T>, c->nw, 128, 0, c->M, c->na, c->nb, c->KA, c->KT, c->split, (const cplx<T>*)theta,
+           (T*)c->thp, (T*)c->thp_lo);
+    afqmc_status st = do_fb_energy_planar<T>(c, nullptr, c->eloc_scratch);
+    if (st) return st;
+    epre = c->eloc_scratch;
+  }
+  for (int s = 0; s < n_steps; ++s) {
+    const T* xs = (const T*)x + (size_t)s * c->nw * c->ng;
+    afqmc_status st = do_propagate<T>(c, phi, xs, fb, ovlp, weight, theta, epre, flags);
+    if (st) return st;
+    st = do_fb_energy_planar<T>(c, fb, el + (size_t)s * c->nw);
+    if (st) return st;
+    epre = el + (size_t)s * c->nw;
+  }
+  return AFQMC_OK;
+}
+
+}  // namespace
+
+// ================================================================================================
+extern "C" {
+
+afqmc_status afqmc_query_bytes(const afqmc_params* p, size_t* const_bytes, size_t* work_bytes) {
+  afqmc_status s = check_params(p, g_init_err);
+  if (s) return s;
+  if (!const_bytes || !work_bytes) { snprintf(g_init_err, 256, "null output pointer"); return AFQMC_EINVAL; }
+  afqmc_ctx tmp;
+  memset(&tmp, 0, sizeof(tmp));
+  tmp.p = *p;
+  tmp.split = (p->gemm_path == 2);
+  carve(p, &tmp, nullptr, nullptr, const_bytes, work_bytes);
+  return AFQMC_OK;
+}
+
+afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1, const double* L_chol,
+                        const double* psiT_a, const double* psiT_b, const double* C_act, const double* det_coeff,
+                        const int32_t* det_exc, void* const_mem, void* work_mem, void* stream) {
+  (void)C_act; (void)det_coeff; (void)det_exc;
+  if (!out) { snprintf(g_init_err, 256, "out is NULL"); return AFQMC_EINVAL; }
+  *out = nullptr;
+  afqmc_status s = check_params(p, g_init_err);
+  if (s) return s;
+  if (!h1 || !L_chol || !psiT_a || (p->n_beta && !psiT_b) || !const_mem || !work_mem) {
+    snprintf(g_init_err, 256, "null input pointer");
+    return AFQMC_EINVAL;
+  }
+  if (((uintptr_t)const_mem & 255) || ((uintptr_t)work_mem & 255)) {
+    snprintf(g_init_err, 256, "const_mem / work_mem must be 256-byte aligned");
+    return AFQMC_EINVAL;
+  }
+  // h and every L_g must be symmetric: the kernels rely on it
+  const int M = p->M;
+  double amax = 0.0;
+  for (size_t e = 0; e < (size_t)M * M; ++e) amax = fmax(amax, fabs(h1[e]));
+  for (int i = 0; i < M; ++i)
+    for (int j = 0; j < i; ++j)
+      if (fabs(h1[(size_t)i * M + j] - h1[(size_t)j * M + i]) > 1e-10 * (amax + 1e-300)) {
+        snprintf(g_init_err, 256, "h1 is not symmetric");
+        return AFQMC_EINVAL;
+      }
+  for (int g = 0; g < p->n_chol; ++g) {
+    const double* Lg = L_chol + (size_t)g * M * M;
+    double lm = 0.0;
+    for (size_t e = 0; e < (size_t)M * M; ++e) lm = fmax(lm, fabs(Lg[e]));
+    if (!isfinite(lm)) { snprintf(g_init_err, 256, "L_chol contains non-finite values"); return AFQMC_EINVAL; }
+    for (int i = 0; i < M; ++i)
+      for (int j = 0; j < i; ++j)
+        if (fabs(Lg[(size_t)i * M + j] - Lg[(size_t)j * M + i]) > 1e-10 * (lm + 1e-300)) {
+          snprintf(g_init_err, 256, "L_chol[g] is not symmetric");
+          return AFQMC_EINVAL;
+        }
+  }
+  afqmc_ctx* c = new (std::nothrow) afqmc_ctx;
+  if (!c) { snprintf(g_init_err, 256, "host allocation failed"); return AFQMC_ENOMEM; }
+  memset(c, 0, sizeof(*c));
+  c->p = *p;
+  c->stream = (cudaStream_t)stream;
+  c->path = 1;
+  c->split = 0;
+  size_t cb, wb;
+  carve(p, c, (char*)const_mem, (char*)work_mem, &cb, &wb);
+  if (p->precision) {
+    taylor_pick<double>(c->M, c->nt, c->tay_cw, c->tay_nch);
+    c->tay_smem = taylor_smem_bytes<double>(c->M, c->MP, c->tay_nch, (c->tay_cw + 3) & ~3);
+    c->green_smem = green_smem_bytes<double>(c->M, c->na, c->nb);
+  } else {
+    taylor_pick<float>(c->M, c->nt, c->tay_cw, c->tay_nch);
+    c->tay_smem = taylor_smem_bytes<float>(c->M, c->MP, c->tay_nch, (c->tay_cw + 3) & ~3);
+    c->green_smem = green_smem_bytes<float>(c->M, c->na, c->nb);
+  }
+  c->tay_threads = (int)rup((size_t)c->M * c->tay_nch, 32);
+  if (c->tay_smem > 227 * 1024) {
+    s = fail(nullptr, AFQMC_EUNSUPPORTED, "Taylor kernel tile exceeds shared memory");
+    delete c;
+    return s;
+  }
+  if (c->green_smem > 48 * 1024) {
+    cudaError_t e = p->precision ? cudaFuncSetAttribute(k_green<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->green_smem)
+                                 : cudaFuncSetAttribute(k_green<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->green_smem);
+    if (e != cudaSuccess) { snprintf(g_init_err, 256, "CUDA: %s", cudaGetErrorString(e)); delete c; return AFQMC_ECUDA; }
+  }
+  s = p->precision ? init_device<double>(c, h1, L_chol, psiT_a, psiT_b) : init_device<float>(c, h1, L_chol, psiT_a, psiT_b);
+  if (s) {
+    memcpy(g_init_err, c->err, 256);
+    delete c;
+    return s;
+  }
+  c->launches = 0;
+  *out = c;
+  return AFQMC_OK;
+}
+
+void afqmc_destroy(afqmc_ctx* ctx) { delete ctx; }
+
+const char* afqmc_last_error(const afqmc_ctx* ctx) { return ctx ? ctx->err : g_init_err; }
+
+int64_t afqmc_launch_count(const afqmc_ctx* ctx) { return ctx ? ctx->launches : 0; }
+int32_t afqmc_gemm_path(const afqmc_ctx* ctx) { return ctx ? ctx->path : 0; }
+
+#define NEED(c, cond, msg) \
+  do { if (!(cond)) return fail((c), AFQMC_EINVAL, "%s", msg); } while (0)
+#define DISPATCH(c, fn, ...) ((c)->p.precision ? fn<double>(__VA_ARGS__) : fn<float>(__VA_ARGS__))
+
+afqmc_status afqmc_overlap_green(afqmc_ctx* c, const void* phi, void* ovlp, void* theta, void* G_or_null, int32_t* flags) {
+  if (!c) return AFQMC_EINVAL;
+  c->err[0] = 0;
+  NEED(c, phi && ovlp && theta, "afqmc_overlap_green: null pointer");
+  if (c->nw == 0) return AFQMC_OK;
+  afqmc_status s = DISPATCH(c, run_green, c, phi, ovlp, theta, 0, nullptr, nullptr, flags);
+  if (s) return s;
+  if (G_or_null) {
+    dim3 grid((c->M * c->M + 255) / 256, c->nw, 2);
+    if (c->p.precision)
+      LAUNCH(c, k_gfull<double>, grid, 256, 0, c->M, c->na, c->nb, (const cplx<double>*)theta, (const double*)c->psi_a,
+             (const double*)c->psi_b, (cplx<double>*)G_or_null);
+    else
+      LAUNCH(c, k_gfull<float>, grid, 256, 0, c->M, c->na, c->nb, (const cplx<float>*)theta, (const float*)c->psi_a,
+             (const float*)c->psi_b, (cplx<float>*)G_or_null);
+  }
+  return AFQMC_OK;
+}
+
+afqmc_status afqmc_force_bias(afqmc_ctx* c, const void* phi, const void* theta, void* fb) {
+  (void)phi;
+  if (!c) return AFQMC_EINVAL;
+  c->err[0] = 0;
+  NEED(c, theta && fb, "afqmc_force_bias: null pointer");
+  if (c->nw == 0) return AFQMC_OK;
+  return DISPATCH(c, do_force_bias, c, theta, fb);
+}
+
+afqmc_status afqmc_propagate(afqmc_ctx* c, void* phi, const void* x, const void* fb, void* ovlp, double* weight, void* theta,
+                             const void* eloc_pre, int32_t* flags) {
+  if (!c) return AFQMC_EINVAL;
+  c->err[0] = 0;
+  NEED(c, phi && x && fb && ovlp && weight && theta, "afqmc_propagate: null pointer");
+  NEED(c, c->p.weight_mode == 0 || eloc_pre, "afqmc_propagate: weight_mode 1 needs eloc_pre");
+  if (c->nw == 0) return AFQMC_OK;
+  return DISPATCH(c, do_propagate, c, phi, x, fb, ovlp, weight, theta, eloc_pre, flags);
+}
+
+afqmc_status afqmc_local_energy(afqmc_ctx* c, const void* phi, const void* theta, void* eloc) {
+  (void)phi;
+  if (!c) return AFQMC_EINVAL;
+  c->err[0] = 0;
+  NEED(c, theta && eloc, "afqmc_local_energy: null pointer");
+  if (c->nw == 0) return AFQMC_OK;
+  if (c->p.precision) {
+    LAUNCH(c, k_planarize<double>, c->nw, 128, 0, c->M, c->na, c->nb, c->KA, c->KT, c->split, (const cplx<double>*)theta,
+           (double*)c->thp, (double*)c->thp_lo);
+    return do_fb_energy_planar<double>(c, nullptr, (zcplx*)eloc);
+  }
+  LAUNCH(c, k_planarize<float>, c->nw, 128, 0, c->M, c->na, c->nb, c->KA, c->KT, c->split, (const cplx<float>*)theta,
+         (float*)c->thp, (float*)c->thp_lo);
+  return do_fb_energy_planar<float>(c, nullptr, (zcplx*)eloc);
+}
+
+afqmc_status afqmc_step(afqmc_ctx* c, void* phi, double* weight, void* ovlp, void* theta, void* fb, const void* x,
+                        int32_t n_steps, void* eloc, int32_t* flags) {
+  if (!c) return AFQMC_EINVAL;
+  c->err[0] = 0;
+  NEED(c, n_steps >= 0, "afqmc_step: n_steps < 0");
+  if (c->nw == 0 || n_steps == 0) return AFQMC_OK;
+  NEED(c, phi && weight && ovlp && theta && fb && x && eloc, "afqmc_step: null pointer");
+  return DISPATCH(c, do_step, c, phi, weight, ovlp, theta, fb, x, n_steps, eloc, flags);
+}
+
+afqmc_status afqmc_step_host(afqmc_ctx* c, void* phi_h, double* weight_h, void* ovlp_h, const void* x_h, int32_t n_steps,
+                             void* eloc_h, int32_t* flags_h, size_t* h2d_bytes, size_t* d2h_bytes) {
+  if (!c) return AFQMC_EINVAL;
+  c->err[0] = 0;
+  NEED(c, n_steps >= 0, "afqmc_step_host: n_steps < 0");
+  if (h2d_bytes) *h2d_bytes = 0;
+  if (d2h_bytes) *d2h_bytes = 0;
+  if (c->nw == 0) return AFQMC_OK;
+  NEED(c, phi_h && weight_h && ovlp_h && (x_h || n_steps == 0) && (eloc_h || n_steps == 0), "afqmc_step_host: null pointer");
+  const size_t nw = c->nw, ts = c->ts;
+  const size_t phi_b = nw * c->M * c->nt * 2 * ts, x_b = nw * c->ng * ts;
+  size_t up = 0, down = 0;
+  cudaStream_t st = c->stream;
+  CUDA_OK(c, cudaMemcpyAsync(c->h_phi, phi_h, phi_b, cudaMemcpyHostToDevice, st));
+  CUDA_OK(c, cudaMemcpyAsync(c->h_weight, weight_h, nw * 8, cudaMemcpyHostToDevice, st));
+  CUDA_OK(c, cudaMemsetAsync(c->h_flags, 0, nw * 4, st));
+  up += phi_b + nw * 8;
+  afqmc_status s = afqmc_overlap_green(c, c->h_phi, c->h_ovlp, c->h_theta, nullptr, c->h_flags);
+  if (s) return s;
+  s = afqmc_force_bias(c, c->h_phi, c->h_theta, c->h_fb);
+  if (s) return s;
+  for (int i = 0; i < n_steps; ++i) {
+    CUDA_OK(c, cudaMemcpyAsync(c->h_x, (const char*)x_h + (size_t)i * x_b, x_b, cudaMemcpyHostToDevice, st));
+    up += x_b;
+    s = afqmc_step(c, c->h_phi, c->h_weight, c->h_ovlp, c->h_theta, c->h_fb, c->h_x, 1, c->h_eloc, c->h_flags);
+    if (s) return s;
+    CUDA_OK(c, cudaMemcpyAsync((char*)eloc_h + (size_t)i * nw * 16, c->h_eloc, nw * 16, cudaMemcpyDeviceToHost, st));
+    down += nw * 16;
+  }
+  CUDA_OK(c, cudaMemcpyAsync(phi_h, c->h_phi, phi_b, cudaMemcpyDeviceToHost, st));
+  CUDA_OK(c, cudaMemcpyAsync(weight_h, c->h_weight, nw * 8, cudaMemcpyDeviceToHost, st));
+  CUDA_OK(c, cudaMemcpyAsync(ovlp_h, c->h_ovlp, nw * 16, cudaMemcpyDeviceToHost, st));
+  down += phi_b + nw * 8 + nw * 16;
+  if (flags_h) {
+    CUDA_OK(c, cudaMemcpyAsync(flags_h, c->h_flags, nw * 4, cudaMemcpyDeviceToHost, st));
+    down += nw * 4;
+  }
+  CUDA_OK(c, cudaStreamSynchronize(st));
+  if (h2d_bytes) *h2d_bytes = up;
+  if (d2h_bytes) *d2h_bytes = down;
+  return AFQMC_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,242 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the FP64 oracle, same seeded inputs.
+
+Protocols:
+  stage  : each entry point alone on random complex non-orthonormal walkers
+  A      : per-step re-synchronised, all walkers, 10 steps
+  B      : free-running from the common initial state, graded on walkers alive in the oracle
+  C      : free-running on the `tame` variant (sigma_L / 10), all walkers
+Tolerances: 1e-5 (FP64 path) / 2e-4 (FP32 path) per north_star.
+"""
+import numpy as np
+import pytest
+
+from oracle import afqmc_oracle as orc
+from workloads import make_workload, random_walkers
+
+from . import gpu_harness as H
+
+pytestmark = pytest.mark.gpu
+
+# (cfg, variant, n_walkers used in the element-by-element comparison, steps)
+SMALL = {1: 64, 2: 96, 3: 40, 5: 6}
+
+
+def _wl(cfg, variant="raw"):
+    return make_workload(cfg, variant)
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 5])
+def test_stage_overlap_green_forcebias_energy(cfg):
+    import torch
+    wl = _wl(cfg)
+    nw = SMALL[cfg]
+    tol = H.tol_for(wl)
+    ini, _ = H.oracle_init(wl)
+    phi = random_walkers(wl, nw, seed=11)
+    ctx = H.make_ctx(wl, nw)
+    st = H.DeviceState(ctx, phi)
+    G = torch.zeros(nw, 2, wl.M, wl.M, dtype=ctx.cdtype, device=ctx.device)
+    ctx.afqmc_overlap_green(st.phi, st.ovlp, st.theta, G, st.flags)
+    ctx.afqmc_force_bias(st.phi, st.theta, st.fb)
+    eloc = torch.zeros(nw, dtype=torch.complex128, device=ctx.device)
+    ctx.afqmc_local_energy(st.phi, st.theta, eloc)
+    out = st.host()
+    S, theta, Gref = orc.o_green(wl.psi_a, wl.psi_b, phi, want_G=True)
+    fa, fb = orc.o_force_bias(ini["R"], theta, wl.n_alpha)
+    E = orc.o_local_energy(ini, theta, fa, fb, wl.n_alpha)
+    errs = dict(S=H.rel_abs(out["S"], S), theta=H.rel_fro(out["theta"], theta),
+                G=H.rel_fro(G.cpu().numpy().astype(np.complex128), Gref), f=H.rel_fro(out["f"], fa + fb),
+                E=H.rel_abs(eloc.cpu().numpy(), E))
+    print(f"cfg{cfg} stage errors: {errs}")
+    assert np.all(out["flags"] == 0)
+    for k, v in errs.items():
+        assert v < tol, (k, v)
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 5])
+def test_stage_propagate(cfg):
+    import torch
+    wl = _wl(cfg)
+    nw = SMALL[cfg]
+    tol = H.tol_for(wl)
+    ini, _ = H.oracle_init(wl)
+    phi = random_walkers(wl, nw, seed=5, spread=0.1)
+    ost = orc.o_seed_state(ini, phi, wl.n_alpha)
+    x = wl.fields(1, nw)[0]
+    new, rec = orc.o_step(ini, ost, x, wl.n_alpha, K=wl.K, E0=wl.E0)
+    ctx = H.make_ctx(wl, nw)
+    st = H.DeviceState(ctx, phi)
+    st.seed()
+    xd = torch.tensor(x, dtype=ctx.rdtype, device=ctx.device)
+    ctx.afqmc_propagate(st.phi, xd, st.fb, st.ovlp, st.weight, st.theta, None, st.flags)
+    out = st.host()
+    errs = dict(phi=H.rel_fro(out["phi"], rec["phi"]), S=H.rel_abs(out["S"], rec["S"]),
+                theta=H.rel_fro(out["theta"], rec["theta"]),
+                w=H.weight_err(out["w"], rec, ost.w, wl.dt, wl.E0))
+    print(f"cfg{cfg} propagate errors: {errs}")
+    for k, v in errs.items():
+        assert v < tol, (k, v)
+
+
+def _protocol_A(wl, nw, steps, gemm_path=0):
+    """Per-step re-synchronised: the GPU starts every step from the oracle's recorded state."""
+    tol = H.tol_for(wl)
+    ini, trial = H.oracle_init(wl)
+    ost = orc.o_seed_state(ini, wl.walkers(nw), wl.n_alpha, trial=trial)
+    xs = wl.fields(steps, nw)
+    ctx = H.make_ctx(wl, nw, gemm_path=gemm_path)
+    worst = {}
+    for n in range(steps):
+        new, rec = orc.o_step(ini, ost, xs[n], wl.n_alpha, K=wl.K, E0=wl.E0, trial=trial)
+        st = H.DeviceState(ctx, ost.phi, weight=ost.w)
+        st.seed()
+        g0 = st.host()
+        eloc = st.step(xs[n:n + 1])[0]
+        out = st.host()
+        alive = np.isfinite(rec["S"]) & np.isfinite(rec["eloc"])
+        errs = dict(S0=H.rel_abs(g0["S"][alive], ost.S[alive]), f_used=H.rel_fro(g0["f"][alive], rec["f_used"][alive]),
+                    phi=H.rel_fro(out["phi"][alive], rec["phi"][alive]), S=H.rel_abs(out["S"][alive], rec["S"][alive]),
+                    f=H.rel_fro(out["f"][alive], rec["f"][alive]), E=H.rel_abs(eloc[alive], rec["eloc"][alive]),
+                    w=H.weight_err(out["w"][alive], {k: v[alive] for k, v in rec.items() if k in ("w", "absI")},
+                                   ost.w[alive], wl.dt, wl.E0))
+        # a dead/alive flip is accepted iff |cos dtheta|_ora < tol
+        flip = ((out["w"] == 0) != (rec["w"] == 0)) & alive
+        assert np.all(np.abs(rec["cosd"][flip]) < tol), "dead/alive flip away from cos=0"
+        for k, v in errs.items():
+            worst[k] = max(worst.get(k, 0.0), v)
+        ost = new
+    print(f"cfg{wl.cfg}/{wl.variant} protocol A worst over {steps} steps: {worst}")
+    for k, v in worst.items():
+        assert v < tol, (k, v)
+    return worst
+
+
+@pytest.mark.parametrize("cfg,variant", [(1, "raw"), (1, "mf"), (2, "raw"), (2, "mf"), (3, "raw"), (3, "mf"), (5, "mf")])
+def test_protocol_A_resync(cfg, variant):
+    wl = _wl(cfg, variant)
+    steps = 10 if cfg != 5 else 3
+    _protocol_A(wl, SMALL[cfg], steps)
+
+
+def _free_run(wl, nw, steps):
+    ini, trial = H.oracle_init(wl)
+    ost = orc.o_seed_state(ini, wl.walkers(nw), wl.n_alpha, trial=trial)
+    xs = wl.fields(steps, nw)
+    ctx = H.make_ctx(wl, nw)
+    st = H.DeviceState(ctx, wl.walkers(nw))
+    st.seed()
+    eloc = st.step(xs)           # one afqmc_step call over all steps
+    recs = []
+    for n in range(steps):
+        w_prev = ost.w
+        ost, rec = orc.o_step(ini, ost, xs[n], wl.n_alpha, K=wl.K, E0=wl.E0, trial=trial)
+        rec["w_prev"] = w_prev
+        recs.append(rec)
+    return st.host(), eloc, recs, ost
+
+
+@pytest.mark.parametrize("cfg,variant", [(1, "raw"), (2, "raw"), (3, "mf")])
+def test_protocol_B_free_running_alive(cfg, variant):
+    """Free-running; graded on walkers alive in the oracle at the last step (final state) and at
+    every step for the energies."""
+    wl = _wl(cfg, variant)
+    nw, steps = SMALL[cfg], 10
+    tol = H.tol_for(wl)
+    out, eloc, recs, ost = _free_run(wl, nw, steps)
+    worstE = 0.0
+    for n in range(steps):
+        alive = recs[n]["w"] > 0
+        if np.any(alive):
+            worstE = max(worstE, H.rel_abs(eloc[n][alive], recs[n]["eloc"][alive]))
+    alive = ost.w > 0
+    errs = dict(E=worstE)
+    if np.any(alive):
+        errs.update(phi=H.rel_fro(out["phi"][alive], ost.phi[alive]), S=H.rel_abs(out["S"][alive], ost.S[alive]),
+                    w=H.rel_abs(out["w"][alive], ost.w[alive]))
+    dead = ~alive
+    assert np.all(np.isfinite(out["phi"][dead].view(np.float64))) or wl.precision == "c64"
+    print(f"cfg{cfg}/{variant} protocol B ({int(alive.sum())}/{nw} alive): {errs}")
+    for k, v in errs.items():
+        assert v < tol, (k, v)
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_protocol_C_tame(cfg):
+    wl = _wl(cfg, "tame")
+    nw = SMALL[cfg]
+    steps = 10 if cfg != 2 else 50
+    tol = H.tol_for(wl)
+    out, eloc, recs, ost = _free_run(wl, nw, steps)
+    assert np.all(ost.w > 0)
+    errs = dict(phi=H.rel_fro(out["phi"], ost.phi), S=H.rel_abs(out["S"], ost.S), w=H.rel_abs(out["w"], ost.w),
+                f=H.rel_fro(out["f"], ost.f_a + ost.f_b), E=H.rel_abs(eloc[-1], recs[-1]["eloc"]))
+    print(f"cfg{cfg}/tame protocol C after {steps} steps: {errs}")
+    for k, v in errs.items():
+        assert v < tol, (k, v)
+
+
+def test_step_host_matches_device_step():
+    wl = _wl(2, "tame")
+    nw, steps = 64, 3
+    ctx = H.make_ctx(wl, nw)
+    st = H.DeviceState(ctx, wl.walkers(nw))
+    st.seed()
+    xs = wl.fields(steps, nw)
+    eloc_d = st.step(xs)
+    d = st.host()
+    phi_h = wl.walkers(nw).astype(np.complex64)
+    w_h = np.ones(nw)
+    S_h = np.zeros(nw, dtype=np.complex128)
+    e_h = np.zeros((steps, nw), dtype=np.complex128)
+    f_h = np.zeros(nw, dtype=np.int32)
+    up, down = ctx.afqmc_step_host(phi_h, w_h, S_h, xs.astype(np.float32), steps, e_h, f_h)
+    assert up == phi_h.nbytes + w_h.nbytes + xs.astype(np.float32).nbytes
+    assert down == phi_h.nbytes + w_h.nbytes + S_h.nbytes + e_h.nbytes + f_h.nbytes
+    np.testing.assert_array_equal(phi_h.astype(np.complex128), d["phi"])
+    np.testing.assert_array_equal(w_h, d["w"])
+    np.testing.assert_array_equal(S_h, d["S"])
+    np.testing.assert_allclose(e_h, eloc_d, rtol=1e-12)
+    assert ctx.launch_count > 0
+
+
+def test_edge_cases():
+    import torch
+    import paper_1804_03310_b200 as afq
+    # ragged / odd sizes, n_beta = 0, a single walker, and the empty batch
+    for (M, na, nb, ng, nw, prec) in [(7, 3, 2, 5, 3, "c128"), (9, 2, 0, 33, 1, "c64"), (13, 4, 3, 17, 5, "c64"),
+                                      (6, 2, 2, 4, 0, "c64")]:
+        wl = make_workload(1, "raw", overrides=dict(M=M, n_alpha=na, n_beta=nb, n_chol=ng, n_walkers=max(nw, 1),
+                                                    precision=prec))
+        ini, _ = H.oracle_init(wl)
+        ctx = H.make_ctx(wl, nw)
+        if nw == 0:
+            empty = torch.zeros(0, M, na + nb, dtype=ctx.cdtype, device=ctx.device)
+            z = torch.zeros(0, dtype=torch.complex128, device=ctx.device)
+            ctx.afqmc_overlap_green(empty, z, empty, None, None)
+            assert ctx.launch_count == 0
+            continue
+        phi = random_walkers(wl, nw, seed=3, spread=0.1)
+        ost = orc.o_seed_state(ini, phi, wl.n_alpha)
+        st = H.DeviceState(ctx, phi)
+        st.seed()
+        xs = wl.fields(2, nw)
+        eloc = st.step(xs)
+        for n in range(2):
+            ost, rec = orc.o_step(ini, ost, xs[n], wl.n_alpha, K=wl.K)
+        out = st.host()
+        tol = H.tol_for(wl)
+        assert H.rel_fro(out["phi"], ost.phi) < tol
+        assert H.rel_abs(out["S"], ost.S) < tol
+        assert H.rel_abs(eloc[-1], rec["eloc"]) < tol
+
+
+def test_singular_walker_sets_flag():
+    wl = _wl(1)
+    ctx = H.make_ctx(wl, 4)
+    phi = wl.walkers(4).copy()
+    phi[2, :, 1] = phi[2, :, 0]          # two equal alpha columns -> singular overlap matrix
+    st = H.DeviceState(ctx, phi)
+    st.seed()
+    out = st.host()
+    assert out["flags"][2] & 1
+    assert np.all(out["flags"][[0, 1, 3]] == 0)
