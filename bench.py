@@ -1,0 +1,300 @@
+#!/usr/bin/env python
+"""bench.py -- walker-steps/s of the ph-AFQMC walker step (propagate + energy every step, both spins).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--cfg 5] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (shift -> assemble -> Taylor -> overlap/weights -> force
+bias -> local energy) over all N_w walkers of the workload.  The workload is BASELINE.json's config 5
+(M=200, 13+12 electrons, N_chol=1000, 2048 complex64 walkers) unless --cfg says otherwise; inputs are
+seeded synthetic tensors of that shape (workloads/gen.py).
+Prints ONE JSON line on rank 0 (contract in the task statement; keys `roofline`, `cpu_baseline`, `e2e`,
+`clocks`, `gpu_launches` included).  N > 1: launched under torchrun, every rank runs an independent
+replica of the batch ("weak"), time = max over ranks (NCCL all-reduce of the device time).
+--impl reference times the FP64 CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "walker-steps/sec (propagate+energy)"
+UNIT = "walker-steps/s"
+
+
+def workload_name(wl):
+    return (f"cfg{wl.cfg} M={wl.M} N=({wl.n_alpha},{wl.n_beta}) N_chol={wl.n_chol} N_w={wl.n_walkers} "
+            f"{wl.precision} K={wl.K} n_det={wl.n_det}")
+
+
+def flops_per_walker_step(wl):
+    """Algorithmic (useful, real) flops per stage per walker-step."""
+    M, na, nb, ng, K = wl.M, wl.n_alpha, wl.n_beta, wl.n_chol, wl.K
+    nt = na + nb
+    return dict(assemble=4.0 * ng * M * M,                       # real x complex: 2 planes x 2 flop
+                force_bias=4.0 * ng * M * nt,
+                taylor=8.0 * M * M * nt * K + 2 * 4.0 * M * M * nt,
+                energy=4.0 * ((M * na) ** 2 + (M * nb) ** 2),
+                green=4.0 * M * (na * na + nb * nb) + 8.0 * M * (na * na + nb * nb))
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm=d["hbm_gbs"], bf16_burst=d["bf16_tflops"], bf16_sust=d["bf16_tflops_sustained"],
+                    sm_max_mhz=d.get("sm_max_mhz", 1965.0), source="measured")
+    return dict(hbm=6650.0, bf16_burst=1590.0, bf16_sust=1400.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        super().__init__(daemon=True)
+        self.index, self.rows, self._stop = index, [], threading.Event()
+
+    def run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
+                self.rows.append([c.strip() for c in out.strip().split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def stop(self):
+        self._stop.set()
+        self.join(timeout=6)
+        sm, mx, reasons = [], 0.0, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = max(mx, float(r[1]))
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                continue
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=mx or None, reasons=sorted(reasons),
+                    samples=len(sm))
+
+
+def time_oracle(wl, target_s=12.0):
+    """The FP64 numpy oracle as it stands, on the host cores: walker-steps/s on a bounded sample."""
+    from oracle import afqmc_oracle as orc
+    from tests import gpu_harness as H
+    cores = len(os.sched_getaffinity(0))
+    ini, trial = H.oracle_init(wl)
+    nw = min(wl.n_walkers, 8)
+    done, t_total, nsteps = 0, 0.0, 0
+    while True:
+        ost = orc.o_seed_state(ini, wl.walkers(nw), wl.n_alpha, trial=trial)
+        x = wl.fields(1, nw)[0]
+        t0 = time.perf_counter()
+        orc.o_step(ini, ost, x, wl.n_alpha, K=wl.K, E0=wl.E0, trial=trial)
+        dt = time.perf_counter() - t0
+        t_total += dt; done += nw; nsteps += 1
+        if t_total >= target_s or nsteps >= 64:
+            break
+        if dt < 1.0 and nw < wl.n_walkers:
+            nw = min(wl.n_walkers, nw * 4)
+    return dict(value=done / t_total, unit=UNIT, cores=cores, kind="oracle",
+                sample=f"{nsteps} oracle step(s) over {done} walker-steps of {workload_name(wl)} "
+                       f"({t_total:.1f} s CPU wall, numpy/BLAS threads = all {cores} cores, init excluded)")
+
+
+def run_reference(args):
+    from workloads import make_workload
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    wl = make_workload(args.cfg, args.variant)
+    budget = max(4.0, min(120.0, 8.0 * (args.steps + args.warmup)))
+    t0 = time.perf_counter()
+    base = time_oracle(wl, target_s=budget)
+    line = dict(metric=METRIC, value=base["value"], unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
+                ms_per_step=1e3 * wl.n_walkers / base["value"], higher_is_better=True, scaling="weak",
+                vs_baseline=None, dtype="f64", data="synthetic", impl="reference",
+                config=dict(workload=workload_name(wl), variant=args.variant),
+                cpu_baseline=base,
+                e2e=dict(value=base["value"], unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
+                wall_s=time.perf_counter() - t0)
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from tests import gpu_harness as H
+    from workloads import make_workload
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+
+    wl = make_workload(args.cfg, args.variant)
+    nw, K, W = wl.n_walkers, args.steps, max(args.warmup, 3)
+    import paper_1804_03310_b200 as afq
+    p = afq.make_params(wl.M, wl.n_alpha, wl.n_beta, wl.n_chol, nw, wl.precision, wl.dt, taylor_order=wl.K,
+                        E0=wl.E0, n_det=wl.n_det, n_act=wl.n_act, gemm_path=args.gemm_path)
+    kw = {}
+    if wl.n_det > 1:
+        kw = dict(C_act=wl.C_act, det_coeff=wl.det_coeff, det_exc=wl.det_exc)
+    ctx = afq.AfqmcContext(p, wl.h, wl.L, wl.psi_a, wl.psi_b, device=f"cuda:{local}", **kw)
+    dev = ctx.device
+    # fields: every rank its own seed (replicas are independent); a fresh draw per step, resident in HBM
+    rng = np.random.default_rng(1000 + rank)
+    nfield = min(K, 8)
+    x = torch.tensor(rng.standard_normal((nfield, nw, wl.n_chol)), dtype=ctx.rdtype, device=dev)
+    phi0 = torch.tensor(wl.walkers(nw), dtype=ctx.cdtype, device=dev)
+    st = H.DeviceState(ctx, wl.walkers(nw))
+    eloc = torch.zeros(1, nw, dtype=torch.complex128, device=dev)
+
+    def reseed():
+        # walkers restart from the trial (the literal configs kill every walker in ~8 steps)
+        st.phi.copy_(phi0); st.weight.fill_(1.0); st.flags.zero_()
+        st.seed()
+
+    def one_step(i):
+        ctx.afqmc_step(st.phi, st.weight, st.ovlp, st.theta, st.fb, x[i % nfield], 1, eloc, st.flags)
+
+    reseed()
+    for i in range(W):
+        one_step(i)
+    torch.cuda.synchronize()
+    reseed()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+    ctx.afqmc_profile_enable(True)
+    l0 = ctx.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for i in range(K):
+        if i and i % 6 == 0:
+            reseed()           # inside the timed region: counted (2 extra small kernels + copies)
+        one_step(i)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    launches = ctx.launch_count - l0
+    prof = ctx.afqmc_profile_read()
+    ctx.afqmc_profile_enable(False)
+    clocks = sampler.stop() if sampler else None
+    tmax = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.barrier()
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms_max = float(tmax.item())
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----
+    Ke = min(K, 4)
+    phi_h = torch.tensor(wl.walkers(nw), dtype=ctx.cdtype).pin_memory()
+    w_h = torch.ones(nw, dtype=torch.float64).pin_memory()
+    S_h = torch.zeros(nw, dtype=torch.complex128).pin_memory()
+    x_h = torch.tensor(rng.standard_normal((Ke, nw, wl.n_chol)), dtype=ctx.rdtype).pin_memory()
+    e_h = torch.zeros(Ke, nw, dtype=torch.complex128).pin_memory()
+    f_h = torch.zeros(nw, dtype=torch.int32).pin_memory()
+    phi_keep = phi_h.clone()
+    ctx.afqmc_step_host(phi_h, w_h, S_h, x_h, 1, e_h, f_h)      # warm
+    phi_h.copy_(phi_keep); w_h.fill_(1.0)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    up, down = ctx.afqmc_step_host(phi_h, w_h, S_h, x_h, Ke, e_h, f_h)   # synchronises internally
+    t_e2e = time.perf_counter() - t0
+    te = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    t_e2e = float(te.item())
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    pk = peaks()
+    fl = flops_per_walker_step(wl)
+    value = world * nw * K / (ms_max * 1e-3)
+    # dominant kernel: the one-body-operator assembly GEMM (H6)
+    a_ms, a_n = prof["assemble"]
+    a_flops = fl["assemble"] * nw
+    if ctx.gemm_path == 2:
+        bound, peak, peak_note = "tensor", 0.5 * pk["bf16_sust"], (
+            f"TF32 dense = {pk['source']} sustained BF16 {pk['bf16_sust']} TF/s x nominal TF32/BF16 ratio 0.5; "
+            "3xTF32 issues 3x the algorithmic flops, so frac <= 1/3 by construction")
+        dtype = "tf32x3"
+    else:
+        fp32_peak = 148 * 128 * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
+        bound, peak, peak_note = "alu", fp32_peak, "FP32 FMA: 148 SMs x 128 lanes x 2 flop x clocks.max.sm (DESIGN.md)"
+        dtype = "f32" if wl.precision == "c64" else "f64"
+        if wl.precision == "c128":
+            peak, peak_note = fp32_peak / 2, "FP64 FMA: 148 SMs x 64 lanes x 2 flop x clocks.max.sm (DESIGN.md)"
+    achieved = a_flops * a_n / (a_ms * 1e-3) / 1e12 if a_ms > 0 else None
+    stage_ms = {k: (v[0] / v[1] if v[1] else None) for k, v in prof.items()}
+    stage_tflops = {k: (fl[k] * nw / (stage_ms[k] * 1e-3) / 1e12 if stage_ms.get(k) else None) for k in fl}
+    base = None
+    if not args.no_cpu_baseline:
+        base = time_oracle(wl, target_s=args.cpu_seconds)
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=K, warmup=W, ms_per_step=ms_max / K,
+                higher_is_better=True, scaling="weak", vs_baseline=None, dtype=dtype, data="synthetic",
+                config=dict(workload=workload_name(wl), variant=args.variant, global_walkers=world * nw,
+                            parallelism=f"replicas x{world}" if world > 1 else "single GPU",
+                            l2="per-step working set (A_w buffer %.0f MB + operands) exceeds the 126 MB L2; no flush"
+                               % (nw * wl.M * wl.M * 2 * (4 if wl.precision == "c64" else 8) / 1e6),
+                            gemm_path={1: "simt", 2: "tcgen05-3xtf32"}[ctx.gemm_path]),
+                clocks=clocks, gpu_launches=launches,
+                e2e=dict(value=world * nw * Ke / t_e2e, unit=UNIT, h2d_bytes_per_step=up / Ke, d2h_bytes_per_step=down / Ke,
+                         steps=Ke, note="afqmc_step_host: pinned host buffers, H2D of walkers+fields and D2H of "
+                                        "walkers/weights/overlaps/energies inside the timed region"),
+                roofline=dict(bound=bound, kernel="H6 assemble GEMM A_w = sum_g z_g L_g", achieved=achieved, peak=peak,
+                              unit="TFLOP/s", frac=(achieved / peak) if achieved else None, traffic=None,
+                              peak_source=peak_note, launches_timed=a_n, ms_per_launch=stage_ms["assemble"]),
+                stages_ms=stage_ms, stages_tflops=stage_tflops, cpu_baseline=base)
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=12)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--cfg", type=int, default=5)
+    ap.add_argument("--variant", default="mf")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--gemm-path", type=int, default=0)
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

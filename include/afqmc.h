@@ -150,6 +150,23 @@ AFQMC_API afqmc_status afqmc_step_host(afqmc_ctx* ctx, void* phi_h, double* weig
 /* Number of kernels this context has launched since init (bench.py's gpu_launches). */
 AFQMC_API int64_t afqmc_launch_count(const afqmc_ctx* ctx);
 
+/* Per-stage device timing with CUDA events recorded on the context's stream around the stage's
+ * kernels (bench.py's roofline line).  enable != 0 creates the events and resets the counters;
+ * enable == 0 destroys them.  afqmc_profile_read may be called after the caller has synchronised the
+ * stream: total_ms = sum of the elapsed times of the (at most 64) recorded executions, launches =
+ * how many were recorded. */
+enum {
+  AFQMC_STAGE_SHIFT = 0,      /* H5 */
+  AFQMC_STAGE_ASSEMBLE = 1,   /* H6: A_w = sum_g z_g L_g GEMM */
+  AFQMC_STAGE_TAYLOR = 2,     /* H7 */
+  AFQMC_STAGE_GREEN = 3,      /* H1-H3 + H8 (+ H10 overlap part) */
+  AFQMC_STAGE_FORCE_BIAS = 4, /* H4 GEMM + finish */
+  AFQMC_STAGE_ENERGY = 5,     /* H9 GEMMs / H10 energy */
+  AFQMC_N_STAGES = 6
+};
+AFQMC_API afqmc_status afqmc_profile_enable(afqmc_ctx* ctx, int32_t enable);
+AFQMC_API afqmc_status afqmc_profile_read(afqmc_ctx* ctx, int32_t stage, double* total_ms, int32_t* launches);
+
 /* Which contraction path the context resolved to: 1 = SIMT, 2 = tcgen05 3xTF32. */
 AFQMC_API int32_t afqmc_gemm_path(const afqmc_ctx* ctx);
 

@@ -19,7 +19,9 @@ FLAG_SINGULAR, FLAG_NONFINITE, FLAG_KILLED = 1, 2, 4
 
 SYMBOLS = ["afqmc_query_bytes", "afqmc_init", "afqmc_destroy", "afqmc_last_error", "afqmc_overlap_green",
            "afqmc_force_bias", "afqmc_propagate", "afqmc_local_energy", "afqmc_step", "afqmc_step_host",
-           "afqmc_launch_count", "afqmc_gemm_path"]
+           "afqmc_launch_count", "afqmc_gemm_path", "afqmc_profile_enable", "afqmc_profile_read"]
+
+STAGES = ["shift", "assemble", "taylor", "green", "force_bias", "energy"]
 
 
 class AfqmcParams(C.Structure):
@@ -65,6 +67,10 @@ def load_library():
     lib.afqmc_launch_count.restype = C.c_int64
     lib.afqmc_gemm_path.argtypes = [vp]
     lib.afqmc_gemm_path.restype = C.c_int32
+    lib.afqmc_profile_enable.argtypes = [vp, C.c_int32]
+    lib.afqmc_profile_read.argtypes = [vp, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_int32)]
+    lib.afqmc_profile_enable.restype = C.c_int
+    lib.afqmc_profile_read.restype = C.c_int
     for name in ("afqmc_query_bytes", "afqmc_init", "afqmc_overlap_green", "afqmc_force_bias", "afqmc_propagate",
                  "afqmc_local_energy", "afqmc_step", "afqmc_step_host"):
         getattr(lib, name).restype = C.c_int
@@ -155,6 +161,18 @@ class AfqmcContext:
     @property
     def gemm_path(self) -> int:
         return int(self._lib.afqmc_gemm_path(self._ctx))
+
+    def afqmc_profile_enable(self, enable=True):
+        self._chk(self._lib.afqmc_profile_enable(self._ctx, 1 if enable else 0))
+
+    def afqmc_profile_read(self):
+        """{stage name: (total_ms, recorded executions)}; synchronise the stream first."""
+        out = {}
+        for i, name in enumerate(STAGES):
+            ms, n = C.c_double(0), C.c_int32(0)
+            self._chk(self._lib.afqmc_profile_read(self._ctx, i, C.byref(ms), C.byref(n)))
+            out[name] = (ms.value, n.value)
+        return out
 
     # ---- same names as the C ABI; tensors are torch CUDA tensors ----
     def afqmc_overlap_green(self, phi, ovlp, theta, G=None, flags=None):

@@ -56,6 +56,10 @@ struct afqmc_ctx {
   double *Ld, *hd, *hpd, *Rd, *hrotd, *ex[4], *psid;
   char err[256];
   int64_t launches;
+  // optional per-stage timing (afqmc_profile_enable)
+  int prof;
+  cudaEvent_t pev[AFQMC_N_STAGES][64][2];
+  int pcount[AFQMC_N_STAGES];
 };
 
 namespace {
@@ -79,6 +83,19 @@ afqmc_status fail(afqmc_ctx* c, afqmc_status s, const char* fmt, const char* a =
     cudaError_t e_ = cudaGetLastError();                                              \
     if (e_ != cudaSuccess) return fail((c), AFQMC_ECUDA, #kern ": %s", cudaGetErrorString(e_)); \
   } while (0)
+
+struct StageScope {
+  afqmc_ctx* c; int stage; int slot;
+  StageScope(afqmc_ctx* c_, int stage_) : c(c_), stage(stage_), slot(-1) {
+    if (c->prof && c->pcount[stage] < 64) {
+      slot = c->pcount[stage]++;
+      cudaEventRecord(c->pev[stage][slot][0], c->stream);
+    }
+  }
+  ~StageScope() {
+    if (slot >= 0) cudaEventRecord(c->pev[stage][slot][1], c->stream);
+  }
+};
 
 // Taylor kernel configuration: chunk width CW (compile-time), chunks, threads.
 template <typename T> int taylor_maxt(int cw) {
@@ -267,6 +284,7 @@ afqmc_status run_green(afqmc_ctx* c, const void* phi, void* ovlp, void* theta, i
   g.ovlp = (zcplx*)ovlp; g.do_weight = do_weight; g.cshift = c->cshift; g.weight = weight;
   g.eloc_pre = (const zcplx*)eloc_pre; g.weight_mode = c->p.weight_mode; g.dt = c->p.dt; g.E0 = c->p.E0;
   g.flags = flags;
+  StageScope sc(c, AFQMC_STAGE_GREEN);
   LAUNCH(c, k_green<T>, c->nw, 128, c->green_smem, g);
   return AFQMC_OK;
 }
@@ -282,6 +300,7 @@ afqmc_status run_gemm(afqmc_ctx* c, const T* A, int lda, int m, const T* B, int 
 
 // per-spin traces f^s_g = sum R^s_g[a][k] Theta_s[k][a] from the planar Theta in ctx->thp
 template <typename T> afqmc_status run_fb_gemm(afqmc_ctx* c) {
+  StageScope sc(c, AFQMC_STAGE_FORCE_BIAS);
   for (int s = 0; s < 2; ++s) {
     int n = s ? c->nb : c->na, soff = s ? c->KA : 0, Ks = s ? c->KB : c->KA;
     if (!n) continue;
@@ -294,6 +313,7 @@ template <typename T> afqmc_status run_fb_gemm(afqmc_ctx* c) {
 }
 
 template <typename T> afqmc_status run_energy_gemm(afqmc_ctx* c, zcplx* eloc) {
+  StageScope sc(c, AFQMC_STAGE_ENERGY);
   for (int s = 0; s < 2; ++s) {
     int n = s ? c->nb : c->na, soff = s ? c->KA : 0, Ks = s ? c->KB : c->KA;
     if (!n) continue;
@@ -310,6 +330,7 @@ template <typename T> afqmc_status run_taylor(afqmc_ctx* c, void* phi) {
   TaylorArgs<T> g;
   g.M = c->M; g.MP = c->MP; g.nt = c->nt; g.K = c->p.taylor_order; g.nchunks = c->tay_nch;
   g.phi = (cplx<T>*)phi; g.A = (const T*)c->Abuf; g.Eh = (const T*)c->Eh;
+  StageScope sc(c, AFQMC_STAGE_TAYLOR);
 #define TAY_CASE(CW)                                                                                        \
   case CW: {                                                                                                \
     constexpr int MT = sizeof(T) == 4 ? (((CW + 3) & ~3) >= 16 ? 448 : ((CW + 3) & ~3) >= 12 ? 576 : ((CW + 3) & ~3) >= 8 ? 768 : 1024) \
@@ -338,11 +359,18 @@ template <typename T> afqmc_status run_taylor(afqmc_ctx* c, void* phi) {
 template <typename T>
 afqmc_status do_propagate(afqmc_ctx* c, void* phi, const void* x, const void* fb, void* ovlp, double* weight, void* theta,
                           const void* eloc_pre, int32_t* flags) {
-  LAUNCH(c, k_shift<T>, c->nw, 128, 0, c->ng, c->NGP, c->p.dt, (const cplx<T>*)fb, (const T*)x, (T*)c->Z, (T*)c->Z_lo,
-         c->split, c->cshift);
-  EpiAssemble<T> epi;
-  epi.out = (T*)c->Abuf; epi.M = c->M; epi.MP = c->MP; epi.m_real = c->M * c->M; epi.n_real = 2 * c->nw;
-  afqmc_status st = run_gemm<T>(c, (const T*)c->Lt, c->NGP, c->M * c->M, (const T*)c->Z, c->NGP, 2 * c->nw, c->NGP, epi);
+  {
+    StageScope sc(c, AFQMC_STAGE_SHIFT);
+    LAUNCH(c, k_shift<T>, c->nw, 128, 0, c->ng, c->NGP, c->p.dt, (const cplx<T>*)fb, (const T*)x, (T*)c->Z, (T*)c->Z_lo,
+           c->split, c->cshift);
+  }
+  afqmc_status st;
+  {
+    StageScope sc(c, AFQMC_STAGE_ASSEMBLE);
+    EpiAssemble<T> epi;
+    epi.out = (T*)c->Abuf; epi.M = c->M; epi.MP = c->MP; epi.m_real = c->M * c->M; epi.n_real = 2 * c->nw;
+    st = run_gemm<T>(c, (const T*)c->Lt, c->NGP, c->M * c->M, (const T*)c->Z, c->NGP, 2 * c->nw, c->NGP, epi);
+  }
   if (st) return st;
   st = run_taylor<T>(c, phi);
   if (st) return st;
@@ -485,7 +513,44 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
   return AFQMC_OK;
 }
 
-void afqmc_destroy(afqmc_ctx* ctx) { delete ctx; }
+void afqmc_destroy(afqmc_ctx* ctx) {
+  if (!ctx) return;
+  afqmc_profile_enable(ctx, 0);
+  delete ctx;
+}
+
+afqmc_status afqmc_profile_enable(afqmc_ctx* c, int32_t enable) {
+  if (!c) return AFQMC_EINVAL;
+  if (c->prof) {
+    for (int s = 0; s < AFQMC_N_STAGES; ++s)
+      for (int i = 0; i < 64; ++i) { cudaEventDestroy(c->pev[s][i][0]); cudaEventDestroy(c->pev[s][i][1]); }
+    c->prof = 0;
+  }
+  memset(c->pcount, 0, sizeof(c->pcount));
+  if (enable) {
+    for (int s = 0; s < AFQMC_N_STAGES; ++s)
+      for (int i = 0; i < 64; ++i) {
+        CUDA_OK(c, cudaEventCreate(&c->pev[s][i][0]));
+        CUDA_OK(c, cudaEventCreate(&c->pev[s][i][1]));
+      }
+    c->prof = 1;
+  }
+  return AFQMC_OK;
+}
+
+afqmc_status afqmc_profile_read(afqmc_ctx* c, int32_t stage, double* total_ms, int32_t* launches) {
+  if (!c || stage < 0 || stage >= AFQMC_N_STAGES || !total_ms || !launches) return AFQMC_EINVAL;
+  double tot = 0.0;
+  int n = c->prof ? c->pcount[stage] : 0;
+  for (int i = 0; i < n; ++i) {
+    float ms = 0.f;
+    CUDA_OK(c, cudaEventElapsedTime(&ms, c->pev[stage][i][0], c->pev[stage][i][1]));
+    tot += ms;
+  }
+  *total_ms = tot;
+  *launches = n;
+  return AFQMC_OK;
+}
 
 const char* afqmc_last_error(const afqmc_ctx* ctx) { return ctx ? ctx->err : g_init_err; }
 

@@ -90,6 +90,7 @@ template <typename T> inline size_t green_smem_bytes(int M, int na, int nb) {
   size_t b = (size_t)M * nt * sizeof(cplx<T>);          // phi_s
   b += (size_t)2 * ns * (2 * ns + 1) * sizeof(cplx<T>); // aug per spin
   b += (size_t)2 * ns * sizeof(cplx<T>);                // fac per spin
+  b = (b + 15) & ~size_t(15);
   b += 2 * sizeof(zcplx) + 4 * sizeof(int);
   return (b + 15) & ~size_t(15);
 }
@@ -122,7 +123,7 @@ __global__ void __launch_bounds__(128) k_green(GreenArgs<T> g) {
   cplx<T>* phi_s = reinterpret_cast<cplx<T>*>(smem_raw);
   cplx<T>* aug = phi_s + (size_t)M * nt;
   cplx<T>* fac = aug + 2 * ns * ld;
-  zcplx* dets = reinterpret_cast<zcplx*>(fac + 2 * ns);
+  zcplx* dets = reinterpret_cast<zcplx*>(smem_raw + ((((size_t)M * nt + 2 * ns * ld + 2 * ns) * sizeof(cplx<T>) + 15) & ~size_t(15)));
   int* sing = reinterpret_cast<int*>(dets + 2);
 
   const cplx<T>* phi_w = g.phi + (size_t)w * M * nt;

@@ -74,13 +74,20 @@ class DeviceState:
 
 
 # ---- error norms (R11): never elementwise-relative -------------------------------------------
-def rel_fro(a, b):
-    """max over walkers of ||a_w - b_w||_F / ||b_w||_F (b = oracle)."""
+def rel_fro(a, b, floor=0.0):
+    """max over walkers of ||a_w - b_w||_F / max(||b_w||_F, floor) (b = oracle).  `floor` is the natural
+    scale of the quantity when the oracle value itself vanishes (the force bias of the mean-field
+    subtracted inputs is exactly 0 at the trial)."""
     a = a.reshape(a.shape[0], -1)
     b = b.reshape(b.shape[0], -1)
-    den = np.linalg.norm(b, axis=1)
+    den = np.maximum(np.linalg.norm(b, axis=1), floor)
     den = np.where(den == 0, 1.0, den)
     return float(np.max(np.linalg.norm(a - b, axis=1) / den)) if a.shape[0] else 0.0
+
+
+def fb_floor(ini):
+    """Scale below which a force-bias norm counts as zero: 1e-3 ||R||_F (f = R . Theta, ||Theta|| = O(1))."""
+    return 1e-3 * float(np.sqrt(sum(np.sum(R * R) for R in ini["R"])))
 
 
 def rel_abs(a, b):

@@ -94,9 +94,9 @@ def _protocol_A(wl, nw, steps, gemm_path=0):
         eloc = st.step(xs[n:n + 1])[0]
         out = st.host()
         alive = np.isfinite(rec["S"]) & np.isfinite(rec["eloc"])
-        errs = dict(S0=H.rel_abs(g0["S"][alive], ost.S[alive]), f_used=H.rel_fro(g0["f"][alive], rec["f_used"][alive]),
+        errs = dict(S0=H.rel_abs(g0["S"][alive], ost.S[alive]), f_used=H.rel_fro(g0["f"][alive], rec["f_used"][alive], H.fb_floor(ini)),
                     phi=H.rel_fro(out["phi"][alive], rec["phi"][alive]), S=H.rel_abs(out["S"][alive], rec["S"][alive]),
-                    f=H.rel_fro(out["f"][alive], rec["f"][alive]), E=H.rel_abs(eloc[alive], rec["eloc"][alive]),
+                    f=H.rel_fro(out["f"][alive], rec["f"][alive], H.fb_floor(ini)), E=H.rel_abs(eloc[alive], rec["eloc"][alive]),
                     w=H.weight_err(out["w"][alive], {k: v[alive] for k, v in rec.items() if k in ("w", "absI")},
                                    ost.w[alive], wl.dt, wl.E0))
         # a dead/alive flip is accepted iff |cos dtheta|_ora < tol
