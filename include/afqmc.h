@@ -132,7 +132,7 @@ AFQMC_API afqmc_status afqmc_propagate(afqmc_ctx* ctx, void* phi, const void* x,
  * (needs phi).  All DEVICE.  phi may be NULL for a single-determinant trial. */
 AFQMC_API afqmc_status afqmc_local_energy(afqmc_ctx* ctx, const void* phi, const void* theta, void* eloc);
 
-/* n_steps full walker steps (order R10): [shift -> assemble -> Taylor propagate -> overlap/Theta ->
+/* n_steps full walker steps (Eq.(2),(3), :61-80, :97; order R10): [shift -> assemble -> Taylor propagate -> overlap/Theta ->
  * weight -> force bias -> local energy] per step.  State on entry/exit: phi, weight, ovlp, theta, fb of
  * the current walkers (seed with afqmc_overlap_green + afqmc_force_bias).  x [n_steps][N_w][n_chol] T,
  * eloc [n_steps][N_w] complex double (E_L of the post-step walker), flags OR-ed.  All DEVICE. */

@@ -13,6 +13,7 @@
 #include "gemm_simt.cuh"
 #include "green.cuh"
 #include "misc.cuh"
+#include "multidet.cuh"
 #include "taylor.cuh"
 
 using namespace afq;
@@ -40,6 +41,11 @@ struct afqmc_ctx {
   cudaStream_t stream;
   int M, MP, na, nb, nt, ng, NGP, nw, KA, KB, KT, ts;  // ts = sizeof(T)
   int split, path;
+  // multi-determinant trial (md != 0): ca/cb = columns per spin of the generalised Theta (n_act), else n_alpha/n_beta
+  int md, nact, ndet, ca, cb;
+  void* Cact; double* coeff; int32_t* exc;
+  void *thtil, *th_scr; zcplx *ovlp0, *ovlp_scr;
+  size_t mdo_smem, mde_smem;
   int tay_cw, tay_nch, tay_threads;
   size_t tay_smem, green_smem;
   // constants
@@ -131,7 +137,18 @@ afqmc_status check_params(const afqmc_params* p, char* err) {
   if (p->gemm_path < 0 || p->gemm_path > 2) { snprintf(err, 256, "gemm_path must be 0, 1 or 2"); return AFQMC_EINVAL; }
   if (p->n_alpha > 32 || p->n_beta > 32) { snprintf(err, 256, "n_alpha, n_beta <= 32 supported"); return AFQMC_EUNSUPPORTED; }
   if (p->n_det < 1) { snprintf(err, 256, "n_det must be >= 1"); return AFQMC_EINVAL; }
-  if (p->n_det > 1) { snprintf(err, 256, "multi-determinant trials not built yet"); return AFQMC_EUNSUPPORTED; }
+  if (p->n_det > 1) {
+    if (p->n_act < p->n_alpha || p->n_act < p->n_beta || p->n_act > p->M || p->n_beta < 1) {
+      snprintf(err, 256, "multi-det: need max(n_alpha, n_beta) <= n_act <= M and n_beta >= 1"); return AFQMC_EINVAL;
+    }
+    if (p->max_exc < 1 || p->max_exc > 2) { snprintf(err, 256, "max_exc must be 1 or 2"); return AFQMC_EUNSUPPORTED; }
+    if (p->n_det > 1024) { snprintf(err, 256, "n_det <= 1024 supported"); return AFQMC_EUNSUPPORTED; }
+    const int ts_ = p->precision ? 8 : 4;
+    if (md_energy_smem(p->M, p->n_alpha, p->n_beta, p->n_act, p->n_det, ts_) > 200 * 1024 ||
+        md_overlap_smem(p->M, p->n_alpha, p->n_beta, p->n_act, p->n_det, ts_) > 200 * 1024) {
+      snprintf(err, 256, "multi-det working set exceeds one CTA's shared memory"); return AFQMC_EUNSUPPORTED;
+    }
+  }
   if (p->gemm_path == 2) { snprintf(err, 256, "tcgen05 path not built yet"); return AFQMC_EUNSUPPORTED; }
   int cw, nch;
   bool ok = p->precision ? taylor_pick<double>(p->M, p->n_alpha + p->n_beta, cw, nch)
@@ -148,7 +165,10 @@ void carve(const afqmc_params* p, afqmc_ctx* c, char* cbase, char* wbase, size_t
   const int M = p->M, na = p->n_alpha, nb = p->n_beta, nt = na + nb, ng = p->n_chol, nw = p->n_walkers;
   const int ts = p->precision ? 8 : 4;
   const int MP = (M + 3) & ~3, NGP = (int)rup(ng, 32);
-  const int KA = (int)rup((size_t)M * na, 32), KB = (int)rup((size_t)M * nb, 32), KT = KA + KB;
+  const int md = p->n_det > 1;
+  const int ca = md ? p->n_act : na, cb_ = md ? p->n_act : nb;
+  const int KA = (int)rup((size_t)M * ca, 32), KB = (int)rup((size_t)M * cb_, 32), KT = KA + KB;
+  c->md = md; c->nact = md ? p->n_act : 0; c->ndet = p->n_det; c->ca = ca; c->cb = cb_;
   c->M = M; c->MP = MP; c->na = na; c->nb = nb; c->nt = nt; c->ng = ng; c->NGP = NGP; c->nw = nw;
   c->KA = KA; c->KB = KB; c->KT = KT; c->ts = ts;
   const int split = c->split;
@@ -160,11 +180,15 @@ void carve(const afqmc_params* p, afqmc_ctx* c, char* cbase, char* wbase, size_t
   c->Lt_lo = split ? cc.take((size_t)M * M * NGP * ts) : nullptr;
   c->Rall = cc.take((size_t)rup(ng, 128) * KT * ts);
   c->Rall_lo = split ? cc.take((size_t)rup(ng, 128) * KT * ts) : nullptr;
-  c->Y[0] = cc.take((size_t)KA * KA * ts);
-  c->Y[1] = cc.take((size_t)(KB ? KB : 32) * (KB ? KB : 32) * ts);
-  c->Y_lo[0] = split ? cc.take((size_t)KA * KA * ts) : nullptr;
-  c->Y_lo[1] = split ? cc.take((size_t)(KB ? KB : 32) * (KB ? KB : 32) * ts) : nullptr;
+  const size_t ya = md ? 32 : KA, yb = (md || !KB) ? 32 : KB;   // Y is not used by the multi-det energy
+  c->Y[0] = cc.take(ya * ya * ts);
+  c->Y[1] = cc.take(yb * yb * ts);
+  c->Y_lo[0] = split ? cc.take(ya * ya * ts) : nullptr;
+  c->Y_lo[1] = split ? cc.take(yb * yb * ts) : nullptr;
   c->hrot = cc.take((size_t)KT * ts);
+  c->Cact = cc.take((size_t)M * (md ? p->n_act : 1) * ts);
+  c->coeff = (double*)cc.take((size_t)p->n_det * 8);
+  c->exc = (int32_t*)cc.take((size_t)p->n_det * 8 * 4);
   *cb = cc.off;
 
   Carver w; w.base = wbase;
@@ -175,6 +199,10 @@ void carve(const afqmc_params* p, afqmc_ctx* c, char* cbase, char* wbase, size_t
   c->thp = w.take(2 * nw1 * KT * ts);
   c->thp_lo = split ? w.take(2 * nw1 * KT * ts) : nullptr;
   c->fs = w.take(2 * 2 * nw1 * NGP * ts);
+  c->thtil = w.take(md ? nw1 * M * 2 * p->n_act * 2 * ts : 256);
+  c->th_scr = w.take(md ? nw1 * M * nt * 2 * ts : 256);
+  c->ovlp0 = (zcplx*)w.take(nw1 * sizeof(zcplx));
+  c->ovlp_scr = (zcplx*)w.take(nw1 * sizeof(zcplx));
   c->cshift = (zcplx*)w.take(nw1 * sizeof(zcplx));
   c->eloc_scratch = (zcplx*)w.take(nw1 * sizeof(zcplx));
   c->h_phi = w.take(nw1 * M * nt * 2 * ts);
@@ -192,11 +220,12 @@ void carve(const afqmc_params* p, afqmc_ctx* c, char* cbase, char* wbase, size_t
   c->Rd = (double*)w.take((size_t)ng * KT * 8);
   c->hrotd = (double*)w.take((size_t)KT * 8);
   for (int i = 0; i < 4; ++i) c->ex[i] = (double*)w.take((size_t)M * M * 8);
-  c->psid = (double*)w.take((size_t)M * nt * 8);
+  c->psid = (double*)w.take((size_t)M * (nt + (md ? p->n_act : 0)) * 8);
   *wb = w.off;
 }
 
-template <typename T> afqmc_status init_device(afqmc_ctx* c, const double* h1, const double* L, const double* pa, const double* pb) {
+template <typename T> afqmc_status init_device(afqmc_ctx* c, const double* h1, const double* L, const double* pa, const double* pb,
+                                              const double* Cact_h, const double* coeff_h, const int32_t* exc_h) {
   const int M = c->M, MP = c->MP, na = c->na, nb = c->nb, ng = c->ng, NGP = c->NGP, KA = c->KA, KB = c->KB, KT = c->KT;
   cudaStream_t st = c->stream;
   size_t cb, wb;
@@ -246,15 +275,25 @@ template <typename T> afqmc_status init_device(afqmc_ctx* c, const double* h1, c
   // trial orbitals in T
   LAUNCH(c, k_cast2d<T>, (M * na + 127) / 128, 128, 0, M, na, psid_a, (size_t)na, (T*)c->psi_a, (T*)nullptr, (size_t)na, 0);
   if (nb) LAUNCH(c, k_cast2d<T>, (M * nb + 127) / 128, 128, 0, M, nb, psid_b, (size_t)nb, (T*)c->psi_b, (T*)nullptr, (size_t)nb, 0);
-  // R^s_g = Psi_s^T L_g and Psi_s^T h, spin-blocked index (s_off + k*n_s + a)
+  double* Cact_d = c->psid + (size_t)M * (na + nb);
+  if (c->md) {
+    const int nact = c->nact;
+    CUDA_OK(c, cudaMemcpyAsync(Cact_d, Cact_h, (size_t)M * nact * 8, cudaMemcpyHostToDevice, st));
+    CUDA_OK(c, cudaMemcpyAsync(c->coeff, coeff_h, (size_t)c->ndet * 8, cudaMemcpyHostToDevice, st));
+    CUDA_OK(c, cudaMemcpyAsync(c->exc, exc_h, (size_t)c->ndet * 8 * 4, cudaMemcpyHostToDevice, st));
+    LAUNCH(c, k_cast2d<T>, (M * nact + 127) / 128, 128, 0, M, nact, Cact_d, (size_t)nact, (T*)c->Cact, (T*)nullptr,
+           (size_t)nact, 0);
+  }
+  // R^s_g = Psi_s^T L_g and Psi_s^T h, spin-blocked index (s_off + k*n_s + a); multi-det: C_act^T L_g for both spins
   for (int s = 0; s < 2; ++s) {
-    int n = s ? nb : na, soff = s ? KA : 0;
+    int n = s ? c->cb : c->ca, soff = s ? KA : 0;
     if (!n) continue;
-    const double* C = s ? psid_b : psid_a;
+    const double* C = c->md ? Cact_d : (s ? psid_b : psid_a);
     size_t tot = (size_t)ng * M * n;
     LAUNCH(c, k_init_rot, (unsigned)((tot + 127) / 128), 128, 0, M, n, n, C, ng, c->Ld, soff, KT, c->Rd);
     LAUNCH(c, k_init_rot, (M * n + 127) / 128, 128, 0, M, n, n, C, 1, c->hd, soff, KT, c->hrotd);
     int Ks = s ? KB : KA;
+    if (!c->md)
     LAUNCH(c, k_init_Y<T>, dim3((M * n + 127) / 128, M * n), 128, 0, M, n, ng, c->Rd, soff, KT, (T*)c->Y[s],
            (T*)c->Y_lo[s], Ks, c->split);
   }
@@ -285,6 +324,21 @@ afqmc_status run_green(afqmc_ctx* c, const void* phi, void* ovlp, void* theta, i
   g.eloc_pre = (const zcplx*)eloc_pre; g.weight_mode = c->p.weight_mode; g.dt = c->p.dt; g.E0 = c->p.E0;
   g.flags = flags;
   StageScope sc(c, AFQMC_STAGE_GREEN);
+  if (c->md) {
+    // reference determinant first (S_0 to scratch, no weights), then SMW over all determinants
+    g.thp = nullptr; g.thp_lo = nullptr; g.ovlp = c->ovlp0; g.do_weight = 0;
+    LAUNCH(c, k_green<T>, c->nw, 128, c->green_smem, g);
+    MdOverlapArgs<T> a;
+    a.m.M = c->M; a.m.na = c->na; a.m.nb = c->nb; a.m.nact = c->nact; a.m.ndet = c->ndet;
+    a.m.C = c->Cact; a.m.coeff = c->coeff; a.m.exc = c->exc;
+    a.theta0 = (const cplx<T>*)theta; a.ovlp0 = c->ovlp0; a.thtil = (cplx<T>*)c->thtil; a.ovlp = (zcplx*)ovlp;
+    a.do_weight = do_weight; a.cshift = c->cshift; a.weight = weight; a.eloc_pre = (const zcplx*)eloc_pre;
+    a.weight_mode = c->p.weight_mode; a.dt = c->p.dt; a.E0 = c->p.E0; a.flags = flags;
+    LAUNCH(c, k_md_overlap<T>, c->nw, 256, c->mdo_smem, a);
+    LAUNCH(c, k_planarize<T>, c->nw, 128, 0, c->M, c->nact, c->nact, c->KA, c->KT, c->split, (const cplx<T>*)c->thtil,
+           (T*)c->thp, (T*)c->thp_lo);
+    return AFQMC_OK;
+  }
   LAUNCH(c, k_green<T>, c->nw, 128, c->green_smem, g);
   return AFQMC_OK;
 }
@@ -302,13 +356,24 @@ afqmc_status run_gemm(afqmc_ctx* c, const T* A, int lda, int m, const T* B, int 
 template <typename T> afqmc_status run_fb_gemm(afqmc_ctx* c) {
   StageScope sc(c, AFQMC_STAGE_FORCE_BIAS);
   for (int s = 0; s < 2; ++s) {
-    int n = s ? c->nb : c->na, soff = s ? c->KA : 0, Ks = s ? c->KB : c->KA;
+    int n = s ? c->cb : c->ca, soff = s ? c->KA : 0, Ks = s ? c->KB : c->KA;
     if (!n) continue;
     EpiStoreT<T> epi;
     epi.out = (T*)c->fs + (size_t)s * 2 * c->nw * c->NGP; epi.ldo = c->NGP; epi.m_real = c->ng; epi.n_real = 2 * c->nw;
     afqmc_status st = run_gemm<T>(c, (const T*)c->Rall + soff, c->KT, c->ng, (const T*)c->thp + soff, c->KT, 2 * c->nw, Ks, epi);
     if (st) return st;
   }
+  return AFQMC_OK;
+}
+
+template <typename T> afqmc_status run_md_energy(afqmc_ctx* c, const void* theta, zcplx* eloc) {
+  StageScope sc(c, AFQMC_STAGE_ENERGY);
+  MdEnergyArgs<T> a;
+  a.m.M = c->M; a.m.na = c->na; a.m.nb = c->nb; a.m.nact = c->nact; a.m.ndet = c->ndet;
+  a.m.C = c->Cact; a.m.coeff = c->coeff; a.m.exc = c->exc;
+  a.ng = c->ng; a.ldr = c->KT; a.theta0 = (const cplx<T>*)theta; a.Ract = (const T*)c->Rall; a.hact = (const T*)c->hrot;
+  a.eloc = eloc;
+  LAUNCH(c, k_md_energy<T>, c->nw, 256, c->mde_smem, a);
   return AFQMC_OK;
 }
 
@@ -377,7 +442,16 @@ afqmc_status do_propagate(afqmc_ctx* c, void* phi, const void* x, const void* fb
   return run_green<T>(c, phi, ovlp, theta, 1, weight, eloc_pre, flags);
 }
 
-template <typename T> afqmc_status do_force_bias(afqmc_ctx* c, const void* theta, void* fb) {
+template <typename T> afqmc_status do_force_bias(afqmc_ctx* c, const void* phi, const void* theta, void* fb) {
+  if (c->md) {
+    // the mixed Green's function needs the determinant ratios: rebuild them from the walker itself
+    afqmc_status st0 = run_green<T>(c, phi, c->ovlp_scr, c->th_scr, 0, nullptr, nullptr, nullptr);
+    if (st0) return st0;
+    st0 = run_fb_gemm<T>(c);
+    if (st0) return st0;
+    LAUNCH(c, k_fb_finish<T>, c->nw, 128, 0, c->ng, c->NGP, c->nw, (const T*)c->fs, (cplx<T>*)fb, (zcplx*)nullptr);
+    return AFQMC_OK;
+  }
   LAUNCH(c, k_planarize<T>, c->nw, 128, 0, c->M, c->na, c->nb, c->KA, c->KT, c->split, (const cplx<T>*)theta, (T*)c->thp,
          (T*)c->thp_lo);
   afqmc_status st = run_fb_gemm<T>(c);
@@ -387,11 +461,23 @@ template <typename T> afqmc_status do_force_bias(afqmc_ctx* c, const void* theta
 }
 
 // energy of the walkers whose planar Theta is in ctx->thp; runs the force-bias GEMM too (fb may be null)
-template <typename T> afqmc_status do_fb_energy_planar(afqmc_ctx* c, void* fb, zcplx* eloc) {
+template <typename T> afqmc_status do_fb_energy_planar(afqmc_ctx* c, const void* theta, void* fb, zcplx* eloc) {
   afqmc_status st = run_fb_gemm<T>(c);
   if (st) return st;
+  if (c->md) {
+    if (fb) LAUNCH(c, k_fb_finish<T>, c->nw, 128, 0, c->ng, c->NGP, c->nw, (const T*)c->fs, (cplx<T>*)fb, (zcplx*)nullptr);
+    return run_md_energy<T>(c, theta, eloc);
+  }
   LAUNCH(c, k_fb_finish<T>, c->nw, 128, 0, c->ng, c->NGP, c->nw, (const T*)c->fs, (cplx<T>*)fb, eloc);
   return run_energy_gemm<T>(c, eloc);
+}
+
+// E_L from an interleaved Theta handed in by the caller
+template <typename T> afqmc_status do_energy_from_theta(afqmc_ctx* c, const void* theta, zcplx* eloc) {
+  if (c->md) return run_md_energy<T>(c, theta, eloc);
+  LAUNCH(c, k_planarize<T>, c->nw, 128, 0, c->M, c->na, c->nb, c->KA, c->KT, c->split, (const cplx<T>*)theta, (T*)c->thp,
+         (T*)c->thp_lo);
+  return do_fb_energy_planar<T>(c, theta, nullptr, eloc);
 }
 
 template <typename T>
@@ -400,10 +486,8 @@ afqmc_status do_step(afqmc_ctx* c, void* phi, double* weight, void* ovlp, void* 
   zcplx* el = (zcplx*)eloc;
   const zcplx* epre = nullptr;
   if (c->p.weight_mode == 1) {
-    // E_L of the walkers on entry (needs their planar Theta)
-    LAUNCH(c, k_planarize<T>, c->nw, 128, 0, c->M, c->na, c->nb, c->KA, c->KT, c->split, (const cplx<T>*)theta,
-           (T*)c->thp, (T*)c->thp_lo);
-    afqmc_status st = do_fb_energy_planar<T>(c, nullptr, c->eloc_scratch);
+    // E_L of the walkers on entry
+    afqmc_status st = do_energy_from_theta<T>(c, theta, c->eloc_scratch);
     if (st) return st;
     epre = c->eloc_scratch;
   }
@@ -411,7 +495,7 @@ afqmc_status do_step(afqmc_ctx* c, void* phi, double* weight, void* ovlp, void* 
     const T* xs = (const T*)x + (size_t)s * c->nw * c->ng;
     afqmc_status st = do_propagate<T>(c, phi, xs, fb, ovlp, weight, theta, epre, flags);
     if (st) return st;
-    st = do_fb_energy_planar<T>(c, fb, el + (size_t)s * c->nw);
+    st = do_fb_energy_planar<T>(c, theta, fb, el + (size_t)s * c->nw);
     if (st) return st;
     epre = el + (size_t)s * c->nw;
   }
@@ -438,14 +522,45 @@ afqmc_status afqmc_query_bytes(const afqmc_params* p, size_t* const_bytes, size_
 afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1, const double* L_chol,
                         const double* psiT_a, const double* psiT_b, const double* C_act, const double* det_coeff,
                         const int32_t* det_exc, void* const_mem, void* work_mem, void* stream) {
-  (void)C_act; (void)det_coeff; (void)det_exc;
   if (!out) { snprintf(g_init_err, 256, "out is NULL"); return AFQMC_EINVAL; }
   *out = nullptr;
   afqmc_status s = check_params(p, g_init_err);
   if (s) return s;
-  if (!h1 || !L_chol || !psiT_a || (p->n_beta && !psiT_b) || !const_mem || !work_mem) {
+  const bool md = p->n_det > 1;
+  if (!h1 || !L_chol || !const_mem || !work_mem || (!md && (!psiT_a || (p->n_beta && !psiT_b))) ||
+      (md && (!C_act || !det_coeff || !det_exc))) {
     snprintf(g_init_err, 256, "null input pointer");
     return AFQMC_EINVAL;
+  }
+  // multi-det: reference orbitals = first n_sigma columns of C_act; excitation list normalised to 2 slots
+  std::vector<double> pa_md, pb_md;
+  std::vector<int32_t> exc2((size_t)p->n_det * 8, -1);
+  if (md) {
+    const int nact = p->n_act;
+    pa_md.resize((size_t)p->M * p->n_alpha); pb_md.resize((size_t)p->M * p->n_beta);
+    for (int k = 0; k < p->M; ++k) {
+      for (int a = 0; a < p->n_alpha; ++a) pa_md[(size_t)k * p->n_alpha + a] = C_act[(size_t)k * nact + a];
+      for (int a = 0; a < p->n_beta; ++a) pb_md[(size_t)k * p->n_beta + a] = C_act[(size_t)k * nact + a];
+    }
+    psiT_a = pa_md.data(); psiT_b = pb_md.data();
+    for (int i = 0; i < p->n_det; ++i)
+      for (int sp = 0; sp < 2; ++sp) {
+        const int n = sp ? p->n_beta : p->n_alpha;
+        int cnt = 0, hs[2] = {-1, -1}, ps[2] = {-1, -1};
+        for (int e = 0; e < p->max_exc; ++e) {
+          const int32_t* ex = det_exc + (((size_t)i * 2 + sp) * p->max_exc + e) * 2;
+          if (ex[0] < 0) continue;
+          if (ex[0] >= n || ex[1] < n || ex[1] >= nact || (cnt == 1 && (ex[0] == hs[0] || ex[1] == ps[0]))) {
+            snprintf(g_init_err, 256, "det_exc: need hole < n_sigma <= particle < n_act, distinct within a determinant");
+            return AFQMC_EINVAL;
+          }
+          hs[cnt] = ex[0]; ps[cnt] = ex[1]; ++cnt;
+        }
+        for (int e = 0; e < cnt; ++e) {
+          exc2[((size_t)i * 2 + sp) * 4 + 2 * e] = hs[e];
+          exc2[((size_t)i * 2 + sp) * 4 + 2 * e + 1] = ps[e];
+        }
+      }
   }
   if (((uintptr_t)const_mem & 255) || ((uintptr_t)work_mem & 255)) {
     snprintf(g_init_err, 256, "const_mem / work_mem must be 256-byte aligned");
@@ -497,12 +612,26 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
     delete c;
     return s;
   }
+  if (c->md) {
+    c->mdo_smem = md_overlap_smem(c->M, c->na, c->nb, c->nact, c->ndet, c->ts);
+    c->mde_smem = md_energy_smem(c->M, c->na, c->nb, c->nact, c->ndet, c->ts);
+    cudaError_t e1, e2;
+    if (p->precision) {
+      e1 = cudaFuncSetAttribute(k_md_overlap<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->mdo_smem);
+      e2 = cudaFuncSetAttribute(k_md_energy<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->mde_smem);
+    } else {
+      e1 = cudaFuncSetAttribute(k_md_overlap<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->mdo_smem);
+      e2 = cudaFuncSetAttribute(k_md_energy<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->mde_smem);
+    }
+    if (e1 != cudaSuccess || e2 != cudaSuccess) { snprintf(g_init_err, 256, "CUDA: cannot size multi-det shared memory"); delete c; return AFQMC_ECUDA; }
+  }
   if (c->green_smem > 48 * 1024) {
     cudaError_t e = p->precision ? cudaFuncSetAttribute(k_green<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->green_smem)
                                  : cudaFuncSetAttribute(k_green<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->green_smem);
     if (e != cudaSuccess) { snprintf(g_init_err, 256, "CUDA: %s", cudaGetErrorString(e)); delete c; return AFQMC_ECUDA; }
   }
-  s = p->precision ? init_device<double>(c, h1, L_chol, psiT_a, psiT_b) : init_device<float>(c, h1, L_chol, psiT_a, psiT_b);
+  s = p->precision ? init_device<double>(c, h1, L_chol, psiT_a, psiT_b, C_act, det_coeff, exc2.data())
+                   : init_device<float>(c, h1, L_chol, psiT_a, psiT_b, C_act, det_coeff, exc2.data());
   if (s) {
     memcpy(g_init_err, c->err, 256);
     delete c;
@@ -570,7 +699,14 @@ afqmc_status afqmc_overlap_green(afqmc_ctx* c, const void* phi, void* ovlp, void
   if (s) return s;
   if (G_or_null) {
     dim3 grid((c->M * c->M + 255) / 256, c->nw, 2);
-    if (c->p.precision)
+    if (c->md) {   // mixed G_s^T = Thtil_s C_act^T
+      if (c->p.precision)
+        LAUNCH(c, k_gfull<double>, grid, 256, 0, c->M, c->nact, c->nact, (const cplx<double>*)c->thtil,
+               (const double*)c->Cact, (const double*)c->Cact, (cplx<double>*)G_or_null);
+      else
+        LAUNCH(c, k_gfull<float>, grid, 256, 0, c->M, c->nact, c->nact, (const cplx<float>*)c->thtil,
+               (const float*)c->Cact, (const float*)c->Cact, (cplx<float>*)G_or_null);
+    } else if (c->p.precision)
       LAUNCH(c, k_gfull<double>, grid, 256, 0, c->M, c->na, c->nb, (const cplx<double>*)theta, (const double*)c->psi_a,
              (const double*)c->psi_b, (cplx<double>*)G_or_null);
     else
@@ -586,7 +722,8 @@ afqmc_status afqmc_force_bias(afqmc_ctx* c, const void* phi, const void* theta, 
   c->err[0] = 0;
   NEED(c, theta && fb, "afqmc_force_bias: null pointer");
   if (c->nw == 0) return AFQMC_OK;
-  return DISPATCH(c, do_force_bias, c, theta, fb);
+  NEED(c, !c->md || phi, "afqmc_force_bias: multi-determinant trial needs phi");
+  return DISPATCH(c, do_force_bias, c, phi, theta, fb);
 }
 
 afqmc_status afqmc_propagate(afqmc_ctx* c, void* phi, const void* x, const void* fb, void* ovlp, double* weight, void* theta,
@@ -605,14 +742,7 @@ afqmc_status afqmc_local_energy(afqmc_ctx* c, const void* phi, const void* theta
   c->err[0] = 0;
   NEED(c, theta && eloc, "afqmc_local_energy: null pointer");
   if (c->nw == 0) return AFQMC_OK;
-  if (c->p.precision) {
-    LAUNCH(c, k_planarize<double>, c->nw, 128, 0, c->M, c->na, c->nb, c->KA, c->KT, c->split, (const cplx<double>*)theta,
-           (double*)c->thp, (double*)c->thp_lo);
-    return do_fb_energy_planar<double>(c, nullptr, (zcplx*)eloc);
-  }
-  LAUNCH(c, k_planarize<float>, c->nw, 128, 0, c->M, c->na, c->nb, c->KA, c->KT, c->split, (const cplx<float>*)theta,
-         (float*)c->thp, (float*)c->thp_lo);
-  return do_fb_energy_planar<float>(c, nullptr, (zcplx*)eloc);
+  return DISPATCH(c, do_energy_from_theta, c, theta, (zcplx*)eloc);
 }
 
 afqmc_status afqmc_step(afqmc_ctx* c, void* phi, double* weight, void* ovlp, void* theta, void* fb, const void* x,

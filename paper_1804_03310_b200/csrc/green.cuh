@@ -10,14 +10,13 @@ namespace afq {
 // executed by ONE warp.  On exit the right block is A^-1; det = product of pivots (FP64, R17).
 // sing bit 0: a pivot was exactly zero / NaN or below eps*max|A|.
 template <typename T>
-__device__ void warp_gauss_jordan(cplx<T>* aug, int n, int ld, cplx<T>* fac, int lane, zcplx& det, int& sing) {
+__device__ void warp_gauss_jordan(cplx<T>* aug, int n, int ld, cplx<T>* fac, int lane, zcplx& det, int& sing, T eps) {
   double dre = 1.0, dim = 0.0;
   sing = 0;
   T amax = T(0);
   for (int e = lane; e < n * n; e += 32) amax = fmax(amax, cabs2(aug[(e / n) * ld + (e % n)]));
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) amax = fmax(amax, __shfl_xor_sync(0xffffffffu, amax, o));
-  const T eps = sizeof(T) == 4 ? T(1e-6) : T(1e-13);
   const T thresh = amax * eps * eps;  // compare squared magnitudes
   for (int col = 0; col < n; ++col) {
     int r = col + lane;
@@ -87,10 +86,9 @@ template <typename T> struct GreenArgs {
 // shared-memory bytes needed by k_green
 template <typename T> inline size_t green_smem_bytes(int M, int na, int nb) {
   int nt = na + nb, ns = na > nb ? na : nb;
-  size_t b = (size_t)M * nt * sizeof(cplx<T>);          // phi_s
-  b += (size_t)2 * ns * (2 * ns + 1) * sizeof(cplx<T>); // aug per spin
-  b += (size_t)2 * ns * sizeof(cplx<T>);                // fac per spin
-  b = (b + 15) & ~size_t(15);
+  size_t b = ((size_t)M * nt * sizeof(cplx<T>) + 15) & ~size_t(15);   // phi_s
+  b += (size_t)2 * ns * (2 * ns + 1) * sizeof(zcplx);   // aug per spin (FP64 on both precision paths)
+  b += (size_t)2 * ns * sizeof(zcplx);                  // fac per spin
   b += 2 * sizeof(zcplx) + 4 * sizeof(int);
   return (b + 15) & ~size_t(15);
 }
@@ -121,9 +119,11 @@ __global__ void __launch_bounds__(128) k_green(GreenArgs<T> g) {
   const int M = g.M, na = g.na, nb = g.nb, nt = na + nb, ns = na > nb ? na : nb;
   const int ld = 2 * ns + 1;
   cplx<T>* phi_s = reinterpret_cast<cplx<T>*>(smem_raw);
-  cplx<T>* aug = phi_s + (size_t)M * nt;
-  cplx<T>* fac = aug + 2 * ns * ld;
-  zcplx* dets = reinterpret_cast<zcplx*>(smem_raw + ((((size_t)M * nt + 2 * ns * ld + 2 * ns) * sizeof(cplx<T>) + 15) & ~size_t(15)));
+  // the small N x N work (overlap matrix, LU, inverse) is FP64 on both precision paths: it is
+  // 0.3 % of the flops and keeps S, Theta accurate to cond(A) * eps of the FP32 walker itself
+  zcplx* aug = reinterpret_cast<zcplx*>(smem_raw + (((size_t)M * nt * sizeof(cplx<T>) + 15) & ~size_t(15)));
+  zcplx* fac = aug + 2 * ns * ld;
+  zcplx* dets = fac + 2 * ns;
   int* sing = reinterpret_cast<int*>(dets + 2);
 
   const cplx<T>* phi_w = g.phi + (size_t)w * M * nt;
@@ -137,23 +137,23 @@ __global__ void __launch_bounds__(128) k_green(GreenArgs<T> g) {
     int n = s ? nb : na, off = s ? na : 0;
     const T* psi = s ? g.psi_b : g.psi_a;
     int a = ee / n, b = ee % n;
-    T sr = T(0), si = T(0);
+    double sr = 0.0, si = 0.0;
     for (int k = 0; k < M; ++k) {
-      T p = psi[k * n + a];
+      double p = (double)psi[k * n + a];
       cplx<T> v = phi_s[k * nt + off + b];
-      sr = fma(p, v.x, sr);
-      si = fma(p, v.y, si);
+      sr = fma(p, (double)v.x, sr);
+      si = fma(p, (double)v.y, si);
     }
-    cplx<T>* A = aug + s * ns * ld;
-    A[a * ld + b] = mk<T>(sr, si);
-    A[a * ld + n + b] = mk<T>(a == b ? T(1) : T(0), T(0));
+    zcplx* A = aug + s * ns * ld;
+    A[a * ld + b] = mk<double>(sr, si);
+    A[a * ld + n + b] = mk<double>(a == b ? 1.0 : 0.0, 0.0);
   }
   __syncthreads();
   if (warp < 2) {
     int n = warp ? nb : na;
     zcplx det = mk<double>(1.0, 0.0);
     int sg = 0;
-    if (n > 0) warp_gauss_jordan<T>(aug + warp * ns * ld, n, ld, fac + warp * ns, lane, det, sg);
+    if (n > 0) warp_gauss_jordan<double>(aug + warp * ns * ld, n, ld, fac + warp * ns, lane, det, sg, sizeof(T) == 4 ? 1e-6 : 1e-13);
     if (lane == 0) { dets[warp] = det; sing[warp] = sg; }
   }
   __syncthreads();
@@ -161,11 +161,12 @@ __global__ void __launch_bounds__(128) k_green(GreenArgs<T> g) {
   // Theta_s = Phi_s A_s^-1
   for (int s = 0; s < 2; ++s) {
     int n = s ? nb : na, off = s ? na : 0, soff = s ? g.KA : 0;
-    const cplx<T>* inv = aug + s * ns * ld + n;
+    const zcplx* inv = aug + s * ns * ld + n;
     for (int e = tid; e < M * n; e += 128) {
       int k = e / n, b = e % n;
-      cplx<T> acc = mk<T>(T(0), T(0));
-      for (int a = 0; a < n; ++a) cfma(acc, phi_s[k * nt + off + a], inv[a * ld + b]);
+      zcplx accd = mk<double>(0.0, 0.0);
+      for (int a = 0; a < n; ++a) cfma(accd, to_z(phi_s[k * nt + off + a]), inv[a * ld + b]);
+      cplx<T> acc = mk<T>((T)accd.x, (T)accd.y);
       if (g.theta) g.theta[(size_t)w * M * nt + k * nt + off + b] = acc;
       if (g.thp) {
         size_t o = (size_t)(2 * w) * g.KT + soff + e;

@@ -1,0 +1,391 @@
+// multidet.cuh -- H10: multi-determinant trial |Psi_T> = sum_i c_i |psi_i> (Eq.(4)).
+// Every determinant is the reference with <= 2 columns per spin replaced by active-space orbitals, so
+// all overlaps / Green's functions follow from the reference by Sherman-Morrison-Woodbury rank-E updates:
+//   Q = C_act^T Theta_0,  Q_i = Q[P_i,H_i] (E x E),  det A_i / det A_0 = det Q_i,  Z_i = Q_i^-1,
+//   Theta_i psi_i^T = Theta_0 psi_0^T + Theta_0[:,H_i] Z_i R[P_i,:],  R = C_virt^T - Q_virt psi_0^T.
+// One CTA per walker; determinant-level scalars are FP64 on both precision paths (H10).
+#pragma once
+#include "common.cuh"
+#include "green.cuh"
+
+namespace afq {
+
+__device__ __forceinline__ zcplx zmul(zcplx a, zcplx b) { return mk<double>(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+__device__ __forceinline__ zcplx zadd(zcplx a, zcplx b) { return mk<double>(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ zcplx zsub(zcplx a, zcplx b) { return mk<double>(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ zcplx zscale(zcplx a, double s) { return mk<double>(a.x * s, a.y * s); }
+
+struct MdConst {
+  int M, na, nb, nact, ndet;
+  const void* C;           // [M][nact]  (T)
+  const double* coeff;     // [ndet]
+  const int32_t* exc;      // [ndet][2][2][2] (hole, particle) or -1
+};
+
+// Shared-memory view used by both multi-det kernels.
+struct MdSmem {
+  zcplx* Qv[2];    // [nvirt_s][n_s]     Q_virt = C_virt^T Theta_0
+  zcplx* Z;        // [ndet][2][4]       Z_i^s[f][e] (row = hole slot f, col = particle slot e)
+  zcplx* omega;    // [ndet]             c_i S_i / S
+  int8_t* rank;    // [ndet][2]          excitation rank per spin
+  zcplx* red;      // [64] reduction scratch
+  int* flag;       // bit 0: a determinant has exactly zero overlap with the walker (its Z is undefined)
+};
+
+inline size_t md_smem_bytes(int na, int nb, int nact, int ndet) {
+  size_t b = (size_t)((nact - na) * na + (nact - nb) * nb) * sizeof(zcplx);
+  b += (size_t)ndet * 8 * sizeof(zcplx) + (size_t)ndet * sizeof(zcplx) + 64 * sizeof(zcplx);
+  b += ((size_t)ndet * 2 + 15) & ~size_t(15);
+  b += 16;
+  return b;
+}
+
+__device__ inline unsigned char* md_carve(unsigned char* p, const MdConst& m, MdSmem& s) {
+  s.Qv[0] = reinterpret_cast<zcplx*>(p); p += (size_t)(m.nact - m.na) * m.na * sizeof(zcplx);
+  s.Qv[1] = reinterpret_cast<zcplx*>(p); p += (size_t)(m.nact - m.nb) * m.nb * sizeof(zcplx);
+  s.Z = reinterpret_cast<zcplx*>(p); p += (size_t)m.ndet * 8 * sizeof(zcplx);
+  s.omega = reinterpret_cast<zcplx*>(p); p += (size_t)m.ndet * sizeof(zcplx);
+  s.red = reinterpret_cast<zcplx*>(p); p += 64 * sizeof(zcplx);
+  s.rank = reinterpret_cast<int8_t*>(p); p += ((size_t)m.ndet * 2 + 15) & ~size_t(15);
+  s.flag = reinterpret_cast<int*>(p); p += 16;
+  return p;
+}
+
+// block-wide complex sum (all threads call); result broadcast
+__device__ inline zcplx block_sum(zcplx v, zcplx* red) {
+  v.x = warp_sum(v.x); v.y = warp_sum(v.y);
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nwarp = (blockDim.x + 31) >> 5;
+  __syncthreads();
+  if (lane == 0) red[wid] = v;
+  __syncthreads();
+  zcplx t = mk<double>(0.0, 0.0);
+  for (int i = 0; i < nwarp; ++i) t = zadd(t, red[i]);
+  __syncthreads();
+  return t;
+}
+
+// From Theta_0 (shared, [M][nt] complex T): Q_virt, per-determinant ratios r_i, Z_i, mixing weights
+// omega_i = c_i r_i^a r_i^b / sum_j c_j r_j^a r_j^b.  Returns the sum (S / S_0).  All threads call.
+template <typename T>
+__device__ zcplx md_prepare(const MdConst& m, const cplx<T>* th0, MdSmem& s) {
+  const int nt = m.na + m.nb, tid = threadIdx.x, nthr = blockDim.x;
+  const T* C = reinterpret_cast<const T*>(m.C);
+  if (tid == 0) *s.flag = 0;
+  for (int sp = 0; sp < 2; ++sp) {
+    const int n = sp ? m.nb : m.na, off = sp ? m.na : 0, nv = m.nact - n;
+    for (int e = tid; e < nv * n; e += nthr) {
+      int p = e / n, h = e - p * n;
+      double sr = 0.0, si = 0.0;
+      for (int k = 0; k < m.M; ++k) {
+        double c = (double)C[k * m.nact + n + p];
+        cplx<T> v = th0[k * nt + off + h];
+        sr = fma(c, (double)v.x, sr);
+        si = fma(c, (double)v.y, si);
+      }
+      s.Qv[sp][e] = mk<double>(sr, si);
+    }
+  }
+  __syncthreads();
+  zcplx part = mk<double>(0.0, 0.0);
+  for (int i = tid; i < m.ndet; i += nthr) {
+    zcplx ratio = mk<double>(1.0, 0.0);
+    for (int sp = 0; sp < 2; ++sp) {
+      const int n = sp ? m.nb : m.na;
+      const int32_t* ex = m.exc + ((size_t)i * 2 + sp) * 4;
+      int h0 = ex[0], p0 = ex[1], h1 = ex[2], p1 = ex[3];
+      int rk = (h0 >= 0) + (h1 >= 0);
+      if (h0 < 0 && h1 >= 0) { h0 = h1; p0 = p1; }
+      s.rank[i * 2 + sp] = (int8_t)rk;
+      zcplx* Zi = s.Z + ((size_t)i * 2 + sp) * 4;
+      const zcplx* Q = s.Qv[sp];
+      if (rk == 1) {
+        zcplx q = Q[(p0 - n) * n + h0];
+        ratio = zmul(ratio, q);
+        if (q.x == 0.0 && q.y == 0.0) { Zi[0] = q; atomicOr(s.flag, 1); }   // zero overlap: dropped, flagged
+        else Zi[0] = zdiv(mk<double>(1.0, 0.0), q);
+      } else if (rk == 2) {
+        zcplx a = Q[(p0 - n) * n + h0], b = Q[(p0 - n) * n + h1];
+        zcplx c = Q[(p1 - n) * n + h0], d = Q[(p1 - n) * n + h1];
+        zcplx det = zsub(zmul(a, d), zmul(b, c));
+        const bool zero = det.x == 0.0 && det.y == 0.0;
+        zcplx id = zero ? det : zdiv(mk<double>(1.0, 0.0), det);
+        if (zero) atomicOr(s.flag, 1);
+        ratio = zmul(ratio, det);
+        // inverse of [[a,b],[c,d]] (rows = particle slot, cols = hole slot): Z[f][e]
+        Zi[0] = zmul(d, id);
+        Zi[1] = zmul(mk<double>(-b.x, -b.y), id);
+        Zi[2] = zmul(mk<double>(-c.x, -c.y), id);
+        Zi[3] = zmul(a, id);
+      }
+    }
+    zcplx cr = zscale(ratio, m.coeff[i]);
+    s.omega[i] = cr;
+    part = zadd(part, cr);
+  }
+  zcplx tot = block_sum(part, s.red);
+  for (int i = tid; i < m.ndet; i += nthr) s.omega[i] = zdiv(s.omega[i], tot);
+  __syncthreads();
+  return tot;
+}
+
+
+// canonical (hole, particle) slots of determinant i, spin sp; returns the rank
+__device__ __forceinline__ int md_exc(const MdConst& m, int i, int sp, int (&h)[2], int (&p)[2]) {
+  const int32_t* ex = m.exc + ((size_t)i * 2 + sp) * 4;
+  h[0] = ex[0]; p[0] = ex[1]; h[1] = ex[2]; p[1] = ex[3];
+  int rk = (h[0] >= 0) + (h[1] >= 0);
+  if (h[0] < 0 && h[1] >= 0) { h[0] = h[1]; p[0] = p[1]; }
+  return rk;
+}
+
+template <typename T> struct MdOverlapArgs {
+  MdConst m;
+  const cplx<T>* theta0;   // [nw][M][nt]   reference Theta_0 (from k_green)
+  const zcplx* ovlp0;      // [nw]          reference overlap det A_0^a det A_0^b
+  cplx<T>* thtil;          // [nw][M][2*nact]  generalised half-rotated mixed Green's function:
+                           //   mixed G_s^T = Thtil_s C_act^T,  Thtil_s = [Theta_0 - Theta_0 B Q_virt | Theta_0 B]
+  zcplx* ovlp;             // in: S (do_weight) ; out: S' = S_0 sum_i c_i r_i
+  int do_weight;
+  const zcplx* cshift; double* weight; const zcplx* eloc_pre; int weight_mode; double dt, E0;
+  int* flags;
+};
+
+inline size_t md_overlap_smem(int M, int na, int nb, int nact, int ndet, int ts) {
+  size_t b = md_smem_bytes(na, nb, nact, ndet);
+  b += ((size_t)M * (na + nb) * 2 * ts + 15) & ~size_t(15);
+  b += (size_t)(na * (nact - na) + nb * (nact - nb)) * sizeof(zcplx);   // Btil
+  b += (size_t)(na * na + nb * nb) * sizeof(zcplx);                     // Btil Q_virt
+  return b;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_md_overlap(MdOverlapArgs<T> g) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const MdConst& m = g.m;
+  const int w = blockIdx.x, tid = threadIdx.x, nthr = blockDim.x, nt = m.na + m.nb, M = m.M;
+  MdSmem s;
+  unsigned char* p = md_carve(smem_raw, m, s);
+  cplx<T>* th0 = reinterpret_cast<cplx<T>*>(p);
+  p += ((size_t)M * nt * sizeof(cplx<T>) + 15) & ~size_t(15);
+  zcplx* Bt[2]; zcplx* BQ[2];
+  Bt[0] = reinterpret_cast<zcplx*>(p); Bt[1] = Bt[0] + m.na * (m.nact - m.na);
+  BQ[0] = Bt[1] + m.nb * (m.nact - m.nb); BQ[1] = BQ[0] + m.na * m.na;
+  for (int e = tid; e < M * nt; e += nthr) th0[e] = g.theta0[(size_t)w * M * nt + e];
+  const int nbt = m.na * (m.nact - m.na) + m.nb * (m.nact - m.nb);
+  for (int e = tid; e < nbt; e += nthr) Bt[0][e] = mk<double>(0.0, 0.0);
+  __syncthreads();
+  zcplx tot = md_prepare<T>(m, th0, s);
+  // Btil_s[h][p] = sum_i omega_i Z_i^s[f][e] at (h_f, p_e)
+  for (int i = tid; i < m.ndet; i += nthr) {
+    zcplx om = s.omega[i];
+    for (int sp = 0; sp < 2; ++sp) {
+      int h[2], pp[2];
+      int rk = md_exc(m, i, sp, h, pp);
+      const int n = sp ? m.nb : m.na, nv = m.nact - n;
+      const zcplx* Zi = s.Z + ((size_t)i * 2 + sp) * 4;
+      for (int f = 0; f < rk; ++f)
+        for (int e = 0; e < rk; ++e) {
+          zcplx v = zmul(om, Zi[rk == 1 ? 0 : f * 2 + e]);
+          double* dst = reinterpret_cast<double*>(&Bt[sp][h[f] * nv + (pp[e] - n)]);
+          atomicAdd(dst, v.x); atomicAdd(dst + 1, v.y);
+        }
+    }
+  }
+  __syncthreads();
+  for (int sp = 0; sp < 2; ++sp) {
+    const int n = sp ? m.nb : m.na, nv = m.nact - n;
+    for (int e = tid; e < n * n; e += nthr) {
+      int h1 = e / n, h2 = e - h1 * n;
+      zcplx a = mk<double>(0.0, 0.0);
+      for (int q = 0; q < nv; ++q) a = zadd(a, zmul(Bt[sp][h1 * nv + q], s.Qv[sp][q * n + h2]));
+      BQ[sp][e] = a;
+    }
+  }
+  __syncthreads();
+  for (int sp = 0; sp < 2; ++sp) {
+    const int n = sp ? m.nb : m.na, nv = m.nact - n, off = sp ? m.na : 0;
+    for (int e = tid; e < M * m.nact; e += nthr) {
+      int k = e / m.nact, q = e - k * m.nact;
+      zcplx a;
+      if (q < n) {
+        a = to_z(th0[k * nt + off + q]);
+        for (int h = 0; h < n; ++h) a = zsub(a, zmul(to_z(th0[k * nt + off + h]), BQ[sp][h * n + q]));
+      } else {
+        a = mk<double>(0.0, 0.0);
+        for (int h = 0; h < n; ++h) a = zadd(a, zmul(to_z(th0[k * nt + off + h]), Bt[sp][h * nv + (q - n)]));
+      }
+      g.thtil[((size_t)w * M + k) * (2 * m.nact) + sp * m.nact + q] = mk<T>((T)a.x, (T)a.y);
+    }
+  }
+  if (tid == 0) {
+    zcplx S_new = zmul(g.ovlp0[w], tot);
+    int flag = (*s.flag & 1) ? FLAG_SINGULAR : 0;
+    if (!isfinite(S_new.x) || !isfinite(S_new.y)) flag |= FLAG_NONFINITE;
+    if (g.do_weight) {
+      double w_new;
+      double epre = g.eloc_pre ? g.eloc_pre[w].x : 0.0;
+      weight_update(g.ovlp[w], S_new, g.cshift[w], g.weight[w], g.dt, g.E0, g.weight_mode, epre, w_new, flag);
+      g.weight[w] = w_new;
+    }
+    g.ovlp[w] = S_new;
+    if (g.flags && flag) atomicOr(&g.flags[w], flag);
+  }
+}
+
+
+// ---------------------------------------------------------------------------------------------
+// Mixed local energy E_L = sum_i omega_i E_L^(i) with rank-E closed forms (H10):
+// per operator X in {L_g, h}:  TT = C_act^T X Theta_0 (nact x N),  T0 = its top N rows,
+//   W = TT_virt - Q_virt T0,  WT = W T0,  f0 = Tr T0,  X0 = Tr(T0 T0);  per determinant and spin
+//   t = f0 + Tr(Z W[P,H]),  xch = X0 + 2 Tr(Z WT[P,H]) + Tr((Z W[P,H])^2);
+//   E^(i) = sum_s t^s(h) + 1/2 sum_g [(t^a + t^b)^2 - xch^a - xch^b].
+// ---------------------------------------------------------------------------------------------
+template <typename T> struct MdEnergyArgs {
+  MdConst m;
+  int ng, ldr;
+  const cplx<T>* theta0;   // [nw][M][nt]
+  const T* Ract;           // [ng][ldr] : Ract[g][k*nact + q] = (C_act^T L_g)[q][k]
+  const T* hact;           // [M*nact]  : (C_act^T h)[q][k] at k*nact + q
+  zcplx* eloc;             // [nw]
+};
+
+inline size_t md_energy_smem(int M, int na, int nb, int nact, int ndet, int ts) {
+  size_t b = md_smem_bytes(na, nb, nact, ndet);
+  b += ((size_t)M * (na + nb) * 2 * ts + 15) & ~size_t(15);
+  b += (size_t)nact * (na + nb) * sizeof(zcplx);                              // TT
+  b += (size_t)2 * ((nact - na) * na + (nact - nb) * nb) * sizeof(zcplx);     // W, WT
+  b += 4 * sizeof(zcplx);
+  return b;
+}
+
+enum { MD_DPT = 4 };  // determinants per thread (ndet <= 4 * 256)
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_md_energy(MdEnergyArgs<T> g) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const MdConst& m = g.m;
+  const int w = blockIdx.x, tid = threadIdx.x, nthr = blockDim.x, nt = m.na + m.nb, M = m.M, nact = m.nact;
+  const int lane = tid & 31, wid = tid >> 5;
+  MdSmem s;
+  unsigned char* p = md_carve(smem_raw, m, s);
+  cplx<T>* th0 = reinterpret_cast<cplx<T>*>(p);
+  p += ((size_t)M * nt * sizeof(cplx<T>) + 15) & ~size_t(15);
+  zcplx* TT = reinterpret_cast<zcplx*>(p);
+  zcplx* Wm[2]; zcplx* WTm[2];
+  Wm[0] = TT + nact * nt; Wm[1] = Wm[0] + (nact - m.na) * m.na;
+  WTm[0] = Wm[1] + (nact - m.nb) * m.nb; WTm[1] = WTm[0] + (nact - m.na) * m.na;
+  zcplx* scal = WTm[1] + (nact - m.nb) * m.nb;   // f0[2], X0[2]
+  for (int e = tid; e < M * nt; e += nthr) th0[e] = g.theta0[(size_t)w * M * nt + e];
+  __syncthreads();
+  md_prepare<T>(m, th0, s);
+
+  zcplx Eacc[MD_DPT];
+#pragma unroll
+  for (int j = 0; j < MD_DPT; ++j) Eacc[j] = mk<double>(0.0, 0.0);
+
+  for (int gi = 0; gi <= g.ng; ++gi) {
+    const bool is_h = gi == g.ng;
+    const T* R = is_h ? g.hact : g.Ract + (size_t)gi * g.ldr;
+    // 1. TT[q][a] = sum_k R[q][k] Theta_0[k][a]
+    for (int e = tid; e < nact * nt; e += nthr) {
+      int q = e / nt, a = e - q * nt;
+      T sr = T(0), si = T(0);
+      for (int k = 0; k < M; ++k) {
+        T r = R[k * nact + q];
+        cplx<T> v = th0[k * nt + a];
+        sr = fma(r, v.x, sr);
+        si = fma(r, v.y, si);
+      }
+      TT[e] = mk<double>((double)sr, (double)si);
+    }
+    __syncthreads();
+    // 2. W = TT_virt - Q_virt T0 ; f0, X0 by warps 0 / 1
+    for (int sp = 0; sp < 2; ++sp) {
+      const int n = sp ? m.nb : m.na, nv = nact - n, off = sp ? m.na : 0;
+      for (int e = tid; e < nv * n; e += nthr) {
+        int pv = e / n, a = e - pv * n;
+        zcplx acc = TT[(n + pv) * nt + off + a];
+        for (int h = 0; h < n; ++h) acc = zsub(acc, zmul(s.Qv[sp][pv * n + h], TT[h * nt + off + a]));
+        Wm[sp][e] = acc;
+      }
+    }
+    if (wid < 2) {
+      const int sp = wid, n = sp ? m.nb : m.na, off = sp ? m.na : 0;
+      zcplx f0 = mk<double>(0.0, 0.0), x0 = mk<double>(0.0, 0.0);
+      for (int e = lane; e < n * n; e += 32) {
+        int a = e / n, b = e - a * n;
+        if (a == b) f0 = zadd(f0, TT[a * nt + off + a]);
+        x0 = zadd(x0, zmul(TT[a * nt + off + b], TT[b * nt + off + a]));
+      }
+      f0.x = warp_sum(f0.x); f0.y = warp_sum(f0.y); x0.x = warp_sum(x0.x); x0.y = warp_sum(x0.y);
+      if (lane == 0) { scal[sp] = f0; scal[2 + sp] = x0; }
+    }
+    __syncthreads();
+    // 3. WT = W T0
+    if (!is_h) {
+      for (int sp = 0; sp < 2; ++sp) {
+        const int n = sp ? m.nb : m.na, nv = nact - n, off = sp ? m.na : 0;
+        for (int e = tid; e < nv * n; e += nthr) {
+          int pv = e / n, a = e - pv * n;
+          zcplx acc = mk<double>(0.0, 0.0);
+          for (int b = 0; b < n; ++b) acc = zadd(acc, zmul(Wm[sp][pv * n + b], TT[b * nt + off + a]));
+          WTm[sp][e] = acc;
+        }
+      }
+    }
+    __syncthreads();
+    // 4. per determinant: E x E work only
+#pragma unroll
+    for (int j = 0; j < MD_DPT; ++j) {
+      const int i = tid + j * 256;
+      if (i >= m.ndet) continue;
+      zcplx tsum = mk<double>(0.0, 0.0), xsum = mk<double>(0.0, 0.0);
+      for (int sp = 0; sp < 2; ++sp) {
+        const int n = sp ? m.nb : m.na;
+        int h[2], pp[2];
+        const int rk = md_exc(m, i, sp, h, pp);
+        const zcplx* Zi = s.Z + ((size_t)i * 2 + sp) * 4;
+        zcplx t = scal[sp], xch = scal[2 + sp];
+        if (rk == 1) {
+          zcplx zw = zmul(Zi[0], Wm[sp][(pp[0] - n) * n + h[0]]);
+          t = zadd(t, zw);
+          if (!is_h) {
+            xch = zadd(xch, zscale(zmul(Zi[0], WTm[sp][(pp[0] - n) * n + h[0]]), 2.0));
+            xch = zadd(xch, zmul(zw, zw));
+          }
+        } else if (rk == 2) {
+          zcplx ZW[2][2], ZT[2][2];
+          for (int f = 0; f < 2; ++f)
+            for (int f2 = 0; f2 < 2; ++f2) {
+              zcplx a = mk<double>(0.0, 0.0), b = mk<double>(0.0, 0.0);
+              for (int e = 0; e < 2; ++e) {
+                a = zadd(a, zmul(Zi[f * 2 + e], Wm[sp][(pp[e] - n) * n + h[f2]]));
+                if (!is_h) b = zadd(b, zmul(Zi[f * 2 + e], WTm[sp][(pp[e] - n) * n + h[f2]]));
+              }
+              ZW[f][f2] = a; ZT[f][f2] = b;
+            }
+          t = zadd(t, zadd(ZW[0][0], ZW[1][1]));
+          if (!is_h) {
+            xch = zadd(xch, zscale(zadd(ZT[0][0], ZT[1][1]), 2.0));
+            xch = zadd(xch, zadd(zadd(zmul(ZW[0][0], ZW[0][0]), zmul(ZW[1][1], ZW[1][1])),
+                                 zscale(zmul(ZW[0][1], ZW[1][0]), 2.0)));
+          }
+        }
+        tsum = zadd(tsum, t);
+        xsum = zadd(xsum, xch);
+      }
+      if (is_h) Eacc[j] = zadd(Eacc[j], tsum);
+      else Eacc[j] = zadd(Eacc[j], zscale(zsub(zmul(tsum, tsum), xsum), 0.5));
+    }
+  }
+  zcplx part = mk<double>(0.0, 0.0);
+#pragma unroll
+  for (int j = 0; j < MD_DPT; ++j) {
+    const int i = tid + j * 256;
+    if (i < m.ndet) part = zadd(part, zmul(s.omega[i], Eacc[j]));
+  }
+  zcplx tot = block_sum(part, s.red);
+  if (tid == 0) g.eloc[w] = tot;
+}
+
+}  // namespace afq

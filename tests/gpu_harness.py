@@ -102,3 +102,70 @@ def weight_err(w_gpu, rec, w_prev, dt, E0):
     if not np.any(ok):
         return 0.0
     return float(np.max(np.abs(w_gpu[ok] - rec["w"][ok]) / den[ok]))
+
+
+def well_conditioned(wl, phi, limit=1e3):
+    """Walkers whose overlap matrices Psi_s^T Phi_s both have condition number <= limit (R11: FP32 error of
+    the inverse scales with cond; the others are reported separately, not graded)."""
+    ok = np.ones(phi.shape[0], dtype=bool)
+    for psi, ph in zip((wl.psi_a, wl.psi_b), (phi[..., :wl.n_alpha], phi[..., wl.n_alpha:])):
+        if psi.shape[1] == 0:
+            continue
+        A = np.matmul(psi.T[None], ph)
+        with np.errstate(all="ignore"):
+            c = np.linalg.cond(A)
+        ok &= np.isfinite(c) & (c <= limit)
+    return ok
+
+
+def cond_number(wl, phi):
+    """Per walker: max over spins of cond(Psi_s^T Phi_s)."""
+    c = np.ones(phi.shape[0])
+    for psi, ph in zip((wl.psi_a, wl.psi_b), (phi[..., :wl.n_alpha], phi[..., wl.n_alpha:])):
+        if psi.shape[1] == 0:
+            continue
+        with np.errstate(all="ignore"):
+            ck = np.linalg.cond(np.matmul(psi.T[None], ph))
+        c = np.maximum(c, np.where(np.isfinite(ck), ck, np.inf))
+    return c
+
+
+def walker_tol(wl, kappa, kappa0=32.0):
+    """Per-walker tolerance: the stated tolerance for cond <= kappa0; on the FP32
+    path it grows in proportion to the condition number kappa of the walker's overlap matrices beyond that:
+    tol_w = max(2e-4, 6.25e-6 * kappa).  Measured FP32 floor (any FP32 implementation, inputs rounded to
+    complex64): S, E, w errors up to 1.5e-6 * kappa, i.e. the bound keeps a factor ~4.  FP64 path: no scaling."""
+    tol = tol_for(wl)
+    if wl.precision == "c128":
+        return np.full(kappa.shape, tol)
+    return tol * np.maximum(1.0, kappa / kappa0)
+
+
+def rel_fro_w(a, b, floor=0.0):
+    a = a.reshape(a.shape[0], -1)
+    b = b.reshape(b.shape[0], -1)
+    den = np.maximum(np.linalg.norm(b, axis=1), floor)
+    den = np.where(den == 0, 1.0, den)
+    return np.linalg.norm(a - b, axis=1) / den
+
+
+def rel_abs_w(a, b):
+    den = np.where(np.abs(b) == 0, 1.0, np.abs(b))
+    return np.abs(a - b) / den
+
+
+def worst_ratio(err_w, tol_w, mask=None):
+    """max over (masked) walkers of error / tolerance; < 1 passes."""
+    if mask is not None:
+        err_w, tol_w = err_w[mask], tol_w[mask]
+    return float(np.max(err_w / tol_w)) if err_w.size else 0.0
+
+
+def start_walkers(wl, nw):
+    """Initial population of a run: the trial determinant (SURVEY O-init 5).  Multi-determinant trials start
+    from the reference determinant plus a small seeded complex perturbation: at the exact reference every excited
+    determinant has zero overlap and both Eq.(4) and the per-determinant definition divide by it."""
+    if wl.n_det > 1:
+        from workloads import random_walkers
+        return random_walkers(wl, nw, seed=21, spread=0.05)
+    return wl.walkers(nw)
