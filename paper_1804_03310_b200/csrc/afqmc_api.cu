@@ -11,6 +11,7 @@
 
 #include "common.cuh"
 #include "gemm_simt.cuh"
+#include "gemm_tf32.cuh"
 #include "green.cuh"
 #include "misc.cuh"
 #include "multidet.cuh"
@@ -60,6 +61,7 @@ struct afqmc_ctx {
   int32_t* h_flags;
   // init staging (FP64)
   double *Ld, *hd, *hpd, *Rd, *hrotd, *ex[4], *psid;
+  tc::Maps map_asm, map_fb[2], map_en[2];   // TMA descriptors of the tcgen05 path (path == 2)
   char err[256];
   int64_t launches;
   // optional per-stage timing (afqmc_profile_enable)
@@ -149,7 +151,10 @@ afqmc_status check_params(const afqmc_params* p, char* err) {
       snprintf(err, 256, "multi-det working set exceeds one CTA's shared memory"); return AFQMC_EUNSUPPORTED;
     }
   }
-  if (p->gemm_path == 2) { snprintf(err, 256, "tcgen05 path not built yet"); return AFQMC_EUNSUPPORTED; }
+  if (p->gemm_path == 2 && (p->precision != 0 || p->n_det > 1)) {
+    snprintf(err, 256, "gemm_path 2 (tcgen05 3xTF32) needs precision 0 and a single-determinant trial");
+    return AFQMC_EUNSUPPORTED;
+  }
   int cw, nch;
   bool ok = p->precision ? taylor_pick<double>(p->M, p->n_alpha + p->n_beta, cw, nch)
                          : taylor_pick<float>(p->M, p->n_alpha + p->n_beta, cw, nch);
@@ -352,12 +357,29 @@ afqmc_status run_gemm(afqmc_ctx* c, const T* A, int lda, int m, const T* B, int 
   return AFQMC_OK;
 }
 
+template <class Epi>
+afqmc_status run_gemm_tc(afqmc_ctx* c, const tc::Maps& maps, int m, int n, int K, Epi epi) {
+  dim3 grid((n + tc::BN - 1) / tc::BN, (m + tc::BM - 1) / tc::BM);
+  auto kern = tc::k_gemm_tf32<Epi>;
+  LAUNCH(c, kern, grid, tc::THREADS, tc::SMEM_BYTES, maps, K, epi);
+  return AFQMC_OK;
+}
+
 // per-spin traces f^s_g = sum R^s_g[a][k] Theta_s[k][a] from the planar Theta in ctx->thp
 template <typename T> afqmc_status run_fb_gemm(afqmc_ctx* c) {
   StageScope sc(c, AFQMC_STAGE_FORCE_BIAS);
   for (int s = 0; s < 2; ++s) {
     int n = s ? c->cb : c->ca, soff = s ? c->KA : 0, Ks = s ? c->KB : c->KA;
     if (!n) continue;
+    if constexpr (sizeof(T) == 4) {
+      if (c->path == 2) {
+        tc::EpiStoreT e2;
+        e2.out = (float*)c->fs + (size_t)s * 2 * c->nw * c->NGP; e2.ldo = c->NGP; e2.m_real = c->ng; e2.n_real = 2 * c->nw;
+        afqmc_status st2 = run_gemm_tc(c, c->map_fb[s], c->ng, 2 * c->nw, Ks, e2);
+        if (st2) return st2;
+        continue;
+      }
+    }
     EpiStoreT<T> epi;
     epi.out = (T*)c->fs + (size_t)s * 2 * c->nw * c->NGP; epi.ldo = c->NGP; epi.m_real = c->ng; epi.n_real = 2 * c->nw;
     afqmc_status st = run_gemm<T>(c, (const T*)c->Rall + soff, c->KT, c->ng, (const T*)c->thp + soff, c->KT, 2 * c->nw, Ks, epi);
@@ -382,6 +404,16 @@ template <typename T> afqmc_status run_energy_gemm(afqmc_ctx* c, zcplx* eloc) {
   for (int s = 0; s < 2; ++s) {
     int n = s ? c->nb : c->na, soff = s ? c->KA : 0, Ks = s ? c->KB : c->KA;
     if (!n) continue;
+    if constexpr (sizeof(T) == 4) {
+      if (c->path == 2) {
+        tc::EpiEnergy e2;
+        e2.thp = (const float*)c->thp; e2.thp_lo = (const float*)c->thp_lo; e2.KT = c->KT; e2.soff = soff;
+        e2.hrot = (const float*)c->hrot + soff; e2.eloc = (double*)eloc; e2.m_real = c->M * n; e2.n_real = 2 * c->nw;
+        afqmc_status st2 = run_gemm_tc(c, c->map_en[s], c->M * n, 2 * c->nw, Ks, e2);
+        if (st2) return st2;
+        continue;
+      }
+    }
     EpiEnergy<T> epi;
     epi.thp = (const T*)c->thp; epi.thp_lo = (const T*)c->thp_lo; epi.KT = c->KT; epi.soff = soff;
     epi.hrot = (const T*)c->hrot + soff; epi.eloc = (double*)eloc; epi.m_real = c->M * n; epi.n_real = 2 * c->nw;
@@ -432,9 +464,20 @@ afqmc_status do_propagate(afqmc_ctx* c, void* phi, const void* x, const void* fb
   afqmc_status st;
   {
     StageScope sc(c, AFQMC_STAGE_ASSEMBLE);
+    bool done = false;
+    if constexpr (sizeof(T) == 4) {
+      if (c->path == 2) {
+        tc::EpiAssemble e2;
+        e2.out = (float*)c->Abuf; e2.M = c->M; e2.MP = c->MP; e2.m_real = c->M * c->M; e2.n_real = 2 * c->nw;
+        st = run_gemm_tc(c, c->map_asm, c->M * c->M, 2 * c->nw, c->NGP, e2);
+        done = true;
+      }
+    }
+    if (!done) {
     EpiAssemble<T> epi;
     epi.out = (T*)c->Abuf; epi.M = c->M; epi.MP = c->MP; epi.m_real = c->M * c->M; epi.n_real = 2 * c->nw;
     st = run_gemm<T>(c, (const T*)c->Lt, c->NGP, c->M * c->M, (const T*)c->Z, c->NGP, 2 * c->nw, c->NGP, epi);
+    }
   }
   if (st) return st;
   st = run_taylor<T>(c, phi);
@@ -514,7 +557,7 @@ afqmc_status afqmc_query_bytes(const afqmc_params* p, size_t* const_bytes, size_
   afqmc_ctx tmp;
   memset(&tmp, 0, sizeof(tmp));
   tmp.p = *p;
-  tmp.split = (p->gemm_path == 2);
+  tmp.split = (p->gemm_path == 2);   // auto resolves to SIMT (see afqmc_init)
   carve(p, &tmp, nullptr, nullptr, const_bytes, work_bytes);
   return AFQMC_OK;
 }
@@ -593,8 +636,8 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
   memset(c, 0, sizeof(*c));
   c->p = *p;
   c->stream = (cudaStream_t)stream;
-  c->path = 1;
-  c->split = 0;
+  c->path = p->gemm_path == 2 ? 2 : 1;
+  c->split = c->path == 2;
   size_t cb, wb;
   carve(p, c, (char*)const_mem, (char*)work_mem, &cb, &wb);
   if (p->precision) {
@@ -629,6 +672,37 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
     cudaError_t e = p->precision ? cudaFuncSetAttribute(k_green<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->green_smem)
                                  : cudaFuncSetAttribute(k_green<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->green_smem);
     if (e != cudaSuccess) { snprintf(g_init_err, 256, "CUDA: %s", cudaGetErrorString(e)); delete c; return AFQMC_ECUDA; }
+  }
+  if (c->path == 2 && c->nw > 0) {
+    using namespace tc;
+    bool ok = true;
+    const uint64_t nrow = 2 * (uint64_t)c->nw;
+    ok &= make_map(&c->map_asm.a_hi, c->Lt, c->NGP, (uint64_t)c->M * c->M, c->NGP, BM);
+    ok &= make_map(&c->map_asm.a_lo, c->Lt_lo, c->NGP, (uint64_t)c->M * c->M, c->NGP, BM);
+    ok &= make_map(&c->map_asm.b_hi, c->Z, c->NGP, nrow, c->NGP, BN);
+    ok &= make_map(&c->map_asm.b_lo, c->Z_lo, c->NGP, nrow, c->NGP, BN);
+    for (int sp = 0; sp < 2; ++sp) {
+      const int n = sp ? c->nb : c->na, soff = sp ? c->KA : 0, Ks = sp ? c->KB : c->KA;
+      if (!n) continue;
+      const float* R = (const float*)c->Rall + soff; const float* Rl = (const float*)c->Rall_lo + soff;
+      const float* th = (const float*)c->thp + soff; const float* thl = (const float*)c->thp_lo + soff;
+      ok &= make_map(&c->map_fb[sp].a_hi, R, Ks, c->ng, c->KT, BM);
+      ok &= make_map(&c->map_fb[sp].a_lo, Rl, Ks, c->ng, c->KT, BM);
+      ok &= make_map(&c->map_fb[sp].b_hi, th, Ks, nrow, c->KT, BN);
+      ok &= make_map(&c->map_fb[sp].b_lo, thl, Ks, nrow, c->KT, BN);
+      ok &= make_map(&c->map_en[sp].a_hi, c->Y[sp], Ks, (uint64_t)c->M * n, Ks, BM);
+      ok &= make_map(&c->map_en[sp].a_lo, c->Y_lo[sp], Ks, (uint64_t)c->M * n, Ks, BM);
+      c->map_en[sp].b_hi = c->map_fb[sp].b_hi;
+      c->map_en[sp].b_lo = c->map_fb[sp].b_lo;
+    }
+    cudaError_t e1 = cudaFuncSetAttribute(k_gemm_tf32<tc::EpiStoreT>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    cudaError_t e2 = cudaFuncSetAttribute(k_gemm_tf32<tc::EpiAssemble>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    cudaError_t e3 = cudaFuncSetAttribute(k_gemm_tf32<tc::EpiEnergy>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    if (!ok || e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) {
+      snprintf(g_init_err, 256, "tcgen05 path: tensor-map / shared-memory set-up failed");
+      delete c;
+      return AFQMC_ECUDA;
+    }
   }
   s = p->precision ? init_device<double>(c, h1, L_chol, psiT_a, psiT_b, C_act, det_coeff, exc2.data())
                    : init_device<float>(c, h1, L_chol, psiT_a, psiT_b, C_act, det_coeff, exc2.data());

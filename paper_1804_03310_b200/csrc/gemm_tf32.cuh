@@ -1,0 +1,259 @@
+// gemm_tf32.cuh -- tcgen05 / TMEM / TMA "NT" GEMM with the 3xTF32 operand split (sm_100a only).
+//   C[m][n] = sum_k A[m][k] B[n][k],  A = A_hi + A_lo, B = B_hi + B_lo (each plane exactly TF32),
+//   C ~= A_lo B_hi + A_hi B_lo + A_hi B_hi  accumulated in FP32 in TMEM (error ~ 2^-22, DESIGN.md
+//   "Precision split").  Operands are K-major FP32 planes in HBM, moved by TMA (128B swizzle) into a
+//   2-stage shared-memory ring; one elected thread issues tcgen05.mma.kind::tf32 (M=128, N=256, K=8);
+//   four epilogue warps read the 128 x 256 accumulator with tcgen05.ld and apply the fused epilogue.
+// Used for H4 (force bias), H6 (operator assembly), H9 (energy): PAPER.md:59, :80, :87.
+#pragma once
+#include <cuda.h>
+#include "common.cuh"
+
+namespace afq {
+namespace tc {
+
+enum { BM = 128, BN = 256, BK = 32, STAGES = 2, UMMA_K = 8, TMEM_COLS = 256, THREADS = 192 };
+enum { A_BYTES = BM * BK * 4, B_BYTES = BN * BK * 4, STAGE_BYTES = 2 * A_BYTES + 2 * B_BYTES };
+enum { SMEM_BYTES = STAGES * STAGE_BYTES + 1024 };
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n.reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+      ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
+      : "memory");
+}
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint64_t* bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
+               : "memory");
+}
+// D[tmem] (+)= A[smem] * B[smem], kind::tf32, one CTA
+__device__ __forceinline__ void umma_tf32(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
+      "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}"
+      ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc)
+      : "memory");
+}
+// K-major, SWIZZLE_128B shared-memory matrix descriptor (rows 128 B apart, 8-row atoms 1024 B apart)
+__device__ __forceinline__ uint64_t make_desc(uint32_t saddr) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr & 0x3FFFF) >> 4);          // start address, bits [0,14)
+  d |= (uint64_t)1 << 16;                           // leading byte offset (unused for swizzled K-major), bits [16,30)
+  d |= (uint64_t)(1024 >> 4) << 32;                 // stride byte offset = 1024 B, bits [32,46)
+  d |= (uint64_t)1 << 46;                           // descriptor version (sm_100)
+  d |= (uint64_t)2 << 61;                           // layout type SWIZZLE_128B
+  return d;
+}
+// instruction descriptor: FP32 accumulate, TF32 x TF32, both K-major, M x N
+__host__ __device__ constexpr uint32_t make_idesc(int M, int N) {
+  return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+// 32 lanes x 32 columns of FP32 accumulators -> 32 registers per thread (thread = TMEM lane)
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32]) {
+  uint32_t r[32];
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr));
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+  for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
+}
+
+struct Maps {
+  CUtensorMap a_hi, a_lo, b_hi, b_lo;   // 2-D {K, rows}, box {BK, BM} / {BK, BN}, SWIZZLE_128B
+};
+
+
+// ---- epilogues: called per epilogue thread with its accumulator row and 32 consecutive columns -------------
+struct EpiStoreT {      // H4: out[col][row]
+  float* out; int ldo, m_real, n_real;
+  __device__ __forceinline__ void operator()(int r, int c0, const float (&v)[32]) const {
+    if (r >= m_real) return;
+#pragma unroll
+    for (int j = 0; j < 32; ++j)
+      if (c0 + j < n_real) out[(size_t)(c0 + j) * ldo + r] = v[j];
+  }
+};
+struct EpiAssemble {    // H6: row = i*M + j, col = 2w + p -> A[w][i][p][MP] (+ j)
+  float* out; int M, MP, m_real, n_real;
+  __device__ __forceinline__ void operator()(int r, int c0, const float (&v)[32]) const {
+    if (r >= m_real) return;
+    const int ii = r / M, jj = r - ii * M;
+#pragma unroll
+    for (int j = 0; j < 32; ++j) {
+      const int c = c0 + j;
+      if (c < n_real) out[((size_t)(c >> 1) * M + ii) * (2 * MP) + (c & 1) * MP + jj] = v[j];
+    }
+  }
+};
+struct EpiEnergy {      // H9: eloc[w] += sum_rows v[row] (0.5 C[row][w] + hrot[row]), v = Theta plane (hi + lo)
+  const float* thp; const float* thp_lo; int KT, soff; const float* hrot; double* eloc; int m_real, n_real;
+  __device__ __forceinline__ void operator()(int r, int c0, const float (&v)[32]) const {
+    const bool rok = r < m_real;
+    const float hr = rok ? hrot[r] : 0.f;
+#pragma unroll
+    for (int j = 0; j < 32; j += 2) {
+      const int c = c0 + j;            // even: real plane of walker c/2
+      double er = 0.0, ei = 0.0;
+      if (rok && c < n_real) {
+        const size_t o = (size_t)c * KT + soff + r;
+        const float vr = thp[o] + thp_lo[o], vi = thp[o + KT] + thp_lo[o + KT];
+        const float ur = 0.5f * v[j] + hr, ui = 0.5f * v[j + 1];
+        er = (double)(vr * ur - vi * ui);
+        ei = (double)(vr * ui + vi * ur);
+      }
+      er = warp_sum(er); ei = warp_sum(ei);
+      if ((threadIdx.x & 31) == 0 && c < n_real) { atomicAdd(&eloc[c], er); atomicAdd(&eloc[c + 1], ei); }
+    }
+  }
+};
+
+template <class Epi>
+__global__ void __launch_bounds__(THREADS, 1) k_gemm_tf32(const __grid_constant__ Maps maps, int K, Epi epi) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  __shared__ __align__(8) uint64_t full_bar[STAGES];
+  __shared__ __align__(8) uint64_t empty_bar[STAGES];
+  __shared__ __align__(8) uint64_t tmem_full_bar;
+  __shared__ uint32_t tmem_base_s;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int m0 = blockIdx.y * BM, n0 = blockIdx.x * BN;
+  const int nkb = K / BK;
+
+  if (warp == 0 && lane == 0) {
+#pragma unroll
+    for (int s = 0; s < STAGES; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
+    mbar_init(&tmem_full_bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.a_hi) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.a_lo) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.b_hi) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.b_lo) : "memory");
+  }
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)),
+                 "r"((uint32_t)TMEM_COLS)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_base_s;
+
+  if (warp == 0) {
+    if (lane == 0) {   // ===== TMA producer =====
+      for (int kb = 0; kb < nkb; ++kb) {
+        const int s = kb % STAGES;
+        const uint32_t ph = (kb / STAGES) & 1;
+        mbar_wait(&empty_bar[s], ph ^ 1);
+        uint8_t* st = smem + (size_t)s * STAGE_BYTES;
+        mbar_expect_tx(&full_bar[s], STAGE_BYTES);
+        tma_load_2d(st, &maps.a_hi, &full_bar[s], kb * BK, m0);
+        tma_load_2d(st + A_BYTES, &maps.a_lo, &full_bar[s], kb * BK, m0);
+        tma_load_2d(st + 2 * A_BYTES, &maps.b_hi, &full_bar[s], kb * BK, n0);
+        tma_load_2d(st + 2 * A_BYTES + B_BYTES, &maps.b_lo, &full_bar[s], kb * BK, n0);
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {   // ===== MMA issuer =====
+      constexpr uint32_t idesc = make_idesc(BM, BN);
+      for (int kb = 0; kb < nkb; ++kb) {
+        const int s = kb % STAGES;
+        const uint32_t ph = (kb / STAGES) & 1;
+        mbar_wait(&full_bar[s], ph);
+        tc_fence_after();
+        const uint32_t sa = smem_u32(smem + (size_t)s * STAGE_BYTES);
+        const uint64_t a_hi = make_desc(sa), a_lo = make_desc(sa + A_BYTES);
+        const uint64_t b_hi = make_desc(sa + 2 * A_BYTES), b_lo = make_desc(sa + 2 * A_BYTES + B_BYTES);
+#pragma unroll
+        for (int k = 0; k < BK / UMMA_K; ++k) {
+          const uint64_t adv = (uint64_t)((k * UMMA_K * 4) >> 4);
+          umma_tf32(tmem, a_lo + adv, b_hi + adv, idesc, (kb | k) ? 1u : 0u);
+          umma_tf32(tmem, a_hi + adv, b_lo + adv, idesc, 1u);
+          umma_tf32(tmem, a_hi + adv, b_hi + adv, idesc, 1u);
+        }
+        tc_commit(&empty_bar[s]);                    // frees the stage once these MMAs have read it
+        if (kb == nkb - 1) tc_commit(&tmem_full_bar);
+      }
+    }
+  } else {             // ===== epilogue warps 2..5: TMEM lane quarter = warp % 4 =====
+    const int q = warp & 3;
+    mbar_wait(&tmem_full_bar, 0);
+    tc_fence_after();
+    const int row = m0 + q * 32 + lane;
+#pragma unroll 1
+    for (int cb = 0; cb < BN / 32; ++cb) {
+      float v[32];
+      tmem_ld32(tmem + ((uint32_t)(q * 32) << 16) + cb * 32, v);
+      epi(row, n0 + cb * 32, v);
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    __syncwarp();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"((uint32_t)TMEM_COLS) : "memory");
+  }
+}
+
+// ---- host: tensor maps ------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+inline EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  return fn;
+}
+
+// K-major FP32 plane [rows][ld], logical extent {K, rows}; box {BK, box_rows}; out-of-range rows read as 0
+inline bool make_map(CUtensorMap* m, const void* base, uint64_t K, uint64_t rows, uint64_t ld, uint32_t box_rows) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn) return false;
+  cuuint64_t dims[2] = {K, rows};
+  cuuint64_t strides[1] = {ld * 4};
+  cuuint32_t box[2] = {BK, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void*>(base), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+}  // namespace tc
+}  // namespace afq

@@ -169,3 +169,11 @@ def start_walkers(wl, nw):
         from workloads import random_walkers
         return random_walkers(wl, nw, seed=21, spread=0.05)
     return wl.walkers(nw)
+
+
+def energy_err_w(e_gpu, e_ora, f_ora):
+    """|E - E_ora| / max(|E_ora|, 1/2 ||f_ora||^2): E_L is a sum of terms of size 1/2 sum_g |f_g|^2 that partly
+    cancel, so the error is measured against the largest of them (same idea as the weight metric, R11)."""
+    den = np.maximum(np.abs(e_ora), 0.5 * np.sum(np.abs(f_ora) ** 2, axis=-1))
+    den = np.where(den == 0, 1.0, den)
+    return np.abs(e_gpu - e_ora) / den

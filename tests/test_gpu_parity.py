@@ -129,7 +129,7 @@ def _protocol_A(wl, nw, steps, gemm_path=0):
         den_w = np.where(den_w > 0, den_w, 1.0)
         errs = dict(S0=H.rel_abs_w(g0["S"], ost.S), f_used=H.rel_fro_w(g0["f"], rec["f_used"], floor),
                     phi=H.rel_fro_w(out["phi"], rec["phi"]), S=H.rel_abs_w(out["S"], rec["S"]),
-                    f=H.rel_fro_w(out["f"], rec["f"], floor), E=H.rel_abs_w(eloc, rec["eloc"]),
+                    f=H.rel_fro_w(out["f"], rec["f"], floor), E=H.energy_err_w(eloc, rec["eloc"], rec["f"]),
                     w=np.abs(out["w"] - rec["w"]) / den_w)
         # a dead/alive flip is accepted iff |cos dtheta|_ora < tolerance of that walker
         flip = ((out["w"] == 0) != (rec["w"] == 0)) & ok
@@ -189,7 +189,7 @@ def test_protocol_B_free_running_alive(cfg, variant):
         alive = (recs[n]["w"] > 0) & np.isfinite(kappa)
         n_alive.append(int(alive.sum()))
         if np.any(alive):
-            e = H.rel_abs_w(eloc[n], recs[n]["eloc"])
+            e = H.energy_err_w(eloc[n], recs[n]["eloc"], recs[n]["f"])
             worstE = max(worstE, H.worst_ratio(e, (n + 1) * H.walker_tol(wl, kappa), alive))
             rawE = max(rawE, float(np.max(e[alive])))
     alive = (ost.w > 0) & np.isfinite(kappa)
@@ -285,3 +285,39 @@ def test_singular_walker_sets_flag():
     out = st.host()
     assert out["flags"][2] & 1
     assert np.all(out["flags"][[0, 1, 3]] == 0)
+
+
+# ---- tcgen05 3xTF32 contraction path (gemm_path = 2): same oracle, same tolerances -------------------------
+@pytest.mark.parametrize("cfg", [2, 3, 5])
+def test_tcgen05_stage_forcebias_energy_propagate(cfg):
+    import torch
+    wl = _wl(cfg)
+    nw = {2: 200, 3: 136, 5: 6}[cfg]      # ragged against the 256-column tile (2 nw = 400 / 272 / 12)
+    tol = H.tol_for(wl)
+    ini, _ = H.oracle_init(wl)
+    phi = random_walkers(wl, nw, seed=5, spread=0.1)
+    ctx = H.make_ctx(wl, nw, gemm_path=2)
+    assert ctx.gemm_path == 2
+    st = H.DeviceState(ctx, phi)
+    st.seed()
+    eloc = torch.zeros(nw, dtype=torch.complex128, device=ctx.device)
+    ctx.afqmc_local_energy(st.phi, st.theta, eloc)
+    g0 = st.host()
+    ost = orc.o_seed_state(ini, phi, wl.n_alpha)
+    x = wl.fields(1, nw)[0]
+    new, rec = orc.o_step(ini, ost, x, wl.n_alpha, K=wl.K, E0=wl.E0)
+    xd = torch.tensor(x, dtype=ctx.rdtype, device=ctx.device)
+    ctx.afqmc_propagate(st.phi, xd, st.fb, st.ovlp, st.weight, st.theta, None, st.flags)
+    out = st.host()
+    errs = dict(f=H.rel_fro(g0["f"], ost.f_a + ost.f_b), E=H.rel_abs(eloc.cpu().numpy(), ost.eloc),
+                phi=H.rel_fro(out["phi"], rec["phi"]), S=H.rel_abs(out["S"], rec["S"]),
+                w=H.weight_err(out["w"], rec, ost.w, wl.dt, wl.E0))
+    print(f"cfg{cfg} tcgen05 3xTF32 stage errors: {errs}")
+    for k, v in errs.items():
+        assert v < tol, (k, v)
+
+
+@pytest.mark.parametrize("cfg,variant", [(3, "mf"), (5, "mf")])
+def test_protocol_A_resync_tcgen05(cfg, variant):
+    wl = _wl(cfg, variant)
+    _protocol_A(wl, SMALL[cfg], {5: 3}.get(cfg, 10), gemm_path=2)
