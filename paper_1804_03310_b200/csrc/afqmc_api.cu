@@ -125,6 +125,12 @@ struct Layout {
   size_t const_bytes, work_bytes;
 };
 
+// gemm_path 0 (auto): tcgen05 3xTF32 wherever it exists (complex64, single determinant), else SIMT
+int resolve_path(const afqmc_params* p) {
+  if (p->gemm_path) return p->gemm_path;
+  return (p->precision == 0 && p->n_det == 1) ? 2 : 1;
+}
+
 afqmc_status check_params(const afqmc_params* p, char* err) {
   if (!p) { snprintf(err, 256, "params is NULL"); return AFQMC_EINVAL; }
   if (p->M < 1 || p->n_alpha < 1 || p->n_beta < 0 || p->n_chol < 1 || p->n_walkers < 0 ||
@@ -557,7 +563,7 @@ afqmc_status afqmc_query_bytes(const afqmc_params* p, size_t* const_bytes, size_
   afqmc_ctx tmp;
   memset(&tmp, 0, sizeof(tmp));
   tmp.p = *p;
-  tmp.split = (p->gemm_path == 2);   // auto resolves to SIMT (see afqmc_init)
+  tmp.split = resolve_path(p) == 2;
   carve(p, &tmp, nullptr, nullptr, const_bytes, work_bytes);
   return AFQMC_OK;
 }
@@ -636,7 +642,7 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
   memset(c, 0, sizeof(*c));
   c->p = *p;
   c->stream = (cudaStream_t)stream;
-  c->path = p->gemm_path == 2 ? 2 : 1;
+  c->path = resolve_path(p);
   c->split = c->path == 2;
   size_t cb, wb;
   carve(p, c, (char*)const_mem, (char*)work_mem, &cb, &wb);

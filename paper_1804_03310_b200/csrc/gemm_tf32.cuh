@@ -12,7 +12,12 @@
 namespace afq {
 namespace tc {
 
-enum { BM = 128, BN = 256, BK = 32, STAGES = 2, UMMA_K = 8, TMEM_COLS = 256, THREADS = 192 };
+enum { BM = 128, BN = 256, BK = 32, STAGES = 2, UMMA_K = 8, TMEM_COLS = 512, THREADS = 320 };
+// The tensor pipe adds into its FP32 accumulator with truncation, so the error of one long accumulation grows
+// linearly with K (measured 6.4e-9 per K element: 1.7e-5 at K = 2600).  The accumulation is therefore cut into
+// chunks of CHUNK_KB k-blocks (128 K elements); each chunk lands in one of two TMEM buffers and is added to a
+// running FP32 sum in registers (round-to-nearest) by the epilogue warps while the next chunk is being issued.
+enum { CHUNK_KB = 4, EPI_WARPS = 8, COLS_PER_WARP = BN / 2 };
 enum { A_BYTES = BM * BK * 4, B_BYTES = BN * BK * 4, STAGE_BYTES = 2 * A_BYTES + 2 * B_BYTES };
 enum { SMEM_BYTES = STAGES * STAGE_BYTES + 1024 };
 
@@ -142,23 +147,26 @@ __global__ void __launch_bounds__(THREADS, 1) k_gemm_tf32(const __grid_constant_
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   __shared__ __align__(8) uint64_t full_bar[STAGES];
   __shared__ __align__(8) uint64_t empty_bar[STAGES];
-  __shared__ __align__(8) uint64_t tmem_full_bar;
+  __shared__ __align__(8) uint64_t tmem_full_bar[2];
+  __shared__ __align__(8) uint64_t tmem_empty_bar[2];
   __shared__ uint32_t tmem_base_s;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int m0 = blockIdx.y * BM, n0 = blockIdx.x * BN;
   const int nkb = K / BK;
+  const int nchunk = (nkb + CHUNK_KB - 1) / CHUNK_KB;
 
-  if (warp == 0 && lane == 0) {
+  if (warp == EPI_WARPS && lane == 0) {
 #pragma unroll
     for (int s = 0; s < STAGES; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
-    mbar_init(&tmem_full_bar, 1);
+#pragma unroll
+    for (int b = 0; b < 2; ++b) { mbar_init(&tmem_full_bar[b], 1); mbar_init(&tmem_empty_bar[b], EPI_WARPS); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.a_hi) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.a_lo) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.b_hi) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.b_lo) : "memory");
   }
-  if (warp == 1) {
+  if (warp == EPI_WARPS + 1) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)),
                  "r"((uint32_t)TMEM_COLS)
                  : "memory");
@@ -169,7 +177,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_gemm_tf32(const __grid_constant_
   tc_fence_after();
   const uint32_t tmem = tmem_base_s;
 
-  if (warp == 0) {
+  if (warp == EPI_WARPS) {
     if (lane == 0) {   // ===== TMA producer =====
       for (int kb = 0; kb < nkb; ++kb) {
         const int s = kb % STAGES;
@@ -183,43 +191,68 @@ __global__ void __launch_bounds__(THREADS, 1) k_gemm_tf32(const __grid_constant_
         tma_load_2d(st + 2 * A_BYTES + B_BYTES, &maps.b_lo, &full_bar[s], kb * BK, n0);
       }
     }
-  } else if (warp == 1) {
+  } else if (warp == EPI_WARPS + 1) {
     if (lane == 0) {   // ===== MMA issuer =====
       constexpr uint32_t idesc = make_idesc(BM, BN);
       for (int kb = 0; kb < nkb; ++kb) {
         const int s = kb % STAGES;
         const uint32_t ph = (kb / STAGES) & 1;
+        const int ci = kb / CHUNK_KB, buf = ci & 1;
+        const bool chunk_start = (kb % CHUNK_KB) == 0;
+        if (chunk_start) {   // the epilogue must have drained this TMEM buffer
+          mbar_wait(&tmem_empty_bar[buf], ((ci >> 1) & 1) ^ 1);
+          tc_fence_after();
+        }
         mbar_wait(&full_bar[s], ph);
         tc_fence_after();
+        const uint32_t d = tmem + buf * BN;
         const uint32_t sa = smem_u32(smem + (size_t)s * STAGE_BYTES);
         const uint64_t a_hi = make_desc(sa), a_lo = make_desc(sa + A_BYTES);
         const uint64_t b_hi = make_desc(sa + 2 * A_BYTES), b_lo = make_desc(sa + 2 * A_BYTES + B_BYTES);
 #pragma unroll
         for (int k = 0; k < BK / UMMA_K; ++k) {
           const uint64_t adv = (uint64_t)((k * UMMA_K * 4) >> 4);
-          umma_tf32(tmem, a_lo + adv, b_hi + adv, idesc, (kb | k) ? 1u : 0u);
-          umma_tf32(tmem, a_hi + adv, b_lo + adv, idesc, 1u);
-          umma_tf32(tmem, a_hi + adv, b_hi + adv, idesc, 1u);
+          umma_tf32(d, a_lo + adv, b_hi + adv, idesc, (chunk_start && k == 0) ? 0u : 1u);
+          umma_tf32(d, a_hi + adv, b_lo + adv, idesc, 1u);
+          umma_tf32(d, a_hi + adv, b_hi + adv, idesc, 1u);
         }
         tc_commit(&empty_bar[s]);                    // frees the stage once these MMAs have read it
-        if (kb == nkb - 1) tc_commit(&tmem_full_bar);
+        if ((kb % CHUNK_KB) == CHUNK_KB - 1 || kb == nkb - 1) tc_commit(&tmem_full_bar[buf]);
       }
     }
-  } else {             // ===== epilogue warps 2..5: TMEM lane quarter = warp % 4 =====
-    const int q = warp & 3;
-    mbar_wait(&tmem_full_bar, 0);
-    tc_fence_after();
+  } else {             // ===== epilogue warps 0..7: TMEM lane quarter = warp % 4, column half = warp / 4 =====
+    const int q = warp & 3, half = warp >> 2;
     const int row = m0 + q * 32 + lane;
-#pragma unroll 1
-    for (int cb = 0; cb < BN / 32; ++cb) {
+    float acc[COLS_PER_WARP];
+#pragma unroll
+    for (int i = 0; i < COLS_PER_WARP; ++i) acc[i] = 0.f;
+    for (int ci = 0; ci < nchunk; ++ci) {
+      const int buf = ci & 1;
+      mbar_wait(&tmem_full_bar[buf], (ci >> 1) & 1);
+      tc_fence_after();
+      const uint32_t t0 = tmem + ((uint32_t)(q * 32) << 16) + buf * BN + half * COLS_PER_WARP;
+#pragma unroll
+      for (int cb = 0; cb < COLS_PER_WARP / 32; ++cb) {
+        float v[32];
+        tmem_ld32(t0 + cb * 32, v);
+#pragma unroll
+        for (int j = 0; j < 32; ++j) acc[cb * 32 + j] += v[j];
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&tmem_empty_bar[buf])) : "memory");
+    }
+#pragma unroll
+    for (int cb = 0; cb < COLS_PER_WARP / 32; ++cb) {
       float v[32];
-      tmem_ld32(tmem + ((uint32_t)(q * 32) << 16) + cb * 32, v);
-      epi(row, n0 + cb * 32, v);
+#pragma unroll
+      for (int j = 0; j < 32; ++j) v[j] = acc[cb * 32 + j];
+      epi(row, n0 + half * COLS_PER_WARP + cb * 32, v);
     }
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 1) {
+  if (warp == EPI_WARPS + 1) {
     __syncwarp();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"((uint32_t)TMEM_COLS) : "memory");
   }
