@@ -52,8 +52,10 @@ def test_query_bytes_and_argument_errors(afq):
     p = afq.make_params(200, 13, 12, 1000, 2048, "c64", 0.005)
     cb, wb = afq.afqmc_query_bytes(p)
     assert cb % 256 == 0 and wb % 256 == 0
-    # L^T (160 MB) + R (20 MB) + Y (2624^2 + 2400^2 floats) dominate the constants
-    assert 2.0e8 < cb < 3.0e8 and wb > 2048 * 200 * 200 * 8
+    # L^T (160 MB) + R (20 MB) + Y (2624^2 + 2400^2 floats) dominate the constants; x2 for the TF32 hi/lo planes
+    assert 4.0e8 < cb < 5.0e8 and wb > 2048 * 200 * 200 * 8
+    cb1, _ = afq.afqmc_query_bytes(afq.make_params(200, 13, 12, 1000, 2048, "c64", 0.005, gemm_path=1))
+    assert 2.0e8 < cb1 < 3.0e8
     bad = [afq.make_params(0, 1, 1, 4, 4, "c64", 0.01), afq.make_params(8, 9, 1, 4, 4, "c64", 0.01),
            afq.make_params(8, 2, 2, 4, 4, "c64", -1.0), afq.make_params(8, 2, 2, 4, 4, "c64", 0.01, taylor_order=0),
            afq.make_params(8, 2, 2, 4, 4, "c64", 0.01, n_det=3, n_act=1)]
