@@ -161,7 +161,8 @@ def run_ours(args):
     ctx = afq.AfqmcContext(p, wl.h, wl.L, wl.psi_a, wl.psi_b, device=f"cuda:{local}", **kw)
     dev = ctx.device
     # fields: every rank its own seed (replicas are independent); a fresh draw per step, resident in HBM
-    rng = np.random.default_rng(1000 + rank)
+    from paper_1804_03310_b200 import dist as D
+    rng = np.random.default_rng(D.rank_seed(1000, rank))
     nfield = min(K, 8)
     x = torch.tensor(rng.standard_normal((nfield, nw, wl.n_chol)), dtype=ctx.rdtype, device=dev)
     phi0 = torch.tensor(wl.walkers(nw), dtype=ctx.cdtype, device=dev)
@@ -203,11 +204,9 @@ def run_ours(args):
     prof = ctx.afqmc_profile_read()
     ctx.afqmc_profile_enable(False)
     clocks = sampler.stop() if sampler else None
-    tmax = torch.tensor([ms], dtype=torch.float64, device=dev)
     if world > 1:
         dist.barrier()
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms_max = float(tmax.item())
+    ms_max = D.max_over_ranks(ms, dev)
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----
     Ke = min(K, 4)
@@ -226,10 +225,7 @@ def run_ours(args):
     t0 = time.perf_counter()
     up, down = ctx.afqmc_step_host(phi_h, w_h, S_h, x_h, Ke, e_h, f_h)   # synchronises internally
     t_e2e = time.perf_counter() - t0
-    te = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    t_e2e = float(te.item())
+    t_e2e = D.max_over_ranks(t_e2e, dev)
 
     if rank != 0:
         if world > 1:
@@ -237,7 +233,7 @@ def run_ours(args):
         return
     pk = peaks()
     fl = flops_per_walker_step(wl)
-    value = world * nw * K / (ms_max * 1e-3)
+    value = D.whole_job_rate(nw * K, world, ms_max * 1e-3)
     # dominant kernel: the one-body-operator assembly GEMM (H6)
     a_ms, a_n = prof["assemble"]
     a_flops = fl["assemble"] * nw

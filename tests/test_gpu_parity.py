@@ -321,3 +321,29 @@ def test_tcgen05_stage_forcebias_energy_propagate(cfg):
 def test_protocol_A_resync_tcgen05(cfg, variant):
     wl = _wl(cfg, variant)
     _protocol_A(wl, SMALL[cfg], {5: 3}.get(cfg, 10), gemm_path=2)
+
+
+def test_full_size_sampled_walkers():
+    """bench.py's launch configuration (cfg 5, all 2048 walkers, default contraction path): two free-running steps,
+    compared on sampled walkers the oracle recomputes one by one (walkers are independent)."""
+    wl = _wl(5, "mf")
+    nw, steps = wl.n_walkers, 2
+    tol = H.tol_for(wl)
+    ini, _ = H.oracle_init(wl)
+    xs = wl.fields(steps, nw)
+    ctx = H.make_ctx(wl, nw)
+    st = H.DeviceState(ctx, wl.walkers(nw))
+    st.seed()
+    eloc = st.step(xs)
+    out = st.host()
+    idx = np.array([0, 1, 255, 256, 1023, 1531, 2046, 2047])
+    ost = orc.o_seed_state(ini, wl.walkers(nw)[idx], wl.n_alpha)
+    for n in range(steps):
+        ost, rec = orc.o_step(ini, ost, xs[n][idx], wl.n_alpha, K=wl.K, E0=wl.E0)
+    errs = dict(phi=H.rel_fro(out["phi"][idx], ost.phi), S=H.rel_abs(out["S"][idx], ost.S),
+                w=H.rel_abs(out["w"][idx], ost.w), f=H.rel_fro(out["f"][idx], ost.f_a + ost.f_b),
+                E=H.rel_abs(eloc[-1][idx], rec["eloc"]))
+    print(f"cfg5 full size (path {ctx.gemm_path}), sampled walkers: {errs}")
+    assert np.all(np.isfinite(out["phi"].view(np.float64)))
+    for k, v in errs.items():
+        assert v < tol, (k, v)
