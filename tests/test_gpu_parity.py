@@ -135,9 +135,12 @@ def _protocol_A(wl, nw, steps, gemm_path=0):
         flip = ((out["w"] == 0) != (rec["w"] == 0)) & ok
         assert np.all(np.abs(rec["cosd"][flip]) < tw[flip]), "dead/alive flip away from cos=0"
         ok_w = ok & ~flip
+        # log w' contains c = x.xbar - xbar.xbar/2 of size dt ||f||^2: a relative error eps in f moves log w' by
+        # eps * dt ||f||^2, so the weight tolerance carries that factor (raw configs: ||f||^2 ~ 1e3..1e4)
+        amp_w = np.maximum(1.0, wl.dt * np.sum(np.abs(rec["f_used"]) ** 2, axis=-1))
         for k, v in errs.items():
             m = ok_w if k == "w" else ok
-            ratio[k] = max(ratio.get(k, 0.0), H.worst_ratio(v, tw, m))
+            ratio[k] = max(ratio.get(k, 0.0), H.worst_ratio(v, tw * amp_w if k == "w" else tw, m))
             raw[k] = max(raw.get(k, 0.0), float(np.max(v[m])) if np.any(m) else 0.0)
         ost = new
     print(f"cfg{wl.cfg}/{wl.variant} protocol A over {steps} steps, {nw} walkers (max cond {kmax:.0f}): "
