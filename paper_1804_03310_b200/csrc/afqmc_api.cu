@@ -16,6 +16,7 @@
 #include "misc.cuh"
 #include "multidet.cuh"
 #include "taylor.cuh"
+#include "taylor_tc.cuh"
 
 using namespace afq;
 
@@ -61,7 +62,8 @@ struct afqmc_ctx {
   int32_t* h_flags;
   // init staging (FP64)
   double *Ld, *hd, *hpd, *Rd, *hrotd, *ex[4], *psid;
-  tc::Maps map_asm, map_fb[2], map_en[2];   // TMA descriptors of the tcgen05 path (path == 2)
+  tc::Maps map_asm, map_fb[2], map_en[2];
+  int tay_tc; void *Abuf_lo, *Eh_lo; tt::TaylorMaps map_tay; tt::TaylorTcArgs tay_args; size_t tay_tc_smem; int n_sm;   // TMA descriptors of the tcgen05 path (path == 2)
   char err[256];
   int64_t launches;
   // optional per-stage timing (afqmc_profile_enable)
@@ -187,6 +189,7 @@ void carve(const afqmc_params* p, afqmc_ctx* c, char* cbase, char* wbase, size_t
   c->psi_a = cc.take((size_t)M * na * ts);
   c->psi_b = cc.take((size_t)M * (nb ? nb : 1) * ts);
   c->Eh = cc.take((size_t)M * MP * ts);
+  c->Eh_lo = split ? cc.take((size_t)M * MP * ts) : nullptr;
   c->Lt = cc.take((size_t)M * M * NGP * ts);
   c->Lt_lo = split ? cc.take((size_t)M * M * NGP * ts) : nullptr;
   c->Rall = cc.take((size_t)rup(ng, 128) * KT * ts);
@@ -207,6 +210,7 @@ void carve(const afqmc_params* p, afqmc_ctx* c, char* cbase, char* wbase, size_t
   c->Z = w.take(2 * nw1 * NGP * ts);
   c->Z_lo = split ? w.take(2 * nw1 * NGP * ts) : nullptr;
   c->Abuf = w.take(nw1 * M * 2 * MP * ts);
+  c->Abuf_lo = split ? w.take(nw1 * M * 2 * MP * ts) : nullptr;
   c->thp = w.take(2 * nw1 * KT * ts);
   c->thp_lo = split ? w.take(2 * nw1 * KT * ts) : nullptr;
   c->fs = w.take(2 * 2 * nw1 * NGP * ts);
@@ -283,6 +287,8 @@ template <typename T> afqmc_status init_device(afqmc_ctx* c, const double* h1, c
     double* t = E; E = Tm; Tm = t;
   }
   LAUNCH(c, k_cast2d<T>, (mm + 127) / 128, 128, 0, M, M, E, (size_t)M, (T*)c->Eh, (T*)nullptr, (size_t)MP, 0);
+  if (c->tay_tc)   // TF32 hi / lo planes of E_h for the tensor-pipe Taylor kernel (the SIMT kernel never runs then)
+    LAUNCH(c, k_cast2d<T>, (mm + 127) / 128, 128, 0, M, M, E, (size_t)M, (T*)c->Eh, (T*)c->Eh_lo, (size_t)MP, 1);
   // trial orbitals in T
   LAUNCH(c, k_cast2d<T>, (M * na + 127) / 128, 128, 0, M, na, psid_a, (size_t)na, (T*)c->psi_a, (T*)nullptr, (size_t)na, 0);
   if (nb) LAUNCH(c, k_cast2d<T>, (M * nb + 127) / 128, 128, 0, M, nb, psid_b, (size_t)nb, (T*)c->psi_b, (T*)nullptr, (size_t)nb, 0);
@@ -434,6 +440,15 @@ template <typename T> afqmc_status run_taylor(afqmc_ctx* c, void* phi) {
   g.M = c->M; g.MP = c->MP; g.nt = c->nt; g.K = c->p.taylor_order; g.nchunks = c->tay_nch;
   g.phi = (cplx<T>*)phi; g.A = (const T*)c->Abuf; g.Eh = (const T*)c->Eh;
   StageScope sc(c, AFQMC_STAGE_TAYLOR);
+  if constexpr (sizeof(T) == 4) {
+    if (c->tay_tc) {
+      tt::TaylorTcArgs a = c->tay_args;
+      a.phi = (cplx<float>*)phi;
+      const int grid = c->nw < c->n_sm ? c->nw : c->n_sm;
+      LAUNCH(c, tt::k_taylor_tc, grid, tt::NTHREADS, c->tay_tc_smem, c->map_tay, a);
+      return AFQMC_OK;
+    }
+  }
 #define TAY_CASE(CW)                                                                                        \
   case CW: {                                                                                                \
     constexpr int MT = sizeof(T) == 4 ? (((CW + 3) & ~3) >= 16 ? 448 : ((CW + 3) & ~3) >= 12 ? 576 : ((CW + 3) & ~3) >= 8 ? 768 : 1024) \
@@ -474,7 +489,7 @@ afqmc_status do_propagate(afqmc_ctx* c, void* phi, const void* x, const void* fb
     if constexpr (sizeof(T) == 4) {
       if (c->path == 2) {
         tc::EpiAssemble e2;
-        e2.out = (float*)c->Abuf; e2.M = c->M; e2.MP = c->MP; e2.m_real = c->M * c->M; e2.n_real = 2 * c->nw;
+        e2.out = (float*)c->Abuf; e2.out_lo = c->tay_tc ? (float*)c->Abuf_lo : nullptr; e2.M = c->M; e2.MP = c->MP; e2.m_real = c->M * c->M; e2.n_real = 2 * c->nw;
         st = run_gemm_tc(c, c->map_asm, c->M * c->M, 2 * c->nw, c->NGP, e2);
         done = true;
       }
@@ -678,6 +693,33 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
     cudaError_t e = p->precision ? cudaFuncSetAttribute(k_green<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->green_smem)
                                  : cudaFuncSetAttribute(k_green<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->green_smem);
     if (e != cudaSuccess) { snprintf(g_init_err, 256, "CUDA: %s", cudaGetErrorString(e)); delete c; return AFQMC_ECUDA; }
+  }
+  c->tay_tc = (c->path == 2 && c->M <= 256 && c->nt <= 32 && c->nw > 0);
+  if (c->tay_tc) {
+    tt::TaylorTcArgs& a = c->tay_args;
+    a.M = c->M; a.MP = c->MP; a.nt = c->nt; a.K = p->taylor_order; a.nw = c->nw;
+    a.mtiles = (c->M + 127) / 128;
+    a.rows_last = (int)rup((size_t)(c->M - 128 * (a.mtiles - 1)), 8);
+    a.nkb = (c->M + 31) / 32;
+    a.phi = nullptr;
+    c->tay_tc_smem = tt::smem_bytes(a.nkb);
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
+    bool ok = true;
+    for (int hl = 0; hl < 2; ++hl)
+      for (int v = 0; v < 2; ++v) {
+        const uint32_t rows = v ? (uint32_t)a.rows_last : 128u;
+        ok &= tc::make_map(&c->map_tay.A[hl][v], hl ? c->Abuf_lo : c->Abuf, 2 * (uint64_t)c->MP, (uint64_t)c->nw * c->M,
+                           2 * (uint64_t)c->MP, rows);
+        ok &= tc::make_map(&c->map_tay.E[hl][v], hl ? c->Eh_lo : c->Eh, (uint64_t)c->MP, (uint64_t)c->M, (uint64_t)c->MP, rows);
+      }
+    cudaError_t e0 = cudaFuncSetAttribute(tt::k_taylor_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tay_tc_smem);
+    if (!ok || e0 != cudaSuccess || c->n_sm <= 0) {
+      snprintf(g_init_err, 256, "tensor-pipe Taylor kernel: tensor-map / shared-memory set-up failed");
+      delete c;
+      return AFQMC_ECUDA;
+    }
   }
   if (c->path == 2 && c->nw > 0) {
     using namespace tc;

@@ -107,15 +107,24 @@ struct EpiStoreT {      // H4: out[col][row]
       if (c0 + j < n_real) out[(size_t)(c0 + j) * ldo + r] = v[j];
   }
 };
-struct EpiAssemble {    // H6: row = i*M + j, col = 2w + p -> A[w][i][p][MP] (+ j)
-  float* out; int M, MP, m_real, n_real;
+struct EpiAssemble {    // H6: row = i*M + j, col = 2w + p -> A[w][i][p][MP] (+ j); out_lo != null: TF32 hi / lo planes
+  float* out; float* out_lo; int M, MP, m_real, n_real;
   __device__ __forceinline__ void operator()(int r, int c0, const float (&v)[32]) const {
     if (r >= m_real) return;
     const int ii = r / M, jj = r - ii * M;
 #pragma unroll
     for (int j = 0; j < 32; ++j) {
       const int c = c0 + j;
-      if (c < n_real) out[((size_t)(c >> 1) * M + ii) * (2 * MP) + (c & 1) * MP + jj] = v[j];
+      if (c < n_real) {
+        const size_t o = ((size_t)(c >> 1) * M + ii) * (2 * MP) + (c & 1) * MP + jj;
+        if (out_lo) {
+          float hi, lo;
+          tf32_split(v[j], hi, lo);
+          out[o] = hi; out_lo[o] = lo;
+        } else {
+          out[o] = v[j];
+        }
+      }
     }
   }
 };
