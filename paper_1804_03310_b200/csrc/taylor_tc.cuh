@@ -1,11 +1,13 @@
 // taylor_tc.cuh -- H7 on the tensor pipe: Phi' = E_h [sum_{k<=K} A^k/k!] E_h Phi  (R3, R9).
 // Persistent CTAs, one walker at a time.  Every product X * T (X = E_h real or A_w complex symmetric, T complex
 // M x N_t) is a set of real tcgen05.mma.kind::tf32 products with the 3xTF32 split:
-//     D_re = X_r T_r - X_i T_i ,  D_im = X_r T_i + X_i T_r      (the minus sign via the descriptor's negate-B bit)
+//     D1 = X_r [T_r | T_i] ,  D2 = X_i [T_r | T_i]  (N = 64 each; a small N makes the a-operand's shared-memory
+//     reads the bound, so re and im share one MMA);  D_re = D1[0:32] - D2[32:64],  D_im = D1[32:64] + D2[0:32]
+//     are combined by the epilogue warps.
 // a-operand: 128-row x 32-column tiles of X (hi / lo planes) streamed by TMA through a 3-stage ring;
-// b-operand: T as four K-major planes (T_r, T_i) x (hi, lo), [32 rows (walker columns)][KP] in shared memory,
+// b-operand: T as two K-major planes (hi, lo), [64 rows = T_r columns | T_i columns][KP] in shared memory,
 //            rewritten by the epilogue warps after every Taylor term (generic -> async proxy fence);
-// accumulators: TMEM, 64 columns per 128-row tile (32 re | 32 im).  The running sum P lives in registers.
+// accumulators: TMEM, 64 columns per (128-row tile, plane, chunk).  The running sum P lives in registers.
 // Supported: M <= 256, N_t <= 32 (else the SIMT kernel of taylor.cuh runs).
 #pragma once
 #include "gemm_tf32.cuh"
@@ -15,7 +17,7 @@ namespace tt {
 
 using namespace tc;
 
-enum { NST = 3, TILE_BYTES = 128 * 128, STG_BYTES = 2 * TILE_BYTES, PLANE_KB_BYTES = 32 * 128, EPW = 8, NTHREADS = (EPW + 2) * 32 };
+enum { NST = 3, TILE_BYTES = 128 * 128, STG_BYTES = 2 * TILE_BYTES, PLANE_KB_BYTES = 64 * 128, EPW = 8, NTHREADS = (EPW + 2) * 32 };
 
 struct TaylorMaps {
   CUtensorMap A[2][2];   // [hi/lo][0: 128-row box, 1: last-tile box]  over Abuf viewed as [N_w*M][2*MP]
@@ -25,12 +27,15 @@ struct TaylorMaps {
 struct TaylorTcArgs {
   int M, MP, nt, K, nw;
   int mtiles, rows_last, nkb;   // 128-row tiles, rows of the last one (multiple of 8), 32-column k-blocks
+  int nch, chunk_kb;            // accumulation chunks per tile (each its own 64 TMEM columns) and k-blocks per chunk:
+                                // the tensor pipe truncates when it adds into its accumulator, so one long chain
+                                // drifts; chunks are summed round-to-nearest in registers by the epilogue warps
   cplx<float>* phi;             // [nw][M][nt] in/out
 };
 
-inline size_t smem_bytes(int nkb) { return (size_t)4 * nkb * PLANE_KB_BYTES + (size_t)NST * STG_BYTES + 1024; }
+inline size_t smem_bytes(int nkb) { return (size_t)2 * nkb * PLANE_KB_BYTES + (size_t)NST * STG_BYTES + 1024; }
 
-// byte offset of element (row b, column j) inside one K-major SWIZZLE_128B plane
+// byte offset of element (row b in 0..63, column j) inside one K-major SWIZZLE_128B plane
 __device__ __forceinline__ uint32_t plane_off(int b, int j) {
   const int kb = j >> 5, jj = j & 31;
   return (uint32_t)(kb * PLANE_KB_BYTES + b * 128 + ((((jj >> 2) ^ (b & 7)) << 4) | ((jj & 3) << 2)));
@@ -47,13 +52,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int M = g.M, nt = g.nt, nkb = g.nkb, mtiles = g.mtiles;
   const uint32_t plane_bytes = (uint32_t)nkb * PLANE_KB_BYTES;
-  uint8_t* planes = smem;                                   // [Tr_hi | Tr_lo | Ti_hi | Ti_lo]
-  uint8_t* stages = smem + 4 * (size_t)plane_bytes;
+  uint8_t* planes = smem;                                   // [hi plane | lo plane], rows 0-31 T_r, 32-63 T_i
+  uint8_t* stages = smem + 2 * (size_t)plane_bytes;
   const int nphase = g.K + 2;
-  const uint32_t tmem_cols = mtiles > 1 ? 128u : 64u;
+  const uint32_t tmem_cols = 512u;
 
   // zero the planes once: rows >= nt and columns >= M must stay 0 for the whole kernel
-  for (uint32_t o = threadIdx.x * 16; o < 4 * plane_bytes; o += NTHREADS * 16)
+  for (uint32_t o = threadIdx.x * 16; o < 2 * plane_bytes; o += NTHREADS * 16)
     *reinterpret_cast<uint4*>(planes + o) = make_uint4(0, 0, 0, 0);
   if (warp == EPW && lane == 0) {
     for (int s = 0; s < NST; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
@@ -101,8 +106,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
     }
   } else if (warp == EPW + 1) {
     if (lane == 0) {   // ===== MMA issuer =====
-      constexpr uint32_t idesc = make_idesc(128, 32);
-      constexpr uint32_t idesc_negb = idesc | (1u << 14);
+      constexpr uint32_t idesc = make_idesc(128, 64);
       const uint32_t pl = smem_u32(planes);
       uint32_t it = 0, gph = 0;
       for (int w = blockIdx.x; w < g.nw; w += gridDim.x)
@@ -111,31 +115,23 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
           mbar_wait(&b_ready_bar, gph & 1);               // T planes of this phase are in shared memory
           tc_fence_after();
           for (int mt = 0; mt < mtiles; ++mt) {
-            const uint32_t d_re = tmem + mt * 64, d_im = d_re + 32;
             for (int kb = 0; kb < nkb; ++kb)
               for (int p = 0; p < (cx ? 2 : 1); ++p, ++it) {
+                const uint32_t d = tmem + ((mt * 2 + p) * g.nch + kb / g.chunk_kb) * 64;
                 const int s = it % NST;
                 mbar_wait(&full_bar[s], (it / NST) & 1);
                 tc_fence_after();
                 const uint32_t sa = smem_u32(stages + (size_t)s * STG_BYTES);
                 const uint64_t x_hi = make_desc(sa), x_lo = make_desc(sa + TILE_BYTES);
                 const uint32_t kboff = (uint32_t)kb * PLANE_KB_BYTES;
-                const uint64_t tr_hi = make_desc(pl + kboff), tr_lo = make_desc(pl + plane_bytes + kboff);
-                const uint64_t ti_hi = make_desc(pl + 2 * plane_bytes + kboff), ti_lo = make_desc(pl + 3 * plane_bytes + kboff);
-                // p == 0: D_re += X_r T_r, D_im += X_r T_i ;  p == 1: D_re -= X_i T_i, D_im += X_i T_r
-                const uint64_t bre_hi = p ? ti_hi : tr_hi, bre_lo = p ? ti_lo : tr_lo;
-                const uint64_t bim_hi = p ? tr_hi : ti_hi, bim_lo = p ? tr_lo : ti_lo;
-                const uint32_t id_re = p ? idesc_negb : idesc;
-                const bool first = kb == 0 && p == 0;
+                const uint64_t t_hi = make_desc(pl + kboff), t_lo = make_desc(pl + plane_bytes + kboff);
+                const bool first = (kb % g.chunk_kb) == 0;
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
                   const uint64_t adv = (uint64_t)(k * 2);   // 8 tf32 = 32 bytes = 2 x 16 B
-                  umma_tf32(d_re, x_lo + adv, bre_hi + adv, id_re, (first && k == 0) ? 0u : 1u);
-                  umma_tf32(d_re, x_hi + adv, bre_lo + adv, id_re, 1u);
-                  umma_tf32(d_re, x_hi + adv, bre_hi + adv, id_re, 1u);
-                  umma_tf32(d_im, x_lo + adv, bim_hi + adv, idesc, (first && k == 0) ? 0u : 1u);
-                  umma_tf32(d_im, x_hi + adv, bim_lo + adv, idesc, 1u);
-                  umma_tf32(d_im, x_hi + adv, bim_hi + adv, idesc, 1u);
+                  umma_tf32(d, x_lo + adv, t_hi + adv, idesc, (first && k == 0) ? 0u : 1u);
+                  umma_tf32(d, x_hi + adv, t_lo + adv, idesc, 1u);
+                  umma_tf32(d, x_hi + adv, t_hi + adv, idesc, 1u);
                 }
                 tc_commit(&empty_bar[s]);
               }
@@ -145,8 +141,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
     }
   } else {   // ===== epilogue warps 0..7: TMEM lane quarter = warp & 3, half = warp >> 2 (0: real part, 1: imaginary) =====
     const int q = warp & 3, half = warp >> 2;
-    uint8_t* pl_hi = planes + (size_t)(2 * half) * plane_bytes;       // T_r or T_i, hi
-    uint8_t* pl_lo = pl_hi + plane_bytes;
+    uint8_t* pl_hi = planes;
+    uint8_t* pl_lo = planes + plane_bytes;
+    const int rb = half * 32;                 // plane row base: T_r rows 0-31, T_i rows 32-63
     uint32_t gph = 0;
     float P[2][32];
     for (int w = blockIdx.x; w < g.nw; w += gridDim.x) {
@@ -156,7 +153,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
         const int j = e / nt, b = e - j * nt;
         float hi, lo;
         tf32_split(phi_w[2 * e + half], hi, lo);
-        const uint32_t o = plane_off(b, j);
+        const uint32_t o = plane_off(rb + b, j);
         *reinterpret_cast<float*>(pl_hi + o) = hi;
         *reinterpret_cast<float*>(pl_lo + o) = lo;
       }
@@ -171,8 +168,23 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
 #pragma unroll
         for (int mt = 0; mt < 2; ++mt) {
           if (mt < mtiles) {
+            // D_re = D1[0:32] - D2[32:64] ; D_im = D1[32:64] + D2[0:32], summed over the accumulation chunks
             float v[32];
-            tmem_ld32(tmem + ((uint32_t)(q * 32) << 16) + mt * 64 + half * 32, v);
+            const bool cxp = ph >= 1 && ph <= g.K;
+            const uint32_t tl = tmem + ((uint32_t)(q * 32) << 16);
+#pragma unroll
+            for (int b = 0; b < 32; ++b) v[b] = 0.f;
+            for (int ch = 0; ch < g.nch; ++ch) {
+              float u[32];
+              tmem_ld32(tl + ((mt * 2 + 0) * g.nch + ch) * 64 + half * 32, u);
+#pragma unroll
+              for (int b = 0; b < 32; ++b) v[b] += u[b];
+              if (cxp) {
+                tmem_ld32(tl + ((mt * 2 + 1) * g.nch + ch) * 64 + (1 - half) * 32, u);
+#pragma unroll
+                for (int b = 0; b < 32; ++b) v[b] = half ? v[b] + u[b] : v[b] - u[b];
+              }
+            }
             const int i = mt * 128 + q * 32 + lane;     // output row = basis index
 #pragma unroll
             for (int b = 0; b < 32; ++b) {
@@ -183,14 +195,16 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
             }
             if (i < M) {
               if (last_phase) {
-                for (int b = 0; b < nt; ++b) phi_w[2 * (i * nt + b) + half] = v[b];
+#pragma unroll
+                for (int b = 0; b < 32; ++b)
+                  if (b < nt) phi_w[2 * (i * nt + b) + half] = v[b];
               } else {
 #pragma unroll
                 for (int b = 0; b < 32; ++b) {
                   if (b < nt) {
                     float hi, lo;
                     tf32_split(v[b], hi, lo);
-                    const uint32_t o = plane_off(b, i);
+                    const uint32_t o = plane_off(rb + b, i);
                     *reinterpret_cast<float*>(pl_hi + o) = hi;
                     *reinterpret_cast<float*>(pl_lo + o) = lo;
                   }
