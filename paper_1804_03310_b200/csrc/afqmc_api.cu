@@ -694,7 +694,9 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
                                  : cudaFuncSetAttribute(k_green<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->green_smem);
     if (e != cudaSuccess) { snprintf(g_init_err, 256, "CUDA: %s", cudaGetErrorString(e)); delete c; return AFQMC_ECUDA; }
   }
-  c->tay_tc = (c->path == 2 && c->M <= 256 && c->nt <= 32 && c->nw > 0);
+  // tensor-pipe Taylor kernel for 96 <= M <= 256: below that a 128-row tile is mostly padding and the FP32 SIMT
+  // kernel is both competitive and free of the tensor pipe's truncation bias
+  c->tay_tc = (c->path == 2 && c->M >= 96 && c->M <= 256 && c->nt <= 32 && c->nw > 0);
   if (c->tay_tc) {
     tt::TaylorTcArgs& a = c->tay_args;
     a.M = c->M; a.MP = c->MP; a.nt = c->nt; a.K = p->taylor_order; a.nw = c->nw;
