@@ -47,6 +47,7 @@ struct afqmc_ctx {
   int md, nact, ndet, ca, cb;
   void* Cact; double* coeff; int32_t* exc;
   void *thtil, *th_scr; zcplx *ovlp0, *ovlp_scr;
+  void *RactT, *thT, *TTg; int MPK;
   size_t mdo_smem, mde_smem;
   int tay_cw, tay_nch, tay_threads;
   size_t tay_smem, green_smem;
@@ -203,6 +204,8 @@ void carve(const afqmc_params* p, afqmc_ctx* c, char* cbase, char* wbase, size_t
   c->Cact = cc.take((size_t)M * (md ? p->n_act : 1) * ts);
   c->coeff = (double*)cc.take((size_t)p->n_det * 8);
   c->exc = (int32_t*)cc.take((size_t)p->n_det * 8 * 4);
+  c->MPK = (int)rup(M, 8);
+  c->RactT = cc.take(md ? (size_t)(ng + 1) * p->n_act * c->MPK * ts : 256);
   *cb = cc.off;
 
   Carver w; w.base = wbase;
@@ -216,6 +219,8 @@ void carve(const afqmc_params* p, afqmc_ctx* c, char* cbase, char* wbase, size_t
   c->fs = w.take(2 * 2 * nw1 * NGP * ts);
   c->thtil = w.take(md ? nw1 * M * 2 * p->n_act * 2 * ts : 256);
   c->th_scr = w.take(md ? nw1 * M * nt * 2 * ts : 256);
+  c->thT = w.take(md ? nw1 * 2 * nt * c->MPK * ts : 256);
+  c->TTg = w.take(md ? nw1 * (ng + 1) * p->n_act * nt * 2 * ts : 256);
   c->ovlp0 = (zcplx*)w.take(nw1 * sizeof(zcplx));
   c->ovlp_scr = (zcplx*)w.take(nw1 * sizeof(zcplx));
   c->cshift = (zcplx*)w.take(nw1 * sizeof(zcplx));
@@ -314,6 +319,10 @@ template <typename T> afqmc_status init_device(afqmc_ctx* c, const double* h1, c
     LAUNCH(c, k_init_Y<T>, dim3((M * n + 127) / 128, M * n), 128, 0, M, n, ng, c->Rd, soff, KT, (T*)c->Y[s],
            (T*)c->Y_lo[s], Ks, c->split);
   }
+  if (c->md) {
+    size_t tot = (size_t)(ng + 1) * c->nact * M;
+    LAUNCH(c, k_init_ractT<T>, (unsigned)((tot + 127) / 128), 128, 0, ng, c->nact, M, c->MPK, c->Rd, KT, c->hrotd, (T*)c->RactT);
+  }
   {
     size_t tot = (size_t)ng * KT;
     LAUNCH(c, k_cast2d<T>, (unsigned)((tot + 127) / 128), 128, 0, ng, KT, c->Rd, (size_t)KT, (T*)c->Rall, (T*)c->Rall_lo,
@@ -344,7 +353,7 @@ afqmc_status run_green(afqmc_ctx* c, const void* phi, void* ovlp, void* theta, i
   if (c->md) {
     // reference determinant first (S_0 to scratch, no weights), then SMW over all determinants
     g.thp = nullptr; g.thp_lo = nullptr; g.ovlp = c->ovlp0; g.do_weight = 0;
-    LAUNCH(c, k_green<T>, c->nw, 128, c->green_smem, g);
+    LAUNCH(c, k_green<T>, c->nw, 256, c->green_smem, g);
     MdOverlapArgs<T> a;
     a.m.M = c->M; a.m.na = c->na; a.m.nb = c->nb; a.m.nact = c->nact; a.m.ndet = c->ndet;
     a.m.C = c->Cact; a.m.coeff = c->coeff; a.m.exc = c->exc;
@@ -356,7 +365,7 @@ afqmc_status run_green(afqmc_ctx* c, const void* phi, void* ovlp, void* theta, i
            (T*)c->thp, (T*)c->thp_lo);
     return AFQMC_OK;
   }
-  LAUNCH(c, k_green<T>, c->nw, 128, c->green_smem, g);
+  LAUNCH(c, k_green<T>, c->nw, 256, c->green_smem, g);
   return AFQMC_OK;
 }
 
@@ -405,8 +414,17 @@ template <typename T> afqmc_status run_md_energy(afqmc_ctx* c, const void* theta
   MdEnergyArgs<T> a;
   a.m.M = c->M; a.m.na = c->na; a.m.nb = c->nb; a.m.nact = c->nact; a.m.ndet = c->ndet;
   a.m.C = c->Cact; a.m.coeff = c->coeff; a.m.exc = c->exc;
-  a.ng = c->ng; a.ldr = c->KT; a.theta0 = (const cplx<T>*)theta; a.Ract = (const T*)c->Rall; a.hact = (const T*)c->hrot;
+  a.ng = c->ng; a.ldr = c->KT; a.theta0 = (const cplx<T>*)theta; a.TTg = (const cplx<T>*)c->TTg;
   a.eloc = eloc;
+  // TT[w][g][q][a] = sum_k (C_act^T X_g)[q][k] Theta_0[w][k][a] for every g (and h) in one GEMM over all walkers
+  LAUNCH(c, k_thT<T>, c->nw, 128, 0, c->M, c->nt, c->MPK, (const cplx<T>*)theta, (T*)c->thT);
+  {
+    EpiTT<T> epi;
+    epi.out = (T*)c->TTg; epi.ng1 = c->ng + 1; epi.nact = c->nact; epi.nt = c->nt;
+    epi.m_real = (c->ng + 1) * c->nact; epi.n_real = c->nw * 2 * c->nt;
+    afqmc_status st = run_gemm<T>(c, (const T*)c->RactT, c->MPK, epi.m_real, (const T*)c->thT, c->MPK, epi.n_real, c->MPK, epi);
+    if (st) return st;
+  }
   LAUNCH(c, k_md_energy<T>, c->nw, 256, c->mde_smem, a);
   return AFQMC_OK;
 }

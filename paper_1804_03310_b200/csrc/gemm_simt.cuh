@@ -102,6 +102,28 @@ template <typename T> struct EpiEnergy {
   }
 };
 
+// H10: row = g*nact + q, col = (w*2 + p)*nt + a  ->  TT[w][g][q][a] (interleaved complex)
+template <typename T> struct EpiTT {
+  T* out; int ng1, nact, nt; int m_real, n_real;
+  template <int TM, int TN>
+  __device__ void operator()(T (&acc)[TM][TN], int r0, int r1, int c0, int c1, void*) const {
+#pragma unroll
+    for (int j = 0; j < TN; ++j) {
+      int c = j < TN / 2 ? c0 + j : c1 + j - TN / 2;
+      if (c >= n_real) continue;
+      int w = c / (2 * nt), rem = c - w * 2 * nt;
+      int p = rem / nt, a = rem - p * nt;
+#pragma unroll
+      for (int i = 0; i < TM; ++i) {
+        int r = i < TM / 2 ? r0 + i : r1 + i - TM / 2;
+        if (r >= m_real) continue;
+        int g = r / nact, q = r - g * nact;
+        out[((((size_t)w * ng1 + g) * nact + q) * nt + a) * 2 + p] = acc[i][j];
+      }
+    }
+  }
+};
+
 // grid = (ceil(N/BN), ceil(M/BM)), 256 threads.
 template <typename T, class Epi>
 __global__ void __launch_bounds__(256) k_gemm_nt(const T* __restrict__ A, int lda, int m_rows,

@@ -133,20 +133,32 @@ struct EpiEnergy {      // H9: eloc[w] += sum_rows v[row] (0.5 C[row][w] + hrot[
   __device__ __forceinline__ void operator()(int r, int c0, const float (&v)[32]) const {
     const bool rok = r < m_real;
     const float hr = rok ? hrot[r] : 0.f;
+    const int lane = threadIdx.x & 31;
+    float x[32];             // x[2p] / x[2p+1] = this row's contribution to Re / Im of walker (c0/2 + p)
 #pragma unroll
     for (int j = 0; j < 32; j += 2) {
-      const int c = c0 + j;            // even: real plane of walker c/2
-      double er = 0.0, ei = 0.0;
+      const int c = c0 + j;
+      float er = 0.f, ei = 0.f;
       if (rok && c < n_real) {
         const size_t o = (size_t)c * KT + soff + r;
         const float vr = thp[o] + thp_lo[o], vi = thp[o + KT] + thp_lo[o + KT];
         const float ur = 0.5f * v[j] + hr, ui = 0.5f * v[j + 1];
-        er = (double)(vr * ur - vi * ui);
-        ei = (double)(vr * ui + vi * ur);
+        er = vr * ur - vi * ui;
+        ei = vr * ui + vi * ur;
       }
-      er = warp_sum(er); ei = warp_sum(ei);
-      if ((threadIdx.x & 31) == 0 && c < n_real) { atomicAdd(&eloc[c], er); atomicAdd(&eloc[c + 1], ei); }
+      x[j] = er; x[j + 1] = ei;
     }
+    // transpose-reduce over the 32 rows of this warp: 31 shuffles, lane l ends with the sum of x[l]
+#pragma unroll
+    for (int s = 16; s >= 1; s >>= 1) {
+#pragma unroll
+      for (int i = 0; i < s; ++i) {
+        const float keep = (lane & s) ? x[i + s] : x[i];
+        const float send = (lane & s) ? x[i] : x[i + s];
+        x[i] = keep + __shfl_xor_sync(0xffffffffu, send, s);
+      }
+    }
+    if (c0 + lane < n_real) atomicAdd(&eloc[c0 + lane], (double)x[0]);
   }
 };
 

@@ -113,9 +113,9 @@ __device__ inline void weight_update(zcplx S_old, zcplx S_new, zcplx c, double w
 }
 
 template <typename T>
-__global__ void __launch_bounds__(128) k_green(GreenArgs<T> g) {
+__global__ void __launch_bounds__(256) k_green(GreenArgs<T> g) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nthr = blockDim.x;
   const int M = g.M, na = g.na, nb = g.nb, nt = na + nb, ns = na > nb ? na : nb;
   const int ld = 2 * ns + 1;
   cplx<T>* phi_s = reinterpret_cast<cplx<T>*>(smem_raw);
@@ -127,11 +127,11 @@ __global__ void __launch_bounds__(128) k_green(GreenArgs<T> g) {
   int* sing = reinterpret_cast<int*>(dets + 2);
 
   const cplx<T>* phi_w = g.phi + (size_t)w * M * nt;
-  for (int e = tid; e < M * nt; e += 128) phi_s[e] = phi_w[e];
+  for (int e = tid; e < M * nt; e += nthr) phi_s[e] = phi_w[e];
   __syncthreads();
 
   // A_s[a][b] = sum_k psi_s[k][a] phi[k][off+b]  (real x complex), augmented with the identity
-  for (int e = tid; e < na * na + nb * nb; e += 128) {
+  for (int e = tid; e < na * na + nb * nb; e += nthr) {
     int s = e >= na * na;
     int ee = s ? e - na * na : e;
     int n = s ? nb : na, off = s ? na : 0;
@@ -162,7 +162,7 @@ __global__ void __launch_bounds__(128) k_green(GreenArgs<T> g) {
   for (int s = 0; s < 2; ++s) {
     int n = s ? nb : na, off = s ? na : 0, soff = s ? g.KA : 0;
     const zcplx* inv = aug + s * ns * ld + n;
-    for (int e = tid; e < M * n; e += 128) {
+    for (int e = tid; e < M * n; e += nthr) {
       int k = e / n, b = e % n;
       zcplx accd = mk<double>(0.0, 0.0);
       for (int a = 0; a < n; ++a) cfma(accd, to_z(phi_s[k * nt + off + a]), inv[a * ld + b]);

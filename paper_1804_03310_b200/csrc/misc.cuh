@@ -185,4 +185,30 @@ __global__ void k_cast2d(int nr, int nc, const double* src, size_t lds, T* dst, 
   }
 }
 
+
+// ---- multi-determinant energy: operands of the TT = C_act^T X Theta_0 GEMM (X = L_g for all g, then h) ----
+// thT[((w*2+p)*nt + a)*MPK + k] = Re/Im Theta_0[w][k][a]   (K-major rows (walker, plane, column), zero padded)
+template <typename T>
+__global__ void __launch_bounds__(128) k_thT(int M, int nt, int MPK, const cplx<T>* theta, T* thT) {
+  const int w = blockIdx.x;
+  for (int e = threadIdx.x; e < M * nt; e += blockDim.x) {
+    int k = e / nt, a = e - k * nt;
+    cplx<T> v = theta[(size_t)w * M * nt + e];
+    thT[((size_t)(w * 2 + 0) * nt + a) * MPK + k] = v.x;
+    thT[((size_t)(w * 2 + 1) * nt + a) * MPK + k] = v.y;
+  }
+}
+// RactT[(g*nact + q)*MPK + k] = (C_act^T L_g)[q][k] for g < ng, (C_act^T h)[q][k] for g == ng
+template <typename T>
+__global__ void k_init_ractT(int ng, int nact, int M, int MPK, const double* Rd, int KT, const double* hrotd, T* out) {
+  size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  size_t tot = (size_t)(ng + 1) * nact * M;
+  if (e >= tot) return;
+  int k = (int)(e % M);
+  int q = (int)((e / M) % nact);
+  int g = (int)(e / ((size_t)M * nact));
+  double v = g < ng ? Rd[(size_t)g * KT + k * nact + q] : hrotd[k * nact + q];
+  out[((size_t)g * nact + q) * MPK + k] = (T)v;
+}
+
 }  // namespace afq

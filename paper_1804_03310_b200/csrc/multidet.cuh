@@ -244,8 +244,8 @@ template <typename T> struct MdEnergyArgs {
   MdConst m;
   int ng, ldr;
   const cplx<T>* theta0;   // [nw][M][nt]
-  const T* Ract;           // [ng][ldr] : Ract[g][k*nact + q] = (C_act^T L_g)[q][k]
-  const T* hact;           // [M*nact]  : (C_act^T h)[q][k] at k*nact + q
+  const cplx<T>* TTg;      // [nw][ng+1][nact][nt] : TT = C_act^T X Theta_0 for X = L_0..L_{ng-1}, h  (batched GEMM,
+                           //                        run before this kernel; H10)
   zcplx* eloc;             // [nw]
 };
 
@@ -285,19 +285,9 @@ __global__ void __launch_bounds__(256) k_md_energy(MdEnergyArgs<T> g) {
 
   for (int gi = 0; gi <= g.ng; ++gi) {
     const bool is_h = gi == g.ng;
-    const T* R = is_h ? g.hact : g.Ract + (size_t)gi * g.ldr;
-    // 1. TT[q][a] = sum_k R[q][k] Theta_0[k][a]
-    for (int e = tid; e < nact * nt; e += nthr) {
-      int q = e / nt, a = e - q * nt;
-      T sr = T(0), si = T(0);
-      for (int k = 0; k < M; ++k) {
-        T r = R[k * nact + q];
-        cplx<T> v = th0[k * nt + a];
-        sr = fma(r, v.x, sr);
-        si = fma(r, v.y, si);
-      }
-      TT[e] = mk<double>((double)sr, (double)si);
-    }
+    // 1. TT[q][a] = (C_act^T X Theta_0)[q][a], precomputed for all X by one GEMM over all walkers
+    const cplx<T>* src = g.TTg + ((size_t)w * (g.ng + 1) + gi) * nact * nt;
+    for (int e = tid; e < nact * nt; e += nthr) TT[e] = to_z(src[e]);
     __syncthreads();
     // 2. W = TT_virt - Q_virt T0 ; f0, X0 by warps 0 / 1
     for (int sp = 0; sp < 2; ++sp) {

@@ -277,3 +277,19 @@ def test_closed_shell_invariant():
     for n in range(3):
         st, _ = O.o_step(ini, st, x[n], wl.n_alpha)
         assert np.allclose(st.phi[..., :2], st.phi[..., 2:], atol=1e-14)
+
+
+def test_oracle_trajectory_fixture():
+    """The oracle's own cfg-1 trajectory is frozen in tests/golden/cfg1_raw_10steps.txt (written by the oracle-only
+    script beside it; NOT a paper value -- the paper prints none).  A change here must cite the passage or DESIGN.md
+    reading that justifies it."""
+    import importlib.util
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("write_oracle_fixture", os.path.join(here, "write_oracle_fixture.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    want = np.loadtxt(os.path.join(here, "cfg1_raw_10steps.txt"))
+    got = np.array(mod.trajectory(), dtype=float)
+    assert got.shape == want.shape
+    np.testing.assert_allclose(got, want, rtol=1e-9, atol=1e-12)
