@@ -425,7 +425,16 @@ template <typename T> afqmc_status run_md_energy(afqmc_ctx* c, const void* theta
     afqmc_status st = run_gemm<T>(c, (const T*)c->RactT, c->MPK, epi.m_real, (const T*)c->thT, c->MPK, epi.n_real, c->MPK, epi);
     if (st) return st;
   }
-  LAUNCH(c, k_md_energy<T>, c->nw, 256, c->mde_smem, a);
+  const int dpt = (c->ndet + MD_THREADS - 1) / MD_THREADS;
+#define MDE_LAUNCH(D)                                                                                              \
+  {                                                                                                                \
+    auto kern = k_md_energy<T, D>;                                                                                 \
+    if (c->mde_smem > 48 * 1024)                                                                                   \
+      CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->mde_smem));       \
+    LAUNCH(c, kern, c->nw, MD_THREADS, c->mde_smem, a);                                                            \
+  }
+  if (dpt <= 1) MDE_LAUNCH(1) else if (dpt <= 2) MDE_LAUNCH(2) else if (dpt <= 4) MDE_LAUNCH(4) else MDE_LAUNCH(8)
+#undef MDE_LAUNCH
   return AFQMC_OK;
 }
 
@@ -700,10 +709,10 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
     cudaError_t e1, e2;
     if (p->precision) {
       e1 = cudaFuncSetAttribute(k_md_overlap<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->mdo_smem);
-      e2 = cudaFuncSetAttribute(k_md_energy<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->mde_smem);
+      e2 = cudaSuccess;
     } else {
       e1 = cudaFuncSetAttribute(k_md_overlap<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->mdo_smem);
-      e2 = cudaFuncSetAttribute(k_md_energy<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->mde_smem);
+      e2 = cudaSuccess;
     }
     if (e1 != cudaSuccess || e2 != cudaSuccess) { snprintf(g_init_err, 256, "CUDA: cannot size multi-det shared memory"); delete c; return AFQMC_ECUDA; }
   }

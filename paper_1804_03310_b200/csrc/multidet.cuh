@@ -252,60 +252,84 @@ template <typename T> struct MdEnergyArgs {
 inline size_t md_energy_smem(int M, int na, int nb, int nact, int ndet, int ts) {
   size_t b = md_smem_bytes(na, nb, nact, ndet);
   b += ((size_t)M * (na + nb) * 2 * ts + 15) & ~size_t(15);
-  b += (size_t)nact * (na + nb) * sizeof(zcplx);                              // TT
-  b += (size_t)2 * ((nact - na) * na + (nact - nb) * nb) * sizeof(zcplx);     // W, WT
-  b += 4 * sizeof(zcplx);
+  const size_t nw_ = (size_t)(nact - na) * na + (size_t)(nact - nb) * nb;
+  // TT, W, WT, Q_virt copy, Z copy, 4 scalars: complex T (the bulk arithmetic follows the walker precision;
+  // per-determinant energies and the final mixture are accumulated in FP64)
+  b += ((size_t)nact * (na + nb) + 3 * nw_ + (size_t)ndet * 8 + 4) * 2 * ts + 16;
   return b;
 }
 
-enum { MD_DPT = 4 };  // determinants per thread (ndet <= 4 * 256)
+enum { MD_THREADS = 128 };  // determinants per thread DPT in {1, 2, 4, 8} (ndet <= 8 * 128)
 
-template <typename T>
-__global__ void __launch_bounds__(256) k_md_energy(MdEnergyArgs<T> g) {
+template <typename T, int MD_DPT>
+__global__ void __launch_bounds__(MD_THREADS) k_md_energy(MdEnergyArgs<T> g) {
+  typedef cplx<T> C;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const MdConst& m = g.m;
   const int w = blockIdx.x, tid = threadIdx.x, nthr = blockDim.x, nt = m.na + m.nb, M = m.M, nact = m.nact;
   const int lane = tid & 31, wid = tid >> 5;
   MdSmem s;
   unsigned char* p = md_carve(smem_raw, m, s);
-  cplx<T>* th0 = reinterpret_cast<cplx<T>*>(p);
-  p += ((size_t)M * nt * sizeof(cplx<T>) + 15) & ~size_t(15);
-  zcplx* TT = reinterpret_cast<zcplx*>(p);
-  zcplx* Wm[2]; zcplx* WTm[2];
-  Wm[0] = TT + nact * nt; Wm[1] = Wm[0] + (nact - m.na) * m.na;
-  WTm[0] = Wm[1] + (nact - m.nb) * m.nb; WTm[1] = WTm[0] + (nact - m.na) * m.na;
-  zcplx* scal = WTm[1] + (nact - m.nb) * m.nb;   // f0[2], X0[2]
+  C* th0 = reinterpret_cast<C*>(p);
+  p += ((size_t)M * nt * sizeof(C) + 15) & ~size_t(15);
+  const int nwa = (nact - m.na) * m.na, nwb = (nact - m.nb) * m.nb;
+  C* TT = reinterpret_cast<C*>(p);
+  C* Wm[2]; C* WTm[2]; C* Qc[2];
+  Wm[0] = TT + nact * nt; Wm[1] = Wm[0] + nwa;
+  WTm[0] = Wm[1] + nwb; WTm[1] = WTm[0] + nwa;
+  Qc[0] = WTm[1] + nwb; Qc[1] = Qc[0] + nwa;
+  C* Zc = Qc[1] + nwb;                 // [ndet][2][4]
+  C* scal = Zc + (size_t)m.ndet * 8;   // f0[2], X0[2]
   for (int e = tid; e < M * nt; e += nthr) th0[e] = g.theta0[(size_t)w * M * nt + e];
   __syncthreads();
   md_prepare<T>(m, th0, s);
+  for (int e = tid; e < nwa + nwb; e += nthr) Qc[0][e] = mk<T>((T)s.Qv[0][e].x, (T)s.Qv[0][e].y);
+  for (int e = tid; e < m.ndet * 8; e += nthr) Zc[e] = mk<T>((T)s.Z[e].x, (T)s.Z[e].y);
 
   zcplx Eacc[MD_DPT];
 #pragma unroll
   for (int j = 0; j < MD_DPT; ++j) Eacc[j] = mk<double>(0.0, 0.0);
+  // excitation pattern of this thread's determinants (constant over the gamma loop): packed 4 x 8 bits per spin
+  uint32_t pat[MD_DPT][2]; int rks[MD_DPT];
+#pragma unroll
+  for (int j = 0; j < MD_DPT; ++j) {
+    const int i = tid + j * MD_THREADS;
+    rks[j] = 0; pat[j][0] = pat[j][1] = 0;
+    if (i < m.ndet)
+      for (int sp = 0; sp < 2; ++sp) {
+        int h[2], pp[2];
+        const int rk = md_exc(m, i, sp, h, pp);
+        const int n = sp ? m.nb : m.na;
+        rks[j] |= rk << (2 * sp);
+        pat[j][sp] = (uint32_t)(h[0] & 255) | ((uint32_t)((pp[0] - n) & 255) << 8) | ((uint32_t)(h[1] & 255) << 16) |
+                     ((uint32_t)((pp[1] - n) & 255) << 24);
+      }
+  }
+  __syncthreads();
 
   for (int gi = 0; gi <= g.ng; ++gi) {
     const bool is_h = gi == g.ng;
     // 1. TT[q][a] = (C_act^T X Theta_0)[q][a], precomputed for all X by one GEMM over all walkers
-    const cplx<T>* src = g.TTg + ((size_t)w * (g.ng + 1) + gi) * nact * nt;
-    for (int e = tid; e < nact * nt; e += nthr) TT[e] = to_z(src[e]);
+    const C* src = g.TTg + ((size_t)w * (g.ng + 1) + gi) * nact * nt;
+    for (int e = tid; e < nact * nt; e += nthr) TT[e] = src[e];
     __syncthreads();
     // 2. W = TT_virt - Q_virt T0 ; f0, X0 by warps 0 / 1
     for (int sp = 0; sp < 2; ++sp) {
       const int n = sp ? m.nb : m.na, nv = nact - n, off = sp ? m.na : 0;
       for (int e = tid; e < nv * n; e += nthr) {
         int pv = e / n, a = e - pv * n;
-        zcplx acc = TT[(n + pv) * nt + off + a];
-        for (int h = 0; h < n; ++h) acc = zsub(acc, zmul(s.Qv[sp][pv * n + h], TT[h * nt + off + a]));
+        C acc = TT[(n + pv) * nt + off + a];
+        for (int h = 0; h < n; ++h) acc = csub(acc, cmul(Qc[sp][pv * n + h], TT[h * nt + off + a]));
         Wm[sp][e] = acc;
       }
     }
     if (wid < 2) {
       const int sp = wid, n = sp ? m.nb : m.na, off = sp ? m.na : 0;
-      zcplx f0 = mk<double>(0.0, 0.0), x0 = mk<double>(0.0, 0.0);
+      C f0 = mk<T>(T(0), T(0)), x0 = mk<T>(T(0), T(0));
       for (int e = lane; e < n * n; e += 32) {
         int a = e / n, b = e - a * n;
-        if (a == b) f0 = zadd(f0, TT[a * nt + off + a]);
-        x0 = zadd(x0, zmul(TT[a * nt + off + b], TT[b * nt + off + a]));
+        if (a == b) f0 = cadd(f0, TT[a * nt + off + a]);
+        x0 = cadd(x0, cmul(TT[a * nt + off + b], TT[b * nt + off + a]));
       }
       f0.x = warp_sum(f0.x); f0.y = warp_sum(f0.y); x0.x = warp_sum(x0.x); x0.y = warp_sum(x0.y);
       if (lane == 0) { scal[sp] = f0; scal[2 + sp] = x0; }
@@ -317,61 +341,70 @@ __global__ void __launch_bounds__(256) k_md_energy(MdEnergyArgs<T> g) {
         const int n = sp ? m.nb : m.na, nv = nact - n, off = sp ? m.na : 0;
         for (int e = tid; e < nv * n; e += nthr) {
           int pv = e / n, a = e - pv * n;
-          zcplx acc = mk<double>(0.0, 0.0);
-          for (int b = 0; b < n; ++b) acc = zadd(acc, zmul(Wm[sp][pv * n + b], TT[b * nt + off + a]));
+          C acc = mk<T>(T(0), T(0));
+          for (int b = 0; b < n; ++b) cfma(acc, Wm[sp][pv * n + b], TT[b * nt + off + a]);
           WTm[sp][e] = acc;
         }
       }
+      __syncthreads();
     }
-    __syncthreads();
     // 4. per determinant: E x E work only
 #pragma unroll
     for (int j = 0; j < MD_DPT; ++j) {
-      const int i = tid + j * 256;
+      const int i = tid + j * MD_THREADS;
       if (i >= m.ndet) continue;
-      zcplx tsum = mk<double>(0.0, 0.0), xsum = mk<double>(0.0, 0.0);
+      C tsum = mk<T>(T(0), T(0)), xsum = mk<T>(T(0), T(0));
+#pragma unroll
       for (int sp = 0; sp < 2; ++sp) {
         const int n = sp ? m.nb : m.na;
-        int h[2], pp[2];
-        const int rk = md_exc(m, i, sp, h, pp);
-        const zcplx* Zi = s.Z + ((size_t)i * 2 + sp) * 4;
-        zcplx t = scal[sp], xch = scal[2 + sp];
+        const int rk = (rks[j] >> (2 * sp)) & 3;
+        const uint32_t pt = pat[j][sp];
+        const int h0 = pt & 255, p0 = (pt >> 8) & 255, h1 = (pt >> 16) & 255, p1 = (pt >> 24) & 255;
+        const C* Zi = Zc + ((size_t)i * 2 + sp) * 4;
+        C t = scal[sp], xch = scal[2 + sp];
         if (rk == 1) {
-          zcplx zw = zmul(Zi[0], Wm[sp][(pp[0] - n) * n + h[0]]);
-          t = zadd(t, zw);
+          C zw = cmul(Zi[0], Wm[sp][p0 * n + h0]);
+          t = cadd(t, zw);
           if (!is_h) {
-            xch = zadd(xch, zscale(zmul(Zi[0], WTm[sp][(pp[0] - n) * n + h[0]]), 2.0));
-            xch = zadd(xch, zmul(zw, zw));
+            C zt = cmul(Zi[0], WTm[sp][p0 * n + h0]);
+            xch = cadd(xch, mk<T>(2 * zt.x, 2 * zt.y));
+            cfma(xch, zw, zw);
           }
         } else if (rk == 2) {
-          zcplx ZW[2][2], ZT[2][2];
-          for (int f = 0; f < 2; ++f)
-            for (int f2 = 0; f2 < 2; ++f2) {
-              zcplx a = mk<double>(0.0, 0.0), b = mk<double>(0.0, 0.0);
-              for (int e = 0; e < 2; ++e) {
-                a = zadd(a, zmul(Zi[f * 2 + e], Wm[sp][(pp[e] - n) * n + h[f2]]));
-                if (!is_h) b = zadd(b, zmul(Zi[f * 2 + e], WTm[sp][(pp[e] - n) * n + h[f2]]));
-              }
-              ZW[f][f2] = a; ZT[f][f2] = b;
-            }
-          t = zadd(t, zadd(ZW[0][0], ZW[1][1]));
+          // (Z W)[f][f'] = sum_e Z[f][e] W[p_e][h_f']
+          const C w00 = Wm[sp][p0 * n + h0], w01 = Wm[sp][p0 * n + h1], w10 = Wm[sp][p1 * n + h0], w11 = Wm[sp][p1 * n + h1];
+          const C z00 = Zi[0], z01 = Zi[1], z10 = Zi[2], z11 = Zi[3];
+          C a00 = cmul(z00, w00); cfma(a00, z01, w10);
+          C a01 = cmul(z00, w01); cfma(a01, z01, w11);
+          C a10 = cmul(z10, w00); cfma(a10, z11, w10);
+          C a11 = cmul(z10, w01); cfma(a11, z11, w11);
+          t = cadd(t, cadd(a00, a11));
           if (!is_h) {
-            xch = zadd(xch, zscale(zadd(ZT[0][0], ZT[1][1]), 2.0));
-            xch = zadd(xch, zadd(zadd(zmul(ZW[0][0], ZW[0][0]), zmul(ZW[1][1], ZW[1][1])),
-                                 zscale(zmul(ZW[0][1], ZW[1][0]), 2.0)));
+            const C v00 = WTm[sp][p0 * n + h0], v10 = WTm[sp][p1 * n + h0], v01 = WTm[sp][p0 * n + h1], v11 = WTm[sp][p1 * n + h1];
+            C b00 = cmul(z00, v00); cfma(b00, z01, v10);
+            C b11 = cmul(z10, v01); cfma(b11, z11, v11);
+            xch = cadd(xch, mk<T>(2 * (b00.x + b11.x), 2 * (b00.y + b11.y)));
+            cfma(xch, a00, a00); cfma(xch, a11, a11);
+            C cr = cmul(a01, a10);
+            xch = cadd(xch, mk<T>(2 * cr.x, 2 * cr.y));
           }
         }
-        tsum = zadd(tsum, t);
-        xsum = zadd(xsum, xch);
+        tsum = cadd(tsum, t);
+        xsum = cadd(xsum, xch);
       }
-      if (is_h) Eacc[j] = zadd(Eacc[j], tsum);
-      else Eacc[j] = zadd(Eacc[j], zscale(zsub(zmul(tsum, tsum), xsum), 0.5));
+      if (is_h) {
+        Eacc[j].x += (double)tsum.x; Eacc[j].y += (double)tsum.y;
+      } else {
+        C e2 = csub(cmul(tsum, tsum), xsum);
+        Eacc[j].x += 0.5 * (double)e2.x; Eacc[j].y += 0.5 * (double)e2.y;
+      }
     }
+    __syncthreads();
   }
   zcplx part = mk<double>(0.0, 0.0);
 #pragma unroll
   for (int j = 0; j < MD_DPT; ++j) {
-    const int i = tid + j * 256;
+    const int i = tid + j * MD_THREADS;
     if (i < m.ndet) part = zadd(part, zmul(s.omega[i], Eacc[j]));
   }
   zcplx tot = block_sum(part, s.red);
