@@ -154,6 +154,7 @@ afqmc_status check_params(const afqmc_params* p, char* err) {
     }
     if (p->max_exc < 1 || p->max_exc > 2) { snprintf(err, 256, "max_exc must be 1 or 2"); return AFQMC_EUNSUPPORTED; }
     if (p->n_det > 1024) { snprintf(err, 256, "n_det <= 1024 supported"); return AFQMC_EUNSUPPORTED; }
+    if (p->n_act * (p->n_alpha + p->n_beta) > 1024) { snprintf(err, 256, "n_act * N_t <= 1024 supported"); return AFQMC_EUNSUPPORTED; }
     const int ts_ = p->precision ? 8 : 4;
     if (md_energy_smem(p->M, p->n_alpha, p->n_beta, p->n_act, p->n_det, ts_) > 200 * 1024 ||
         md_overlap_smem(p->M, p->n_alpha, p->n_beta, p->n_act, p->n_det, ts_) > 200 * 1024) {

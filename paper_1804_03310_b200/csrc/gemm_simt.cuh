@@ -102,7 +102,7 @@ template <typename T> struct EpiEnergy {
   }
 };
 
-// H10: row = g*nact + q, col = (w*2 + p)*nt + a  ->  TT[w][g][q][a] (interleaved complex)
+// H10: row = g*nact + q, col = (w*nt + a)*2 + p  ->  TT[w][g][q][a] (interleaved complex; columns contiguous)
 template <typename T> struct EpiTT {
   T* out; int ng1, nact, nt; int m_real, n_real;
   template <int TM, int TN>
@@ -112,13 +112,12 @@ template <typename T> struct EpiTT {
       int c = j < TN / 2 ? c0 + j : c1 + j - TN / 2;
       if (c >= n_real) continue;
       int w = c / (2 * nt), rem = c - w * 2 * nt;
-      int p = rem / nt, a = rem - p * nt;
 #pragma unroll
       for (int i = 0; i < TM; ++i) {
         int r = i < TM / 2 ? r0 + i : r1 + i - TM / 2;
         if (r >= m_real) continue;
         int g = r / nact, q = r - g * nact;
-        out[((((size_t)w * ng1 + g) * nact + q) * nt + a) * 2 + p] = acc[i][j];
+        out[(((size_t)w * ng1 + g) * nact + q) * (2 * nt) + rem] = acc[i][j];
       }
     }
   }

@@ -187,15 +187,15 @@ __global__ void k_cast2d(int nr, int nc, const double* src, size_t lds, T* dst, 
 
 
 // ---- multi-determinant energy: operands of the TT = C_act^T X Theta_0 GEMM (X = L_g for all g, then h) ----
-// thT[((w*2+p)*nt + a)*MPK + k] = Re/Im Theta_0[w][k][a]   (K-major rows (walker, plane, column), zero padded)
+// thT[((w*nt + a)*2 + p)*MPK + k] = Re/Im Theta_0[w][k][a]   (K-major rows (walker, column, plane), zero padded)
 template <typename T>
 __global__ void __launch_bounds__(128) k_thT(int M, int nt, int MPK, const cplx<T>* theta, T* thT) {
   const int w = blockIdx.x;
   for (int e = threadIdx.x; e < M * nt; e += blockDim.x) {
     int k = e / nt, a = e - k * nt;
     cplx<T> v = theta[(size_t)w * M * nt + e];
-    thT[((size_t)(w * 2 + 0) * nt + a) * MPK + k] = v.x;
-    thT[((size_t)(w * 2 + 1) * nt + a) * MPK + k] = v.y;
+    thT[(((size_t)w * nt + a) * 2 + 0) * MPK + k] = v.x;
+    thT[(((size_t)w * nt + a) * 2 + 1) * MPK + k] = v.y;
   }
 }
 // RactT[(g*nact + q)*MPK + k] = (C_act^T L_g)[q][k] for g < ng, (C_act^T h)[q][k] for g == ng

@@ -255,7 +255,7 @@ inline size_t md_energy_smem(int M, int na, int nb, int nact, int ndet, int ts) 
   const size_t nw_ = (size_t)(nact - na) * na + (size_t)(nact - nb) * nb;
   // TT, W, WT, Q_virt copy, Z copy, 4 scalars: complex T (the bulk arithmetic follows the walker precision;
   // per-determinant energies and the final mixture are accumulated in FP64)
-  b += ((size_t)nact * (na + nb) + 3 * nw_ + (size_t)ndet * 8 + 4) * 2 * ts + 16;
+  b += ((size_t)2 * nact * (na + nb) + 3 * nw_ + (size_t)ndet * 8 + 4) * 2 * ts + 16;   // TT is double buffered
   return b;
 }
 
@@ -273,9 +273,9 @@ __global__ void __launch_bounds__(MD_THREADS) k_md_energy(MdEnergyArgs<T> g) {
   C* th0 = reinterpret_cast<C*>(p);
   p += ((size_t)M * nt * sizeof(C) + 15) & ~size_t(15);
   const int nwa = (nact - m.na) * m.na, nwb = (nact - m.nb) * m.nb;
-  C* TT = reinterpret_cast<C*>(p);
+  C* TT0 = reinterpret_cast<C*>(p);
   C* Wm[2]; C* WTm[2]; C* Qc[2];
-  Wm[0] = TT + nact * nt; Wm[1] = Wm[0] + nwa;
+  Wm[0] = TT0 + 2 * nact * nt; Wm[1] = Wm[0] + nwa;
   WTm[0] = Wm[1] + nwb; WTm[1] = WTm[0] + nwa;
   Qc[0] = WTm[1] + nwb; Qc[1] = Qc[0] + nwa;
   C* Zc = Qc[1] + nwb;                 // [ndet][2][4]
@@ -307,12 +307,24 @@ __global__ void __launch_bounds__(MD_THREADS) k_md_energy(MdEnergyArgs<T> g) {
   }
   __syncthreads();
 
+  // 1. TT[q][a] = (C_act^T X Theta_0)[q][a], precomputed for all X by one GEMM over all walkers; the tile of the
+  //    next X is fetched into registers while this one is processed (double buffer in shared memory)
+  enum { TTPF = 8 };   // nact * nt <= TTPF * MD_THREADS (checked on the host)
+  const C* srcw = g.TTg + (size_t)w * (g.ng + 1) * nact * nt;
+  for (int e = tid; e < nact * nt; e += nthr) TT0[e] = srcw[e];
+  __syncthreads();
   for (int gi = 0; gi <= g.ng; ++gi) {
     const bool is_h = gi == g.ng;
-    // 1. TT[q][a] = (C_act^T X Theta_0)[q][a], precomputed for all X by one GEMM over all walkers
-    const C* src = g.TTg + ((size_t)w * (g.ng + 1) + gi) * nact * nt;
-    for (int e = tid; e < nact * nt; e += nthr) TT[e] = src[e];
-    __syncthreads();
+    C* TT = TT0 + (gi & 1) * nact * nt;
+    C pre[TTPF];
+    if (gi < g.ng) {
+      const C* src = srcw + (size_t)(gi + 1) * nact * nt;
+#pragma unroll
+      for (int u = 0; u < TTPF; ++u) {
+        const int e = tid + u * MD_THREADS;
+        if (e < nact * nt) pre[u] = src[e];
+      }
+    }
     // 2. W = TT_virt - Q_virt T0 ; f0, X0 by warps 0 / 1
     for (int sp = 0; sp < 2; ++sp) {
       const int n = sp ? m.nb : m.na, nv = nact - n, off = sp ? m.na : 0;
@@ -397,6 +409,14 @@ __global__ void __launch_bounds__(MD_THREADS) k_md_energy(MdEnergyArgs<T> g) {
       } else {
         C e2 = csub(cmul(tsum, tsum), xsum);
         Eacc[j].x += 0.5 * (double)e2.x; Eacc[j].y += 0.5 * (double)e2.y;
+      }
+    }
+    if (gi < g.ng) {
+      C* TTn = TT0 + ((gi + 1) & 1) * nact * nt;
+#pragma unroll
+      for (int u = 0; u < TTPF; ++u) {
+        const int e = tid + u * MD_THREADS;
+        if (e < nact * nt) TTn[e] = pre[u];
       }
     }
     __syncthreads();
