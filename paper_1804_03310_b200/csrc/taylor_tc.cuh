@@ -46,7 +46,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   __shared__ __align__(8) uint64_t full_bar[NST];
   __shared__ __align__(8) uint64_t empty_bar[NST];
-  __shared__ __align__(8) uint64_t tmem_full_bar;
+  __shared__ __align__(8) uint64_t tmem_full_bar[2];   // per 128-row tile: tile 0 is post-processed while tile 1 is issued
   __shared__ __align__(8) uint64_t b_ready_bar;
   __shared__ uint32_t tmem_base_s;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -62,7 +62,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
     *reinterpret_cast<uint4*>(planes + o) = make_uint4(0, 0, 0, 0);
   if (warp == EPW && lane == 0) {
     for (int s = 0; s < NST; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
-    mbar_init(&tmem_full_bar, 1);
+    mbar_init(&tmem_full_bar[0], 1); mbar_init(&tmem_full_bar[1], 1);
     mbar_init(&b_ready_bar, EPW);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -135,8 +135,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
                 }
                 tc_commit(&empty_bar[s]);
               }
+            tc_commit(&tmem_full_bar[mt]);
           }
-          tc_commit(&tmem_full_bar);
         }
     }
   } else {   // ===== epilogue warps 0..7: TMEM lane quarter = warp & 3, half = warp >> 2 (0: real part, 1: imaginary) =====
@@ -150,9 +150,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
       float* phi_w = reinterpret_cast<float*>(g.phi + (size_t)w * M * nt);
       // phase-0 operand: planes <- Phi_w  (row b = walker column, column j = basis index)
       for (int e = (warp & 3) * 32 + lane; e < M * nt; e += 128) {
-        const int j = e / nt, b = e - j * nt;
+        const int b = e / M, j = e - b * M;     // lanes along j: conflict-free plane writes
         float hi, lo;
-        tf32_split(phi_w[2 * e + half], hi, lo);
+        tf32_split(phi_w[2 * (j * nt + b) + half], hi, lo);
         const uint32_t o = plane_off(rb + b, j);
         *reinterpret_cast<float*>(pl_hi + o) = hi;
         *reinterpret_cast<float*>(pl_lo + o) = lo;
@@ -161,49 +161,56 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
       __syncwarp();
       if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&b_ready_bar)) : "memory");
       for (int ph = 0; ph < nphase; ++ph, ++gph) {
-        mbar_wait(&tmem_full_bar, gph & 1);
-        tc_fence_after();
         const bool last_phase = ph == nphase - 1;
         const float scale = (ph >= 1 && ph <= g.K) ? 1.0f / (float)ph : 1.0f;
+        const bool cxp = ph >= 1 && ph <= g.K;
+        const uint32_t tl = tmem + ((uint32_t)(q * 32) << 16);
+        float vv[2][32];
+        // pass 1 (tile 0 overlaps the MMAs of tile 1): D_re = D1[0:32] - D2[32:64], D_im = D1[32:64] + D2[0:32],
+        // summed over the accumulation chunks; scale, add into the running sum
 #pragma unroll
         for (int mt = 0; mt < 2; ++mt) {
           if (mt < mtiles) {
-            // D_re = D1[0:32] - D2[32:64] ; D_im = D1[32:64] + D2[0:32], summed over the accumulation chunks
-            float v[32];
-            const bool cxp = ph >= 1 && ph <= g.K;
-            const uint32_t tl = tmem + ((uint32_t)(q * 32) << 16);
+            mbar_wait(&tmem_full_bar[mt], gph & 1);
+            tc_fence_after();
 #pragma unroll
-            for (int b = 0; b < 32; ++b) v[b] = 0.f;
+            for (int b = 0; b < 32; ++b) vv[mt][b] = 0.f;
             for (int ch = 0; ch < g.nch; ++ch) {
               float u[32];
               tmem_ld32(tl + ((mt * 2 + 0) * g.nch + ch) * 64 + half * 32, u);
 #pragma unroll
-              for (int b = 0; b < 32; ++b) v[b] += u[b];
+              for (int b = 0; b < 32; ++b) vv[mt][b] += u[b];
               if (cxp) {
                 tmem_ld32(tl + ((mt * 2 + 1) * g.nch + ch) * 64 + (1 - half) * 32, u);
 #pragma unroll
-                for (int b = 0; b < 32; ++b) v[b] = half ? v[b] + u[b] : v[b] - u[b];
+                for (int b = 0; b < 32; ++b) vv[mt][b] = half ? vv[mt][b] + u[b] : vv[mt][b] - u[b];
               }
             }
-            const int i = mt * 128 + q * 32 + lane;     // output row = basis index
 #pragma unroll
             for (int b = 0; b < 32; ++b) {
-              float t = v[b] * scale;
+              float t = vv[mt][b] * scale;
               if (ph == 0) P[mt][b] = t; else P[mt][b] += t;
               if (ph == g.K) t = P[mt][b];               // operand of the closing E_h product is the sum
-              v[b] = t;
+              vv[mt][b] = t;
             }
+          }
+        }
+        // pass 2: every MMA of this phase has completed, the T planes may be overwritten
+#pragma unroll
+        for (int mt = 0; mt < 2; ++mt) {
+          if (mt < mtiles) {
+            const int i = mt * 128 + q * 32 + lane;     // output row = basis index
             if (i < M) {
               if (last_phase) {
 #pragma unroll
                 for (int b = 0; b < 32; ++b)
-                  if (b < nt) phi_w[2 * (i * nt + b) + half] = v[b];
+                  if (b < nt) phi_w[2 * (i * nt + b) + half] = vv[mt][b];
               } else {
 #pragma unroll
                 for (int b = 0; b < 32; ++b) {
                   if (b < nt) {
                     float hi, lo;
-                    tf32_split(v[b], hi, lo);
+                    tf32_split(vv[mt][b], hi, lo);
                     const uint32_t o = plane_off(rb + b, i);
                     *reinterpret_cast<float*>(pl_hi + o) = hi;
                     *reinterpret_cast<float*>(pl_lo + o) = lo;
