@@ -64,6 +64,7 @@ struct afqmc_ctx {
   // init staging (FP64)
   double *Ld, *hd, *hpd, *Rd, *hrotd, *ex[4], *psid;
   tc::Maps map_asm, map_fb[2], map_en[2];
+  int nblk; int2* blk;   // symmetric block list of the tcgen05 assembly GEMM
   int tay_tc; void *Abuf_lo, *Eh_lo; tt::TaylorMaps map_tay; tt::TaylorTcArgs tay_args; size_t tay_tc_smem; int n_sm;   // TMA descriptors of the tcgen05 path (path == 2)
   char err[256];
   int64_t launches;
@@ -192,8 +193,15 @@ void carve(const afqmc_params* p, afqmc_ctx* c, char* cbase, char* wbase, size_t
   c->psi_b = cc.take((size_t)M * (nb ? nb : 1) * ts);
   c->Eh = cc.take((size_t)M * MP * ts);
   c->Eh_lo = split ? cc.take((size_t)M * MP * ts) : nullptr;
-  c->Lt = cc.take((size_t)M * M * NGP * ts);
-  c->Lt_lo = split ? cc.take((size_t)M * M * NGP * ts) : nullptr;
+  // tcgen05 path: only the 8 x 16 blocks (i-block, j-block) that touch the upper triangle of the symmetric A_w
+  c->nblk = 0;
+  for (int ib = 0; ib * 8 < M; ++ib)
+    for (int jb = 0; jb * 16 < M; ++jb)
+      if (ib * 8 <= jb * 16 + 15) ++c->nblk;
+  const size_t lt_rows = split ? (size_t)c->nblk * 128 : (size_t)M * M;
+  c->Lt = cc.take(lt_rows * NGP * ts);
+  c->Lt_lo = split ? cc.take(lt_rows * NGP * ts) : nullptr;
+  c->blk = (int2*)cc.take((size_t)(c->nblk ? c->nblk : 1) * sizeof(int2));
   c->Rall = cc.take((size_t)rup(ng, 128) * KT * ts);
   c->Rall_lo = split ? cc.take((size_t)rup(ng, 128) * KT * ts) : nullptr;
   const size_t ya = md ? 32 : KA, yb = (md || !KB) ? 32 : KB;   // Y is not used by the multi-det energy
@@ -330,7 +338,17 @@ template <typename T> afqmc_status init_device(afqmc_ctx* c, const double* h1, c
            (size_t)KT, c->split);
     LAUNCH(c, k_cast2d<T>, (KT + 127) / 128, 128, 0, 1, KT, c->hrotd, (size_t)KT, (T*)c->hrot, (T*)nullptr, (size_t)KT, 0);
   }
-  // Lt[ij][g] = L[g][ij]  (K-major operand of the assembly GEMM)
+  // Lt[ij][g] = L[g][ij]  (K-major operand of the assembly GEMM); tcgen05 path: symmetric block packing
+  if (c->split) {
+    std::vector<int2> tab;
+    for (int ib = 0; ib * 8 < M; ++ib)
+      for (int jb = 0; jb * 16 < M; ++jb)
+        if (ib * 8 <= jb * 16 + 15) tab.push_back(make_int2(ib, jb));
+    CUDA_OK(c, cudaMemcpyAsync(c->blk, tab.data(), tab.size() * sizeof(int2), cudaMemcpyHostToDevice, st));
+    CUDA_OK(c, cudaStreamSynchronize(st));
+    size_t tot = (size_t)c->nblk * 128 * ng;
+    LAUNCH(c, k_pack_Lt<T>, (unsigned)((tot + 255) / 256), 256, 0, M, ng, NGP, c->nblk, c->blk, c->Ld, (T*)c->Lt, (T*)c->Lt_lo);
+  } else
   LAUNCH(c, k_transpose_cast<T>, dim3((ng + 31) / 32, (mm + 31) / 32), dim3(32, 8), 0, mm, ng, c->Ld, (size_t)mm,
          (T*)c->Lt, (T*)c->Lt_lo, (size_t)NGP, c->split);
   CUDA_OK(c, cudaStreamSynchronize(st));
@@ -517,8 +535,14 @@ afqmc_status do_propagate(afqmc_ctx* c, void* phi, const void* x, const void* fb
     if constexpr (sizeof(T) == 4) {
       if (c->path == 2) {
         tc::EpiAssemble e2;
-        e2.out = (float*)c->Abuf; e2.out_lo = c->tay_tc ? (float*)c->Abuf_lo : nullptr; e2.M = c->M; e2.MP = c->MP; e2.m_real = c->M * c->M; e2.n_real = 2 * c->nw;
-        st = run_gemm_tc(c, c->map_asm, c->M * c->M, 2 * c->nw, c->NGP, e2);
+        e2.out = (float*)c->Abuf; e2.out_lo = c->tay_tc ? (float*)c->Abuf_lo : nullptr; e2.blk = c->blk; e2.M = c->M; e2.MP = c->MP; e2.m_real = c->nblk * 128; e2.n_real = 2 * c->nw;
+        st = run_gemm_tc(c, c->map_asm, c->nblk * 128, 2 * c->nw, c->NGP, e2);
+        if (!st) {
+          const int nt32 = (c->M + 31) / 32;
+          dim3 sg(nt32 * (nt32 + 1) / 2, c->nw);
+          LAUNCH(c, k_symmetrize<float>, sg, dim3(32, 8), 0, c->M, c->MP, (float*)c->Abuf,
+                 c->tay_tc ? (float*)c->Abuf_lo : (float*)nullptr);
+        }
         done = true;
       }
     }
@@ -761,8 +785,8 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
     using namespace tc;
     bool ok = true;
     const uint64_t nrow = 2 * (uint64_t)c->nw;
-    ok &= make_map(&c->map_asm.a_hi, c->Lt, c->NGP, (uint64_t)c->M * c->M, c->NGP, BM);
-    ok &= make_map(&c->map_asm.a_lo, c->Lt_lo, c->NGP, (uint64_t)c->M * c->M, c->NGP, BM);
+    ok &= make_map(&c->map_asm.a_hi, c->Lt, c->NGP, (uint64_t)c->nblk * 128, c->NGP, BM);
+    ok &= make_map(&c->map_asm.a_lo, c->Lt_lo, c->NGP, (uint64_t)c->nblk * 128, c->NGP, BM);
     ok &= make_map(&c->map_asm.b_hi, c->Z, c->NGP, nrow, c->NGP, BN);
     ok &= make_map(&c->map_asm.b_lo, c->Z_lo, c->NGP, nrow, c->NGP, BN);
     for (int sp = 0; sp < 2; ++sp) {

@@ -107,23 +107,37 @@ struct EpiStoreT {      // H4: out[col][row]
       if (c0 + j < n_real) out[(size_t)(c0 + j) * ldo + r] = v[j];
   }
 };
-struct EpiAssemble {    // H6: row = i*M + j, col = 2w + p -> A[w][i][p][MP] (+ j); out_lo != null: TF32 hi / lo planes
-  float* out; float* out_lo; int M, MP, m_real, n_real;
+// H6: col = 2w + p -> A[w][i][p][MP] (+ j); out_lo != null: TF32 hi / lo planes.
+// blk == null: row = i*M + j (all M^2 elements).  blk != null: A_w is symmetric, only the 8 x 16 element blocks that
+// touch the upper triangle are computed: row = block*128 + (i % 8)*16 + (j % 16), blk[block] = (i / 8, j / 16); lanes
+// run along j (64-byte segments).  The lower triangle is filled afterwards by k_symmetrize (misc.cuh).
+struct EpiAssemble {
+  float* out; float* out_lo; const int2* blk; int M, MP, m_real, n_real;
+  __device__ __forceinline__ void put(size_t o, float v) const {
+    if (out_lo) {
+      float hi, lo;
+      tf32_split(v, hi, lo);
+      out[o] = hi; out_lo[o] = lo;
+    } else {
+      out[o] = v;
+    }
+  }
   __device__ __forceinline__ void operator()(int r, int c0, const float (&v)[32]) const {
     if (r >= m_real) return;
-    const int ii = r / M, jj = r - ii * M;
+    int ii, jj;
+    if (blk) {
+      const int2 b = blk[r >> 7];
+      ii = b.x * 8 + ((r >> 4) & 7); jj = b.y * 16 + (r & 15);
+      if (ii >= M || jj >= M) return;
+    } else {
+      ii = r / M; jj = r - ii * M;
+    }
 #pragma unroll
     for (int j = 0; j < 32; ++j) {
       const int c = c0 + j;
       if (c < n_real) {
-        const size_t o = ((size_t)(c >> 1) * M + ii) * (2 * MP) + (c & 1) * MP + jj;
-        if (out_lo) {
-          float hi, lo;
-          tf32_split(v[j], hi, lo);
-          out[o] = hi; out_lo[o] = lo;
-        } else {
-          out[o] = v[j];
-        }
+        const size_t base = (size_t)(c >> 1) * M * (2 * MP) + (c & 1) * MP;
+        put(base + (size_t)ii * (2 * MP) + jj, v[j]);
       }
     }
   }

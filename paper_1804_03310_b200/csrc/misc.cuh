@@ -211,4 +211,56 @@ __global__ void k_init_ractT(int ng, int nact, int M, int MPK, const double* Rd,
   out[((size_t)g * nact + q) * MPK + k] = (T)v;
 }
 
+
+// Symmetric-packed K-major L for the tcgen05 assembly GEMM: row = block*128 + (i%8)*16 + (j%16) (see tc::EpiAssemble)
+template <typename T>
+__global__ void k_pack_Lt(int M, int ng, int NGP, int nblk, const int2* blk, const double* L, T* Lt, T* Lt_lo) {
+  size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= (size_t)nblk * 128 * ng) return;
+  int g = (int)(e % ng), r = (int)(e / ng);
+  const int2 b = blk[r >> 7];
+  int i = b.x * 8 + ((r >> 4) & 7), j = b.y * 16 + (r & 15);
+  double v = (i < M && j < M) ? L[(size_t)g * M * M + (size_t)i * M + j] : 0.0;
+  float hi, lo;
+  tf32_split((float)v, hi, lo);
+  Lt[(size_t)r * NGP + g] = (T)hi;
+  Lt_lo[(size_t)r * NGP + g] = (T)lo;
+}
+
+
+// A[w][i][p][j] := A[w][j][p][i] for i > j (A_w is symmetric; the assembly GEMM wrote the upper blocks only).
+// grid = (tile pairs TI >= TJ, walkers), block = 32 x 8; each CTA moves one 32 x 32 tile of both planes of both
+// buffers (hi / lo) through shared memory: 16 independent loads per thread in flight.
+template <typename T>
+__global__ void __launch_bounds__(256) k_symmetrize(int M, int MP, T* A, T* A_lo) {
+  __shared__ T tile[4][32][33];
+  int t = blockIdx.x, TI = 0;
+  while (t > TI) { t -= TI + 1; ++TI; }
+  const int TJ = t;                        // TI >= TJ
+  const int nbuf = A_lo ? 2 : 1;
+  const size_t woff = ((size_t)blockIdx.y * M) * (2 * MP);
+  const int tx = threadIdx.x, ty = threadIdx.y;
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    if (q >= 2 * nbuf) break;
+    const T* src = (q >> 1 ? A_lo : A) + woff + (q & 1) * MP;
+#pragma unroll
+    for (int r = ty; r < 32; r += 8) {
+      int j = TJ * 32 + r, i = TI * 32 + tx;
+      tile[q][r][tx] = (j < M && i < M) ? src[(size_t)j * (2 * MP) + i] : T(0);
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    if (q >= 2 * nbuf) break;
+    T* dst = (q >> 1 ? A_lo : A) + woff + (q & 1) * MP;
+#pragma unroll
+    for (int r = ty; r < 32; r += 8) {
+      int i = TI * 32 + r, j = TJ * 32 + tx;
+      if (i < M && j < M && i > j) dst[(size_t)i * (2 * MP) + j] = tile[q][tx][r];
+    }
+  }
+}
+
 }  // namespace afq

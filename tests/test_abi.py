@@ -53,7 +53,7 @@ def test_query_bytes_and_argument_errors(afq):
     cb, wb = afq.afqmc_query_bytes(p)
     assert cb % 256 == 0 and wb % 256 == 0
     # L^T (160 MB) + R (20 MB) + Y (2624^2 + 2400^2 floats) dominate the constants; x2 for the TF32 hi/lo planes
-    assert 4.0e8 < cb < 5.0e8 and wb > 2048 * 200 * 200 * 8
+    assert 3.0e8 < cb < 4.0e8 and wb > 2048 * 200 * 200 * 8   # L^T is symmetric-block packed on this path
     cb1, _ = afq.afqmc_query_bytes(afq.make_params(200, 13, 12, 1000, 2048, "c64", 0.005, gemm_path=1))
     assert 2.0e8 < cb1 < 3.0e8
     bad = [afq.make_params(0, 1, 1, 4, 4, "c64", 0.01), afq.make_params(8, 9, 1, 4, 4, "c64", 0.01),
