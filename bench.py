@@ -234,22 +234,49 @@ def run_ours(args):
     pk = peaks()
     fl = flops_per_walker_step(wl)
     value = D.whole_job_rate(nw * K, world, ms_max * 1e-3)
-    # dominant kernel: the one-body-operator assembly GEMM (H6)
-    a_ms, a_n = prof["assemble"]
-    a_flops = fl["assemble"] * nw
+    # roofline of the dominant kernel = the stage with the largest device time (CUDA events on the launching
+    # stream, afqmc_profile_*); the H6 assembly GEMM is always reported beside it as `roofline_h6`
+    M_, ng_ = wl.M, wl.n_chol
     if ctx.gemm_path == 2:
-        bound, peak, peak_note = "tensor", 0.5 * pk["bf16_burst"], (
-            f"TF32 dense = {pk['source']} burst BF16 {pk['bf16_burst']} TF/s x nominal TF32/BF16 ratio 0.5 (the kernel runs "
-            f"~1 ms inside a ~5 ms step, no power-cap reason active; sustained figure would be {0.5 * pk['bf16_sust']:.0f}); "
+        # the tcgen05 assembly GEMM exploits A = A^T: its algorithmic work is the upper triangle only
+        fl["assemble"] = 4.0 * ng_ * M_ * (M_ + 1) / 2
+        peak, peak_note = 0.5 * pk["bf16_burst"], (
+            f"TF32 dense = {pk['source']} burst BF16 {pk['bf16_burst']} TF/s x nominal TF32/BF16 ratio 0.5 (each kernel runs "
+            f"1-2 ms inside a ~5 ms step, no power-cap reason active; sustained figure would be {0.5 * pk['bf16_sust']:.0f}); "
             "achieved counts ALGORITHMIC flops and 3xTF32 issues 3x of them, so frac <= 1/3 by construction")
-        dtype = "tf32x3"
+        bound, dtype = "tensor", "tf32x3"
     else:
         fp32_peak = 148 * 128 * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
         bound, peak, peak_note = "alu", fp32_peak, "FP32 FMA: 148 SMs x 128 lanes x 2 flop x clocks.max.sm (DESIGN.md)"
         dtype = "f32" if wl.precision == "c64" else "f64"
         if wl.precision == "c128":
             peak, peak_note = fp32_peak / 2, "FP64 FMA: 148 SMs x 64 lanes x 2 flop x clocks.max.sm (DESIGN.md)"
-    achieved = a_flops * a_n / (a_ms * 1e-3) / 1e12 if a_ms > 0 else None
+    names = dict(assemble="H6 assembly GEMM A_w = sum_g z_g L_g (tc::k_gemm_tf32<EpiAssemble> / k_gemm_nt)",
+                 taylor="H7 Taylor propagator (tt::k_taylor_tc / k_taylor)",
+                 energy="H9 energy GEMMs + fused dot (or H10 multi-det energy)", force_bias="H4 force-bias GEMMs",
+                 green="H1-H3/H8 overlap, LU, Theta, weights (k_green)")
+    traffic_ncu = {"assemble": 1.306e9, "taylor": 2.10e9} if (ctx.gemm_path == 2 and args.cfg == 5) else {}
+
+    def roof(stage):
+        ms, n = prof[stage]
+        if not n or ms <= 0 or stage not in fl:
+            return None
+        ach = fl[stage] * nw * n / (ms * 1e-3) / 1e12
+        r = dict(bound=bound, kernel=names[stage], achieved=ach, peak=peak, unit="TFLOP/s", frac=ach / peak,
+                 traffic=traffic_ncu.get(stage), peak_source=peak_note, launches_timed=n, ms_per_launch=ms / n)
+        if ctx.gemm_path == 2:
+            r["issued_frac"] = 3.0 * ach / peak
+        if stage == "green":      # HBM-bound stage: bytes, not flops
+            cb = 8 if wl.precision == "c64" else 16
+            byts = nw * wl.M * wl.n_t * cb * (2 + (2 if ctx.gemm_path == 2 else 1))
+            r.update(bound="hbm", achieved=byts * n / (ms * 1e-3) / 1e9, peak=pk["hbm"], unit="GB/s",
+                     peak_source=f"{pk['source']} HBM copy bandwidth")
+            r["frac"] = r["achieved"] / r["peak"]
+            r.pop("issued_frac", None)
+        return r
+
+    timed = {k: v[0] / v[1] for k, v in prof.items() if v[1] and k in names}
+    dominant = max(timed, key=timed.get) if timed else "assemble"
     stage_ms = {k: (v[0] / v[1] if v[1] else None) for k, v in prof.items()}
     stage_tflops = {k: (fl[k] * nw / (stage_ms[k] * 1e-3) / 1e12 if stage_ms.get(k) else None) for k in fl}
     base = None
@@ -266,12 +293,7 @@ def run_ours(args):
                 e2e=dict(value=world * nw * Ke / t_e2e, unit=UNIT, h2d_bytes_per_step=up / Ke, d2h_bytes_per_step=down / Ke,
                          steps=Ke, note="afqmc_step_host: pinned host buffers, H2D of walkers+fields and D2H of "
                                         "walkers/weights/overlaps/energies inside the timed region"),
-                roofline=dict(bound=bound, kernel="H6 assemble GEMM A_w = sum_g z_g L_g", achieved=achieved, peak=peak,
-                              unit="TFLOP/s", frac=(achieved / peak) if achieved else None,
-                              traffic=1.306e9 if (ctx.gemm_path == 2 and args.cfg == 5) else None,
-                              peak_source=peak_note, launches_timed=a_n, ms_per_launch=stage_ms["assemble"],
-                              issued_frac=(3.0 * achieved / peak) if (achieved and ctx.gemm_path == 2) else None,
-                              traffic_note="ncu dram__bytes_read+write per launch: 1.306 GB (profiles/r1_ncu_full.md)"),
+                roofline=roof(dominant), roofline_h6=roof("assemble"),
                 stages_ms=stage_ms, stages_tflops=stage_tflops, cpu_baseline=base)
     print(json.dumps(line))
     if world > 1:

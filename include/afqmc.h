@@ -162,7 +162,8 @@ enum {
   AFQMC_STAGE_GREEN = 3,      /* H1-H3 + H8 (+ H10 overlap part) */
   AFQMC_STAGE_FORCE_BIAS = 4, /* H4 GEMM + finish */
   AFQMC_STAGE_ENERGY = 5,     /* H9 GEMMs / H10 energy */
-  AFQMC_N_STAGES = 6
+  AFQMC_STAGE_SYMMETRIZE = 6, /* H6 tail: lower triangle of A_w from the upper one (tcgen05 path) */
+  AFQMC_N_STAGES = 7
 };
 AFQMC_API afqmc_status afqmc_profile_enable(afqmc_ctx* ctx, int32_t enable);
 AFQMC_API afqmc_status afqmc_profile_read(afqmc_ctx* ctx, int32_t stage, double* total_ms, int32_t* launches);

@@ -21,7 +21,7 @@ SYMBOLS = ["afqmc_query_bytes", "afqmc_init", "afqmc_destroy", "afqmc_last_error
            "afqmc_force_bias", "afqmc_propagate", "afqmc_local_energy", "afqmc_step", "afqmc_step_host",
            "afqmc_launch_count", "afqmc_gemm_path", "afqmc_profile_enable", "afqmc_profile_read"]
 
-STAGES = ["shift", "assemble", "taylor", "green", "force_bias", "energy"]
+STAGES = ["shift", "assemble", "taylor", "green", "force_bias", "energy", "symmetrize"]
 
 
 class AfqmcParams(C.Structure):

@@ -537,12 +537,6 @@ afqmc_status do_propagate(afqmc_ctx* c, void* phi, const void* x, const void* fb
         tc::EpiAssemble e2;
         e2.out = (float*)c->Abuf; e2.out_lo = c->tay_tc ? (float*)c->Abuf_lo : nullptr; e2.blk = c->blk; e2.M = c->M; e2.MP = c->MP; e2.m_real = c->nblk * 128; e2.n_real = 2 * c->nw;
         st = run_gemm_tc(c, c->map_asm, c->nblk * 128, 2 * c->nw, c->NGP, e2);
-        if (!st) {
-          const int nt32 = (c->M + 31) / 32;
-          dim3 sg(nt32 * (nt32 + 1) / 2, c->nw);
-          LAUNCH(c, k_symmetrize<float>, sg, dim3(32, 8), 0, c->M, c->MP, (float*)c->Abuf,
-                 c->tay_tc ? (float*)c->Abuf_lo : (float*)nullptr);
-        }
         done = true;
       }
     }
@@ -550,6 +544,15 @@ afqmc_status do_propagate(afqmc_ctx* c, void* phi, const void* x, const void* fb
     EpiAssemble<T> epi;
     epi.out = (T*)c->Abuf; epi.M = c->M; epi.MP = c->MP; epi.m_real = c->M * c->M; epi.n_real = 2 * c->nw;
     st = run_gemm<T>(c, (const T*)c->Lt, c->NGP, c->M * c->M, (const T*)c->Z, c->NGP, 2 * c->nw, c->NGP, epi);
+    }
+  }
+  if constexpr (sizeof(T) == 4) {
+    if (!st && c->path == 2) {
+      StageScope sc(c, AFQMC_STAGE_SYMMETRIZE);
+      const int nt32 = (c->M + 31) / 32;
+      dim3 sg(nt32 * (nt32 + 1) / 2, c->nw);
+      LAUNCH(c, k_symmetrize<float>, sg, dim3(32, 8), 0, c->M, c->MP, (float*)c->Abuf,
+             c->tay_tc ? (float*)c->Abuf_lo : (float*)nullptr);
     }
   }
   if (st) return st;
