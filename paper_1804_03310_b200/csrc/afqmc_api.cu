@@ -534,9 +534,16 @@ afqmc_status do_propagate(afqmc_ctx* c, void* phi, const void* x, const void* fb
     bool done = false;
     if constexpr (sizeof(T) == 4) {
       if (c->path == 2) {
+        if (c->M % 4 == 0) {   // staged epilogue writes both triangles: no symmetrize pass
+          tc::EpiAssembleSym e3;
+          e3.out = (float*)c->Abuf; e3.out_lo = c->tay_tc ? (float*)c->Abuf_lo : nullptr; e3.blk = c->blk; e3.M = c->M;
+          e3.MP = c->MP; e3.n_real = 2 * c->nw;
+          st = run_gemm_tc(c, c->map_asm, c->nblk * 128, 2 * c->nw, c->NGP, e3);
+          done = true;
+        }
         tc::EpiAssemble e2;
         e2.out = (float*)c->Abuf; e2.out_lo = c->tay_tc ? (float*)c->Abuf_lo : nullptr; e2.blk = c->blk; e2.M = c->M; e2.MP = c->MP; e2.m_real = c->nblk * 128; e2.n_real = 2 * c->nw;
-        st = run_gemm_tc(c, c->map_asm, c->nblk * 128, 2 * c->nw, c->NGP, e2);
+        if (!done) st = run_gemm_tc(c, c->map_asm, c->nblk * 128, 2 * c->nw, c->NGP, e2);
         done = true;
       }
     }
@@ -547,7 +554,7 @@ afqmc_status do_propagate(afqmc_ctx* c, void* phi, const void* x, const void* fb
     }
   }
   if constexpr (sizeof(T) == 4) {
-    if (!st && c->path == 2) {
+    if (!st && c->path == 2 && c->M % 4 != 0) {
       StageScope sc(c, AFQMC_STAGE_SYMMETRIZE);
       const int nt32 = (c->M + 31) / 32;
       dim3 sg(nt32 * (nt32 + 1) / 2, c->nw);
@@ -809,6 +816,7 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
     cudaError_t e1 = cudaFuncSetAttribute(k_gemm_tf32<tc::EpiStoreT>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     cudaError_t e2 = cudaFuncSetAttribute(k_gemm_tf32<tc::EpiAssemble>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     cudaError_t e3 = cudaFuncSetAttribute(k_gemm_tf32<tc::EpiEnergy>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(k_gemm_tf32<tc::EpiAssembleSym>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     if (!ok || e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) {
       snprintf(g_init_err, 256, "tcgen05 path: tensor-map / shared-memory set-up failed");
       delete c;

@@ -99,6 +99,7 @@ struct Maps {
 
 // ---- epilogues: called per epilogue thread with its accumulator row and 32 consecutive columns -------------
 struct EpiStoreT {      // H4: out[col][row]
+  static constexpr bool kStaged = false;
   float* out; int ldo, m_real, n_real;
   __device__ __forceinline__ void operator()(int r, int c0, const float (&v)[32]) const {
     if (r >= m_real) return;
@@ -112,6 +113,7 @@ struct EpiStoreT {      // H4: out[col][row]
 // touch the upper triangle are computed: row = block*128 + (i % 8)*16 + (j % 16), blk[block] = (i / 8, j / 16); lanes
 // run along j (64-byte segments).  The lower triangle is filled afterwards by k_symmetrize (misc.cuh).
 struct EpiAssemble {
+  static constexpr bool kStaged = false;
   float* out; float* out_lo; const int2* blk; int M, MP, m_real, n_real;
   __device__ __forceinline__ void put(size_t o, float v) const {
     if (out_lo) {
@@ -142,7 +144,47 @@ struct EpiAssemble {
     }
   }
 };
+// H6, symmetric and staged (M % 4 == 0): the 128 x 256 tile (one 8 x 16 block of (i, j) for 128 walkers x 2 planes)
+// goes through the now idle stage memory, S[col][i%8][j%16], and leaves as 16-byte vectors in BOTH orientations:
+// A[w][i][p][j..j+3] (64-byte runs) and A[w][j][p][i..i+3] (32-byte runs), so no separate symmetrize pass is needed.
+struct EpiAssembleSym {
+  static constexpr bool kStaged = true;
+  float* out; float* out_lo; const int2* blk; int M, MP, n_real;
+  __device__ __forceinline__ void operator()(int, int, const float (&)[32]) const {}
+  __device__ __forceinline__ void put4(size_t o, float4 v) const {
+    if (out_lo) {
+      float4 h, l;
+      tf32_split(v.x, h.x, l.x); tf32_split(v.y, h.y, l.y); tf32_split(v.z, h.z, l.z); tf32_split(v.w, h.w, l.w);
+      *reinterpret_cast<float4*>(out + o) = h;
+      *reinterpret_cast<float4*>(out_lo + o) = l;
+    } else {
+      *reinterpret_cast<float4*>(out + o) = v;
+    }
+  }
+  // t = thread index among the 256 epilogue threads; S = staged tile, S[c * 128 + ii * 16 + jj]
+  __device__ __forceinline__ void flush(const float* S, int m0, int n0, int t) const {
+    const int2 b = blk[m0 >> 7];
+    const int i0 = b.x * 8, j0 = b.y * 16;
+    for (int u = t; u < 256 * 32; u += 256) {          // direct: (column c, row ii, vector v of 4 jj)
+      const int c = u >> 5, ii = (u >> 2) & 7, v = u & 3;
+      const int col = n0 + c, i = i0 + ii, j = j0 + 4 * v;
+      if (col >= n_real || i >= M || j >= M) continue;
+      const float4 x = *reinterpret_cast<const float4*>(S + c * 128 + ii * 16 + 4 * v);
+      put4((size_t)(col >> 1) * M * (2 * MP) + (col & 1) * MP + (size_t)i * (2 * MP) + j, x);
+    }
+    for (int u = t; u < 256 * 32; u += 256) {          // mirrored: (column c, row jj, vector v of 4 ii)
+      const int c = u >> 5, jj = (u >> 1) & 15, v = u & 1;
+      const int col = n0 + c, j = j0 + jj, i = i0 + 4 * v;
+      if (col >= n_real || i >= M || j >= M) continue;
+      const float* p = S + c * 128 + (4 * v) * 16 + jj;
+      const float4 x = make_float4(p[0], p[16], p[32], p[48]);
+      put4((size_t)(col >> 1) * M * (2 * MP) + (col & 1) * MP + (size_t)j * (2 * MP) + i, x);
+    }
+  }
+};
+
 struct EpiEnergy {      // H9: eloc[w] += sum_rows v[row] (0.5 C[row][w] + hrot[row]), v = Theta plane (hi + lo)
+  static constexpr bool kStaged = false;
   const float* thp; const float* thp_lo; int KT, soff; const float* hrot; double* eloc; int m_real, n_real;
   __device__ __forceinline__ void operator()(int r, int c0, const float (&v)[32]) const {
     const bool rok = r < m_real;
@@ -277,12 +319,21 @@ __global__ void __launch_bounds__(THREADS, 1) k_gemm_tf32(const __grid_constant_
       __syncwarp();
       if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&tmem_empty_bar[buf])) : "memory");
     }
+    if constexpr (Epi::kStaged) {
+      // all MMAs have completed (last tmem_full observed) and no TMA load is pending: the stage memory is free
+      float* S = reinterpret_cast<float*>(smem);
 #pragma unroll
-    for (int cb = 0; cb < COLS_PER_WARP / 32; ++cb) {
-      float v[32];
+      for (int j = 0; j < COLS_PER_WARP; ++j) S[(half * COLS_PER_WARP + j) * BM + q * 32 + lane] = acc[j];
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      epi.flush(S, m0, n0, (int)threadIdx.x);
+    } else {
 #pragma unroll
-      for (int j = 0; j < 32; ++j) v[j] = acc[cb * 32 + j];
-      epi(row, n0 + half * COLS_PER_WARP + cb * 32, v);
+      for (int cb = 0; cb < COLS_PER_WARP / 32; ++cb) {
+        float v[32];
+#pragma unroll
+        for (int j = 0; j < 32; ++j) v[j] = acc[cb * 32 + j];
+        epi(row, n0 + half * COLS_PER_WARP + cb * 32, v);
+      }
     }
   }
   tc_fence_before();
