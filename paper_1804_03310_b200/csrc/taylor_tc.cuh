@@ -1,13 +1,15 @@
 // taylor_tc.cuh -- H7 on the tensor pipe: Phi' = E_h [sum_{k<=K} A^k/k!] E_h Phi  (R3, R9).
 // Persistent CTAs, one walker at a time.  Every product X * T (X = E_h real or A_w complex symmetric, T complex
 // M x N_t) is a set of real tcgen05.mma.kind::tf32 products with the 3xTF32 split:
-//     D1 = X_r [T_r | T_i] ,  D2 = X_i [T_r | T_i]  (N = 64 each; a small N makes the a-operand's shared-memory
-//     reads the bound, so re and im share one MMA);  D_re = D1[0:32] - D2[32:64],  D_im = D1[32:64] + D2[0:32]
-//     are combined by the epilogue warps.
+//     D1 = X_r [T_r | T_i] ,  D2 = X_i [T_r | T_i];  D_re = D1[0:32] - D2[32:64],  D_im = D1[32:64] + D2[0:32]
+//     are combined by the epilogue warps.  Measured: with N this small the kernel is bound by the tensor pipe's
+//     shared-memory operand fetch (~64 B/clk/SM; every MMA re-reads its 4 KB a-operand slice), so the products are
+//     packed into as few, as wide MMAs as possible: X_hi [T_hi | T_lo] is ONE N = 128 MMA (columns 0-63: hi*hi,
+//     64-127: hi*lo) and X_lo T_hi one N = 64 MMA into columns 0-63; the epilogue adds the two column halves.
 // a-operand: 128-row x 32-column tiles of X (hi / lo planes) streamed by TMA through a 3-stage ring;
-// b-operand: T as two K-major planes (hi, lo), [64 rows = T_r columns | T_i columns][KP] in shared memory,
+// b-operand: T K-major in shared memory, per 32-column k-block 128 rows: [T_r, T_i (hi) | T_r, T_i (lo)],
 //            rewritten by the epilogue warps after every Taylor term (generic -> async proxy fence);
-// accumulators: TMEM, 64 columns per (128-row tile, plane, chunk).  The running sum P lives in registers.
+// accumulators: TMEM, 128 columns per (128-row tile, plane).  The running sum P lives in registers.
 // Supported: M <= 256, N_t <= 32 (else the SIMT kernel of taylor.cuh runs).
 #pragma once
 #include "gemm_tf32.cuh"
@@ -17,7 +19,7 @@ namespace tt {
 
 using namespace tc;
 
-enum { NST = 3, TILE_BYTES = 128 * 128, STG_BYTES = 2 * TILE_BYTES, PLANE_KB_BYTES = 64 * 128, EPW = 8, NTHREADS = (EPW + 2) * 32 };
+enum { NST = 3, TILE_BYTES = 128 * 128, STG_BYTES = 2 * TILE_BYTES, PLANE_KB_BYTES = 128 * 128, EPW = 8, NTHREADS = (EPW + 2) * 32 };
 
 struct TaylorMaps {
   CUtensorMap A[2][2];   // [hi/lo][0: 128-row box, 1: last-tile box]  over Abuf viewed as [N_w*M][2*MP]
@@ -33,9 +35,9 @@ struct TaylorTcArgs {
   cplx<float>* phi;             // [nw][M][nt] in/out
 };
 
-inline size_t smem_bytes(int nkb) { return (size_t)2 * nkb * PLANE_KB_BYTES + (size_t)NST * STG_BYTES + 1024; }
+inline size_t smem_bytes(int nkb) { return (size_t)nkb * PLANE_KB_BYTES + (size_t)NST * STG_BYTES + 1024; }
 
-// byte offset of element (row b in 0..63, column j) inside one K-major SWIZZLE_128B plane
+// byte offset of element (row b in 0..127, column j) inside the K-major SWIZZLE_128B T operand
 __device__ __forceinline__ uint32_t plane_off(int b, int j) {
   const int kb = j >> 5, jj = j & 31;
   return (uint32_t)(kb * PLANE_KB_BYTES + b * 128 + ((((jj >> 2) ^ (b & 7)) << 4) | ((jj & 3) << 2)));
@@ -52,13 +54,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int M = g.M, nt = g.nt, nkb = g.nkb, mtiles = g.mtiles;
   const uint32_t plane_bytes = (uint32_t)nkb * PLANE_KB_BYTES;
-  uint8_t* planes = smem;                                   // [hi plane | lo plane], rows 0-31 T_r, 32-63 T_i
-  uint8_t* stages = smem + 2 * (size_t)plane_bytes;
+  uint8_t* planes = smem;                                   // rows 0-31 T_r hi, 32-63 T_i hi, 64-95 T_r lo, 96-127 T_i lo
+  uint8_t* stages = smem + (size_t)plane_bytes;
   const int nphase = g.K + 2;
   const uint32_t tmem_cols = 512u;
 
   // zero the planes once: rows >= nt and columns >= M must stay 0 for the whole kernel
-  for (uint32_t o = threadIdx.x * 16; o < 2 * plane_bytes; o += NTHREADS * 16)
+  for (uint32_t o = threadIdx.x * 16; o < plane_bytes; o += NTHREADS * 16)
     *reinterpret_cast<uint4*>(planes + o) = make_uint4(0, 0, 0, 0);
   if (warp == EPW && lane == 0) {
     for (int s = 0; s < NST; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
@@ -106,7 +108,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
     }
   } else if (warp == EPW + 1) {
     if (lane == 0) {   // ===== MMA issuer =====
-      constexpr uint32_t idesc = make_idesc(128, 64);
+      constexpr uint32_t idesc128 = make_idesc(128, 128), idesc64 = make_idesc(128, 64);
       const uint32_t pl = smem_u32(planes);
       uint32_t it = 0, gph = 0;
       for (int w = blockIdx.x; w < g.nw; w += gridDim.x)
@@ -117,21 +119,20 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
           for (int mt = 0; mt < mtiles; ++mt) {
             for (int kb = 0; kb < nkb; ++kb)
               for (int p = 0; p < (cx ? 2 : 1); ++p, ++it) {
-                const uint32_t d = tmem + ((mt * 2 + p) * g.nch + kb / g.chunk_kb) * 64;
+                const uint32_t d = tmem + (mt * 2 + p) * 128;
                 const int s = it % NST;
                 mbar_wait(&full_bar[s], (it / NST) & 1);
                 tc_fence_after();
                 const uint32_t sa = smem_u32(stages + (size_t)s * STG_BYTES);
                 const uint64_t x_hi = make_desc(sa), x_lo = make_desc(sa + TILE_BYTES);
                 const uint32_t kboff = (uint32_t)kb * PLANE_KB_BYTES;
-                const uint64_t t_hi = make_desc(pl + kboff), t_lo = make_desc(pl + plane_bytes + kboff);
-                const bool first = (kb % g.chunk_kb) == 0;
+                const uint64_t t_all = make_desc(pl + kboff);   // 128 rows: hi then lo; its first 64 rows = T_hi
+                const bool first = kb == 0;
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
                   const uint64_t adv = (uint64_t)(k * 2);   // 8 tf32 = 32 bytes = 2 x 16 B
-                  umma_tf32(d, x_lo + adv, t_hi + adv, idesc, (first && k == 0) ? 0u : 1u);
-                  umma_tf32(d, x_hi + adv, t_lo + adv, idesc, 1u);
-                  umma_tf32(d, x_hi + adv, t_hi + adv, idesc, 1u);
+                  umma_tf32(d, x_hi + adv, t_all + adv, idesc128, (first && k == 0) ? 0u : 1u);
+                  umma_tf32(d, x_lo + adv, t_all + adv, idesc64, 1u);
                 }
                 tc_commit(&empty_bar[s]);
               }
@@ -142,7 +143,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
   } else {   // ===== epilogue warps 0..7: TMEM lane quarter = warp & 3, half = warp >> 2 (0: real part, 1: imaginary) =====
     const int q = warp & 3, half = warp >> 2;
     uint8_t* pl_hi = planes;
-    uint8_t* pl_lo = planes + plane_bytes;
+    uint8_t* pl_lo = planes + 64 * 128;       // lo rows start 64 rows further down inside every k-block
     const int rb = half * 32;                 // plane row base: T_r rows 0-31, T_i rows 32-63
     uint32_t gph = 0;
     float P[2][32];
@@ -175,13 +176,19 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
             tc_fence_after();
 #pragma unroll
             for (int b = 0; b < 32; ++b) vv[mt][b] = 0.f;
-            for (int ch = 0; ch < g.nch; ++ch) {
+            {
               float u[32];
-              tmem_ld32(tl + ((mt * 2 + 0) * g.nch + ch) * 64 + half * 32, u);
+              tmem_ld32(tl + (mt * 2 + 0) * 128 + half * 32, u);              // X_r: hi*hi + lo*hi
+#pragma unroll
+              for (int b = 0; b < 32; ++b) vv[mt][b] += u[b];
+              tmem_ld32(tl + (mt * 2 + 0) * 128 + 64 + half * 32, u);         // X_r: hi*lo
 #pragma unroll
               for (int b = 0; b < 32; ++b) vv[mt][b] += u[b];
               if (cxp) {
-                tmem_ld32(tl + ((mt * 2 + 1) * g.nch + ch) * 64 + (1 - half) * 32, u);
+                tmem_ld32(tl + (mt * 2 + 1) * 128 + (1 - half) * 32, u);
+#pragma unroll
+                for (int b = 0; b < 32; ++b) vv[mt][b] = half ? vv[mt][b] + u[b] : vv[mt][b] - u[b];
+                tmem_ld32(tl + (mt * 2 + 1) * 128 + 64 + (1 - half) * 32, u);
 #pragma unroll
                 for (int b = 0; b < 32; ++b) vv[mt][b] = half ? vv[mt][b] + u[b] : vv[mt][b] - u[b];
               }
