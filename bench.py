@@ -67,7 +67,28 @@ class ClockSampler(threading.Thread):
         super().__init__(daemon=True)
         self.index, self.rows, self._halt = index, [], threading.Event()
 
+    def _nvml_loop(self):
+        import pynvml as nv
+        nv.nvmlInit()
+        h = nv.nvmlDeviceGetHandleByIndex(self.index)
+        mx = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+        bits = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40}
+        get_reasons = getattr(nv, "nvmlDeviceGetCurrentClocksEventReasons", None) or nv.nvmlDeviceGetCurrentClocksThrottleReasons
+        while not self._halt.is_set():
+            sm = nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)
+            r = int(get_reasons(h))
+            pw = nv.nvmlDeviceGetPowerUsage(h) / 1000.0
+            row = [str(sm), str(mx), str(pw)] + [("Active" if r & bits[n] else "Not Active")
+                                                 for n in ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")]
+            self.rows.append(row)
+            self._halt.wait(0.002)
+
     def run(self):
+        try:
+            self._nvml_loop()        # NVML in-process: ~1 ms per sample, so even a 50 ms timed region is covered
+            return
+        except Exception:
+            pass
         while not self._halt.is_set():
             try:
                 out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
@@ -90,8 +111,14 @@ class ClockSampler(threading.Thread):
                         reasons.add(n)
             except Exception:
                 continue
+        pw = []
+        for r in self.rows:
+            try:
+                pw.append(float(r[2]))
+            except Exception:
+                pass
         return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=mx or None, reasons=sorted(reasons),
-                    samples=len(sm))
+                    samples=len(sm), power_w_max=max(pw) if pw else None)
 
 
 def time_oracle(wl, target_s=12.0):
