@@ -46,6 +46,7 @@ struct afqmc_ctx {
   // multi-determinant trial (md != 0): ca/cb = columns per spin of the generalised Theta (n_act), else n_alpha/n_beta
   int md, nact, ndet, ca, cb;
   void* Cact; double* coeff; int32_t* exc;
+  double *psid_ac, *psid_bc;   // FP64 trial orbitals (constants)
   void *thtil, *th_scr; zcplx *ovlp0, *ovlp_scr;
   void *RactT, *thT, *TTg; int MPK;
   size_t mdo_smem, mde_smem;
@@ -191,6 +192,8 @@ void carve(const afqmc_params* p, afqmc_ctx* c, char* cbase, char* wbase, size_t
   Carver cc; cc.base = cbase;
   c->psi_a = cc.take((size_t)M * na * ts);
   c->psi_b = cc.take((size_t)M * (nb ? nb : 1) * ts);
+  c->psid_ac = (double*)cc.take((size_t)M * na * 8);
+  c->psid_bc = (double*)cc.take((size_t)M * (nb ? nb : 1) * 8);
   c->Eh = cc.take((size_t)M * MP * ts);
   c->Eh_lo = split ? cc.take((size_t)M * MP * ts) : nullptr;
   // tcgen05 path: only the 8 x 16 blocks (i-block, j-block) that touch the upper triangle of the symmetric A_w
@@ -303,6 +306,8 @@ template <typename T> afqmc_status init_device(afqmc_ctx* c, const double* h1, c
   LAUNCH(c, k_cast2d<T>, (mm + 127) / 128, 128, 0, M, M, E, (size_t)M, (T*)c->Eh, (T*)nullptr, (size_t)MP, 0);
   if (c->tay_tc)   // TF32 hi / lo planes of E_h for the tensor-pipe Taylor kernel (the SIMT kernel never runs then)
     LAUNCH(c, k_cast2d<T>, (mm + 127) / 128, 128, 0, M, M, E, (size_t)M, (T*)c->Eh, (T*)c->Eh_lo, (size_t)MP, 1);
+  CUDA_OK(c, cudaMemcpyAsync(c->psid_ac, psid_a, (size_t)M * na * 8, cudaMemcpyDeviceToDevice, st));
+  if (nb) CUDA_OK(c, cudaMemcpyAsync(c->psid_bc, psid_b, (size_t)M * nb * 8, cudaMemcpyDeviceToDevice, st));
   // trial orbitals in T
   LAUNCH(c, k_cast2d<T>, (M * na + 127) / 128, 128, 0, M, na, psid_a, (size_t)na, (T*)c->psi_a, (T*)nullptr, (size_t)na, 0);
   if (nb) LAUNCH(c, k_cast2d<T>, (M * nb + 127) / 128, 128, 0, M, nb, psid_b, (size_t)nb, (T*)c->psi_b, (T*)nullptr, (size_t)nb, 0);
@@ -363,6 +368,7 @@ afqmc_status run_green(afqmc_ctx* c, const void* phi, void* ovlp, void* theta, i
   GreenArgs<T> g;
   g.M = c->M; g.na = c->na; g.nb = c->nb; g.nw = c->nw;
   g.phi = (const cplx<T>*)phi; g.psi_a = (const T*)c->psi_a; g.psi_b = (const T*)c->psi_b;
+  g.psid_a = c->psid_ac; g.psid_b = c->psid_bc;
   g.theta = (cplx<T>*)theta; g.thp = (T*)c->thp; g.thp_lo = (T*)c->thp_lo;
   g.KA = c->KA; g.KT = c->KT; g.split = c->split;
   g.ovlp = (zcplx*)ovlp; g.do_weight = do_weight; g.cshift = c->cshift; g.weight = weight;

@@ -64,11 +64,88 @@ __device__ void warp_gauss_jordan(cplx<T>* aug, int n, int ld, cplx<T>* fac, int
   det = mk<double>(dre, dim);
 }
 
+// The same elimination executed by a GROUP of 128 threads (4 warps, named barrier `bar_id`): the serial
+// one-warp version left 6 of the CTA's 8 warps idle and dominated the kernel (ncu: most stall samples at the CTA
+// barrier behind it).  work = [fac (n) | prow (2n)] scratch; ctrl = one int.  Warp 0 of the group does the pivot
+// search and carries det / sing (identical in all its lanes).
+__device__ inline void group_gauss_jordan(zcplx* aug, int n, int ld, zcplx* work, int* ctrl, int gtid, int bar_id,
+                                          zcplx& det, int& sing, double eps) {
+  zcplx* fac = work;
+  zcplx* prow = work + n;
+  const int lane = gtid & 31, gwarp = gtid >> 5;
+  double dre = 1.0, dim = 0.0;
+  sing = 0;
+  double thresh = 0.0;
+  if (gwarp == 0) {
+    double amax = 0.0;
+    for (int e = lane; e < n * n; e += 32) amax = fmax(amax, cabs2(aug[(e / n) * ld + (e % n)]));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) amax = fmax(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+    thresh = amax * eps * eps;
+  }
+  for (int col = 0; col < n; ++col) {
+    if (gwarp == 0) {
+      int r = col + lane;
+      double mag = (r < n) ? cabs2(aug[r * ld + col]) : -1.0;
+      int idx = r;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        double om = __shfl_xor_sync(0xffffffffu, mag, o);
+        int oi = __shfl_xor_sync(0xffffffffu, idx, o);
+        if (om > mag || (om == mag && oi < idx)) { mag = om; idx = oi; }
+      }
+      const bool dead = !(mag > 0.0);
+      if (dead) { sing = 1; dre = 0.0; dim = 0.0; }
+      else {
+        if (mag < thresh) sing = 1;
+        if (idx != col) { dre = -dre; dim = -dim; }
+        zcplx p = aug[idx * ld + col];
+        double nr = dre * p.x - dim * p.y;
+        dim = dre * p.y + dim * p.x;
+        dre = nr;
+      }
+      if (lane == 0) {
+        *ctrl = dead ? -1 : idx;
+        if (!dead) prow[2 * n + 2 * n * n] = cinv(aug[idx * ld + col]);   // one FP64 reciprocal per pivot, not 128
+      }
+    }
+    asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
+    const int piv = *ctrl;
+    if (piv < 0) break;                                   // exactly singular: uniform exit
+    // factors (column col, rows permuted) and the scaled pivot row, both out of place
+    const zcplx ip = prow[2 * n + 2 * n * n];
+    for (int c = gtid; c < 2 * n; c += 128) prow[c] = cmul(aug[piv * ld + c], ip);
+    for (int r = gtid; r < n; r += 128) fac[r] = aug[(r == col ? piv : (r == piv ? col : r)) * ld + col];
+    asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
+    // new row r <- (row col <-> row piv swapped) - fac[r] * prow ; new row col <- prow
+    for (int e = gtid; e < n * 2 * n; e += 128) {
+      const int r = e / (2 * n), c = e - r * 2 * n;
+      zcplx v;
+      if (r == col) v = prow[c];
+      else {
+        const int src = (r == piv) ? col : r;            // the old row `col` moves to position piv
+        v = aug[src * ld + c];
+        const zcplx f = fac[r], pr = prow[c];
+        v.x = fma(-f.x, pr.x, v.x); v.x = fma(f.y, pr.y, v.x);
+        v.y = fma(-f.x, pr.y, v.y); v.y = fma(-f.y, pr.x, v.y);
+      }
+      // rows col and piv are both read and written in this pass: stage the result, store after the barrier
+      prow[2 * n + e] = v;
+    }
+    asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
+    for (int e = gtid; e < n * 2 * n; e += 128) aug[(e / (2 * n)) * ld + (e % (2 * n))] = prow[2 * n + e];
+    asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
+  }
+  det = mk<double>(dre, dim);
+}
+
 template <typename T> struct GreenArgs {
   int M, na, nb, nw;
   const cplx<T>* phi;     // [nw][M][nt]
   const T* psi_a;         // [M][na]
   const T* psi_b;         // [M][nb]
+  const double* psid_a;   // FP64 copies (no per-iteration conversion in the overlap loop)
+  const double* psid_b;
   cplx<T>* theta;         // [nw][M][nt] or null
   T* thp;                 // planar [nw][2][KT]: spin-blocked index s_off + k*n_s + a ; may be null
   T* thp_lo;              // tf32 low plane (split != 0)
@@ -88,8 +165,8 @@ template <typename T> inline size_t green_smem_bytes(int M, int na, int nb) {
   int nt = na + nb, ns = na > nb ? na : nb;
   size_t b = ((size_t)M * nt * sizeof(cplx<T>) + 15) & ~size_t(15);   // phi_s
   b += (size_t)2 * ns * (2 * ns + 1) * sizeof(zcplx);   // aug per spin (FP64 on both precision paths)
-  b += (size_t)2 * ns * sizeof(zcplx);                  // fac per spin
-  b += 2 * sizeof(zcplx) + 4 * sizeof(int);
+  b += (size_t)2 * (3 * ns + 2 * ns * ns + 1) * sizeof(zcplx);   // per spin: fac, scaled pivot row, staged update, 1/pivot
+  b += 2 * sizeof(zcplx) + 8 * sizeof(int);
   return (b + 15) & ~size_t(15);
 }
 
@@ -123,49 +200,97 @@ __global__ void __launch_bounds__(256) k_green(GreenArgs<T> g) {
   // 0.3 % of the flops and keeps S, Theta accurate to cond(A) * eps of the FP32 walker itself
   zcplx* aug = reinterpret_cast<zcplx*>(smem_raw + (((size_t)M * nt * sizeof(cplx<T>) + 15) & ~size_t(15)));
   zcplx* fac = aug + 2 * ns * ld;
-  zcplx* dets = fac + 2 * ns;
+  zcplx* dets = fac + 2 * (3 * ns + 2 * ns * ns + 1);
   int* sing = reinterpret_cast<int*>(dets + 2);
+  int* ctrl = sing + 2;
 
   const cplx<T>* phi_w = g.phi + (size_t)w * M * nt;
   for (int e = tid; e < M * nt; e += nthr) phi_s[e] = phi_w[e];
   __syncthreads();
 
-  // A_s[a][b] = sum_k psi_s[k][a] phi[k][off+b]  (real x complex), augmented with the identity
-  for (int e = tid; e < na * na + nb * nb; e += nthr) {
-    int s = e >= na * na;
-    int ee = s ? e - na * na : e;
-    int n = s ? nb : na, off = s ? na : 0;
-    const T* psi = s ? g.psi_b : g.psi_a;
-    int a = ee / n, b = ee % n;
-    double sr = 0.0, si = 0.0;
-    for (int k = 0; k < M; ++k) {
-      double p = (double)psi[k * n + a];
-      cplx<T> v = phi_s[k * nt + off + b];
-      sr = fma(p, (double)v.x, sr);
-      si = fma(p, (double)v.y, si);
+  // A_s[a][b] = sum_k psi_s[k][a] phi[k][off+b]  (real x complex, FP64), augmented with the identity.
+  // FP64 issue slots are the scarce resource here (conversions included), so one work item = (spin, column b, group
+  // of 4 rows a, half of the k range): phi[k][b] is converted once and reused for 4 rows; halves meet in shared atomics.
+  for (int e = tid; e < 2 * ns * ld; e += nthr) aug[e] = mk<double>(0.0, 0.0);
+  __syncthreads();
+  {
+    const int ga = (na + 3) >> 2, gb = (nb + 3) >> 2;
+    const int items_a = na * ga * 2, items = items_a + nb * gb * 2;
+    for (int e = tid; e < items; e += nthr) {
+      const int s = e >= items_a;
+      const int ee = s ? e - items_a : e;
+      const int n = s ? nb : na, off = s ? na : 0, gn = s ? gb : ga;
+      const double* psi = s ? g.psid_b : g.psid_a;
+      const int kh = ee & 1, b = (ee >> 1) % n, a0 = ((ee >> 1) / n) * 4;
+      (void)gn;
+      const int k0 = kh ? (M >> 1) : 0, k1 = kh ? M : (M >> 1);
+      double sr[4] = {0.0, 0.0, 0.0, 0.0}, si[4] = {0.0, 0.0, 0.0, 0.0};
+      for (int k = k0; k < k1; ++k) {
+        const cplx<T> v = phi_s[k * nt + off + b];
+        const double vr = (double)v.x, vi = (double)v.y;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const double pu = (a0 + u < n) ? psi[k * n + a0 + u] : 0.0;
+          sr[u] = fma(pu, vr, sr[u]);
+          si[u] = fma(pu, vi, si[u]);
+        }
+      }
+      zcplx* A = aug + s * ns * ld;
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+        if (a0 + u < n) {
+          double* dst = reinterpret_cast<double*>(&A[(a0 + u) * ld + b]);
+          atomicAdd(dst, sr[u]); atomicAdd(dst + 1, si[u]);
+        }
     }
-    zcplx* A = aug + s * ns * ld;
-    A[a * ld + b] = mk<double>(sr, si);
-    A[a * ld + n + b] = mk<double>(a == b ? 1.0 : 0.0, 0.0);
+    for (int e = tid; e < na + nb; e += nthr) {
+      const int s = e >= na, a = s ? e - na : e, n = s ? nb : na;
+      aug[s * ns * ld + a * ld + n + a] = mk<double>(1.0, 0.0);
+    }
   }
   __syncthreads();
-  if (warp < 2) {
-    int n = warp ? nb : na;
+  {
+    // warps 0-3 invert A_alpha, warps 4-7 A_beta (named barriers 1 / 2)
+    const int grp = warp >> 2, n = grp ? nb : na;
     zcplx det = mk<double>(1.0, 0.0);
     int sg = 0;
-    if (n > 0) warp_gauss_jordan<double>(aug + warp * ns * ld, n, ld, fac + warp * ns, lane, det, sg, sizeof(T) == 4 ? 1e-6 : 1e-13);
-    if (lane == 0) { dets[warp] = det; sing[warp] = sg; }
+    if (n > 0)
+      group_gauss_jordan(aug + grp * ns * ld, n, ld, fac + grp * (3 * ns + 2 * ns * ns + 1), ctrl + grp, tid & 127, 1 + grp, det, sg,
+                         sizeof(T) == 4 ? 1e-6 : 1e-13);
+    if ((tid & 127) == 0) { dets[grp] = det; sing[grp] = sg; }
   }
   __syncthreads();
 
-  // Theta_s = Phi_s A_s^-1
+  // Theta_s = Phi_s A_s^-1.  FP32 path: the FP64 inverse is split into FP32 hi + lo parts and the product runs on the
+  // FP32 pipe (the walker itself is FP32, so FP64 products bought nothing but FP64 issue slots); FP64 path unchanged.
+  cplx<float>* invf = reinterpret_cast<cplx<float>*>(fac);   // [2 spins][ns*ns][hi, lo] (LU scratch, now free)
+  if constexpr (sizeof(T) == 4) {
+    for (int e = tid; e < na * na + nb * nb; e += nthr) {
+      const int s = e >= na * na, ee = s ? e - na * na : e, n = s ? nb : na;
+      const zcplx v = aug[s * ns * ld + (ee / n) * ld + n + (ee % n)];
+      const float hr = (float)v.x, hi = (float)v.y;
+      invf[(s * ns * ns + ee) * 2 + 0] = mk<float>(hr, hi);
+      invf[(s * ns * ns + ee) * 2 + 1] = mk<float>((float)(v.x - (double)hr), (float)(v.y - (double)hi));
+    }
+    __syncthreads();
+  }
   for (int s = 0; s < 2; ++s) {
     int n = s ? nb : na, off = s ? na : 0, soff = s ? g.KA : 0;
     const zcplx* inv = aug + s * ns * ld + n;
     for (int e = tid; e < M * n; e += nthr) {
       int k = e / n, b = e % n;
       zcplx accd = mk<double>(0.0, 0.0);
-      for (int a = 0; a < n; ++a) cfma(accd, to_z(phi_s[k * nt + off + a]), inv[a * ld + b]);
+      if constexpr (sizeof(T) == 4) {
+        cplx<float> ah = mk<float>(0.f, 0.f), al = mk<float>(0.f, 0.f);
+        for (int a = 0; a < n; ++a) {
+          const cplx<float> ph = mk<float>((float)phi_s[k * nt + off + a].x, (float)phi_s[k * nt + off + a].y);
+          cfma(ah, ph, invf[(s * ns * ns + a * n + b) * 2 + 0]);
+          cfma(al, ph, invf[(s * ns * ns + a * n + b) * 2 + 1]);
+        }
+        accd = mk<double>((double)(ah.x + al.x), (double)(ah.y + al.y));
+      } else {
+        for (int a = 0; a < n; ++a) cfma(accd, to_z(phi_s[k * nt + off + a]), inv[a * ld + b]);
+      }
       cplx<T> acc = mk<T>((T)accd.x, (T)accd.y);
       if (g.theta) g.theta[(size_t)w * M * nt + k * nt + off + b] = acc;
       if (g.thp) {
