@@ -44,7 +44,7 @@ def flops_per_walker_step(wl):
     return dict(assemble=4.0 * ng * M * M,                       # real x complex: 2 planes x 2 flop
                 force_bias=4.0 * ng * M * nt,
                 taylor=8.0 * M * M * nt * K + 2 * 4.0 * M * M * nt,
-                energy=4.0 * ((M * na) ** 2 + (M * nb) ** 2),
+                energy=2.0 * ((M * na) ** 2 + (M * nb) ** 2),   # v^T Y v with Y symmetric: upper triangle only
                 green=4.0 * M * (na * na + nb * nb) + 8.0 * M * (na * na + nb * nb))
 
 

@@ -404,10 +404,10 @@ afqmc_status run_gemm(afqmc_ctx* c, const T* A, int lda, int m, const T* B, int 
 }
 
 template <class Epi>
-afqmc_status run_gemm_tc(afqmc_ctx* c, const tc::Maps& maps, int m, int n, int K, Epi epi) {
+afqmc_status run_gemm_tc(afqmc_ctx* c, const tc::Maps& maps, int m, int n, int K, Epi epi, int tri = 0) {
   dim3 grid((n + tc::BN - 1) / tc::BN, (m + tc::BM - 1) / tc::BM);
   auto kern = tc::k_gemm_tf32<Epi>;
-  LAUNCH(c, kern, grid, tc::THREADS, tc::SMEM_BYTES, maps, K, epi);
+  LAUNCH(c, kern, grid, tc::THREADS, tc::SMEM_BYTES, maps, K, tri, epi);
   return AFQMC_OK;
 }
 
@@ -473,7 +473,7 @@ template <typename T> afqmc_status run_energy_gemm(afqmc_ctx* c, zcplx* eloc) {
         tc::EpiEnergy e2;
         e2.thp = (const float*)c->thp; e2.thp_lo = (const float*)c->thp_lo; e2.KT = c->KT; e2.soff = soff;
         e2.hrot = (const float*)c->hrot + soff; e2.eloc = (double*)eloc; e2.m_real = c->M * n; e2.n_real = 2 * c->nw;
-        afqmc_status st2 = run_gemm_tc(c, c->map_en[s], c->M * n, 2 * c->nw, Ks, e2);
+        afqmc_status st2 = run_gemm_tc(c, c->map_en[s], c->M * n, 2 * c->nw, Ks, e2, 1);
         if (st2) return st2;
         continue;
       }

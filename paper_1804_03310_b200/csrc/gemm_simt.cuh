@@ -58,7 +58,7 @@ template <typename T> struct EpiAssemble {
   }
 };
 
-// H9: per column pair (walker w): e += sum_rows v[row] * (0.5 * C[row][w] + hrot[row]), v = planar Theta
+// H9: per column pair (walker w): e += sum_rows v[row] * (C[row][w] + hrot[row]), C = Y' v, v = planar Theta
 // block of this spin, complex bilinear (no conjugation).  Accumulated into eloc[w] (FP64 atomics).
 template <typename T> struct EpiEnergy {
   const T* thp; const T* thp_lo; int KT; int soff;   // v_re = thp[(2w)*KT + soff + row] (+ lo plane if split)
@@ -86,8 +86,8 @@ template <typename T> struct EpiEnergy {
         size_t o = (size_t)(2 * w) * KT + soff + r;
         T vr = thp[o], vi = thp[o + KT];
         if (thp_lo) { vr += thp_lo[o]; vi += thp_lo[o + KT]; }
-        T ur = T(0.5) * acc[i][j] + hrot[r];
-        T ui = T(0.5) * acc[i][j + 1];
+        T ur = acc[i][j] + hrot[r];          // acc = Y' v with Y' = triu(Y), diagonal halved: v^T Y' v = 1/2 v^T Y v
+        T ui = acc[i][j + 1];
         er += (double)(vr * ur - vi * ui);
         ei += (double)(vr * ui + vi * ur);
       }

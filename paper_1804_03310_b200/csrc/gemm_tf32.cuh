@@ -198,7 +198,7 @@ struct EpiEnergy {      // H9: eloc[w] += sum_rows v[row] (0.5 C[row][w] + hrot[
       if (rok && c < n_real) {
         const size_t o = (size_t)c * KT + soff + r;
         const float vr = thp[o] + thp_lo[o], vi = thp[o + KT] + thp_lo[o + KT];
-        const float ur = 0.5f * v[j] + hr, ui = 0.5f * v[j + 1];
+        const float ur = v[j] + hr, ui = v[j + 1];   // v = Y' Theta with Y' = triu(Y), diag / 2: Theta^T Y' Theta = 1/2 Theta^T Y Theta
         er = vr * ur - vi * ui;
         ei = vr * ui + vi * ur;
       }
@@ -219,7 +219,7 @@ struct EpiEnergy {      // H9: eloc[w] += sum_rows v[row] (0.5 C[row][w] + hrot[
 };
 
 template <class Epi>
-__global__ void __launch_bounds__(THREADS, 1) k_gemm_tf32(const __grid_constant__ Maps maps, int K, Epi epi) {
+__global__ void __launch_bounds__(THREADS, 1) k_gemm_tf32(const __grid_constant__ Maps maps, int K, int tri, Epi epi) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   __shared__ __align__(8) uint64_t full_bar[STAGES];
@@ -229,7 +229,10 @@ __global__ void __launch_bounds__(THREADS, 1) k_gemm_tf32(const __grid_constant_
   __shared__ uint32_t tmem_base_s;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int m0 = blockIdx.y * BM, n0 = blockIdx.x * BN;
-  const int nkb = K / BK;
+  // tri != 0: the a-operand is upper triangular in 128 x 128 blocks (H9: Y' = triu(Y) with half the diagonal), so
+  // the k-blocks left of this row tile are all zero and are skipped
+  const int kb0 = tri ? m0 / BK : 0;
+  const int nkb = K / BK - kb0;
   const int nchunk = (nkb + CHUNK_KB - 1) / CHUNK_KB;
 
   if (warp == EPI_WARPS && lane == 0) {
@@ -262,10 +265,11 @@ __global__ void __launch_bounds__(THREADS, 1) k_gemm_tf32(const __grid_constant_
         mbar_wait(&empty_bar[s], ph ^ 1);
         uint8_t* st = smem + (size_t)s * STAGE_BYTES;
         mbar_expect_tx(&full_bar[s], STAGE_BYTES);
-        tma_load_2d(st, &maps.a_hi, &full_bar[s], kb * BK, m0);
-        tma_load_2d(st + A_BYTES, &maps.a_lo, &full_bar[s], kb * BK, m0);
-        tma_load_2d(st + 2 * A_BYTES, &maps.b_hi, &full_bar[s], kb * BK, n0);
-        tma_load_2d(st + 2 * A_BYTES + B_BYTES, &maps.b_lo, &full_bar[s], kb * BK, n0);
+        const int kc = (kb0 + kb) * BK;
+        tma_load_2d(st, &maps.a_hi, &full_bar[s], kc, m0);
+        tma_load_2d(st + A_BYTES, &maps.a_lo, &full_bar[s], kc, m0);
+        tma_load_2d(st + 2 * A_BYTES, &maps.b_hi, &full_bar[s], kc, n0);
+        tma_load_2d(st + 2 * A_BYTES + B_BYTES, &maps.b_lo, &full_bar[s], kc, n0);
       }
     }
   } else if (warp == EPI_WARPS + 1) {

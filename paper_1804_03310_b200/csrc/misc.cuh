@@ -117,7 +117,9 @@ __global__ void k_init_rot(int M, int n, int ldc, const double* C, int ng, const
   Rd[(size_t)g * KT + soff + r] = s;
 }
 
-// Y^s[(k,a)][(l,b)] = sum_g R[g][(k,a)] R[g][(l,b)] - R[g][(l,a)] R[g][(k,b)]   (Eq.(5); R8)
+// Y^s[(k,a)][(l,b)] = sum_g R[g][(k,a)] R[g][(l,b)] - R[g][(l,a)] R[g][(k,b)]   (Eq.(5); R8).
+// Y is symmetric and only enters through v^T Y v, so what is stored is Y' = upper triangle with the diagonal halved
+// (v^T Y' v = 1/2 v^T Y v): the energy GEMM then skips the all-zero blocks below the diagonal.
 template <typename T>
 __global__ void k_init_Y(int M, int n, int ng, const double* Rd, int soff, int KT, T* Y, T* Y_lo, int ldy, int split) {
   int c = blockIdx.x * blockDim.x + threadIdx.x;
@@ -127,11 +129,12 @@ __global__ void k_init_Y(int M, int n, int ng, const double* Rd, int soff, int K
   int k = r / n, a = r % n, l = c / n, b = c % n;
   const double* R = Rd + soff;
   double s = 0.0;
-  for (int g = 0; g < ng; ++g) {
+  for (int g = 0; g < (c >= r ? ng : 0); ++g) {
     const double* Rg = R + (size_t)g * KT;
     s = fma(Rg[r], Rg[c], s);
     s = fma(-Rg[l * n + a], Rg[k * n + b], s);
   }
+  if (c == r) s *= 0.5;
   size_t o = (size_t)r * ldy + c;
   if (split) {
     float hi, lo;
