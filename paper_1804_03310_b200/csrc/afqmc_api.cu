@@ -130,10 +130,10 @@ struct Layout {
   size_t const_bytes, work_bytes;
 };
 
-// gemm_path 0 (auto): tcgen05 3xTF32 wherever it exists (complex64, single determinant), else SIMT
+// gemm_path 0 (auto): tcgen05 3xTF32 wherever it exists (complex64 walkers), else SIMT
 int resolve_path(const afqmc_params* p) {
   if (p->gemm_path) return p->gemm_path;
-  return (p->precision == 0 && p->n_det == 1) ? 2 : 1;
+  return p->precision == 0 ? 2 : 1;
 }
 
 afqmc_status check_params(const afqmc_params* p, char* err) {
@@ -163,8 +163,8 @@ afqmc_status check_params(const afqmc_params* p, char* err) {
       snprintf(err, 256, "multi-det working set exceeds one CTA's shared memory"); return AFQMC_EUNSUPPORTED;
     }
   }
-  if (p->gemm_path == 2 && (p->precision != 0 || p->n_det > 1)) {
-    snprintf(err, 256, "gemm_path 2 (tcgen05 3xTF32) needs precision 0 and a single-determinant trial");
+  if (p->gemm_path == 2 && p->precision != 0) {
+    snprintf(err, 256, "gemm_path 2 (tcgen05 3xTF32) needs precision 0 (complex64 walkers)");
     return AFQMC_EUNSUPPORTED;
   }
   int cw, nch;
@@ -806,7 +806,7 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
     ok &= make_map(&c->map_asm.b_hi, c->Z, c->NGP, nrow, c->NGP, BN);
     ok &= make_map(&c->map_asm.b_lo, c->Z_lo, c->NGP, nrow, c->NGP, BN);
     for (int sp = 0; sp < 2; ++sp) {
-      const int n = sp ? c->nb : c->na, soff = sp ? c->KA : 0, Ks = sp ? c->KB : c->KA;
+      const int n = sp ? c->cb : c->ca, soff = sp ? c->KA : 0, Ks = sp ? c->KB : c->KA;
       if (!n) continue;
       const float* R = (const float*)c->Rall + soff; const float* Rl = (const float*)c->Rall_lo + soff;
       const float* th = (const float*)c->thp + soff; const float* thl = (const float*)c->thp_lo + soff;
@@ -814,6 +814,7 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
       ok &= make_map(&c->map_fb[sp].a_lo, Rl, Ks, c->ng, c->KT, BM);
       ok &= make_map(&c->map_fb[sp].b_hi, th, Ks, nrow, c->KT, BN);
       ok &= make_map(&c->map_fb[sp].b_lo, thl, Ks, nrow, c->KT, BN);
+      if (c->md) continue;   // the multi-determinant energy does not use Y
       ok &= make_map(&c->map_en[sp].a_hi, c->Y[sp], Ks, (uint64_t)c->M * n, Ks, BM);
       ok &= make_map(&c->map_en[sp].a_lo, c->Y_lo[sp], Ks, (uint64_t)c->M * n, Ks, BM);
       c->map_en[sp].b_hi = c->map_fb[sp].b_hi;
