@@ -48,7 +48,7 @@ struct afqmc_ctx {
   void* Cact; double* coeff; int32_t* exc;
   double *psid_ac, *psid_bc;   // FP64 trial orbitals (constants)
   void *thtil, *th_scr; zcplx *ovlp0, *ovlp_scr;
-  void *RactT, *thT, *TTg; int MPK;
+  void *RactT, *RactT_lo, *thT, *thT_lo, *TTg; int MPK; tc::Maps map_tt;
   size_t mdo_smem, mde_smem;
   int tay_cw, tay_nch, tay_threads;
   size_t tay_smem, green_smem;
@@ -216,8 +216,9 @@ void carve(const afqmc_params* p, afqmc_ctx* c, char* cbase, char* wbase, size_t
   c->Cact = cc.take((size_t)M * (md ? p->n_act : 1) * ts);
   c->coeff = (double*)cc.take((size_t)p->n_det * 8);
   c->exc = (int32_t*)cc.take((size_t)p->n_det * 8 * 4);
-  c->MPK = (int)rup(M, 8);
+  c->MPK = (int)rup(M, 32);   // K of the TT GEMM, padded to the tcgen05 k-block
   c->RactT = cc.take(md ? (size_t)(ng + 1) * p->n_act * c->MPK * ts : 256);
+  c->RactT_lo = (md && split) ? cc.take((size_t)(ng + 1) * p->n_act * c->MPK * ts) : nullptr;
   *cb = cc.off;
 
   Carver w; w.base = wbase;
@@ -232,6 +233,7 @@ void carve(const afqmc_params* p, afqmc_ctx* c, char* cbase, char* wbase, size_t
   c->thtil = w.take(md ? nw1 * M * 2 * p->n_act * 2 * ts : 256);
   c->th_scr = w.take(md ? nw1 * M * nt * 2 * ts : 256);
   c->thT = w.take(md ? nw1 * 2 * nt * c->MPK * ts : 256);
+  c->thT_lo = (md && split) ? w.take(nw1 * 2 * nt * c->MPK * ts) : nullptr;
   c->TTg = w.take(md ? nw1 * (ng + 1) * p->n_act * nt * 2 * ts : 256);
   c->ovlp0 = (zcplx*)w.take(nw1 * sizeof(zcplx));
   c->ovlp_scr = (zcplx*)w.take(nw1 * sizeof(zcplx));
@@ -335,7 +337,7 @@ template <typename T> afqmc_status init_device(afqmc_ctx* c, const double* h1, c
   }
   if (c->md) {
     size_t tot = (size_t)(ng + 1) * c->nact * M;
-    LAUNCH(c, k_init_ractT<T>, (unsigned)((tot + 127) / 128), 128, 0, ng, c->nact, M, c->MPK, c->Rd, KT, c->hrotd, (T*)c->RactT);
+    LAUNCH(c, k_init_ractT<T>, (unsigned)((tot + 127) / 128), 128, 0, ng, c->nact, M, c->MPK, c->Rd, KT, c->hrotd, (T*)c->RactT, (T*)c->RactT_lo);
   }
   {
     size_t tot = (size_t)ng * KT;
@@ -442,8 +444,19 @@ template <typename T> afqmc_status run_md_energy(afqmc_ctx* c, const void* theta
   a.ng = c->ng; a.ldr = c->KT; a.theta0 = (const cplx<T>*)theta; a.TTg = (const cplx<T>*)c->TTg;
   a.eloc = eloc;
   // TT[w][g][q][a] = sum_k (C_act^T X_g)[q][k] Theta_0[w][k][a] for every g (and h) in one GEMM over all walkers
-  LAUNCH(c, k_thT<T>, c->nw, 128, 0, c->M, c->nt, c->MPK, (const cplx<T>*)theta, (T*)c->thT);
-  {
+  LAUNCH(c, k_thT<T>, c->nw, 128, 0, c->M, c->nt, c->MPK, (const cplx<T>*)theta, (T*)c->thT, (T*)c->thT_lo);
+  bool tt_done = false;
+  if constexpr (sizeof(T) == 4) {
+    if (c->path == 2) {
+      tc::EpiTT e2;
+      e2.out = (float*)c->TTg; e2.ng1 = c->ng + 1; e2.nact = c->nact; e2.nt = c->nt;
+      e2.m_real = (c->ng + 1) * c->nact; e2.n_real = c->nw * 2 * c->nt;
+      afqmc_status st = run_gemm_tc(c, c->map_tt, e2.m_real, e2.n_real, c->MPK, e2);
+      if (st) return st;
+      tt_done = true;
+    }
+  }
+  if (!tt_done) {
     EpiTT<T> epi;
     epi.out = (T*)c->TTg; epi.ng1 = c->ng + 1; epi.nact = c->nact; epi.nt = c->nt;
     epi.m_real = (c->ng + 1) * c->nact; epi.n_real = c->nw * 2 * c->nt;
@@ -814,7 +827,16 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
       ok &= make_map(&c->map_fb[sp].a_lo, Rl, Ks, c->ng, c->KT, BM);
       ok &= make_map(&c->map_fb[sp].b_hi, th, Ks, nrow, c->KT, BN);
       ok &= make_map(&c->map_fb[sp].b_lo, thl, Ks, nrow, c->KT, BN);
-      if (c->md) continue;   // the multi-determinant energy does not use Y
+      if (c->md) {           // the multi-determinant energy does not use Y; its TT GEMM has its own operands
+        if (sp == 0) {
+          const uint64_t r1 = (uint64_t)(c->ng + 1) * c->nact, r2 = (uint64_t)c->nw * 2 * c->nt;
+          ok &= make_map(&c->map_tt.a_hi, c->RactT, c->MPK, r1, c->MPK, BM);
+          ok &= make_map(&c->map_tt.a_lo, c->RactT_lo, c->MPK, r1, c->MPK, BM);
+          ok &= make_map(&c->map_tt.b_hi, c->thT, c->MPK, r2, c->MPK, BN);
+          ok &= make_map(&c->map_tt.b_lo, c->thT_lo, c->MPK, r2, c->MPK, BN);
+        }
+        continue;
+      }
       ok &= make_map(&c->map_en[sp].a_hi, c->Y[sp], Ks, (uint64_t)c->M * n, Ks, BM);
       ok &= make_map(&c->map_en[sp].a_lo, c->Y_lo[sp], Ks, (uint64_t)c->M * n, Ks, BM);
       c->map_en[sp].b_hi = c->map_fb[sp].b_hi;
@@ -823,6 +845,7 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
     cudaError_t e1 = cudaFuncSetAttribute(k_gemm_tf32<tc::EpiStoreT>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     cudaError_t e2 = cudaFuncSetAttribute(k_gemm_tf32<tc::EpiAssemble>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     cudaError_t e3 = cudaFuncSetAttribute(k_gemm_tf32<tc::EpiEnergy>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(k_gemm_tf32<tc::EpiTT>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(k_gemm_tf32<tc::EpiAssembleSym>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     if (!ok || e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) {
       snprintf(g_init_err, 256, "tcgen05 path: tensor-map / shared-memory set-up failed");

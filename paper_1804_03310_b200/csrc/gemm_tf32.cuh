@@ -183,6 +183,35 @@ struct EpiAssembleSym {
   }
 };
 
+struct EpiTT {          // H10: row = g*nact + q, col = (w*nt + a)*2 + p -> TT[w][g][q][a] (interleaved complex)
+  static constexpr bool kStaged = false;
+  float* out; int ng1, nact, nt, m_real, n_real;
+  __device__ __forceinline__ void operator()(int r, int c0, const float (&v)[32]) const {
+    if (r >= m_real) return;
+    const int g = r / nact, q = r - g * nact;
+    float* orow = out + ((size_t)g * nact + q) * (2 * nt);
+    const size_t wstride = (size_t)ng1 * nact * (2 * nt);
+    if ((nt & 1) == 0) {     // 2nt % 4 == 0: float4 groups never straddle a walker and stay 16-byte aligned
+#pragma unroll
+      for (int j = 0; j < 32; j += 4) {
+        const int c = c0 + j;
+        if (c < n_real) {
+          const int w = c / (2 * nt), rem = c - w * 2 * nt;
+          *reinterpret_cast<float4*>(orow + w * wstride + rem) = make_float4(v[j], v[j + 1], v[j + 2], v[j + 3]);
+        }
+      }
+    } else {
+#pragma unroll
+      for (int j = 0; j < 32; ++j) {
+        const int c = c0 + j;
+        if (c < n_real) {
+          const int w = c / (2 * nt), rem = c - w * 2 * nt;
+          orow[w * wstride + rem] = v[j];
+        }
+      }
+    }
+  }
+};
 struct EpiEnergy {      // H9: eloc[w] += sum_rows v[row] (0.5 C[row][w] + hrot[row]), v = Theta plane (hi + lo)
   static constexpr bool kStaged = false;
   const float* thp; const float* thp_lo; int KT, soff; const float* hrot; double* eloc; int m_real, n_real;

@@ -192,18 +192,25 @@ __global__ void k_cast2d(int nr, int nc, const double* src, size_t lds, T* dst, 
 // ---- multi-determinant energy: operands of the TT = C_act^T X Theta_0 GEMM (X = L_g for all g, then h) ----
 // thT[((w*nt + a)*2 + p)*MPK + k] = Re/Im Theta_0[w][k][a]   (K-major rows (walker, column, plane), zero padded)
 template <typename T>
-__global__ void __launch_bounds__(128) k_thT(int M, int nt, int MPK, const cplx<T>* theta, T* thT) {
+__global__ void __launch_bounds__(128) k_thT(int M, int nt, int MPK, const cplx<T>* theta, T* thT, T* thT_lo) {
   const int w = blockIdx.x;
   for (int e = threadIdx.x; e < M * nt; e += blockDim.x) {
     int k = e / nt, a = e - k * nt;
     cplx<T> v = theta[(size_t)w * M * nt + e];
-    thT[(((size_t)w * nt + a) * 2 + 0) * MPK + k] = v.x;
-    thT[(((size_t)w * nt + a) * 2 + 1) * MPK + k] = v.y;
+    const size_t o0 = (((size_t)w * nt + a) * 2 + 0) * MPK + k, o1 = o0 + MPK;
+    if (thT_lo) {
+      float h0, l0, h1, l1;
+      tf32_split((float)v.x, h0, l0);
+      tf32_split((float)v.y, h1, l1);
+      thT[o0] = (T)h0; thT[o1] = (T)h1; thT_lo[o0] = (T)l0; thT_lo[o1] = (T)l1;
+    } else {
+      thT[o0] = v.x; thT[o1] = v.y;
+    }
   }
 }
 // RactT[(g*nact + q)*MPK + k] = (C_act^T L_g)[q][k] for g < ng, (C_act^T h)[q][k] for g == ng
 template <typename T>
-__global__ void k_init_ractT(int ng, int nact, int M, int MPK, const double* Rd, int KT, const double* hrotd, T* out) {
+__global__ void k_init_ractT(int ng, int nact, int M, int MPK, const double* Rd, int KT, const double* hrotd, T* out, T* out_lo) {
   size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   size_t tot = (size_t)(ng + 1) * nact * M;
   if (e >= tot) return;
@@ -211,7 +218,14 @@ __global__ void k_init_ractT(int ng, int nact, int M, int MPK, const double* Rd,
   int q = (int)((e / M) % nact);
   int g = (int)(e / ((size_t)M * nact));
   double v = g < ng ? Rd[(size_t)g * KT + k * nact + q] : hrotd[k * nact + q];
-  out[((size_t)g * nact + q) * MPK + k] = (T)v;
+  const size_t o = ((size_t)g * nact + q) * MPK + k;
+  if (out_lo) {
+    float hi, lo;
+    tf32_split((float)v, hi, lo);
+    out[o] = (T)hi; out_lo[o] = (T)lo;
+  } else {
+    out[o] = (T)v;
+  }
 }
 
 
