@@ -43,13 +43,36 @@ __device__ __forceinline__ uint32_t plane_off(int b, int j) {
   return (uint32_t)(kb * PLANE_KB_BYTES + b * 128 + ((((jj >> 2) ^ (b & 7)) << 4) | ((jj & 3) << 2)));
 }
 
+// Staged result [M][nt] complex inside the planes: only the non-padding rows of the first k-blocks are used (chunks of
+// nt plane rows x 128 B = 16 result rows of nt complex, 4 chunks per k-block), so the zero padding the MMAs rely on is
+// never touched.  Needs ceil(M / 16) <= 4 * floor(M / 32) (true for M >= 64).
+__device__ __forceinline__ uint32_t stage_chunk(int c) { return (uint32_t)((c >> 2) * PLANE_KB_BYTES + (c & 3) * (32 * 128)); }
+__device__ __forceinline__ uint32_t stage_row(int i, int nt) { return stage_chunk(i >> 4) + (uint32_t)((i & 15) * nt * 8); }
+__device__ __forceinline__ void sts32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
+__device__ __forceinline__ float2 lds64(uint32_t a) {
+  float2 v;
+  asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(a) : "memory");
+  return v;
+}
+// staged result -> global, 16-row chunks are contiguous on both sides
+__device__ __forceinline__ void stage_flush(uint32_t pl, float2* dst, int M, int nt, int et) {
+  const int per = 16 * nt;
+  for (int c = 0; c * 16 < M; ++c) {
+    const int n = min(16, M - c * 16) * nt;
+    const uint32_t base = pl + stage_chunk(c);
+    for (int idx = et; idx < n; idx += EPW * 32) dst[c * per + idx] = lds64(base + idx * 8);
+  }
+}
+enum { MAXE = 32 };   // complex elements of Phi_w per epilogue thread: M * N_t <= 256 * 32 = MAXE * 256
+
 __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant__ TaylorMaps maps, TaylorTcArgs g) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   __shared__ __align__(8) uint64_t full_bar[NST];
   __shared__ __align__(8) uint64_t empty_bar[NST];
   __shared__ __align__(8) uint64_t tmem_full_bar[2];   // per 128-row tile: tile 0 is post-processed while tile 1 is issued
-  __shared__ __align__(8) uint64_t b_ready_bar;
+  __shared__ __align__(8) uint64_t b_ready_bar[8];     // per (tile, lane quarter) = 32-column k-block of the T operand
+  __shared__ __align__(8) uint64_t t_free_bar[4];      // last tile has consumed k-block kb < 4 of the current T
   __shared__ uint32_t tmem_base_s;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int M = g.M, nt = g.nt, nkb = g.nkb, mtiles = g.mtiles;
@@ -65,7 +88,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
   if (warp == EPW && lane == 0) {
     for (int s = 0; s < NST; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
     mbar_init(&tmem_full_bar[0], 1); mbar_init(&tmem_full_bar[1], 1);
-    mbar_init(&b_ready_bar, EPW);
+    for (int x = 0; x < 8; ++x) mbar_init(&b_ready_bar[x], 2);   // the re and the im warp of that quarter
+    for (int x = 0; x < 4; ++x) mbar_init(&t_free_bar[x], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == EPW + 1) {
@@ -114,10 +138,14 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
       for (int w = blockIdx.x; w < g.nw; w += gridDim.x)
         for (int ph = 0; ph < nphase; ++ph, ++gph) {
           const bool cx = ph >= 1 && ph <= g.K;
-          mbar_wait(&b_ready_bar, gph & 1);               // T planes of this phase are in shared memory
-          tc_fence_after();
           for (int mt = 0; mt < mtiles; ++mt) {
-            for (int kb = 0; kb < nkb; ++kb)
+            for (int kb = 0; kb < nkb; ++kb) {
+              if (mt == 0 && (kb & 3) == 0) {
+                // k-blocks kb..kb+3 of this phase's T are in shared memory, and (all 8 epilogue warps arrive on
+                // them after their TMEM loads) the accumulators of tile kb/4 have been read
+                for (int x = 0; x < 4; ++x) mbar_wait(&b_ready_bar[kb + x], gph & 1);
+                tc_fence_after();
+              }
               for (int p = 0; p < (cx ? 2 : 1); ++p, ++it) {
                 const uint32_t d = tmem + (mt * 2 + p) * 128;
                 const int s = it % NST;
@@ -136,104 +164,162 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
                 }
                 tc_commit(&empty_bar[s]);
               }
+              if (mtiles == 2 && mt == 1 && kb < 4) tc_commit(&t_free_bar[kb]);
+            }
             tc_commit(&tmem_full_bar[mt]);
           }
         }
     }
   } else {   // ===== epilogue warps 0..7: TMEM lane quarter = warp & 3, half = warp >> 2 (0: real part, 1: imaginary) =====
+    // Rows i = mt*128 + q*32 + lane of the product are k-block mt*4+q of the next T operand.  Tile 0 is post-processed
+    // and written back while tile 1 is being issued (each k-block as soon as tile 1 has consumed it), and the next
+    // phase starts on k-blocks 0-3 while tile 1 is post-processed: the tensor pipe does not wait between phases.
     const int q = warp & 3, half = warp >> 2;
-    uint8_t* pl_hi = planes;
-    uint8_t* pl_lo = planes + 64 * 128;       // lo rows start 64 rows further down inside every k-block
+    const uint32_t plu = smem_u32(planes);
+    const uint32_t pl_hi = plu, pl_lo = plu + 64 * 128;   // lo rows start 64 rows further down inside every k-block
     const int rb = half * 32;                 // plane row base: T_r rows 0-31, T_i rows 32-63
     uint32_t gph = 0;
     float P[2][32];
+    const int et = (int)threadIdx.x;      // epilogue threads are 0..255
+    int w_last = -1;
     for (int w = blockIdx.x; w < g.nw; w += gridDim.x) {
       float* phi_w = reinterpret_cast<float*>(g.phi + (size_t)w * M * nt);
-      // phase-0 operand: planes <- Phi_w  (row b = walker column, column j = basis index)
-      for (int e = (warp & 3) * 32 + lane; e < M * nt; e += 128) {
-        const int b = e / M, j = e - b * M;     // lanes along j: conflict-free plane writes
-        float hi, lo;
-        tf32_split(phi_w[2 * (j * nt + b) + half], hi, lo);
-        const uint32_t o = plane_off(rb + b, j);
-        *reinterpret_cast<float*>(pl_hi + o) = hi;
-        *reinterpret_cast<float*>(pl_lo + o) = lo;
+      // phase-0 operand: planes <- Phi_w (row b = walker column, column i = basis index).  Phi_w is read as
+      // consecutive complex numbers (coalesced, all loads in flight at once); every MMA of the previous walker has
+      // completed (each warp has observed tmem_full of its last tile)
+      {
+        float2 f[MAXE / 2];
+        const float2* src = reinterpret_cast<const float2*>(phi_w);
+#pragma unroll
+        for (int k = 0; k < MAXE / 2; ++k) {
+          const int e = et + k * (EPW * 32);
+          if (e < M * nt) f[k] = src[e];
+        }
+        if (w != (int)blockIdx.x) {
+          // the previous walker's result is staged in the planes: write it out before they are overwritten
+          asm volatile("bar.sync 1, 256;" ::: "memory");
+          float2* dst = reinterpret_cast<float2*>(g.phi + (size_t)(w - gridDim.x) * M * nt);
+          stage_flush(plu, dst, M, nt, et);
+          asm volatile("bar.sync 1, 256;" ::: "memory");
+        }
+        int ci = et / nt, cbb = et - ci * nt;            // (row, column) of element e, stepped without divisions
+        const int di = (EPW * 32) / nt, db = (EPW * 32) - di * nt;
+#pragma unroll
+        for (int hb = 0; hb < 2; ++hb) {
+          if (hb == 1) {
+#pragma unroll
+            for (int k = 0; k < MAXE / 2; ++k) {
+              const int e = et + (k + MAXE / 2) * (EPW * 32);
+              if (e < M * nt) f[k] = src[e];
+            }
+          }
+#pragma unroll
+          for (int k = 0; k < MAXE / 2; ++k) {
+            const int e = et + (k + hb * (MAXE / 2)) * (EPW * 32);
+            if (e < M * nt) {
+              float h0, l0, h1, l1;
+              tf32_split(f[k].x, h0, l0);
+              tf32_split(f[k].y, h1, l1);
+              const uint32_t o = plane_off(cbb, ci);
+              sts32(pl_hi + o, h0);
+              sts32(pl_lo + o, l0);
+              sts32(pl_hi + o + 32 * 128, h1);    // T_i rows are 32 rows below the T_r rows
+              sts32(pl_lo + o + 32 * 128, l1);
+            }
+            ci += di; cbb += db;
+            if (cbb >= nt) { cbb -= nt; ++ci; }
+          }
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        tc_fence_before();
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        if (lane == 0)
+          for (int mt = 0; mt < mtiles; ++mt)
+            asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&b_ready_bar[mt * 4 + q])) : "memory");
       }
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      __syncwarp();
-      if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&b_ready_bar)) : "memory");
       for (int ph = 0; ph < nphase; ++ph, ++gph) {
         const bool last_phase = ph == nphase - 1;
         const float scale = (ph >= 1 && ph <= g.K) ? 1.0f / (float)ph : 1.0f;
         const bool cxp = ph >= 1 && ph <= g.K;
         const uint32_t tl = tmem + ((uint32_t)(q * 32) << 16);
-        float vv[2][32];
-        // pass 1 (tile 0 overlaps the MMAs of tile 1): D_re = D1[0:32] - D2[32:64], D_im = D1[32:64] + D2[0:32],
-        // summed over the accumulation chunks; scale, add into the running sum
 #pragma unroll
         for (int mt = 0; mt < 2; ++mt) {
           if (mt < mtiles) {
+            // D_re = D1[0:32] - D2[32:64], D_im = D1[32:64] + D2[0:32]; columns 64.. hold the hi*lo products
+            float v[32];
             mbar_wait(&tmem_full_bar[mt], gph & 1);
             tc_fence_after();
-#pragma unroll
-            for (int b = 0; b < 32; ++b) vv[mt][b] = 0.f;
             {
-              float u[32];
-              tmem_ld32(tl + (mt * 2 + 0) * 128 + half * 32, u);              // X_r: hi*hi + lo*hi
+              float u0[32], u1[32];
+              tmem_ld32x2(tl + (mt * 2 + 0) * 128 + half * 32, tl + (mt * 2 + 0) * 128 + 64 + half * 32, u0, u1);
 #pragma unroll
-              for (int b = 0; b < 32; ++b) vv[mt][b] += u[b];
-              tmem_ld32(tl + (mt * 2 + 0) * 128 + 64 + half * 32, u);         // X_r: hi*lo
-#pragma unroll
-              for (int b = 0; b < 32; ++b) vv[mt][b] += u[b];
+              for (int b = 0; b < 32; ++b) v[b] = u0[b] + u1[b];
               if (cxp) {
-                tmem_ld32(tl + (mt * 2 + 1) * 128 + (1 - half) * 32, u);
+                // (single loads here: a second pair in flight would not fit the 168-register budget beside P)
+                tmem_ld32(tl + (mt * 2 + 1) * 128 + (1 - half) * 32, u0);
 #pragma unroll
-                for (int b = 0; b < 32; ++b) vv[mt][b] = half ? vv[mt][b] + u[b] : vv[mt][b] - u[b];
-                tmem_ld32(tl + (mt * 2 + 1) * 128 + 64 + (1 - half) * 32, u);
+                for (int b = 0; b < 32; ++b) v[b] = half ? v[b] + u0[b] : v[b] - u0[b];
+                tmem_ld32(tl + (mt * 2 + 1) * 128 + 64 + (1 - half) * 32, u0);
 #pragma unroll
-                for (int b = 0; b < 32; ++b) vv[mt][b] = half ? vv[mt][b] + u[b] : vv[mt][b] - u[b];
+                for (int b = 0; b < 32; ++b) v[b] = half ? v[b] + u0[b] : v[b] - u0[b];
               }
             }
 #pragma unroll
             for (int b = 0; b < 32; ++b) {
-              float t = vv[mt][b] * scale;
+              float t = v[b] * scale;
               if (ph == 0) P[mt][b] = t; else P[mt][b] += t;
               if (ph == g.K) t = P[mt][b];               // operand of the closing E_h product is the sum
-              vv[mt][b] = t;
+              v[b] = t;
             }
-          }
-        }
-        // pass 2: every MMA of this phase has completed, the T planes may be overwritten
+            const int i = mt * 128 + q * 32 + lane;       // output row = basis index
+            if (last_phase) {
+              // result rows stay in registers (P is dead) until every MMA has completed, then go to the staging
+              // area inside the planes (the non-padding bytes, all rewritten by the next walker's operand)
 #pragma unroll
-        for (int mt = 0; mt < 2; ++mt) {
-          if (mt < mtiles) {
-            const int i = mt * 128 + q * 32 + lane;     // output row = basis index
-            if (i < M) {
-              if (last_phase) {
+              for (int b = 0; b < 32; ++b) P[mt][b] = v[b];
+              if (mt == mtiles - 1) {
 #pragma unroll
-                for (int b = 0; b < 32; ++b)
-                  if (b < nt) phi_w[2 * (i * nt + b) + half] = vv[mt][b];
-              } else {
+                for (int m2 = 0; m2 < 2; ++m2) {
+                  const int i2 = m2 * 128 + q * 32 + lane;
+                  if (m2 < mtiles && i2 < M) {
+                    const uint32_t srow = plu + stage_row(i2, nt) + half * 4;
 #pragma unroll
-                for (int b = 0; b < 32; ++b) {
-                  if (b < nt) {
-                    float hi, lo;
-                    tf32_split(vv[mt][b], hi, lo);
-                    const uint32_t o = plane_off(rb + b, i);
-                    *reinterpret_cast<float*>(pl_hi + o) = hi;
-                    *reinterpret_cast<float*>(pl_lo + o) = lo;
+                    for (int b = 0; b < 32; ++b)
+                      if (b < nt) sts32(srow + b * 8, P[m2][b]);
                   }
                 }
               }
+            } else {
+              float hi[32], lo[32];
+#pragma unroll
+              for (int b = 0; b < 32; ++b) tf32_split(v[b], hi[b], lo[b]);
+              // k-block mt*4+q of T may be overwritten once every MMA that reads it has completed: for the last
+              // tile that is tmem_full (above), for tile 0 of two the last tile's pass over that k-block
+              if (mt == 0 && mtiles == 2) mbar_wait(&t_free_bar[q], gph & 1);
+              if (i < M) {
+#pragma unroll
+                for (int b = 0; b < 32; ++b)
+                  if (b < nt) {
+                    const uint32_t o = plane_off(rb + b, i);
+                    sts32(pl_hi + o, hi[b]);
+                    sts32(pl_lo + o, lo[b]);
+                  }
+              }
+              asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+              tc_fence_before();
+              __syncwarp();
+              if (lane == 0)
+                asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&b_ready_bar[mt * 4 + q])) : "memory");
             }
           }
         }
-        tc_fence_before();
-        if (!last_phase) {
-          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-          __syncwarp();
-          if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&b_ready_bar)) : "memory");
-        }
       }
+      w_last = w;
+    }
+    if (w_last >= 0) {   // the last walker's result is still staged
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      float2* dst = reinterpret_cast<float2*>(g.phi + (size_t)w_last * M * nt);
+      stage_flush(plu, dst, M, nt, et);
     }
   }
   tc_fence_before();
