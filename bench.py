@@ -264,7 +264,7 @@ def run_ours(args):
     # roofline of the dominant kernel = the stage with the largest device time (CUDA events on the launching
     # stream, afqmc_profile_*); the H6 assembly GEMM is always reported beside it as `roofline_h6`
     M_, ng_ = wl.M, wl.n_chol
-    if ctx.gemm_path == 2:
+    if ctx.gemm_path >= 2:
         # the tcgen05 assembly GEMM exploits A = A^T: its algorithmic work is the upper triangle only
         fl["assemble"] = 4.0 * ng_ * M_ * (M_ + 1) / 2
         peak, peak_note = 0.5 * pk["bf16_burst"], (
@@ -282,7 +282,7 @@ def run_ours(args):
                  taylor="H7 Taylor propagator (tt::k_taylor_tc / k_taylor)",
                  energy="H9 energy GEMMs + fused dot (or H10 multi-det energy)", force_bias="H4 force-bias GEMMs",
                  green="H1-H3/H8 overlap, LU, Theta, weights (k_green)")
-    traffic_ncu = {"assemble": 1.306e9, "taylor": 2.10e9} if (ctx.gemm_path == 2 and args.cfg == 5) else {}
+    traffic_ncu = {"assemble": 1.306e9, "taylor": 2.10e9} if (ctx.gemm_path >= 2 and args.cfg == 5) else {}
 
     def roof(stage):
         ms, n = prof[stage]
@@ -291,11 +291,11 @@ def run_ours(args):
         ach = fl[stage] * nw * n / (ms * 1e-3) / 1e12
         r = dict(bound=bound, kernel=names[stage], achieved=ach, peak=peak, unit="TFLOP/s", frac=ach / peak,
                  traffic=traffic_ncu.get(stage), peak_source=peak_note, launches_timed=n, ms_per_launch=ms / n)
-        if ctx.gemm_path == 2:
+        if ctx.gemm_path >= 2:
             r["issued_frac"] = 3.0 * ach / peak
         if stage == "green":      # HBM-bound stage: bytes, not flops
             cb = 8 if wl.precision == "c64" else 16
-            byts = nw * wl.M * wl.n_t * cb * (2 + (2 if ctx.gemm_path == 2 else 1))
+            byts = nw * wl.M * wl.n_t * cb * (2 + (2 if ctx.gemm_path >= 2 else 1))
             r.update(bound="hbm", achieved=byts * n / (ms * 1e-3) / 1e9, peak=pk["hbm"], unit="GB/s",
                      peak_source=f"{pk['source']} HBM copy bandwidth")
             r["frac"] = r["achieved"] / r["peak"]
@@ -315,7 +315,7 @@ def run_ours(args):
                             parallelism=f"replicas x{world}" if world > 1 else "single GPU",
                             l2="per-step working set (A_w buffer %.0f MB + operands) exceeds the 126 MB L2; no flush"
                                % (nw * wl.M * wl.M * 2 * (4 if wl.precision == "c64" else 8) / 1e6),
-                            gemm_path={1: "simt", 2: "tcgen05-3xtf32"}[ctx.gemm_path]),
+                            gemm_path={1: "simt", 2: "tcgen05-3xtf32", 3: "tcgen05-3xtf32-ctapair"}[ctx.gemm_path]),
                 clocks=clocks, gpu_launches=launches,
                 e2e=dict(value=world * nw * Ke / t_e2e, unit=UNIT, h2d_bytes_per_step=up / Ke, d2h_bytes_per_step=down / Ke,
                          steps=Ke, note="afqmc_step_host: pinned host buffers, H2D of walkers+fields and D2H of "

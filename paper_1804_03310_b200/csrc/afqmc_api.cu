@@ -7,6 +7,7 @@
 #include <stdio.h>
 #include <string.h>
 #include <new>
+#include <algorithm>
 #include <vector>
 
 #include "common.cuh"
@@ -66,6 +67,7 @@ struct afqmc_ctx {
   double *Ld, *hd, *hpd, *Rd, *hrotd, *ex[4], *psid;
   tc::Maps map_asm, map_fb[2], map_en[2];
   int nblk; int2* blk;   // symmetric block list of the tcgen05 assembly GEMM
+  int cta2;   // tcgen05 GEMMs run on CTA pairs (cta_group::2), gemm_path 3
   int tay_tc; void *Abuf_lo, *Eh_lo; tt::TaylorMaps map_tay; tt::TaylorTcArgs tay_args; size_t tay_tc_smem; int n_sm;   // TMA descriptors of the tcgen05 path (path == 2)
   char err[256];
   int64_t launches;
@@ -132,9 +134,11 @@ struct Layout {
 
 // gemm_path 0 (auto): tcgen05 3xTF32 wherever it exists (complex64 walkers), else SIMT
 int resolve_path(const afqmc_params* p) {
-  if (p->gemm_path) return p->gemm_path;
+  if (p->gemm_path) return p->gemm_path >= 2 ? 2 : 1;
   return p->precision == 0 ? 2 : 1;
 }
+// the tcgen05 GEMMs run on CTA pairs unless gemm_path 2 asks for the one-CTA kernels
+int resolve_cta2(const afqmc_params* p) { return resolve_path(p) == 2 && p->gemm_path != 2; }
 
 afqmc_status check_params(const afqmc_params* p, char* err) {
   if (!p) { snprintf(err, 256, "params is NULL"); return AFQMC_EINVAL; }
@@ -147,7 +151,7 @@ afqmc_status check_params(const afqmc_params* p, char* err) {
   if (p->taylor_order < 1 || p->taylor_order > 20) { snprintf(err, 256, "taylor_order must be in 1..20"); return AFQMC_EINVAL; }
   if (p->weight_mode != 0 && p->weight_mode != 1) { snprintf(err, 256, "weight_mode must be 0 or 1"); return AFQMC_EINVAL; }
   if (!(p->dt > 0.0) || !isfinite(p->dt) || !isfinite(p->E0)) { snprintf(err, 256, "dt must be > 0 and finite"); return AFQMC_EINVAL; }
-  if (p->gemm_path < 0 || p->gemm_path > 2) { snprintf(err, 256, "gemm_path must be 0, 1 or 2"); return AFQMC_EINVAL; }
+  if (p->gemm_path < 0 || p->gemm_path > 3) { snprintf(err, 256, "gemm_path must be 0, 1, 2 or 3"); return AFQMC_EINVAL; }
   if (p->n_alpha > 32 || p->n_beta > 32) { snprintf(err, 256, "n_alpha, n_beta <= 32 supported"); return AFQMC_EUNSUPPORTED; }
   if (p->n_det < 1) { snprintf(err, 256, "n_det must be >= 1"); return AFQMC_EINVAL; }
   if (p->n_det > 1) {
@@ -163,8 +167,8 @@ afqmc_status check_params(const afqmc_params* p, char* err) {
       snprintf(err, 256, "multi-det working set exceeds one CTA's shared memory"); return AFQMC_EUNSUPPORTED;
     }
   }
-  if (p->gemm_path == 2 && p->precision != 0) {
-    snprintf(err, 256, "gemm_path 2 (tcgen05 3xTF32) needs precision 0 (complex64 walkers)");
+  if (p->gemm_path >= 2 && p->precision != 0) {
+    snprintf(err, 256, "gemm_path 2/3 (tcgen05 3xTF32) needs precision 0 (complex64 walkers)");
     return AFQMC_EUNSUPPORTED;
   }
   int cw, nch;
@@ -351,6 +355,14 @@ template <typename T> afqmc_status init_device(afqmc_ctx* c, const double* h1, c
     for (int ib = 0; ib * 8 < M; ++ib)
       for (int jb = 0; jb * 16 < M; ++jb)
         if (ib * 8 <= jb * 16 + 15) tab.push_back(make_int2(ib, jb));
+    // order: 32 x 32 super-blocks (4 ib x 2 jb), blocks row-major inside.  Tiles that run at the same time then write
+    // whole 128-byte lines of A_w in both orientations (a block alone writes 64-byte runs (i, j..j+15) and 32-byte
+    // runs (j, i..i+7)), which L2 merges before they reach HBM
+    std::stable_sort(tab.begin(), tab.end(), [](const int2& a, const int2& b) {
+      const int ka[4] = {a.x >> 2, a.y >> 1, a.x, a.y}, kb[4] = {b.x >> 2, b.y >> 1, b.x, b.y};
+      for (int t = 0; t < 4; ++t) if (ka[t] != kb[t]) return ka[t] < kb[t];
+      return false;
+    });
     CUDA_OK(c, cudaMemcpyAsync(c->blk, tab.data(), tab.size() * sizeof(int2), cudaMemcpyHostToDevice, st));
     CUDA_OK(c, cudaStreamSynchronize(st));
     size_t tot = (size_t)c->nblk * 128 * ng;
@@ -406,8 +418,16 @@ afqmc_status run_gemm(afqmc_ctx* c, const T* A, int lda, int m, const T* B, int 
 }
 
 template <class Epi>
-afqmc_status run_gemm_tc(afqmc_ctx* c, const tc::Maps& maps, int m, int n, int K, Epi epi, int tri = 0) {
+afqmc_status run_gemm_tc(afqmc_ctx* c, const tc::Maps& maps, int m, int n, int K, Epi epi, int tri = 0, bool pair_ok = true) {
   dim3 grid((n + tc::BN - 1) / tc::BN, (m + tc::BM - 1) / tc::BM);
+  if (c->cta2 && pair_ok) {
+    const int m_tiles = (int)grid.y;
+    const int n_tiles = (int)grid.x;
+    dim3 grid2(((grid.y + 1) & ~1u) * grid.x);   // CTA pairs = clusters of two adjacent row tiles, 1-D grid
+    auto kern2 = tc::k_gemm_tf32_pair<Epi>;
+    LAUNCH(c, kern2, grid2, tc::THREADS, tc::SMEM_BYTES, maps, K, tri, m_tiles, n_tiles, epi);
+    return AFQMC_OK;
+  }
   auto kern = tc::k_gemm_tf32<Epi>;
   LAUNCH(c, kern, grid, tc::THREADS, tc::SMEM_BYTES, maps, K, tri, epi);
   return AFQMC_OK;
@@ -451,7 +471,8 @@ template <typename T> afqmc_status run_md_energy(afqmc_ctx* c, const void* theta
       tc::EpiTT e2;
       e2.out = (float*)c->TTg; e2.ng1 = c->ng + 1; e2.nact = c->nact; e2.nt = c->nt;
       e2.m_real = (c->ng + 1) * c->nact; e2.n_real = c->nw * 2 * c->nt;
-      afqmc_status st = run_gemm_tc(c, c->map_tt, e2.m_real, e2.n_real, c->MPK, e2);
+      // K is one or two k-blocks here: the epilogue is the whole kernel and the pair's cluster barriers only cost
+      afqmc_status st = run_gemm_tc(c, c->map_tt, e2.m_real, e2.n_real, c->MPK, e2, 0, false);
       if (st) return st;
       tt_done = true;
     }
@@ -740,6 +761,7 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
   c->stream = (cudaStream_t)stream;
   c->path = resolve_path(p);
   c->split = c->path == 2;
+  c->cta2 = resolve_cta2(p);
   size_t cb, wb;
   carve(p, c, (char*)const_mem, (char*)work_mem, &cb, &wb);
   if (p->precision) {
@@ -816,8 +838,8 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
     const uint64_t nrow = 2 * (uint64_t)c->nw;
     ok &= make_map(&c->map_asm.a_hi, c->Lt, c->NGP, (uint64_t)c->nblk * 128, c->NGP, BM);
     ok &= make_map(&c->map_asm.a_lo, c->Lt_lo, c->NGP, (uint64_t)c->nblk * 128, c->NGP, BM);
-    ok &= make_map(&c->map_asm.b_hi, c->Z, c->NGP, nrow, c->NGP, BN);
-    ok &= make_map(&c->map_asm.b_lo, c->Z_lo, c->NGP, nrow, c->NGP, BN);
+    ok &= make_map(&c->map_asm.b_hi, c->Z, c->NGP, nrow, c->NGP, B_BOX);
+    ok &= make_map(&c->map_asm.b_lo, c->Z_lo, c->NGP, nrow, c->NGP, B_BOX);
     for (int sp = 0; sp < 2; ++sp) {
       const int n = sp ? c->cb : c->ca, soff = sp ? c->KA : 0, Ks = sp ? c->KB : c->KA;
       if (!n) continue;
@@ -825,15 +847,15 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
       const float* th = (const float*)c->thp + soff; const float* thl = (const float*)c->thp_lo + soff;
       ok &= make_map(&c->map_fb[sp].a_hi, R, Ks, c->ng, c->KT, BM);
       ok &= make_map(&c->map_fb[sp].a_lo, Rl, Ks, c->ng, c->KT, BM);
-      ok &= make_map(&c->map_fb[sp].b_hi, th, Ks, nrow, c->KT, BN);
-      ok &= make_map(&c->map_fb[sp].b_lo, thl, Ks, nrow, c->KT, BN);
+      ok &= make_map(&c->map_fb[sp].b_hi, th, Ks, nrow, c->KT, B_BOX);
+      ok &= make_map(&c->map_fb[sp].b_lo, thl, Ks, nrow, c->KT, B_BOX);
       if (c->md) {           // the multi-determinant energy does not use Y; its TT GEMM has its own operands
         if (sp == 0) {
           const uint64_t r1 = (uint64_t)(c->ng + 1) * c->nact, r2 = (uint64_t)c->nw * 2 * c->nt;
           ok &= make_map(&c->map_tt.a_hi, c->RactT, c->MPK, r1, c->MPK, BM);
           ok &= make_map(&c->map_tt.a_lo, c->RactT_lo, c->MPK, r1, c->MPK, BM);
-          ok &= make_map(&c->map_tt.b_hi, c->thT, c->MPK, r2, c->MPK, BN);
-          ok &= make_map(&c->map_tt.b_lo, c->thT_lo, c->MPK, r2, c->MPK, BN);
+          ok &= make_map(&c->map_tt.b_hi, c->thT, c->MPK, r2, c->MPK, B_BOX);
+          ok &= make_map(&c->map_tt.b_lo, c->thT_lo, c->MPK, r2, c->MPK, B_BOX);
         }
         continue;
       }
@@ -847,6 +869,11 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
     cudaError_t e3 = cudaFuncSetAttribute(k_gemm_tf32<tc::EpiEnergy>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(k_gemm_tf32<tc::EpiTT>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(k_gemm_tf32<tc::EpiAssembleSym>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(k_gemm_tf32_pair<tc::EpiStoreT>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(k_gemm_tf32_pair<tc::EpiAssemble>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(k_gemm_tf32_pair<tc::EpiEnergy>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(k_gemm_tf32_pair<tc::EpiTT>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(k_gemm_tf32_pair<tc::EpiAssembleSym>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     if (!ok || e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) {
       snprintf(g_init_err, 256, "tcgen05 path: tensor-map / shared-memory set-up failed");
       delete c;
@@ -907,7 +934,7 @@ afqmc_status afqmc_profile_read(afqmc_ctx* c, int32_t stage, double* total_ms, i
 const char* afqmc_last_error(const afqmc_ctx* ctx) { return ctx ? ctx->err : g_init_err; }
 
 int64_t afqmc_launch_count(const afqmc_ctx* ctx) { return ctx ? ctx->launches : 0; }
-int32_t afqmc_gemm_path(const afqmc_ctx* ctx) { return ctx ? ctx->path : 0; }
+int32_t afqmc_gemm_path(const afqmc_ctx* ctx) { return ctx ? (ctx->cta2 ? 3 : ctx->path) : 0; }
 
 #define NEED(c, cond, msg) \
   do { if (!(cond)) return fail((c), AFQMC_EINVAL, "%s", msg); } while (0)

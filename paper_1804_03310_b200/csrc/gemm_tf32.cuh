@@ -20,6 +20,7 @@ enum { BM = 128, BN = 256, BK = 32, STAGES = 2, UMMA_K = 8, TMEM_COLS = 512, THR
 enum { CHUNK_KB = 4, EPI_WARPS = 8, COLS_PER_WARP = BN / 2 };
 enum { A_BYTES = BM * BK * 4, B_BYTES = BN * BK * 4, STAGE_BYTES = 2 * A_BYTES + 2 * B_BYTES };
 enum { SMEM_BYTES = STAGES * STAGE_BYTES + 1024 };
+enum { B_BOX = 128 };   // rows per TMA box of the b-operand maps
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -58,6 +59,45 @@ __device__ __forceinline__ void umma_tf32(uint32_t d_tmem, uint64_t adesc, uint6
   asm volatile(
       "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
       "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}"
+      ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc)
+      : "memory");
+}
+// ---- CTA pair (cta_group::2) forms.  Shared-window addresses of the two CTAs of a pair differ in bit 24; clearing
+// it addresses the even (leader) CTA's copy of the same variable.
+constexpr uint32_t PEER_MASK = 0xFEFFFFFFu;
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// TMA load into this CTA's shared memory, transaction bytes counted on the LEADER CTA's mbarrier
+__device__ __forceinline__ void tma_load_2d_pair(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+      ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar) & PEER_MASK), "r"(c0), "r"(c1)
+      : "memory");
+}
+// arrive on the same barrier in both CTAs of the pair once all MMAs issued so far have completed
+__device__ __forceinline__ void tc_commit_pair(uint64_t* bar) {
+  asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+               ::"r"(smem_u32(bar)), "h"((uint16_t)3)
+               : "memory");
+}
+// arrive on the leader CTA's copy of a barrier
+__device__ __forceinline__ void mbar_arrive_leader(uint64_t* bar) {
+  asm volatile(
+      "{\n.reg .b32 ra;\nmapa.shared::cluster.u32 ra, %0, 0;\nmbarrier.arrive.release.cluster.shared::cluster.b64 _, [ra];\n}"
+      ::"r"(smem_u32(bar))
+      : "memory");
+}
+// D[tmem of both CTAs] (+)= A * B with M = 256 (128 rows per CTA), the N rows of B split between the two CTAs
+__device__ __forceinline__ void umma_tf32_pair(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
+      "tcgen05.mma.cta_group::2.kind::tf32 [%0], %1, %2, %3, p;\n}"
       ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc)
       : "memory");
 }
@@ -312,8 +352,11 @@ __global__ void __launch_bounds__(THREADS, 1) k_gemm_tf32(const __grid_constant_
         const int kc = (kb0 + kb) * BK;
         tma_load_2d(st, &maps.a_hi, &full_bar[s], kc, m0);
         tma_load_2d(st + A_BYTES, &maps.a_lo, &full_bar[s], kc, m0);
+        // the b-operand maps have 128-row boxes (shared with the CTA-pair kernel): two loads per plane
         tma_load_2d(st + 2 * A_BYTES, &maps.b_hi, &full_bar[s], kc, n0);
+        tma_load_2d(st + 2 * A_BYTES + B_BYTES / 2, &maps.b_hi, &full_bar[s], kc, n0 + B_BOX);
         tma_load_2d(st + 2 * A_BYTES + B_BYTES, &maps.b_lo, &full_bar[s], kc, n0);
+        tma_load_2d(st + 2 * A_BYTES + B_BYTES + B_BYTES / 2, &maps.b_lo, &full_bar[s], kc, n0 + B_BOX);
       }
     }
   } else if (warp == EPI_WARPS + 1) {
@@ -389,6 +432,153 @@ __global__ void __launch_bounds__(THREADS, 1) k_gemm_tf32(const __grid_constant_
   if (warp == EPI_WARPS + 1) {
     __syncwarp();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"((uint32_t)TMEM_COLS) : "memory");
+  }
+}
+
+// ---- CTA-pair version: two CTAs of one TPC (cluster of 2 along grid x: a cluster of (1, 2, 1) is rejected at launch for cta_group::2 code) run one 256 x 256 tile with
+// tcgen05.mma.cta_group::2.  Each CTA holds its own 128 rows of A and HALF of the 256 b-operand rows, so every MMA
+// fetches 4 KB + 4 KB per SM for 128 math cycles instead of 4 KB + 8 KB: the shared-memory operand fetch that caps
+// the one-CTA kernel at 66 % of the pipe no longer binds.  The leader (even) CTA issues the MMAs; both CTAs run a
+// TMA producer (transaction bytes of both land on the leader's full barrier) and 8 epilogue warps on their own
+// 128 TMEM lanes.  Stage = 64 KB per CTA, three stages.
+enum { STAGES2 = 3, HB_BYTES = B_BYTES / 2, STAGE2_BYTES = 2 * A_BYTES + 2 * HB_BYTES };
+static_assert(STAGES2 * STAGE2_BYTES + 1024 <= SMEM_BYTES, "pair kernel uses the same dynamic smem size");
+static_assert(STAGES2 * STAGE2_BYTES >= BM * BN * 4, "staged epilogue needs the tile in shared memory");
+
+template <class Epi>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(THREADS, 1)
+k_gemm_tf32_pair(const __grid_constant__ Maps maps, int K, int tri, int m_tiles, int n_tiles, Epi epi) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  __shared__ __align__(8) uint64_t full_bar[STAGES2];     // used in the leader only
+  __shared__ __align__(8) uint64_t empty_bar[STAGES2];    // one in each CTA (multicast commit)
+  __shared__ __align__(8) uint64_t tmem_full_bar[2];      // one in each CTA (multicast commit)
+  __shared__ __align__(8) uint64_t tmem_empty_bar[2];     // leader only: 2 x 8 epilogue warps arrive
+  __shared__ uint32_t tmem_base_s;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+  // 1-D grid of pairs; the column tile varies fastest, so the CTAs running at one time share a few row tiles of A
+  // (each fetched from HBM once) and all of B stays in L2
+  const int pair = blockIdx.x >> 1, mt = (pair / n_tiles) * 2 + (int)rank;
+  const int m0 = mt * BM, n0 = (pair % n_tiles) * BN;
+  const int kb0 = tri ? ((mt & ~1) * BM) / BK : 0;   // the pair starts at the leader's diagonal block
+  const int nkb = K / BK - kb0;
+  const int nchunk = (nkb + CHUNK_KB - 1) / CHUNK_KB;
+
+  if (warp == EPI_WARPS && lane == 0) {
+#pragma unroll
+    for (int s = 0; s < STAGES2; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
+#pragma unroll
+    for (int b = 0; b < 2; ++b) { mbar_init(&tmem_full_bar[b], 1); mbar_init(&tmem_empty_bar[b], 2 * EPI_WARPS); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.a_hi) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.a_lo) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.b_hi) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.b_lo) : "memory");
+  }
+  if (warp == EPI_WARPS + 1) {   // the same warp in both CTAs allocates the pair's TMEM columns
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)),
+                 "r"((uint32_t)TMEM_COLS)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();      // the peer's barriers are initialised before anything is signalled across the pair
+  tc_fence_after();
+  const uint32_t tmem = tmem_base_s;
+
+  if (warp == EPI_WARPS) {
+    if (lane == 0) {   // ===== TMA producer (both CTAs): own A rows, own half of the B rows =====
+      for (int kb = 0; kb < nkb; ++kb) {
+        const int s = kb % STAGES2;
+        const uint32_t ph = (kb / STAGES2) & 1;
+        mbar_wait(&empty_bar[s], ph ^ 1);
+        uint8_t* st = smem + (size_t)s * STAGE2_BYTES;
+        if (rank == 0) mbar_expect_tx(&full_bar[s], 2 * STAGE2_BYTES);
+        const int kc = (kb0 + kb) * BK, nb = n0 + (int)rank * B_BOX;
+        tma_load_2d_pair(st, &maps.a_hi, &full_bar[s], kc, m0);
+        tma_load_2d_pair(st + A_BYTES, &maps.a_lo, &full_bar[s], kc, m0);
+        tma_load_2d_pair(st + 2 * A_BYTES, &maps.b_hi, &full_bar[s], kc, nb);
+        tma_load_2d_pair(st + 2 * A_BYTES + HB_BYTES, &maps.b_lo, &full_bar[s], kc, nb);
+      }
+    }
+  } else if (warp == EPI_WARPS + 1) {
+    if (lane == 0 && rank == 0) {   // ===== MMA issuer (leader CTA) =====
+      constexpr uint32_t idesc = make_idesc(2 * BM, BN);
+      for (int kb = 0; kb < nkb; ++kb) {
+        const int s = kb % STAGES2;
+        const uint32_t ph = (kb / STAGES2) & 1;
+        const int ci = kb / CHUNK_KB, buf = ci & 1;
+        const bool chunk_start = (kb % CHUNK_KB) == 0;
+        if (chunk_start) {   // the epilogue warps of both CTAs must have drained this TMEM buffer
+          mbar_wait(&tmem_empty_bar[buf], ((ci >> 1) & 1) ^ 1);
+          tc_fence_after();
+        }
+        mbar_wait(&full_bar[s], ph);
+        tc_fence_after();
+        const uint32_t d = tmem + buf * BN;
+        const uint32_t sa = smem_u32(smem + (size_t)s * STAGE2_BYTES);
+        const uint64_t a_hi = make_desc(sa), a_lo = make_desc(sa + A_BYTES);
+        const uint64_t b_hi = make_desc(sa + 2 * A_BYTES), b_lo = make_desc(sa + 2 * A_BYTES + HB_BYTES);
+#pragma unroll
+        for (int k = 0; k < BK / UMMA_K; ++k) {
+          const uint64_t adv = (uint64_t)((k * UMMA_K * 4) >> 4);
+          umma_tf32_pair(d, a_lo + adv, b_hi + adv, idesc, (chunk_start && k == 0) ? 0u : 1u);
+          umma_tf32_pair(d, a_hi + adv, b_lo + adv, idesc, 1u);
+          umma_tf32_pair(d, a_hi + adv, b_hi + adv, idesc, 1u);
+        }
+        tc_commit_pair(&empty_bar[s]);
+        if ((kb % CHUNK_KB) == CHUNK_KB - 1 || kb == nkb - 1) tc_commit_pair(&tmem_full_bar[buf]);
+      }
+    }
+  } else {             // ===== epilogue warps 0..7 of each CTA: its own 128 accumulator rows =====
+    const int q = warp & 3, half = warp >> 2;
+    const int row = m0 + q * 32 + lane;
+    float acc[COLS_PER_WARP];
+#pragma unroll
+    for (int i = 0; i < COLS_PER_WARP; ++i) acc[i] = 0.f;
+    for (int ci = 0; ci < nchunk; ++ci) {
+      const int buf = ci & 1;
+      mbar_wait(&tmem_full_bar[buf], (ci >> 1) & 1);
+      tc_fence_after();
+      const uint32_t t0 = tmem + ((uint32_t)(q * 32) << 16) + buf * BN + half * COLS_PER_WARP;
+#pragma unroll
+      for (int cb = 0; cb < COLS_PER_WARP / 32; ++cb) {
+        float v[32];
+        tmem_ld32(t0 + cb * 32, v);
+#pragma unroll
+        for (int j = 0; j < 32; ++j) acc[cb * 32 + j] += v[j];
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive_leader(&tmem_empty_bar[buf]);
+    }
+    if (mt < m_tiles) {   // the grid is padded to an even number of row tiles
+      if constexpr (Epi::kStaged) {
+        // every MMA of the pair has completed (last tmem_full observed), no TMA load is pending: the stages are free
+        float* S = reinterpret_cast<float*>(smem);
+#pragma unroll
+        for (int j = 0; j < COLS_PER_WARP; ++j) S[(half * COLS_PER_WARP + j) * BM + q * 32 + lane] = acc[j];
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        epi.flush(S, m0, n0, (int)threadIdx.x);
+      } else {
+#pragma unroll
+        for (int cb = 0; cb < COLS_PER_WARP / 32; ++cb) {
+          float v[32];
+#pragma unroll
+          for (int j = 0; j < 32; ++j) v[j] = acc[cb * 32 + j];
+          epi(row, n0 + half * COLS_PER_WARP + cb * 32, v);
+        }
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();      // neither CTA leaves while the other may still read its shared memory or signal its barriers
+  if (warp == EPI_WARPS + 1) {
+    __syncwarp();
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"((uint32_t)TMEM_COLS) : "memory");
   }
 }
 

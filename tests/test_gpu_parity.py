@@ -290,17 +290,18 @@ def test_singular_walker_sets_flag():
     assert np.all(out["flags"][[0, 1, 3]] == 0)
 
 
-# ---- tcgen05 3xTF32 contraction path (gemm_path = 2): same oracle, same tolerances -------------------------
+# ---- tcgen05 3xTF32 contraction path (gemm_path = 2: one CTA per tile, 3: CTA pairs): same oracle, same tolerances
+@pytest.mark.parametrize("path", [2, 3])
 @pytest.mark.parametrize("cfg", [2, 3, 5])
-def test_tcgen05_stage_forcebias_energy_propagate(cfg):
+def test_tcgen05_stage_forcebias_energy_propagate(cfg, path):
     import torch
     wl = _wl(cfg)
     nw = {2: 200, 3: 136, 5: 6}[cfg]      # ragged against the 256-column tile (2 nw = 400 / 272 / 12)
     tol = H.tol_for(wl)
     ini, _ = H.oracle_init(wl)
     phi = random_walkers(wl, nw, seed=5, spread=0.1)
-    ctx = H.make_ctx(wl, nw, gemm_path=2)
-    assert ctx.gemm_path == 2
+    ctx = H.make_ctx(wl, nw, gemm_path=path)
+    assert ctx.gemm_path == path
     st = H.DeviceState(ctx, phi)
     st.seed()
     eloc = torch.zeros(nw, dtype=torch.complex128, device=ctx.device)
@@ -315,15 +316,16 @@ def test_tcgen05_stage_forcebias_energy_propagate(cfg):
     errs = dict(f=H.rel_fro(g0["f"], ost.f_a + ost.f_b), E=H.rel_abs(eloc.cpu().numpy(), ost.eloc),
                 phi=H.rel_fro(out["phi"], rec["phi"]), S=H.rel_abs(out["S"], rec["S"]),
                 w=H.weight_err(out["w"], rec, ost.w, wl.dt, wl.E0))
-    print(f"cfg{cfg} tcgen05 3xTF32 stage errors: {errs}")
+    print(f"cfg{cfg} tcgen05 3xTF32 (gemm_path {path}) stage errors: {errs}")
     for k, v in errs.items():
         assert v < tol, (k, v)
 
 
+@pytest.mark.parametrize("path", [2, 3])
 @pytest.mark.parametrize("cfg,variant", [(3, "mf"), (5, "mf")])
-def test_protocol_A_resync_tcgen05(cfg, variant):
+def test_protocol_A_resync_tcgen05(cfg, variant, path):
     wl = _wl(cfg, variant)
-    _protocol_A(wl, SMALL[cfg], {5: 3}.get(cfg, 10), gemm_path=2)
+    _protocol_A(wl, SMALL[cfg], {5: 3}.get(cfg, 10), gemm_path=path)
 
 
 def test_full_size_sampled_walkers():
