@@ -485,6 +485,27 @@ template <typename T> afqmc_status run_md_energy(afqmc_ctx* c, const void* theta
     if (st) return st;
   }
   const int dpt = (c->ndet + MD_THREADS - 1) / MD_THREADS;
+  if constexpr (sizeof(T) == 4) {
+    // batched-gamma kernel (gemm_path 1 keeps the one-operator-at-a-time kernel): n_sigma <= 16, <= 2 determinants per thread (more would spill its per-determinant
+    // registers), tiles that are 16-byte multiples, shared memory that fits
+    const int nmax = c->na > c->nb ? c->na : c->nb;
+    const size_t smb = md_energy_b_smem(c->M, c->na, c->nb, c->nact, c->ndet, c->ts);
+    if (c->path == 2 && nmax <= 16 && dpt <= 2 && ((size_t)c->nact * c->nt * 2 * c->ts) % 16 == 0 && smb <= 200 * 1024) {
+#define MDB_LAUNCH(N, D)                                                                                           \
+  {                                                                                                                \
+    auto kern = k_md_energy_b<T, N, D>;                                                                            \
+    if (smb > 48 * 1024)                                                                                           \
+      CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb));               \
+    LAUNCH(c, kern, c->nw, MD_THREADS, smb, a);                                                                    \
+  }
+#define MDB_PICK(N)                                                                                                \
+  { if (dpt <= 1) MDB_LAUNCH(N, 1) else MDB_LAUNCH(N, 2) }
+      if (nmax <= 8) MDB_PICK(8) else if (nmax <= 12) MDB_PICK(12) else MDB_PICK(16)
+#undef MDB_PICK
+#undef MDB_LAUNCH
+      return AFQMC_OK;
+    }
+  }
 #define MDE_LAUNCH(D)                                                                                              \
   {                                                                                                                \
     auto kern = k_md_energy<T, D>;                                                                                 \

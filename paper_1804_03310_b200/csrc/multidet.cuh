@@ -431,4 +431,217 @@ __global__ void __launch_bounds__(MD_THREADS) k_md_energy(MdEnergyArgs<T> g) {
   if (tid == 0) g.eloc[w] = tot;
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// Batched-gamma version of k_md_energy (same arithmetic).  The kernel above walks the operators one at a time with three
+// CTA barriers each and a fraction of its threads busy; here MDB_G operators are processed per pass:
+//   A. one thread per (operator, spin, virtual row pv): the W row (n x n complex MACs against Q_virt), then the WT row
+//      (n x n more), rows in registers, T0 read from the TT tiles that cp.async double-buffers in shared memory;
+//   A2. f0 = Tr T0 and X0 = Tr(T0 T0) reduced from per-row partials;
+//   B. one thread per determinant, looping over the operators of the batch with its Z and excitation pattern in registers.
+// Three barriers per MDB_G operators.  Needs n_sigma <= NMAX and 16-byte multiples for the tiles (host checks).
+// ---------------------------------------------------------------------------------------------
+enum { MDB_G = 6, MDB_PAD = 2 };   // tiles MDB_PAD complex apart in shared memory: operators of a batch hit different banks
+
+inline size_t md_energy_b_smem(int M, int na, int nb, int nact, int ndet, int ts) {
+  size_t b = md_smem_bytes(na, nb, nact, ndet);
+  b += ((size_t)M * (na + nb) * 2 * ts + 15) & ~size_t(15);
+  const size_t nva = nact - na, nvb = nact - nb, nw_ = nva * na + nvb * nb, nvm = nva > nvb ? nva : nvb;
+  const size_t celems = (size_t)2 * MDB_G * (nact * (na + nb) + MDB_PAD) + (size_t)2 * MDB_G * nw_ + nw_ + (size_t)ndet * 8 +
+                        (size_t)MDB_G * 4 + (size_t)MDB_G * 2 * (nvm ? nvm : 1) * 2;
+  return b + celems * 2 * ts + 32;
+}
+
+template <typename T, int NMAX, int MD_DPT>
+__global__ void __launch_bounds__(MD_THREADS) k_md_energy_b(MdEnergyArgs<T> g) {
+  typedef cplx<T> C;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const MdConst& m = g.m;
+  const int w = blockIdx.x, tid = threadIdx.x, nthr = blockDim.x, nt = m.na + m.nb, M = m.M, nact = m.nact;
+  MdSmem s;
+  unsigned char* p = md_carve(smem_raw, m, s);
+  C* th0 = reinterpret_cast<C*>(p);
+  p += ((size_t)M * nt * sizeof(C) + 15) & ~size_t(15);
+  const int nva = nact - m.na, nvb = nact - m.nb, nvt = nva + nvb, nvm = nva > nvb ? nva : nvb;
+  const int nwa = nva * m.na, nwb = nvb * m.nb, nwt = nwa + nwb, tile = nact * nt;
+  const int tstr = tile + MDB_PAD;             // padded tile stride
+  C* TTb = reinterpret_cast<C*>(p);            // [2][MDB_G][tstr]   (16-byte aligned: cp.async destination)
+  C* Wb = TTb + 2 * MDB_G * tstr;              // [MDB_G][nwa + nwb]
+  C* WTb = Wb + MDB_G * nwt;
+  C* Qc[2]; Qc[0] = WTb + MDB_G * nwt; Qc[1] = Qc[0] + nwa;
+  C* Zc = Qc[1] + nwb;                         // [ndet][2][4]
+  C* scal = Zc + (size_t)m.ndet * 8;           // [MDB_G][f0 a, f0 b, X0 a, X0 b]
+  C* part = scal + MDB_G * 4;                  // [MDB_G][2][nvm][f0, X0]
+  const int nop = g.ng + 1, nbatch = (nop + MDB_G - 1) / MDB_G;
+  const C* srcw = g.TTg + (size_t)w * nop * tile;
+  auto fetch = [&](int bi) {
+    const int g0 = bi * MDB_G, gc = min(MDB_G, nop - g0);
+    const int t16 = (int)((size_t)tile * sizeof(C) / 16);
+    const unsigned char* src = reinterpret_cast<const unsigned char*>(srcw + (size_t)g0 * tile);
+    unsigned char* dst = reinterpret_cast<unsigned char*>(TTb + (size_t)(bi & 1) * MDB_G * tstr);
+    for (int e = tid; e < gc * t16; e += nthr) {
+      const int gl = e / t16, r = e - gl * t16;
+      cp_async16(dst + ((size_t)gl * tstr * sizeof(C) + (size_t)r * 16), src + (size_t)e * 16);
+    }
+    cp_async_commit();
+  };
+  fetch(0);
+
+  for (int e = tid; e < M * nt; e += nthr) th0[e] = g.theta0[(size_t)w * M * nt + e];
+  __syncthreads();
+  md_prepare<T>(m, th0, s);
+  for (int e = tid; e < nwt; e += nthr) Qc[0][e] = mk<T>((T)s.Qv[0][e].x, (T)s.Qv[0][e].y);
+  for (int e = tid; e < m.ndet * 8; e += nthr) Zc[e] = mk<T>((T)s.Z[e].x, (T)s.Z[e].y);
+
+  zcplx Eacc[MD_DPT];
+  uint32_t pat[MD_DPT][2]; int rks[MD_DPT];
+#pragma unroll
+  for (int j = 0; j < MD_DPT; ++j) {
+    Eacc[j] = mk<double>(0.0, 0.0);
+    const int i = tid + j * MD_THREADS;
+    rks[j] = 0; pat[j][0] = pat[j][1] = 0;
+    if (i < m.ndet)
+      for (int sp = 0; sp < 2; ++sp) {
+        int h[2], pp[2];
+        const int rk = md_exc(m, i, sp, h, pp);
+        const int n = sp ? m.nb : m.na;
+        rks[j] |= rk << (2 * sp);
+        pat[j][sp] = (uint32_t)(h[0] & 255) | ((uint32_t)((pp[0] - n) & 255) << 8) | ((uint32_t)(h[1] & 255) << 16) |
+                     ((uint32_t)((pp[1] - n) & 255) << 24);
+      }
+  }
+
+  for (int bi = 0; bi < nbatch; ++bi) {
+    const int g0 = bi * MDB_G, gc = min(MDB_G, nop - g0);
+    if (bi + 1 < nbatch) { fetch(bi + 1); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
+    __syncthreads();   // this batch's tiles have landed; the previous pass no longer reads W / WT / scal
+    const C* TT = TTb + (size_t)(bi & 1) * MDB_G * tstr;
+    // ---- A: W = TT_virt - Q_virt T0 and WT = W T0, one row per thread
+    for (int it = tid; it < gc * nvt; it += nthr) {
+      const int gl = it / nvt, r = it - gl * nvt, sp = r >= nva, pv = sp ? r - nva : r;
+      const int n = sp ? m.nb : m.na, nv = sp ? nvb : nva, off = sp ? m.na : 0;
+      const C* T0 = TT + (size_t)gl * tstr + off;          // T0[h * nt + a]
+      const int wo = gl * nwt + (sp ? nwa : 0) + pv * n;
+      C wr[NMAX];
+#pragma unroll
+      for (int a = 0; a < NMAX; ++a) wr[a] = a < n ? T0[(n + pv) * nt + a] : mk<T>(T(0), T(0));
+      for (int h = 0; h < n; ++h) {
+        const C q = Qc[sp][pv * n + h];
+#pragma unroll
+        for (int a = 0; a < NMAX; ++a)
+          if (a < n) wr[a] = csub(wr[a], cmul(q, T0[h * nt + a]));
+      }
+#pragma unroll
+      for (int a = 0; a < NMAX; ++a)
+        if (a < n) Wb[wo + a] = wr[a];
+      C wt[NMAX];
+#pragma unroll
+      for (int a = 0; a < NMAX; ++a) wt[a] = mk<T>(T(0), T(0));
+      for (int b = 0; b < n; ++b) {
+        const C wb = Wb[wo + b];
+#pragma unroll
+        for (int a = 0; a < NMAX; ++a)
+          if (a < n) cfma(wt[a], wb, T0[b * nt + a]);
+      }
+#pragma unroll
+      for (int a = 0; a < NMAX; ++a)
+        if (a < n) WTb[wo + a] = wt[a];
+      C f0 = mk<T>(T(0), T(0)), x0 = mk<T>(T(0), T(0));
+      for (int a = pv; a < n; a += nv) {
+        f0 = cadd(f0, T0[a * nt + a]);
+        for (int b = 0; b < n; ++b) cfma(x0, T0[a * nt + b], T0[b * nt + a]);
+      }
+      part[((gl * 2 + sp) * nvm + pv) * 2 + 0] = f0;
+      part[((gl * 2 + sp) * nvm + pv) * 2 + 1] = x0;
+    }
+    __syncthreads();
+    // ---- A2: f0, X0 per (operator, spin)
+    for (int it = tid; it < gc * 2; it += nthr) {
+      const int gl = it >> 1, sp = it & 1, n = sp ? m.nb : m.na, nv = sp ? nvb : nva, off = sp ? m.na : 0;
+      C f0 = mk<T>(T(0), T(0)), x0 = mk<T>(T(0), T(0));
+      if (nv > 0) {
+        for (int pv = 0; pv < nv; ++pv) {
+          f0 = cadd(f0, part[((gl * 2 + sp) * nvm + pv) * 2 + 0]);
+          x0 = cadd(x0, part[((gl * 2 + sp) * nvm + pv) * 2 + 1]);
+        }
+      } else {   // no virtual orbital for this spin: nobody computed the partials
+        const C* T0 = TT + (size_t)gl * tstr + off;
+        for (int a = 0; a < n; ++a) {
+          f0 = cadd(f0, T0[a * nt + a]);
+          for (int b = 0; b < n; ++b) cfma(x0, T0[a * nt + b], T0[b * nt + a]);
+        }
+      }
+      scal[gl * 4 + sp] = f0; scal[gl * 4 + 2 + sp] = x0;
+    }
+    __syncthreads();
+    // ---- B: per determinant, E x E work per operator
+#pragma unroll
+    for (int j = 0; j < MD_DPT; ++j) {
+      const int i = tid + j * MD_THREADS;
+      if (i >= m.ndet) continue;
+      C zz[2][4];
+#pragma unroll
+      for (int sp = 0; sp < 2; ++sp)
+#pragma unroll
+        for (int u = 0; u < 4; ++u) zz[sp][u] = Zc[((size_t)i * 2 + sp) * 4 + u];
+      for (int gl = 0; gl < gc; ++gl) {
+        const bool is_h = g0 + gl == g.ng;
+        C tsum = mk<T>(T(0), T(0)), xsum = mk<T>(T(0), T(0));
+#pragma unroll
+        for (int sp = 0; sp < 2; ++sp) {
+          const int n = sp ? m.nb : m.na;
+          const int rk = (rks[j] >> (2 * sp)) & 3;
+          const uint32_t pt = pat[j][sp];
+          const int h0 = pt & 255, p0 = (pt >> 8) & 255, h1 = (pt >> 16) & 255, p1 = (pt >> 24) & 255;
+          const C* Wm = Wb + gl * nwt + (sp ? nwa : 0);
+          const C* WTm = WTb + gl * nwt + (sp ? nwa : 0);
+          C t = scal[gl * 4 + sp], xch = scal[gl * 4 + 2 + sp];
+          if (rk == 1) {
+            C zw = cmul(zz[sp][0], Wm[p0 * n + h0]);
+            t = cadd(t, zw);
+            if (!is_h) {
+              C zt = cmul(zz[sp][0], WTm[p0 * n + h0]);
+              xch = cadd(xch, mk<T>(2 * zt.x, 2 * zt.y));
+              cfma(xch, zw, zw);
+            }
+          } else if (rk == 2) {
+            const C w00 = Wm[p0 * n + h0], w01 = Wm[p0 * n + h1], w10 = Wm[p1 * n + h0], w11 = Wm[p1 * n + h1];
+            const C z00 = zz[sp][0], z01 = zz[sp][1], z10 = zz[sp][2], z11 = zz[sp][3];
+            C a00 = cmul(z00, w00); cfma(a00, z01, w10);
+            C a01 = cmul(z00, w01); cfma(a01, z01, w11);
+            C a10 = cmul(z10, w00); cfma(a10, z11, w10);
+            C a11 = cmul(z10, w01); cfma(a11, z11, w11);
+            t = cadd(t, cadd(a00, a11));
+            if (!is_h) {
+              const C v00 = WTm[p0 * n + h0], v10 = WTm[p1 * n + h0], v01 = WTm[p0 * n + h1], v11 = WTm[p1 * n + h1];
+              C b00 = cmul(z00, v00); cfma(b00, z01, v10);
+              C b11 = cmul(z10, v01); cfma(b11, z11, v11);
+              xch = cadd(xch, mk<T>(2 * (b00.x + b11.x), 2 * (b00.y + b11.y)));
+              cfma(xch, a00, a00); cfma(xch, a11, a11);
+              C cr = cmul(a01, a10);
+              xch = cadd(xch, mk<T>(2 * cr.x, 2 * cr.y));
+            }
+          }
+          tsum = cadd(tsum, t);
+          xsum = cadd(xsum, xch);
+        }
+        if (is_h) {
+          Eacc[j].x += (double)tsum.x; Eacc[j].y += (double)tsum.y;
+        } else {
+          C e2 = csub(cmul(tsum, tsum), xsum);
+          Eacc[j].x += 0.5 * (double)e2.x; Eacc[j].y += 0.5 * (double)e2.y;
+        }
+      }
+    }
+  }
+  zcplx partE = mk<double>(0.0, 0.0);
+#pragma unroll
+  for (int j = 0; j < MD_DPT; ++j) {
+    const int i = tid + j * MD_THREADS;
+    if (i < m.ndet) partE = zadd(partE, zmul(s.omega[i], Eacc[j]));
+  }
+  zcplx tot = block_sum(partE, s.red);
+  if (tid == 0) g.eloc[w] = tot;
+}
+
 }  // namespace afq

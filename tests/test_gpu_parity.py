@@ -53,16 +53,18 @@ def test_stage_overlap_green_forcebias_energy(cfg):
         assert v < tol, (k, v)
 
 
-def test_stage_multidet_overlap_forcebias_energy():
+@pytest.mark.parametrize("path", [0, 1])
+def test_stage_multidet_overlap_forcebias_energy(path):
     """cfg 4 (100 determinants): S, mixed G, mixed f, mixed E_L against the oracle's DEFINITION path (every
-    determinant recomputed directly) -- the GPU uses SMW rank-E closed forms (Eq.(4))."""
+    determinant recomputed directly) -- the GPU uses SMW rank-E closed forms (Eq.(4)).  path 0: tcgen05 GEMMs and the
+    batched-gamma energy kernel; path 1: SIMT GEMMs and the one-operator-at-a-time energy kernel."""
     import torch
     wl = _wl(4)
     nw = SMALL[4]
     tol = H.tol_for(wl)
     ini, trial = H.oracle_init(wl)
     phi = random_walkers(wl, nw, seed=11, spread=0.2)
-    ctx = H.make_ctx(wl, nw)
+    ctx = H.make_ctx(wl, nw, gemm_path=path)
     st = H.DeviceState(ctx, phi)
     G = torch.zeros(nw, 2, wl.M, wl.M, dtype=ctx.cdtype, device=ctx.device)
     ctx.afqmc_overlap_green(st.phi, st.ovlp, st.theta, G, st.flags)
@@ -73,7 +75,7 @@ def test_stage_multidet_overlap_forcebias_energy():
     S, f, E, Gref = orc.o_multidet_definition(ini, trial, phi, wl.n_alpha, want_G=True)
     errs = dict(S=H.rel_abs(out["S"], S), G=H.rel_fro(G.cpu().numpy().astype(np.complex128), Gref),
                 f=H.rel_fro(out["f"], f), E=H.rel_abs(eloc.cpu().numpy(), E))
-    print(f"cfg4 multi-det stage errors: {errs}")
+    print(f"cfg4 multi-det stage errors (gemm_path {ctx.gemm_path}): {errs}")
     for k, v in errs.items():
         assert v < tol, (k, v)
 
