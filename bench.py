@@ -278,11 +278,11 @@ def run_ours(args):
         dtype = "f32" if wl.precision == "c64" else "f64"
         if wl.precision == "c128":
             peak, peak_note = fp32_peak / 2, "FP64 FMA: 148 SMs x 64 lanes x 2 flop x clocks.max.sm (DESIGN.md)"
-    names = dict(assemble="H6 assembly GEMM A_w = sum_g z_g L_g (tc::k_gemm_tf32<EpiAssemble> / k_gemm_nt)",
+    names = dict(assemble="H6 assembly GEMM A_w = sum_g z_g L_g (tc::k_gemm_tf32_pair<EpiAssembleSym> / k_gemm_tf32 / k_gemm_nt)",
                  taylor="H7 Taylor propagator (tt::k_taylor_tc / k_taylor)",
                  energy="H9 energy GEMMs + fused dot (or H10 multi-det energy)", force_bias="H4 force-bias GEMMs",
                  green="H1-H3/H8 overlap, LU, Theta, weights (k_green)")
-    traffic_ncu = {"assemble": 1.306e9, "taylor": 2.10e9} if (ctx.gemm_path >= 2 and args.cfg == 5) else {}
+    traffic_ncu = {"assemble": 2.227e9, "taylor": 2.131e9} if (ctx.gemm_path >= 2 and args.cfg == 5) else {}
 
     def roof(stage):
         ms, n = prof[stage]
