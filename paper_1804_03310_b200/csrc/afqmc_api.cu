@@ -827,12 +827,6 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
     a.mtiles = (c->M + 127) / 128;
     a.rows_last = (int)rup((size_t)(c->M - 128 * (a.mtiles - 1)), 8);
     a.nkb = (c->M + 31) / 32;
-    {
-      const int maxch = 1;   // (kept for the args struct; the kernel now uses one 128-column region per tile and plane)
-      a.chunk_kb = (a.nkb + maxch - 1) / maxch;
-      if (a.chunk_kb < 2 && a.nkb >= 4) a.chunk_kb = 2;
-      a.nch = (a.nkb + a.chunk_kb - 1) / a.chunk_kb;
-    }
     a.phi = nullptr;
     c->tay_tc_smem = tt::smem_bytes(a.nkb);
     int dev = 0;

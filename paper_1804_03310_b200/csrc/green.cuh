@@ -6,64 +6,6 @@
 
 namespace afq {
 
-// Gauss-Jordan with partial pivoting on the augmented n x 2n matrix [A | I] held in shared memory,
-// executed by ONE warp.  On exit the right block is A^-1; det = product of pivots (FP64, R17).
-// sing bit 0: a pivot was exactly zero / NaN or below eps*max|A|.
-template <typename T>
-__device__ void warp_gauss_jordan(cplx<T>* aug, int n, int ld, cplx<T>* fac, int lane, zcplx& det, int& sing, T eps) {
-  double dre = 1.0, dim = 0.0;
-  sing = 0;
-  T amax = T(0);
-  for (int e = lane; e < n * n; e += 32) amax = fmax(amax, cabs2(aug[(e / n) * ld + (e % n)]));
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) amax = fmax(amax, __shfl_xor_sync(0xffffffffu, amax, o));
-  const T thresh = amax * eps * eps;  // compare squared magnitudes
-  for (int col = 0; col < n; ++col) {
-    int r = col + lane;
-    T mag = (r < n) ? cabs2(aug[r * ld + col]) : T(-1);
-    int idx = r;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      T om = __shfl_xor_sync(0xffffffffu, mag, o);
-      int oi = __shfl_xor_sync(0xffffffffu, idx, o);
-      if (om > mag || (om == mag && oi < idx)) { mag = om; idx = oi; }
-    }
-    if (idx != col) {
-      for (int c = lane; c < 2 * n; c += 32) {
-        cplx<T> t = aug[col * ld + c];
-        aug[col * ld + c] = aug[idx * ld + c];
-        aug[idx * ld + c] = t;
-      }
-      dre = -dre; dim = -dim;
-    }
-    __syncwarp();
-    cplx<T> p = aug[col * ld + col];
-    if (!(mag > T(0))) { sing = 1; dre = 0.0; dim = 0.0; break; }
-    if (mag < thresh) sing = 1;
-    double nr = dre * (double)p.x - dim * (double)p.y;
-    dim = dre * (double)p.y + dim * (double)p.x;
-    dre = nr;
-    cplx<T> ip = cinv(p);
-    __syncwarp();
-    for (int c = lane; c < 2 * n; c += 32) aug[col * ld + c] = cmul(aug[col * ld + c], ip);
-    for (int rr = lane; rr < n; rr += 32) fac[rr] = aug[rr * ld + col];
-    __syncwarp();
-    for (int rr = 0; rr < n; ++rr) {
-      if (rr == col) continue;
-      cplx<T> f = fac[rr];
-      for (int c = lane; c < 2 * n; c += 32) {
-        cplx<T> v = aug[rr * ld + c];
-        cplx<T> pr = aug[col * ld + c];
-        v.x = fma(-f.x, pr.x, v.x); v.x = fma(f.y, pr.y, v.x);
-        v.y = fma(-f.x, pr.y, v.y); v.y = fma(-f.y, pr.x, v.y);
-        aug[rr * ld + c] = v;
-      }
-    }
-    __syncwarp();
-  }
-  det = mk<double>(dre, dim);
-}
-
 // The same elimination executed by a GROUP of 128 threads (4 warps, named barrier `bar_id`): the serial
 // one-warp version left 6 of the CTA's 8 warps idle and dominated the kernel (ncu: most stall samples at the CTA
 // barrier behind it).  work = [fac (n) | prow (2n)] scratch; ctrl = one int.  Warp 0 of the group does the pivot

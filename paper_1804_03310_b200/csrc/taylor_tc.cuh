@@ -29,9 +29,6 @@ struct TaylorMaps {
 struct TaylorTcArgs {
   int M, MP, nt, K, nw;
   int mtiles, rows_last, nkb;   // 128-row tiles, rows of the last one (multiple of 8), 32-column k-blocks
-  int nch, chunk_kb;            // accumulation chunks per tile (each its own 64 TMEM columns) and k-blocks per chunk:
-                                // the tensor pipe truncates when it adds into its accumulator, so one long chain
-                                // drifts; chunks are summed round-to-nearest in registers by the epilogue warps
   cplx<float>* phi;             // [nw][M][nt] in/out
 };
 
