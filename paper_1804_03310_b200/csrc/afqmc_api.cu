@@ -68,6 +68,7 @@ struct afqmc_ctx {
   tc::Maps map_asm, map_fb[2], map_en[2];
   int nblk; int2* blk;   // symmetric block list of the tcgen05 assembly GEMM
   int cta2;   // tcgen05 GEMMs run on CTA pairs (cta_group::2), gemm_path 3
+  int ps_ok;  // the persistent pair kernel's shared-memory request was accepted
   int tay_tc; void *Abuf_lo, *Eh_lo; tt::TaylorMaps map_tay; tt::TaylorTcArgs tay_args; size_t tay_tc_smem; int n_sm;   // TMA descriptors of the tcgen05 path (path == 2)
   char err[256];
   int64_t launches;
@@ -423,6 +424,16 @@ afqmc_status run_gemm_tc(afqmc_ctx* c, const tc::Maps& maps, int m, int n, int K
   if (c->cta2 && pair_ok) {
     const int m_tiles = (int)grid.y;
     const int n_tiles = (int)grid.x;
+    if constexpr (Epi::kStaged) {
+      // persistent pairs: the staged epilogue of one tile overlaps the main loop of the next
+      const int n_pairs = (m_tiles + 1) / 2 * n_tiles, slots = c->n_sm / 2;
+      if (!tri && slots > 0 && c->ps_ok) {
+        dim3 gridp(2 * (n_pairs < slots ? n_pairs : slots));
+        auto kernp = tc::k_gemm_tf32_pair_ps<Epi>;
+        LAUNCH(c, kernp, gridp, tc::THREADS, tc::SMEM_PS_BYTES, maps, K, m_tiles, n_tiles, n_pairs, epi);
+        return AFQMC_OK;
+      }
+    }
     dim3 grid2(((grid.y + 1) & ~1u) * grid.x);   // CTA pairs = clusters of two adjacent row tiles, 1-D grid
     auto kern2 = tc::k_gemm_tf32_pair<Epi>;
     LAUNCH(c, kern2, grid2, tc::THREADS, tc::SMEM_BYTES, maps, K, tri, m_tiles, n_tiles, epi);
@@ -783,6 +794,11 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
   c->path = resolve_path(p);
   c->split = c->path == 2;
   c->cta2 = resolve_cta2(p);
+  {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
+  }
   size_t cb, wb;
   carve(p, c, (char*)const_mem, (char*)work_mem, &cb, &wb);
   if (p->precision) {
@@ -889,6 +905,8 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
     if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(k_gemm_tf32_pair<tc::EpiEnergy>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(k_gemm_tf32_pair<tc::EpiTT>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(k_gemm_tf32_pair<tc::EpiAssembleSym>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    c->ps_ok = cudaFuncSetAttribute(k_gemm_tf32_pair_ps<tc::EpiAssembleSym>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_PS_BYTES) == cudaSuccess;
+    (void)cudaGetLastError();
     if (!ok || e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) {
       snprintf(g_init_err, 256, "tcgen05 path: tensor-map / shared-memory set-up failed");
       delete c;

@@ -236,6 +236,26 @@ struct EpiAssembleSym {
       put4((size_t)(col >> 1) * M * (2 * MP) + (col & 1) * MP + (size_t)j * (2 * MP) + i, x);
     }
   }
+  // Quarter r of the tile (persistent kernel): staged column sc = half * 32 + j  <->  tile column half * 128 + r * 32 + j
+  __device__ __forceinline__ void flush_part(const float* S, int m0, int n0, int t, int r) const {
+    const int2 b = blk[m0 >> 7];
+    const int i0 = b.x * 8, j0 = b.y * 16;
+    for (int u = t; u < 64 * 32; u += 256) {           // direct
+      const int sc = u >> 5, ii = (u >> 2) & 7, v = u & 3;
+      const int col = n0 + (sc >> 5) * 128 + r * 32 + (sc & 31), i = i0 + ii, j = j0 + 4 * v;
+      if (col >= n_real || i >= M || j >= M) continue;
+      const float4 x = *reinterpret_cast<const float4*>(S + sc * 128 + ii * 16 + 4 * v);
+      put4((size_t)(col >> 1) * M * (2 * MP) + (col & 1) * MP + (size_t)i * (2 * MP) + j, x);
+    }
+    for (int u = t; u < 64 * 32; u += 256) {           // mirrored
+      const int sc = u >> 5, jj = (u >> 1) & 15, v = u & 1;
+      const int col = n0 + (sc >> 5) * 128 + r * 32 + (sc & 31), j = j0 + jj, i = i0 + 4 * v;
+      if (col >= n_real || i >= M || j >= M) continue;
+      const float* p = S + sc * 128 + (4 * v) * 16 + jj;
+      const float4 x = make_float4(p[0], p[16], p[32], p[48]);
+      put4((size_t)(col >> 1) * M * (2 * MP) + (col & 1) * MP + (size_t)j * (2 * MP) + i, x);
+    }
+  }
 };
 
 struct EpiTT {          // H10: row = g*nact + q, col = (w*nt + a)*2 + p -> TT[w][g][q][a] (interleaved complex)
@@ -576,6 +596,150 @@ k_gemm_tf32_pair(const __grid_constant__ Maps maps, int K, int tri, int m_tiles,
   tc_fence_before();
   __syncthreads();
   cluster_sync_all();      // neither CTA leaves while the other may still read its shared memory or signal its barriers
+  if (warp == EPI_WARPS + 1) {
+    __syncwarp();
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"((uint32_t)TMEM_COLS) : "memory");
+  }
+}
+
+// ---- persistent CTA-pair version for staged epilogues (H6): one pair per TPC loops over the tile pairs.  The operand
+// ring (3 x 64 KB) and the staging area (32 KB, a quarter tile) are separate, so while the 8 epilogue warps of each CTA
+// push the finished tile out in four rounds, the TMA producer and the MMA issuer are already two accumulation chunks
+// into the next tile (the two TMEM buffers are free as soon as the last chunk sits in registers).  Barrier phases run
+// on across tiles (global k-block / chunk counters).
+enum { STG_COLS = 64, STG_BYTES = BM * STG_COLS * 4, SMEM_PS_BYTES = STAGES2 * STAGE2_BYTES + STG_BYTES + 1024 };
+
+template <class Epi>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(THREADS, 1)
+k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps, int K, int m_tiles, int n_tiles, int n_pairs, Epi epi) {
+  static_assert(Epi::kStaged, "persistent kernel is written for the staged epilogue");
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  float* S = reinterpret_cast<float*>(smem + (size_t)STAGES2 * STAGE2_BYTES);
+  __shared__ __align__(8) uint64_t full_bar[STAGES2];     // used in the leader only
+  __shared__ __align__(8) uint64_t empty_bar[STAGES2];
+  __shared__ __align__(8) uint64_t tmem_full_bar[2];
+  __shared__ __align__(8) uint64_t tmem_empty_bar[2];     // leader only: 2 x 8 epilogue warps arrive
+  __shared__ uint32_t tmem_base_s;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+  const int cid = blockIdx.x >> 1, ncl = gridDim.x >> 1;
+  const int nkb = K / BK;
+  const int nchunk = (nkb + CHUNK_KB - 1) / CHUNK_KB;
+
+  if (warp == EPI_WARPS && lane == 0) {
+#pragma unroll
+    for (int s = 0; s < STAGES2; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
+#pragma unroll
+    for (int b = 0; b < 2; ++b) { mbar_init(&tmem_full_bar[b], 1); mbar_init(&tmem_empty_bar[b], 2 * EPI_WARPS); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.a_hi) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.a_lo) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.b_hi) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.b_lo) : "memory");
+  }
+  if (warp == EPI_WARPS + 1) {
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)),
+                 "r"((uint32_t)TMEM_COLS)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();
+  tc_fence_after();
+  const uint32_t tmem = tmem_base_s;
+
+  if (warp == EPI_WARPS) {
+    if (lane == 0) {   // ===== TMA producer (both CTAs) =====
+      uint32_t it = 0;
+      for (int tp = cid; tp < n_pairs; tp += ncl) {
+        const int m0 = ((tp / n_tiles) * 2 + (int)rank) * BM, nb = (tp % n_tiles) * BN + (int)rank * B_BOX;
+        for (int kb = 0; kb < nkb; ++kb, ++it) {
+          const int s = it % STAGES2;
+          mbar_wait(&empty_bar[s], ((it / STAGES2) & 1) ^ 1);
+          uint8_t* st = smem + (size_t)s * STAGE2_BYTES;
+          if (rank == 0) mbar_expect_tx(&full_bar[s], 2 * STAGE2_BYTES);
+          const int kc = kb * BK;
+          tma_load_2d_pair(st, &maps.a_hi, &full_bar[s], kc, m0);
+          tma_load_2d_pair(st + A_BYTES, &maps.a_lo, &full_bar[s], kc, m0);
+          tma_load_2d_pair(st + 2 * A_BYTES, &maps.b_hi, &full_bar[s], kc, nb);
+          tma_load_2d_pair(st + 2 * A_BYTES + HB_BYTES, &maps.b_lo, &full_bar[s], kc, nb);
+        }
+      }
+    }
+  } else if (warp == EPI_WARPS + 1) {
+    if (lane == 0 && rank == 0) {   // ===== MMA issuer (leader CTA) =====
+      constexpr uint32_t idesc = make_idesc(2 * BM, BN);
+      uint32_t it = 0, cg = 0;
+      for (int tp = cid; tp < n_pairs; tp += ncl) {
+        for (int kb = 0; kb < nkb; ++kb, ++it) {
+          const int s = it % STAGES2;
+          const int buf = cg & 1;
+          const bool chunk_start = (kb % CHUNK_KB) == 0;
+          if (chunk_start) {   // both CTAs' epilogue warps have drained this TMEM buffer (two chunks ago)
+            mbar_wait(&tmem_empty_bar[buf], ((cg >> 1) & 1) ^ 1);
+            tc_fence_after();
+          }
+          mbar_wait(&full_bar[s], (it / STAGES2) & 1);
+          tc_fence_after();
+          const uint32_t d = tmem + buf * BN;
+          const uint32_t sa = smem_u32(smem + (size_t)s * STAGE2_BYTES);
+          const uint64_t a_hi = make_desc(sa), a_lo = make_desc(sa + A_BYTES);
+          const uint64_t b_hi = make_desc(sa + 2 * A_BYTES), b_lo = make_desc(sa + 2 * A_BYTES + HB_BYTES);
+#pragma unroll
+          for (int k = 0; k < BK / UMMA_K; ++k) {
+            const uint64_t adv = (uint64_t)((k * UMMA_K * 4) >> 4);
+            umma_tf32_pair(d, a_lo + adv, b_hi + adv, idesc, (chunk_start && k == 0) ? 0u : 1u);
+            umma_tf32_pair(d, a_hi + adv, b_lo + adv, idesc, 1u);
+            umma_tf32_pair(d, a_hi + adv, b_hi + adv, idesc, 1u);
+          }
+          tc_commit_pair(&empty_bar[s]);
+          if ((kb % CHUNK_KB) == CHUNK_KB - 1 || kb == nkb - 1) { tc_commit_pair(&tmem_full_bar[buf]); ++cg; }
+        }
+      }
+    }
+  } else {             // ===== epilogue warps 0..7 of each CTA =====
+    const int q = warp & 3, half = warp >> 2;
+    uint32_t cg = 0;
+    for (int tp = cid; tp < n_pairs; tp += ncl) {
+      const int mt = (tp / n_tiles) * 2 + (int)rank, m0 = mt * BM, n0 = (tp % n_tiles) * BN;
+      float acc[COLS_PER_WARP];
+#pragma unroll
+      for (int i = 0; i < COLS_PER_WARP; ++i) acc[i] = 0.f;
+      for (int ci = 0; ci < nchunk; ++ci, ++cg) {
+        const int buf = cg & 1;
+        mbar_wait(&tmem_full_bar[buf], (cg >> 1) & 1);
+        tc_fence_after();
+        const uint32_t t0 = tmem + ((uint32_t)(q * 32) << 16) + buf * BN + half * COLS_PER_WARP;
+#pragma unroll
+        for (int cb = 0; cb < COLS_PER_WARP / 32; ++cb) {
+          float v[32];
+          tmem_ld32(t0 + cb * 32, v);
+#pragma unroll
+          for (int j = 0; j < 32; ++j) acc[cb * 32 + j] += v[j];
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_leader(&tmem_empty_bar[buf]);
+      }
+      // the tile sits in registers and both TMEM buffers are released: the next tile's MMAs run while it is written out
+      const bool valid = mt < m_tiles;
+#pragma unroll
+      for (int r = 0; r < COLS_PER_WARP / 32; ++r) {
+        asm volatile("bar.sync 1, 256;" ::: "memory");      // the previous round has left the staging area
+        if (valid) {
+#pragma unroll
+          for (int j = 0; j < 32; ++j) S[(half * 32 + j) * BM + q * 32 + lane] = acc[r * 32 + j];
+        }
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        if (valid) epi.flush_part(S, m0, n0, (int)threadIdx.x, r);
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();
   if (warp == EPI_WARPS + 1) {
     __syncwarp();
     asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"((uint32_t)TMEM_COLS) : "memory");
