@@ -21,8 +21,14 @@ Pins (tests/test_oracle_*.py, all `-m "not gpu"`):
   Cholesky <-> V         P7  pivoted Cholesky reproduces V and the energies
   multi-det mixed        P8  Fock-space brute force;  P9 FCI trial => E_L == E_FCI
   whole method           P10 long run vs FCI on cfg 1
+  o_orthonormalize       P12 Fock-space |Phi> = det(R_a) det(R_b) |Q>, Q^+Q = 1, R upper / positive diagonal,
+                             Theta / f / E_L invariance, S' == overlap recomputed from Q
+  o_comb / o_population_control  P13 brute-force tooth counting, copies in {floor, ceil}(N w_i / W),
+                             mean copies over u == N w_i / W, total weight kept
+  o_run                  P14 schedule == hand-unrolled o_step / ortho / comb sequence; mixed estimator unchanged
+                             by orthonormalisation
 No step-level worked numeric example is printed in the paper: parity is pinned only by
-P1-P11 (DESIGN.md says so too).
+P1-P14 (DESIGN.md says so too).
 """
 from __future__ import annotations
 
@@ -364,23 +370,70 @@ def o_multidet_smw(ini, trial, phi, n_alpha, want_G=False):
 
 
 # --------------------------------------------------------------------------------------
-# Long-run helpers (used only by the FCI pin P10): PAPER.md:97 (orthonormalise, comb PC)
+# NEXT-1 / NEXT-2: the two steps either side of the walker step and the paper's
+# schedule.  PAPER.md:97 ("Walker orbitals are orthonormalized after every two propagation steps",
+# local energy "measured every 0.1 Ha^-1", population control "at intervals of 0.1 Ha^-1"),
+# PAPER.md:295 ("a simple combing method").  Also used by the FCI pin P10.
 # --------------------------------------------------------------------------------------
 def o_orthonormalize(phi, S, n_alpha):
-    """QR each spin block; S <- S / (det R_a det R_b) keeps <Psi_T|phi> consistent."""
+    """Thin QR of each spin block, Phi_s = Q_s R_s; the walker becomes Q and S <- S / (det R_a det R_b),
+    because |Phi> = det(R_a) det(R_b) |Q> (a determinant is multilinear and alternating in its columns).
+
+    Reading R21: R has a real positive diagonal -- the one thin QR that is unique -- so LAPACK's
+    Householder factors are re-phased column by column: Q <- Q D, R <- D^* R, D = diag(R_jj / |R_jj|).
+    Returns (Q, S')."""
     out = []
-    S = S.copy()
+    S = np.array(S, dtype=np.complex128, copy=True)
     for ph in split_spin(phi, n_alpha):
+        if ph.shape[2] == 0:
+            out.append(ph)
+            continue
         Q, R = np.linalg.qr(ph)
-        S = S / np.prod(np.diagonal(R, axis1=1, axis2=2), axis=1)
+        d = np.diagonal(R, axis1=1, axis2=2)
+        D = d / np.abs(d)
+        Q = Q * D[:, None, :]
+        S = S / np.prod(np.abs(d), axis=1)
         out.append(Q)
     return np.concatenate(out, axis=2), S
 
 
 def o_comb(w, u):
-    """'Simple combing' population control: returns parent index per new walker.
-    u in [0,1) is the comb offset (passed in); new weights are all sum(w)/N."""
+    """'Simple combing' population control: returns the parent index of each new walker.
+
+    Reading R22: N_w teeth at t_i = (i + u) W / N_w, W = sum w, u in [0,1) drawn by the caller; tooth i
+    selects the first walker p whose running sum c_p = w_0 + ... + w_p (accumulated in index order)
+    exceeds t_i.  Every new walker then carries the weight W / N_w (the population keeps its total weight)."""
     n = w.shape[0]
     cum = np.cumsum(w)
     teeth = (np.arange(n) + u) * (cum[-1] / n)
     return np.searchsorted(cum, teeth, side="right").clip(0, n - 1)
+
+
+def o_population_control(st, u):
+    """Comb the population: every per-walker quantity of the state follows its parent; weights = W / N_w.
+    Returns (new state, parent indices)."""
+    par = o_comb(st.w, u)
+    n = st.w.shape[0]
+    w = np.full(n, np.sum(st.w) / n)
+    return OracleState(st.phi[par], w, st.S[par], st.theta[par], st.f_a[par], st.f_b[par], st.eloc[par]), par
+
+
+def o_run(ini, st, xs, n_alpha, K=6, E0=0.0, energy_every=1, ortho_every=0, pc_every=0, us=(), trial=None):
+    """The paper's schedule around o_step, hybrid weights (mode 0) only.  After step n
+    (1-based): E_L is recorded if n % energy_every == 0; then the walkers are orthonormalised if
+    n % ortho_every == 0; then combed if n % pc_every == 0 with offset us[n / pc_every - 1] (reading R23:
+    measure, orthonormalise, comb, in that order; 0 switches a part off).  Theta, f and E_L do not change
+    under orthonormalisation (Theta = Phi A^-1 is invariant under Phi -> Phi R^-1), so the order of the first
+    two is immaterial.  Returns (state, [(n, w at measurement, E_L)], [parents per comb])."""
+    meas, parents = [], []
+    for n in range(1, xs.shape[0] + 1):
+        st, _ = o_step(ini, st, xs[n - 1], n_alpha, K=K, E0=E0, mode=0, trial=trial)
+        if energy_every and n % energy_every == 0:
+            meas.append((n, st.w.copy(), st.eloc.copy()))
+        if ortho_every and n % ortho_every == 0:
+            phi, S = o_orthonormalize(st.phi, st.S, n_alpha)
+            st = OracleState(phi, st.w, S, st.theta, st.f_a, st.f_b, st.eloc)
+        if pc_every and n % pc_every == 0:
+            st, par = o_population_control(st, us[n // pc_every - 1])
+            parents.append(par)
+    return st, meas, parents
