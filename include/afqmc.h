@@ -148,6 +148,37 @@ AFQMC_API afqmc_status afqmc_step_host(afqmc_ctx* ctx, void* phi_h, double* weig
                              int32_t n_steps, void* eloc_h, int32_t* flags_h, size_t* h2d_bytes,
                              size_t* d2h_bytes);
 
+/* Walker orthonormalisation ("Walker orbitals are orthonormalized after every two
+ * propagation steps"): thin QR of each spin block, Phi_s = Q_s R_s with R_s upper triangular and a real positive
+ * diagonal (the unique thin QR, reading R21; modified Gram-Schmidt in FP64 on both precision paths).  phi (in/out)
+ * becomes Q; ovlp (in/out, complex double [N_w]) becomes S / (det R_a det R_b), since |Phi> = det R_a det R_b |Q>.
+ * Theta, the force bias and E_L are invariant (Theta = Phi A^-1), so theta / fb of the state stay valid.  A walker
+ * with a vanishing or non-finite column is left untouched and flagged (bit 0 / bit 1).  flags may be NULL.
+ * All DEVICE.  EUNSUPPORTED if N_t (M|1) 16 bytes exceed one CTA's shared memory. */
+AFQMC_API afqmc_status afqmc_orthonormalize(afqmc_ctx* ctx, void* phi, void* ovlp, int32_t* flags);
+
+/* "Simple combing" population control (NEXT-1; reading R22): W = sum_w weight, teeth
+ * t_i = (i + u) W / N_w, new walker i = copy of the first walker p whose running sum weight[0] + ... + weight[p]
+ * (accumulated in index order, FP64) exceeds t_i; every new walker gets weight W / N_w.  phi, ovlp, theta, fb follow
+ * their parent (in place; moved through scratch in work_mem).  u in [0, 1) is drawn by the caller (HOST value).
+ * parent (DEVICE int32 [N_w], may be NULL) receives the map.  W == 0 or non-finite: nothing moves, weights kept.
+ * All other pointers DEVICE.  Errors: EINVAL (null, u outside [0, 1)). */
+AFQMC_API afqmc_status afqmc_population_control(afqmc_ctx* ctx, void* phi, double* weight, void* ovlp, void* theta, void* fb,
+                                      double u, int32_t* parent);
+
+/* The paper's schedule around the walker step (NEXT-2; hybrid weights "to minimize evaluations of the
+ * local energy, which is measured every 0.1 Ha^-1", orthonormalisation every 2 steps, population control every
+ * 0.1 Ha^-1).  n_steps steps of [shift -> assemble -> Taylor -> overlap/Theta -> weight -> force bias]; after step n
+ * (1-based), in this order (reading R23): if n % energy_every == 0, E_L of the walkers goes to
+ * eloc[n / energy_every - 1][N_w] and their weights to w_meas[same][N_w] (DEVICE double, may be NULL); if
+ * n % ortho_every == 0, afqmc_orthonormalize; if n % pc_every == 0, afqmc_population_control with
+ * u[n / pc_every - 1] (HOST array, read during the call) and the map to parents[n / pc_every - 1][N_w] (DEVICE, may be
+ * NULL).  0 switches a part off; energy_every = 1, ortho_every = pc_every = 0 is afqmc_step.  Needs weight_mode 0.
+ * x [n_steps][N_w][n_chol] T DEVICE; state arguments as afqmc_step. */
+AFQMC_API afqmc_status afqmc_run(afqmc_ctx* ctx, void* phi, double* weight, void* ovlp, void* theta, void* fb, const void* x,
+                       int32_t n_steps, int32_t energy_every, int32_t ortho_every, int32_t pc_every, const double* u,
+                       void* eloc, double* w_meas, int32_t* parents, int32_t* flags);
+
 /* Number of kernels this context has launched since init (bench.py's gpu_launches). */
 AFQMC_API int64_t afqmc_launch_count(const afqmc_ctx* ctx);
 
@@ -164,7 +195,9 @@ enum {
   AFQMC_STAGE_FORCE_BIAS = 4, /* H4 GEMM + finish */
   AFQMC_STAGE_ENERGY = 5,     /* H9 GEMMs / H10 energy */
   AFQMC_STAGE_SYMMETRIZE = 6, /* H6 tail: lower triangle of A_w from the upper one (tcgen05 path) */
-  AFQMC_N_STAGES = 7
+  AFQMC_STAGE_ORTHO = 7,      /* NEXT-1: walker orthonormalisation */
+  AFQMC_STAGE_POPCTL = 8,     /* NEXT-1: comb population control (3 kernels) */
+  AFQMC_N_STAGES = 9
 };
 AFQMC_API afqmc_status afqmc_profile_enable(afqmc_ctx* ctx, int32_t enable);
 AFQMC_API afqmc_status afqmc_profile_read(afqmc_ctx* ctx, int32_t stage, double* total_ms, int32_t* launches);

@@ -414,7 +414,7 @@ def o_population_control(st, u):
     Returns (new state, parent indices)."""
     par = o_comb(st.w, u)
     n = st.w.shape[0]
-    w = np.full(n, np.sum(st.w) / n)
+    w = np.full(n, np.cumsum(st.w)[-1] / n)            # W = the running sum's last element (R22)
     return OracleState(st.phi[par], w, st.S[par], st.theta[par], st.f_a[par], st.f_b[par], st.eloc[par]), par
 
 

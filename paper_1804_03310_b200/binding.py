@@ -19,9 +19,10 @@ FLAG_SINGULAR, FLAG_NONFINITE, FLAG_KILLED = 1, 2, 4
 
 SYMBOLS = ["afqmc_query_bytes", "afqmc_init", "afqmc_destroy", "afqmc_last_error", "afqmc_overlap_green",
            "afqmc_force_bias", "afqmc_propagate", "afqmc_local_energy", "afqmc_step", "afqmc_step_host",
-           "afqmc_launch_count", "afqmc_gemm_path", "afqmc_profile_enable", "afqmc_profile_read"]
+           "afqmc_launch_count", "afqmc_gemm_path", "afqmc_profile_enable", "afqmc_profile_read",
+           "afqmc_orthonormalize", "afqmc_population_control", "afqmc_run"]
 
-STAGES = ["shift", "assemble", "taylor", "green", "force_bias", "energy", "symmetrize"]
+STAGES = ["shift", "assemble", "taylor", "green", "force_bias", "energy", "symmetrize", "ortho", "popctl"]
 
 
 class AfqmcParams(C.Structure):
@@ -63,6 +64,9 @@ def load_library():
     lib.afqmc_local_energy.argtypes = [vp, vp, vp, vp]
     lib.afqmc_step.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_int32, vp, i32p]
     lib.afqmc_step_host.argtypes = [vp, vp, vp, vp, vp, C.c_int32, vp, i32p, szp, szp]
+    lib.afqmc_orthonormalize.argtypes = [vp, vp, vp, i32p]
+    lib.afqmc_population_control.argtypes = [vp, vp, vp, vp, vp, vp, C.c_double, i32p]
+    lib.afqmc_run.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp, vp, i32p, i32p]
     lib.afqmc_launch_count.argtypes = [vp]
     lib.afqmc_launch_count.restype = C.c_int64
     lib.afqmc_gemm_path.argtypes = [vp]
@@ -72,7 +76,8 @@ def load_library():
     lib.afqmc_profile_enable.restype = C.c_int
     lib.afqmc_profile_read.restype = C.c_int
     for name in ("afqmc_query_bytes", "afqmc_init", "afqmc_overlap_green", "afqmc_force_bias", "afqmc_propagate",
-                 "afqmc_local_energy", "afqmc_step", "afqmc_step_host"):
+                 "afqmc_local_energy", "afqmc_step", "afqmc_step_host", "afqmc_orthonormalize", "afqmc_population_control",
+                 "afqmc_run"):
         getattr(lib, name).restype = C.c_int
     _lib = lib
     return lib
@@ -191,6 +196,21 @@ class AfqmcContext:
     def afqmc_step(self, phi, weight, ovlp, theta, fb, x, n_steps, eloc, flags=None):
         self._chk(self._lib.afqmc_step(self._ctx, _dp(phi), _dp(weight), _dp(ovlp), _dp(theta), _dp(fb), _dp(x),
                                        int(n_steps), _dp(eloc), _dp(flags)))
+
+    def afqmc_orthonormalize(self, phi, ovlp, flags=None):
+        self._chk(self._lib.afqmc_orthonormalize(self._ctx, _dp(phi), _dp(ovlp), _dp(flags)))
+
+    def afqmc_population_control(self, phi, weight, ovlp, theta, fb, u, parent=None):
+        self._chk(self._lib.afqmc_population_control(self._ctx, _dp(phi), _dp(weight), _dp(ovlp), _dp(theta), _dp(fb),
+                                                     float(u), _dp(parent)))
+
+    def afqmc_run(self, phi, weight, ovlp, theta, fb, x, n_steps, energy_every=1, ortho_every=0, pc_every=0, u=None,
+                  eloc=None, w_meas=None, parents=None, flags=None):
+        """u: host sequence of comb offsets in [0, 1), one per population-control event."""
+        ua = None if u is None else np.ascontiguousarray(u, dtype=np.float64)
+        self._chk(self._lib.afqmc_run(self._ctx, _dp(phi), _dp(weight), _dp(ovlp), _dp(theta), _dp(fb), _dp(x),
+                                      int(n_steps), int(energy_every), int(ortho_every), int(pc_every), _hp(ua),
+                                      _dp(eloc), _dp(w_meas), _dp(parents), _dp(flags)))
 
     def afqmc_step_host(self, phi_h, weight_h, ovlp_h, x_h, n_steps, eloc_h, flags_h=None):
         """HOST buffers: numpy arrays or CPU (pinned) torch tensors, updated in place. Returns (h2d, d2h) bytes."""

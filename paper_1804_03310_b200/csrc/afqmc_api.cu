@@ -18,6 +18,7 @@
 #include "multidet.cuh"
 #include "taylor.cuh"
 #include "taylor_tc.cuh"
+#include "popctl.cuh"
 
 using namespace afq;
 
@@ -63,6 +64,9 @@ struct afqmc_ctx {
   zcplx *h_ovlp, *h_eloc;
   double* h_weight;
   int32_t* h_flags;
+  // orthonormalisation / comb population control (popctl.cuh)
+  size_t ortho_smem;
+  void *pc_phi, *pc_theta, *pc_fb; zcplx* pc_ovlp; double *pc_cum, *pc_wnew; int32_t* pc_parent;
   // init staging (FP64)
   double *Ld, *hd, *hpd, *Rd, *hrotd, *ex[4], *psid;
   tc::Maps map_asm, map_fb[2], map_en[2];
@@ -252,6 +256,13 @@ void carve(const afqmc_params* p, afqmc_ctx* c, char* cbase, char* wbase, size_t
   c->h_eloc = (zcplx*)w.take(nw1 * sizeof(zcplx));
   c->h_weight = (double*)w.take(nw1 * sizeof(double));
   c->h_flags = (int32_t*)w.take(nw1 * sizeof(int32_t));
+  c->pc_phi = w.take(nw1 * M * nt * 2 * ts);
+  c->pc_theta = w.take(nw1 * M * nt * 2 * ts);
+  c->pc_fb = w.take(nw1 * ng * 2 * ts);
+  c->pc_ovlp = (zcplx*)w.take(nw1 * sizeof(zcplx));
+  c->pc_cum = (double*)w.take(nw1 * sizeof(double));
+  c->pc_wnew = (double*)w.take(256);
+  c->pc_parent = (int32_t*)w.take(nw1 * sizeof(int32_t));
   // FP64 init staging
   c->Ld = (double*)w.take((size_t)ng * M * M * 8);
   c->hd = (double*)w.take((size_t)M * M * 8);
@@ -700,6 +711,61 @@ afqmc_status do_step(afqmc_ctx* c, void* phi, double* weight, void* ovlp, void* 
   return AFQMC_OK;
 }
 
+template <typename T> afqmc_status do_ortho(afqmc_ctx* c, void* phi, void* ovlp, int32_t* flags) {
+  if (c->ortho_smem > 227 * 1024) return fail(c, AFQMC_EUNSUPPORTED, "%s", "afqmc_orthonormalize: walker exceeds one CTA's shared memory in FP64");
+  StageScope sc(c, AFQMC_STAGE_ORTHO);
+  LAUNCH(c, k_ortho<T>, c->nw, 256, c->ortho_smem, c->M, c->na, c->nb, (cplx<T>*)phi, (zcplx*)ovlp, flags);
+  return AFQMC_OK;
+}
+
+template <typename T>
+afqmc_status do_popctl(afqmc_ctx* c, void* phi, double* weight, void* ovlp, void* theta, void* fb, double u, int32_t* parent) {
+  StageScope sc(c, AFQMC_STAGE_POPCTL);
+  LAUNCH(c, k_comb_parents, 1, 1024, 0, c->nw, (const double*)weight, u, c->pc_cum, c->pc_parent, c->pc_wnew);
+  CombMove m;
+  m.phi = (uint2*)phi; m.theta = (uint2*)theta; m.fb = (uint2*)fb; m.ovlp = (zcplx*)ovlp;
+  m.s_phi = (uint2*)c->pc_phi; m.s_theta = (uint2*)c->pc_theta; m.s_fb = (uint2*)c->pc_fb; m.s_ovlp = c->pc_ovlp;
+  m.words_phi = c->M * c->nt * 2 * c->ts / 8; m.words_fb = c->ng * 2 * c->ts / 8;
+  LAUNCH(c, k_comb_pack, c->nw, 256, 0, m, (const int32_t*)c->pc_parent);
+  LAUNCH(c, k_comb_unpack, c->nw, 256, 0, m, (const int32_t*)c->pc_parent, weight, (const double*)c->pc_wnew);
+  if (parent) CUDA_OK(c, cudaMemcpyAsync(parent, c->pc_parent, (size_t)c->nw * 4, cudaMemcpyDeviceToDevice, c->stream));
+  return AFQMC_OK;
+}
+
+// The paper's schedule around the walker step; hybrid weights only.
+template <typename T>
+afqmc_status do_run(afqmc_ctx* c, void* phi, double* weight, void* ovlp, void* theta, void* fb, const void* x, int n_steps,
+                    int energy_every, int ortho_every, int pc_every, const double* u, void* eloc, double* w_meas,
+                    int32_t* parents, int32_t* flags) {
+  zcplx* el = (zcplx*)eloc;
+  int n_meas = 0, n_pc = 0;
+  for (int s = 1; s <= n_steps; ++s) {
+    const T* xs = (const T*)x + (size_t)(s - 1) * c->nw * c->ng;
+    afqmc_status st = do_propagate<T>(c, phi, xs, fb, ovlp, weight, theta, nullptr, flags);
+    if (st) return st;
+    if (energy_every && s % energy_every == 0) {
+      st = do_fb_energy_planar<T>(c, theta, fb, el + (size_t)n_meas * c->nw);
+      if (st) return st;
+      if (w_meas) CUDA_OK(c, cudaMemcpyAsync(w_meas + (size_t)n_meas * c->nw, weight, (size_t)c->nw * 8, cudaMemcpyDeviceToDevice, c->stream));
+      ++n_meas;
+    } else {   // propagate-only step: the force bias of the new walker, no energy contraction
+      st = run_fb_gemm<T>(c);
+      if (st) return st;
+      LAUNCH(c, k_fb_finish<T>, c->nw, 128, 0, c->ng, c->NGP, c->nw, (const T*)c->fs, (cplx<T>*)fb, (zcplx*)nullptr);
+    }
+    if (ortho_every && s % ortho_every == 0) {
+      st = do_ortho<T>(c, phi, ovlp, flags);
+      if (st) return st;
+    }
+    if (pc_every && s % pc_every == 0) {
+      st = do_popctl<T>(c, phi, weight, ovlp, theta, fb, u[n_pc], parents ? parents + (size_t)n_pc * c->nw : nullptr);
+      if (st) return st;
+      ++n_pc;
+    }
+  }
+  return AFQMC_OK;
+}
+
 }  // namespace
 
 // ================================================================================================
@@ -832,6 +898,12 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
   if (c->green_smem > 48 * 1024) {
     cudaError_t e = p->precision ? cudaFuncSetAttribute(k_green<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->green_smem)
                                  : cudaFuncSetAttribute(k_green<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->green_smem);
+    if (e != cudaSuccess) { snprintf(g_init_err, 256, "CUDA: %s", cudaGetErrorString(e)); delete c; return AFQMC_ECUDA; }
+  }
+  c->ortho_smem = ortho_smem_bytes(c->M, c->nt);
+  if (c->ortho_smem > 48 * 1024 && c->ortho_smem <= 227 * 1024) {
+    cudaError_t e = p->precision ? cudaFuncSetAttribute(k_ortho<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ortho_smem)
+                                 : cudaFuncSetAttribute(k_ortho<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ortho_smem);
     if (e != cudaSuccess) { snprintf(g_init_err, 256, "CUDA: %s", cudaGetErrorString(e)); delete c; return AFQMC_ECUDA; }
   }
   // tensor-pipe Taylor kernel for 96 <= M <= 256: below that a 128-row tile is mostly padding and the FP32 SIMT
@@ -1036,6 +1108,42 @@ afqmc_status afqmc_step(afqmc_ctx* c, void* phi, double* weight, void* ovlp, voi
   if (c->nw == 0 || n_steps == 0) return AFQMC_OK;
   NEED(c, phi && weight && ovlp && theta && fb && x && eloc, "afqmc_step: null pointer");
   return DISPATCH(c, do_step, c, phi, weight, ovlp, theta, fb, x, n_steps, eloc, flags);
+}
+
+afqmc_status afqmc_orthonormalize(afqmc_ctx* c, void* phi, void* ovlp, int32_t* flags) {
+  if (!c) return AFQMC_EINVAL;
+  c->err[0] = 0;
+  NEED(c, phi && ovlp, "afqmc_orthonormalize: null pointer");
+  if (c->nw == 0) return AFQMC_OK;
+  return DISPATCH(c, do_ortho, c, phi, ovlp, flags);
+}
+
+afqmc_status afqmc_population_control(afqmc_ctx* c, void* phi, double* weight, void* ovlp, void* theta, void* fb, double u,
+                                      int32_t* parent) {
+  if (!c) return AFQMC_EINVAL;
+  c->err[0] = 0;
+  NEED(c, u >= 0.0 && u < 1.0, "afqmc_population_control: u must be in [0, 1)");
+  if (c->nw == 0) return AFQMC_OK;
+  NEED(c, phi && weight && ovlp && theta && fb, "afqmc_population_control: null pointer");
+  return DISPATCH(c, do_popctl, c, phi, weight, ovlp, theta, fb, u, parent);
+}
+
+afqmc_status afqmc_run(afqmc_ctx* c, void* phi, double* weight, void* ovlp, void* theta, void* fb, const void* x,
+                       int32_t n_steps, int32_t energy_every, int32_t ortho_every, int32_t pc_every, const double* u,
+                       void* eloc, double* w_meas, int32_t* parents, int32_t* flags) {
+  if (!c) return AFQMC_EINVAL;
+  c->err[0] = 0;
+  NEED(c, n_steps >= 0 && energy_every >= 0 && ortho_every >= 0 && pc_every >= 0, "afqmc_run: negative count");
+  NEED(c, c->p.weight_mode == 0, "afqmc_run: the schedule needs hybrid weights (weight_mode 0, PAPER.md:97)");
+  if (c->nw == 0 || n_steps == 0) return AFQMC_OK;
+  NEED(c, phi && weight && ovlp && theta && fb && x, "afqmc_run: null pointer");
+  NEED(c, eloc || !energy_every || n_steps < energy_every, "afqmc_run: eloc is NULL");
+  if (pc_every && n_steps >= pc_every) {
+    NEED(c, u, "afqmc_run: u is NULL");
+    for (int i = 0; i < n_steps / pc_every; ++i) NEED(c, u[i] >= 0.0 && u[i] < 1.0, "afqmc_run: u must be in [0, 1)");
+  }
+  return DISPATCH(c, do_run, c, phi, weight, ovlp, theta, fb, x, n_steps, energy_every, ortho_every, pc_every, u, eloc,
+                  w_meas, parents, flags);
 }
 
 afqmc_status afqmc_step_host(afqmc_ctx* c, void* phi_h, double* weight_h, void* ovlp_h, const void* x_h, int32_t n_steps,

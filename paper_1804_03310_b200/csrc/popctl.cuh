@@ -1,0 +1,193 @@
+// popctl.cuh -- the two steps either side of the walker step:
+//   k_ortho        walker orthonormalisation, PAPER.md:97 ("orthonormalized after every two propagation steps")
+//   k_comb_parents / k_comb_pack / k_comb_unpack   "simple combing" population control
+// Both are HBM-bound by design (read + write the walker once); the arithmetic is FP64 on both precision paths.
+#pragma once
+#include "common.cuh"
+
+namespace afq {
+
+// ------------------------------------------------------------------------------------------------
+// Thin QR of each spin block by modified Gram-Schmidt, R with a real positive diagonal (reading R21):
+// Phi_s = Q_s R_s, walker <- Q, S <- S / (det R_a det R_b) because |Phi> = det R_a det R_b |Q>.
+// One CTA (256 threads) per walker.  The walker is held in shared memory in FP64, one column after the
+// other with an odd leading dimension (conflict-free both for the transposing load/store and for the column
+// sweeps).  Right-looking elimination without an intermediate scaling: at step j every warp that owns a
+// trailing column k computes d = <v_j, v_k> and n = <v_j, v_j> in one sweep and applies v_k -= (d/n) v_j in a
+// second one; v_j itself is only read, so one CTA barrier per step is enough.  Columns are scaled by 1/|v_j|
+// when the walker is written back.  Theta = Phi A^-1 is invariant, so nothing else of the state changes.
+// ------------------------------------------------------------------------------------------------
+__host__ __device__ inline int ortho_ld(int M) { return M | 1; }
+inline size_t ortho_smem_bytes(int M, int nt) { return (size_t)nt * ortho_ld(M) * sizeof(zcplx) + 72 * sizeof(double); }
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_ortho(int M, int na, int nb, cplx<T>* __restrict__ phi, zcplx* __restrict__ ovlp,
+                                               int32_t* __restrict__ flags) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  zcplx* V = (zcplx*)smem_raw;
+  const int nt = na + nb, ld = ortho_ld(M);
+  double* nrm = (double*)(V + (size_t)nt * ld);   // [nt] squared norms of the orthogonalised columns
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  cplx<T>* g = phi + (size_t)blockIdx.x * M * nt;
+  for (int e = tid; e < M * nt; e += 256) {
+    const int i = e / nt, k = e - i * nt;
+    V[k * ld + i] = to_z(g[e]);
+  }
+  __syncthreads();
+  const int nmax = na > nb ? na : nb;
+  for (int j = 0; j + 1 < nmax; ++j) {
+    // trailing columns of both spins at this step, dealt round-robin to the 8 warps
+    const int ta = na - 1 - j > 0 ? na - 1 - j : 0, tb = nb - 1 - j > 0 ? nb - 1 - j : 0;
+    for (int t = warp; t < ta + tb; t += 8) {
+      const int s_off = t < ta ? 0 : na;
+      const int k = t < ta ? j + 1 + t : j + 1 + (t - ta);
+      const zcplx* vj = V + (size_t)(s_off + j) * ld;
+      zcplx* vk = V + (size_t)(s_off + k) * ld;
+      double dr = 0.0, di = 0.0, nn = 0.0;
+      for (int i = lane; i < M; i += 32) {
+        const zcplx a = vj[i], b = vk[i];
+        dr = fma(a.x, b.x, dr); dr = fma(a.y, b.y, dr);      // conj(a) * b
+        di = fma(a.x, b.y, di); di = fma(-a.y, b.x, di);
+        nn = fma(a.x, a.x, nn); nn = fma(a.y, a.y, nn);
+      }
+      dr = warp_sum(dr); di = warp_sum(di); nn = warp_sum(nn);
+      if (nn > 0.0) {
+        const double cr = dr / nn, ci = di / nn;
+        for (int i = lane; i < M; i += 32) {
+          const zcplx a = vj[i];
+          zcplx b = vk[i];
+          b.x = fma(-cr, a.x, b.x); b.x = fma(ci, a.y, b.x);
+          b.y = fma(-cr, a.y, b.y); b.y = fma(-ci, a.x, b.y);
+          vk[i] = b;
+        }
+      }
+    }
+    __syncthreads();
+  }
+  for (int k = warp; k < nt; k += 8) {
+    const zcplx* vk = V + (size_t)k * ld;
+    double nn = 0.0;
+    for (int i = lane; i < M; i += 32) { const zcplx a = vk[i]; nn = fma(a.x, a.x, nn); nn = fma(a.y, a.y, nn); }
+    nn = warp_sum(nn);
+    if (lane == 0) nrm[k] = nn;
+  }
+  __syncthreads();
+  if (tid < 32) {
+    // det R_a det R_b = prod |v_k| (real, positive); a vanishing or non-finite column flags the walker
+    double r = (tid < nt) ? sqrt(nrm[tid]) : 1.0;
+    int bad = (tid < nt) && !(r > 0.0 && isfinite(r));
+    bad = __any_sync(0xffffffffu, bad);
+    double prod = r;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) prod *= __shfl_xor_sync(0xffffffffu, prod, o);
+    if (nt > 32) {   // n_alpha, n_beta <= 32 each: a second round covers columns 32..63
+      double r2 = (tid + 32 < nt) ? sqrt(nrm[tid + 32]) : 1.0;
+      int bad2 = (tid + 32 < nt) && !(r2 > 0.0 && isfinite(r2));
+      bad |= __any_sync(0xffffffffu, bad2);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) r2 *= __shfl_xor_sync(0xffffffffu, r2, o);
+      prod *= r2;
+    }
+    if (tid == 0) {
+      if (!bad) {
+        zcplx s = ovlp[blockIdx.x];
+        ovlp[blockIdx.x] = mk<double>(s.x / prod, s.y / prod);
+      } else if (flags) {
+        flags[blockIdx.x] |= isfinite(prod) ? FLAG_SINGULAR : FLAG_NONFINITE;
+      }
+      nrm[64] = bad ? 1.0 : 0.0;
+    }
+  }
+  __syncthreads();
+  if (nrm[64] != 0.0) return;   // degenerate walker: left as it was (flagged)
+  for (int e = tid; e < M * nt; e += 256) {
+    const int i = e / nt, k = e - i * nt;
+    const double inv = 1.0 / sqrt(nrm[k]);
+    const zcplx v = V[k * ld + i];
+    g[e] = mk<T>((T)(v.x * inv), (T)(v.y * inv));
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Comb (reading R22): teeth t_i = (i + u) W / N_w; parent(i) = first p with c_p > t_i, c = running sum of w in
+// index order.  The running sum decides integers, so it is accumulated SEQUENTIALLY in FP64 in the same order as
+// the definition (one thread, chunks staged through shared memory by the whole CTA): bit-identical parents.
+// One CTA.  cum [N_w] scratch; wnew[0] = W / N_w, wnew[1] = W.  W == 0 or non-finite: identity map, wnew[0] = -1
+// (the unpack kernel then keeps the weights).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(1024) k_comb_parents(int nw, const double* __restrict__ w, double u, double* __restrict__ cum,
+                                                        int32_t* __restrict__ parent, double* __restrict__ wnew) {
+  __shared__ double buf[1024];
+  __shared__ double carry;
+  const int tid = threadIdx.x;
+  if (tid == 0) carry = 0.0;
+  for (int base = 0; base < nw; base += 1024) {
+    const int n = min(1024, nw - base);
+    if (tid < n) buf[tid] = w[base + tid];
+    __syncthreads();
+    if (tid == 0) {
+      double c = carry;
+      for (int i = 0; i < n; ++i) { c = __dadd_rn(c, buf[i]); buf[i] = c; }
+      carry = c;
+    }
+    __syncthreads();
+    if (tid < n) cum[base + tid] = buf[tid];
+    __syncthreads();
+  }
+  const double W = carry;
+  const bool ok = W > 0.0 && isfinite(W);
+  if (tid == 0) { wnew[0] = ok ? __ddiv_rn(W, (double)nw) : -1.0; wnew[1] = W; }
+  const double step = __ddiv_rn(W, (double)nw);
+  for (int i = tid; i < nw; i += 1024) {
+    int p = i;
+    if (ok) {
+      const double t = __dmul_rn(__dadd_rn((double)i, u), step);
+      int lo = 0, hi = nw;                 // first index with cum > t
+      while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (cum[mid] > t) hi = mid; else lo = mid + 1;
+      }
+      p = lo < nw - 1 ? lo : nw - 1;
+    }
+    parent[i] = p;
+  }
+}
+
+// Walkers whose parent is another slot are first copied (phi, theta, fb, S of the PARENT) into a scratch slot of
+// their own, then (second kernel) from there into place: out of place, so any map is allowed; slots that keep their
+// walker move no bytes.  Sizes in 8-byte words (a complex64 or one double).
+struct CombMove {
+  uint2 *phi, *theta, *fb, *s_phi, *s_theta, *s_fb;
+  zcplx *ovlp, *s_ovlp;
+  int words_phi, words_fb;   // per walker
+};
+
+__global__ void __launch_bounds__(256) k_comb_pack(CombMove m, const int32_t* __restrict__ parent) {
+  const int i = blockIdx.x, p = parent[i];
+  if (p == i) return;
+  const size_t op = (size_t)p * m.words_phi, oi = (size_t)i * m.words_phi;
+  for (int e = threadIdx.x; e < m.words_phi; e += 256) {
+    m.s_phi[oi + e] = m.phi[op + e];
+    m.s_theta[oi + e] = m.theta[op + e];
+  }
+  const size_t fp = (size_t)p * m.words_fb, fi = (size_t)i * m.words_fb;
+  for (int e = threadIdx.x; e < m.words_fb; e += 256) m.s_fb[fi + e] = m.fb[fp + e];
+  if (threadIdx.x == 0) m.s_ovlp[i] = m.ovlp[p];
+}
+
+__global__ void __launch_bounds__(256) k_comb_unpack(CombMove m, const int32_t* __restrict__ parent, double* __restrict__ weight,
+                                                      const double* __restrict__ wnew) {
+  const int i = blockIdx.x;
+  if (threadIdx.x == 0 && wnew[0] >= 0.0) weight[i] = wnew[0];
+  if (parent[i] == i) return;
+  const size_t oi = (size_t)i * m.words_phi;
+  for (int e = threadIdx.x; e < m.words_phi; e += 256) {
+    m.phi[oi + e] = m.s_phi[oi + e];
+    m.theta[oi + e] = m.s_theta[oi + e];
+  }
+  const size_t fi = (size_t)i * m.words_fb;
+  for (int e = threadIdx.x; e < m.words_fb; e += 256) m.fb[fi + e] = m.s_fb[fi + e];
+  if (threadIdx.x == 0) m.ovlp[i] = m.s_ovlp[i];
+}
+
+}  // namespace afq

@@ -163,7 +163,7 @@ def test_P14_schedule_matches_unrolled_sequence():
         if k in (3, 7):
             par = O.o_comb(s2.w, us[k // 4])
             assert np.array_equal(par, parents[k // 4])
-            s2 = O.OracleState(s2.phi[par], np.full(nw, s2.w.sum() / nw), s2.S[par], s2.theta[par], s2.f_a[par],
+            s2 = O.OracleState(s2.phi[par], np.full(nw, np.cumsum(s2.w)[-1] / nw), s2.S[par], s2.theta[par], s2.f_a[par],
                                s2.f_b[par], s2.eloc[par])
     assert np.array_equal(st.phi, s2.phi) and np.array_equal(st.w, s2.w) and np.array_equal(st.S, s2.S)
     # no population control: orthonormalisation every step vs never -> same weights and energies
