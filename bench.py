@@ -236,7 +236,7 @@ def run_ours(args):
     ms_max = D.max_over_ranks(ms, dev)
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----
-    Ke = min(K, 4)
+    Ke = K          # every step uploads its fields and downloads its energies; the walkers go in and out once per call
     phi_h = torch.tensor(wl.walkers(nw), dtype=ctx.cdtype).pin_memory()
     w_h = torch.ones(nw, dtype=torch.float64).pin_memory()
     S_h = torch.zeros(nw, dtype=torch.complex128).pin_memory()
@@ -276,18 +276,28 @@ def run_ours(args):
         ms20 = e0.elapsed_time(e1)
         prof20 = ctx.afqmc_profile_read()
         ctx.afqmc_profile_enable(False)
+        # the literal configs kill the whole population within ~8 steps, so the comb inside the run moves
+        # nothing; its cost is measured on the same state with seeded log-normal weights (sigma 0.5) instead
+        wr = torch.tensor(np.exp(0.5 * np.random.default_rng(7).standard_normal(nw)), dtype=torch.float64, device=dev)
+        st.weight.copy_(wr)
+        ctx.afqmc_profile_enable(True)
+        ctx.afqmc_population_control(st.phi, st.weight, st.ovlp, st.theta, st.fb, 0.5, par20[0])
+        torch.cuda.synchronize()
+        prof_pc = ctx.afqmc_profile_read()
+        ctx.afqmc_profile_enable(False)
         moved = int((par20[0] != torch.arange(nw, device=dev, dtype=torch.int32)).sum().item())
         cb_ = 8 if wl.precision == "c64" else 16
         ob = nw * (2 * wl.M * wl.n_t * cb_ + 32)                       # read + write the walker, read + write S
         o_ms = prof20["ortho"][0] / max(prof20["ortho"][1], 1)
-        p_ms = prof20["popctl"][0] / max(prof20["popctl"][1], 1)
+        p_ms = prof_pc["popctl"][0] / max(prof_pc["popctl"][1], 1)
         pb = moved * 4 * ((2 * wl.M * wl.n_t + wl.n_chol) * cb_ + 16) + nw * 28
         hbm = peaks()["hbm"]
         sched = dict(value=world * nw * ns / (ms20 * 1e-3), unit=UNIT, ms_per_step=ms20 / ns, steps=ns, energy_every=ee,
                      ortho_every=oe, pc_every=pe, gpu_launches=ctx.launch_count - l1,
                      ortho=dict(ms_per_launch=o_ms, bytes=ob, achieved_gbs=ob / (o_ms * 1e-3) / 1e9 if o_ms else None,
                                 frac_hbm=ob / (o_ms * 1e-3) / 1e9 / hbm if o_ms else None),
-                     popctl=dict(ms_per_launch=p_ms, walkers_moved=moved, bytes=pb,
+                     popctl=dict(ms_per_launch=p_ms, ms_inside_run=prof20["popctl"][0], walkers_moved=moved, bytes=pb,
+                                 weights="seeded log-normal, sigma 0.5",
                                  achieved_gbs=pb / (p_ms * 1e-3) / 1e9 if p_ms else None),
                      note="one afqmc_run call: propagate-only steps (no energy contraction) except the measured one")
 

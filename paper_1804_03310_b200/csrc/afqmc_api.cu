@@ -714,7 +714,7 @@ afqmc_status do_step(afqmc_ctx* c, void* phi, double* weight, void* ovlp, void* 
 template <typename T> afqmc_status do_ortho(afqmc_ctx* c, void* phi, void* ovlp, int32_t* flags) {
   if (c->ortho_smem > 227 * 1024) return fail(c, AFQMC_EUNSUPPORTED, "%s", "afqmc_orthonormalize: walker exceeds one CTA's shared memory in FP64");
   StageScope sc(c, AFQMC_STAGE_ORTHO);
-  LAUNCH(c, k_ortho<T>, c->nw, 256, c->ortho_smem, c->M, c->na, c->nb, (cplx<T>*)phi, (zcplx*)ovlp, flags);
+  LAUNCH(c, k_ortho<T>, c->nw, ortho_threads(c->na, c->nb), c->ortho_smem, c->M, c->na, c->nb, (cplx<T>*)phi, (zcplx*)ovlp, flags);
   return AFQMC_OK;
 }
 
@@ -904,6 +904,10 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
   if (c->ortho_smem > 48 * 1024 && c->ortho_smem <= 227 * 1024) {
     cudaError_t e = p->precision ? cudaFuncSetAttribute(k_ortho<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ortho_smem)
                                  : cudaFuncSetAttribute(k_ortho<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ortho_smem);
+    // ask for the full shared-memory carve-out: with the default split only one 80 KB CTA fits an SM (ncu, round 1)
+    if (e == cudaSuccess)
+      e = p->precision ? cudaFuncSetAttribute(k_ortho<double>, cudaFuncAttributePreferredSharedMemoryCarveout, 100)
+                       : cudaFuncSetAttribute(k_ortho<float>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     if (e != cudaSuccess) { snprintf(g_init_err, 256, "CUDA: %s", cudaGetErrorString(e)); delete c; return AFQMC_ECUDA; }
   }
   // tensor-pipe Taylor kernel for 96 <= M <= 256: below that a 128-row tile is mostly padding and the FP32 SIMT

@@ -216,34 +216,68 @@ __global__ void __launch_bounds__(256) k_green(GreenArgs<T> g) {
     }
     __syncthreads();
   }
-  for (int s = 0; s < 2; ++s) {
-    int n = s ? nb : na, off = s ? na : 0, soff = s ? g.KA : 0;
-    const zcplx* inv = aug + s * ns * ld + n;
-    for (int e = tid; e < M * n; e += nthr) {
-      int k = e / n, b = e % n;
-      zcplx accd = mk<double>(0.0, 0.0);
-      if constexpr (sizeof(T) == 4) {
-        cplx<float> ah = mk<float>(0.f, 0.f), al = mk<float>(0.f, 0.f);
-        for (int a = 0; a < n; ++a) {
-          const cplx<float> ph = mk<float>((float)phi_s[k * nt + off + a].x, (float)phi_s[k * nt + off + a].y);
-          cfma(ah, ph, invf[(s * ns * ns + a * n + b) * 2 + 0]);
-          cfma(al, ph, invf[(s * ns * ns + a * n + b) * 2 + 1]);
+  if constexpr (sizeof(T) == 4) {
+    // register tile: one thread = column b of four rows k, k + Mq, k + 2 Mq, k + 3 Mq (Mq = ceil(M/4)); the hi/lo pair of
+    // inv[a][b] is one 16-byte shared load reused by the four rows, and for a fixed row slot consecutive threads
+    // write consecutive elements of Theta and of the planar operand
+    const int Mq = (M + 3) >> 2;
+    for (int s = 0; s < 2; ++s) {
+      const int n = s ? nb : na, off = s ? na : 0, soff = s ? g.KA : 0;
+      const float4* iv = reinterpret_cast<const float4*>(invf) + s * ns * ns;
+      for (int e = tid; e < Mq * n; e += nthr) {
+        const int kg = e / n, b = e - kg * n;
+        cplx<float> ah[4], al[4];
+        int kk[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          ah[u] = mk<float>(0.f, 0.f); al[u] = mk<float>(0.f, 0.f);
+          const int k = kg + u * Mq;
+          kk[u] = k < M ? k : M - 1;
         }
-        accd = mk<double>((double)(ah.x + al.x), (double)(ah.y + al.y));
-      } else {
-        for (int a = 0; a < n; ++a) cfma(accd, to_z(phi_s[k * nt + off + a]), inv[a * ld + b]);
+        for (int a = 0; a < n; ++a) {
+          const float4 v = iv[a * n + b];
+          const cplx<float> vh = mk<float>(v.x, v.y), vl = mk<float>(v.z, v.w);
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const cplx<T> p = phi_s[kk[u] * nt + off + a];
+            const cplx<float> ph = mk<float>((float)p.x, (float)p.y);
+            cfma(ah[u], ph, vh);
+            cfma(al[u], ph, vl);
+          }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int k = kg + u * Mq;
+          if (k >= M) continue;
+          const cplx<T> acc = mk<T>((T)(ah[u].x + al[u].x), (T)(ah[u].y + al[u].y));
+          if (g.theta) g.theta[(size_t)w * M * nt + k * nt + off + b] = acc;
+          if (g.thp) {
+            const size_t o = (size_t)(2 * w) * g.KT + soff + k * n + b;
+            if (g.split) {
+              float h0, l0, h1, l1;
+              tf32_split((float)acc.x, h0, l0);
+              tf32_split((float)acc.y, h1, l1);
+              g.thp[o] = (T)h0; g.thp[o + g.KT] = (T)h1;
+              g.thp_lo[o] = (T)l0; g.thp_lo[o + g.KT] = (T)l1;
+            } else {
+              g.thp[o] = acc.x; g.thp[o + g.KT] = acc.y;
+            }
+          }
+        }
       }
-      cplx<T> acc = mk<T>((T)accd.x, (T)accd.y);
-      if (g.theta) g.theta[(size_t)w * M * nt + k * nt + off + b] = acc;
-      if (g.thp) {
-        size_t o = (size_t)(2 * w) * g.KT + soff + e;
-        if (g.split) {
-          float h0, l0, h1, l1;
-          tf32_split((float)acc.x, h0, l0);
-          tf32_split((float)acc.y, h1, l1);
-          g.thp[o] = (T)h0; g.thp[o + g.KT] = (T)h1;
-          g.thp_lo[o] = (T)l0; g.thp_lo[o + g.KT] = (T)l1;
-        } else {
+    }
+  } else {
+    for (int s = 0; s < 2; ++s) {
+      int n = s ? nb : na, off = s ? na : 0, soff = s ? g.KA : 0;
+      const zcplx* inv = aug + s * ns * ld + n;
+      for (int e = tid; e < M * n; e += nthr) {
+        int k = e / n, b = e % n;
+        zcplx accd = mk<double>(0.0, 0.0);
+        for (int a = 0; a < n; ++a) cfma(accd, to_z(phi_s[k * nt + off + a]), inv[a * ld + b]);
+        cplx<T> acc = mk<T>((T)accd.x, (T)accd.y);
+        if (g.theta) g.theta[(size_t)w * M * nt + k * nt + off + b] = acc;
+        if (g.thp) {
+          size_t o = (size_t)(2 * w) * g.KT + soff + e;
           g.thp[o] = acc.x; g.thp[o + g.KT] = acc.y;
         }
       }

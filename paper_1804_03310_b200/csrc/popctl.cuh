@@ -10,7 +10,7 @@ namespace afq {
 // ------------------------------------------------------------------------------------------------
 // Thin QR of each spin block by modified Gram-Schmidt, R with a real positive diagonal (reading R21):
 // Phi_s = Q_s R_s, walker <- Q, S <- S / (det R_a det R_b) because |Phi> = det R_a det R_b |Q>.
-// One CTA (256 threads) per walker.  The walker is held in shared memory in FP64, one column after the
+// One CTA per walker, one warp per trailing column (ortho_threads).  The walker is held in shared memory in FP64, one column after the
 // other with an odd leading dimension (conflict-free both for the transposing load/store and for the column
 // sweeps).  Right-looking elimination without an intermediate scaling: at step j every warp that owns a
 // trailing column k computes d = <v_j, v_k> and n = <v_j, v_j> in one sweep and applies v_k -= (d/n) v_j in a
@@ -18,58 +18,74 @@ namespace afq {
 // when the walker is written back.  Theta = Phi A^-1 is invariant, so nothing else of the state changes.
 // ------------------------------------------------------------------------------------------------
 __host__ __device__ inline int ortho_ld(int M) { return M | 1; }
-inline size_t ortho_smem_bytes(int M, int nt) { return (size_t)nt * ortho_ld(M) * sizeof(zcplx) + 72 * sizeof(double); }
+inline int ortho_threads(int na, int nb) {
+  int w = na + nb - 2;   // trailing columns of both spins at the first elimination step
+  w = w < 8 ? 8 : (w > 16 ? 16 : w);     // <= 512 threads: two CTAs per SM by registers and (cfg 5) shared memory
+  return 32 * w;
+}
+inline size_t ortho_smem_bytes(int M, int nt) { return (size_t)nt * ortho_ld(M) * sizeof(zcplx) + 136 * sizeof(double); }
 
 template <typename T>
-__global__ void __launch_bounds__(256) k_ortho(int M, int na, int nb, cplx<T>* __restrict__ phi, zcplx* __restrict__ ovlp,
+__global__ void __launch_bounds__(512, 2) k_ortho(int M, int na, int nb, cplx<T>* __restrict__ phi, zcplx* __restrict__ ovlp,
                                                int32_t* __restrict__ flags) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   zcplx* V = (zcplx*)smem_raw;
   const int nt = na + nb, ld = ortho_ld(M);
   double* nrm = (double*)(V + (size_t)nt * ld);   // [nt] squared norms of the orthogonalised columns
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nth = blockDim.x, nwp = nth >> 5;
   cplx<T>* g = phi + (size_t)blockIdx.x * M * nt;
-  for (int e = tid; e < M * nt; e += 256) {
+  for (int e = tid; e < M * nt; e += nth) {
     const int i = e / nt, k = e - i * nt;
     V[k * ld + i] = to_z(g[e]);
   }
   __syncthreads();
   const int nmax = na > nb ? na : nb;
   for (int j = 0; j + 1 < nmax; ++j) {
-    // trailing columns of both spins at this step, dealt round-robin to the 8 warps
+    // trailing columns of both spins at this step, dealt round-robin to the warps (up to 16 per CTA)
     const int ta = na - 1 - j > 0 ? na - 1 - j : 0, tb = nb - 1 - j > 0 ? nb - 1 - j : 0;
-    for (int t = warp; t < ta + tb; t += 8) {
+    for (int t = warp; t < ta + tb; t += nwp) {
       const int s_off = t < ta ? 0 : na;
       const int k = t < ta ? j + 1 + t : j + 1 + (t - ta);
       const zcplx* vj = V + (size_t)(s_off + j) * ld;
       zcplx* vk = V + (size_t)(s_off + k) * ld;
-      double dr = 0.0, di = 0.0, nn = 0.0;
-      for (int i = lane; i < M; i += 32) {
-        const zcplx a = vj[i], b = vk[i];
+      // two rows per iteration on separate accumulators: the sweep is a chain of dependent DFMAs otherwise
+      double dr = 0.0, di = 0.0, nn = 0.0, dr2 = 0.0, di2 = 0.0, nn2 = 0.0;
+      int i = lane;
+      for (; i + 32 < M; i += 64) {
+        const zcplx a = vj[i], b = vk[i], a2 = vj[i + 32], b2 = vk[i + 32];
         dr = fma(a.x, b.x, dr); dr = fma(a.y, b.y, dr);      // conj(a) * b
         di = fma(a.x, b.y, di); di = fma(-a.y, b.x, di);
         nn = fma(a.x, a.x, nn); nn = fma(a.y, a.y, nn);
+        dr2 = fma(a2.x, b2.x, dr2); dr2 = fma(a2.y, b2.y, dr2);
+        di2 = fma(a2.x, b2.y, di2); di2 = fma(-a2.y, b2.x, di2);
+        nn2 = fma(a2.x, a2.x, nn2); nn2 = fma(a2.y, a2.y, nn2);
       }
-      dr = warp_sum(dr); di = warp_sum(di); nn = warp_sum(nn);
+      if (i < M) {
+        const zcplx a = vj[i], b = vk[i];
+        dr = fma(a.x, b.x, dr); dr = fma(a.y, b.y, dr);
+        di = fma(a.x, b.y, di); di = fma(-a.y, b.x, di);
+        nn = fma(a.x, a.x, nn); nn = fma(a.y, a.y, nn);
+      }
+      dr = warp_sum(dr + dr2); di = warp_sum(di + di2); nn = warp_sum(nn + nn2);
       if (nn > 0.0) {
-        const double cr = dr / nn, ci = di / nn;
-        for (int i = lane; i < M; i += 32) {
-          const zcplx a = vj[i];
-          zcplx b = vk[i];
+        const double inv = 1.0 / nn, cr = dr * inv, ci = di * inv;
+        for (int r = lane; r < M; r += 32) {
+          const zcplx a = vj[r];
+          zcplx b = vk[r];
           b.x = fma(-cr, a.x, b.x); b.x = fma(ci, a.y, b.x);
           b.y = fma(-cr, a.y, b.y); b.y = fma(-ci, a.x, b.y);
-          vk[i] = b;
+          vk[r] = b;
         }
       }
     }
     __syncthreads();
   }
-  for (int k = warp; k < nt; k += 8) {
+  for (int k = warp; k < nt; k += nwp) {
     const zcplx* vk = V + (size_t)k * ld;
     double nn = 0.0;
     for (int i = lane; i < M; i += 32) { const zcplx a = vk[i]; nn = fma(a.x, a.x, nn); nn = fma(a.y, a.y, nn); }
     nn = warp_sum(nn);
-    if (lane == 0) nrm[k] = nn;
+    if (lane == 0) { nrm[k] = nn; nrm[72 + k] = 1.0 / sqrt(nn); }
   }
   __syncthreads();
   if (tid < 32) {
@@ -100,9 +116,9 @@ __global__ void __launch_bounds__(256) k_ortho(int M, int na, int nb, cplx<T>* _
   }
   __syncthreads();
   if (nrm[64] != 0.0) return;   // degenerate walker: left as it was (flagged)
-  for (int e = tid; e < M * nt; e += 256) {
+  for (int e = tid; e < M * nt; e += nth) {
     const int i = e / nt, k = e - i * nt;
-    const double inv = 1.0 / sqrt(nrm[k]);
+    const double inv = nrm[72 + k];
     const zcplx v = V[k * ld + i];
     g[e] = mk<T>((T)(v.x * inv), (T)(v.y * inv));
   }
