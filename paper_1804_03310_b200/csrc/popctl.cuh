@@ -13,8 +13,7 @@ namespace afq {
 // One CTA per walker, one warp per trailing column (ortho_threads).  The walker is held in shared memory in FP64, one column after the
 // other with an odd leading dimension (conflict-free both for the transposing load/store and for the column
 // sweeps).  Right-looking elimination without an intermediate scaling: at step j every warp that owns a
-// trailing column k computes d = <v_j, v_k> and n = <v_j, v_j> in one sweep and applies v_k -= (d/n) v_j in a
-// second one; v_j itself is only read, so one CTA barrier per step is enough.  Columns are scaled by 1/|v_j|
+// trailing column k computes d = <v_j, v_k> in one sweep and applies v_k -= (d/|v_j|^2) v_j in a second one; v_j itself is only read, so one CTA barrier per step is enough.  Columns are scaled by 1/|v_j|
 // when the walker is written back.  Theta = Phi A^-1 is invariant, so nothing else of the state changes.
 // ------------------------------------------------------------------------------------------------
 __host__ __device__ inline int ortho_ld(int M) { return M | 1; }
@@ -39,6 +38,19 @@ __global__ void __launch_bounds__(512, 2) k_ortho(int M, int na, int nb, cplx<T>
     V[k * ld + i] = to_z(g[e]);
   }
   __syncthreads();
+  // nrm[k] = |v_k|^2 of the fully orthogonalised column k.  Column 0 of each spin is final from the start; column
+  // j + 1 becomes final in elimination step j, and the warp that updates it accumulates its norm in the same sweep.
+  if (warp < 2) {
+    const int n = warp ? nb : na, c0 = warp ? na : 0;
+    if (n > 0) {
+      const zcplx* v0 = V + (size_t)c0 * ld;
+      double nn = 0.0;
+      for (int i = lane; i < M; i += 32) { const zcplx a = v0[i]; nn = fma(a.x, a.x, nn); nn = fma(a.y, a.y, nn); }
+      nn = warp_sum(nn);
+      if (lane == 0) nrm[c0] = nn;
+    }
+  }
+  __syncthreads();
   const int nmax = na > nb ? na : nb;
   for (int j = 0; j + 1 < nmax; ++j) {
     // trailing columns of both spins at this step, dealt round-robin to the warps (up to 16 per CTA)
@@ -48,25 +60,24 @@ __global__ void __launch_bounds__(512, 2) k_ortho(int M, int na, int nb, cplx<T>
       const int k = t < ta ? j + 1 + t : j + 1 + (t - ta);
       const zcplx* vj = V + (size_t)(s_off + j) * ld;
       zcplx* vk = V + (size_t)(s_off + k) * ld;
+      const double nn = nrm[s_off + j];
       // two rows per iteration on separate accumulators: the sweep is a chain of dependent DFMAs otherwise
-      double dr = 0.0, di = 0.0, nn = 0.0, dr2 = 0.0, di2 = 0.0, nn2 = 0.0;
+      double dr = 0.0, di = 0.0, dr2 = 0.0, di2 = 0.0;
       int i = lane;
       for (; i + 32 < M; i += 64) {
         const zcplx a = vj[i], b = vk[i], a2 = vj[i + 32], b2 = vk[i + 32];
         dr = fma(a.x, b.x, dr); dr = fma(a.y, b.y, dr);      // conj(a) * b
         di = fma(a.x, b.y, di); di = fma(-a.y, b.x, di);
-        nn = fma(a.x, a.x, nn); nn = fma(a.y, a.y, nn);
         dr2 = fma(a2.x, b2.x, dr2); dr2 = fma(a2.y, b2.y, dr2);
         di2 = fma(a2.x, b2.y, di2); di2 = fma(-a2.y, b2.x, di2);
-        nn2 = fma(a2.x, a2.x, nn2); nn2 = fma(a2.y, a2.y, nn2);
       }
       if (i < M) {
         const zcplx a = vj[i], b = vk[i];
         dr = fma(a.x, b.x, dr); dr = fma(a.y, b.y, dr);
         di = fma(a.x, b.y, di); di = fma(-a.y, b.x, di);
-        nn = fma(a.x, a.x, nn); nn = fma(a.y, a.y, nn);
       }
-      dr = warp_sum(dr + dr2); di = warp_sum(di + di2); nn = warp_sum(nn + nn2);
+      dr = warp_sum(dr + dr2); di = warp_sum(di + di2);
+      double nk = 0.0;
       if (nn > 0.0) {
         const double inv = 1.0 / nn, cr = dr * inv, ci = di * inv;
         for (int r = lane; r < M; r += 32) {
@@ -75,18 +86,19 @@ __global__ void __launch_bounds__(512, 2) k_ortho(int M, int na, int nb, cplx<T>
           b.x = fma(-cr, a.x, b.x); b.x = fma(ci, a.y, b.x);
           b.y = fma(-cr, a.y, b.y); b.y = fma(-ci, a.x, b.y);
           vk[r] = b;
+          if (k == j + 1) { nk = fma(b.x, b.x, nk); nk = fma(b.y, b.y, nk); }
         }
+      } else if (k == j + 1) {
+        for (int r = lane; r < M; r += 32) { const zcplx b = vk[r]; nk = fma(b.x, b.x, nk); nk = fma(b.y, b.y, nk); }
+      }
+      if (k == j + 1) {
+        nk = warp_sum(nk);
+        if (lane == 0) nrm[s_off + k] = nk;
       }
     }
     __syncthreads();
   }
-  for (int k = warp; k < nt; k += nwp) {
-    const zcplx* vk = V + (size_t)k * ld;
-    double nn = 0.0;
-    for (int i = lane; i < M; i += 32) { const zcplx a = vk[i]; nn = fma(a.x, a.x, nn); nn = fma(a.y, a.y, nn); }
-    nn = warp_sum(nn);
-    if (lane == 0) { nrm[k] = nn; nrm[72 + k] = 1.0 / sqrt(nn); }
-  }
+  if (tid < nt) nrm[72 + tid] = 1.0 / sqrt(nrm[tid]);
   __syncthreads();
   if (tid < 32) {
     // det R_a det R_b = prod |v_k| (real, positive); a vanishing or non-finite column flags the walker
