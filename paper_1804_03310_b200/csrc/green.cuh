@@ -8,27 +8,36 @@ namespace afq {
 
 // The same elimination executed by a GROUP of 128 threads (4 warps, named barrier `bar_id`): the serial
 // one-warp version left 6 of the CTA's 8 warps idle and dominated the kernel (ncu: most stall samples at the CTA
-// barrier behind it).  work = [fac (n) | prow (2n)] scratch; ctrl = one int.  Warp 0 of the group does the pivot
-// search and carries det / sing (identical in all its lanes).
+// barrier behind it).  work = [fac (n) | prow (2n) | staging copy (2n^2) | 1] scratch.  det / sing are identical in
+// all threads of the group.
 __device__ inline void group_gauss_jordan(zcplx* aug, int n, int ld, zcplx* work, int* ctrl, int gtid, int bar_id,
                                           zcplx& det, int& sing, double eps) {
+  (void)ctrl;
   zcplx* fac = work;
   zcplx* prow = work + n;
-  const int lane = gtid & 31, gwarp = gtid >> 5;
+  const int lane = gtid & 31;
   double dre = 1.0, dim = 0.0;
   sing = 0;
   double thresh = 0.0;
-  if (gwarp == 0) {
+  {
     double amax = 0.0;
     for (int e = lane; e < n * n; e += 32) amax = fmax(amax, cabs2(aug[(e / n) * ld + (e % n)]));
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) amax = fmax(amax, __shfl_xor_sync(0xffffffffu, amax, o));
     thresh = amax * eps * eps;
   }
+  // The matrix ping-pongs between `aug` (row stride ld) and a dense staging copy (row stride 2n): every pivot step reads
+  // one and writes the other, so a step costs two group barriers (factors ready; update done) instead of four, and
+  // there is no copy-back pass.  The pivot search is done by every warp of the group redundantly (same shuffles, same
+  // result): no barrier between the search and the factor computation.
+  zcplx* cur = aug; int lc = ld;
+  zcplx* nxt = prow + 2 * n; int ln = 2 * n;
   for (int col = 0; col < n; ++col) {
-    if (gwarp == 0) {
+    int piv;
+    zcplx ip = mk<double>(0.0, 0.0);
+    {
       int r = col + lane;
-      double mag = (r < n) ? cabs2(aug[r * ld + col]) : -1.0;
+      double mag = (r < n) ? cabs2(cur[r * lc + col]) : -1.0;
       int idx = r;
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) {
@@ -37,27 +46,22 @@ __device__ inline void group_gauss_jordan(zcplx* aug, int n, int ld, zcplx* work
         if (om > mag || (om == mag && oi < idx)) { mag = om; idx = oi; }
       }
       const bool dead = !(mag > 0.0);
-      if (dead) { sing = 1; dre = 0.0; dim = 0.0; }
+      if (dead) { sing = 1; dre = 0.0; dim = 0.0; piv = -1; }
       else {
         if (mag < thresh) sing = 1;
         if (idx != col) { dre = -dre; dim = -dim; }
-        zcplx p = aug[idx * ld + col];
+        const zcplx p = cur[idx * lc + col];
         double nr = dre * p.x - dim * p.y;
         dim = dre * p.y + dim * p.x;
         dre = nr;
-      }
-      if (lane == 0) {
-        *ctrl = dead ? -1 : idx;
-        if (!dead) prow[2 * n + 2 * n * n] = cinv(aug[idx * ld + col]);   // one FP64 reciprocal per pivot, not 128
+        piv = idx;
+        ip = cinv(p);
       }
     }
-    asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
-    const int piv = *ctrl;
-    if (piv < 0) break;                                   // exactly singular: uniform exit
+    if (piv < 0) break;                                   // exactly singular: uniform exit (all warps agree)
     // factors (column col, rows permuted) and the scaled pivot row, both out of place
-    const zcplx ip = prow[2 * n + 2 * n * n];
-    for (int c = gtid; c < 2 * n; c += 128) prow[c] = cmul(aug[piv * ld + c], ip);
-    for (int r = gtid; r < n; r += 128) fac[r] = aug[(r == col ? piv : (r == piv ? col : r)) * ld + col];
+    for (int c = gtid; c < 2 * n; c += 128) prow[c] = cmul(cur[piv * lc + c], ip);
+    for (int r = gtid; r < n; r += 128) fac[r] = cur[(r == col ? piv : (r == piv ? col : r)) * lc + col];
     asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
     // new row r <- (row col <-> row piv swapped) - fac[r] * prow ; new row col <- prow
     for (int e = gtid; e < n * 2 * n; e += 128) {
@@ -66,17 +70,19 @@ __device__ inline void group_gauss_jordan(zcplx* aug, int n, int ld, zcplx* work
       if (r == col) v = prow[c];
       else {
         const int src = (r == piv) ? col : r;            // the old row `col` moves to position piv
-        v = aug[src * ld + c];
+        v = cur[src * lc + c];
         const zcplx f = fac[r], pr = prow[c];
         v.x = fma(-f.x, pr.x, v.x); v.x = fma(f.y, pr.y, v.x);
         v.y = fma(-f.x, pr.y, v.y); v.y = fma(-f.y, pr.x, v.y);
       }
-      // rows col and piv are both read and written in this pass: stage the result, store after the barrier
-      prow[2 * n + e] = v;
+      nxt[r * ln + c] = v;
     }
     asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
-    for (int e = gtid; e < n * 2 * n; e += 128) aug[(e / (2 * n)) * ld + (e % (2 * n))] = prow[2 * n + e];
-    asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
+    zcplx* t = cur; cur = nxt; nxt = t;
+    const int tl = lc; lc = ln; ln = tl;
+  }
+  if (cur != aug) {   // odd number of completed steps: the result is in the staging copy
+    for (int e = gtid; e < n * 2 * n; e += 128) aug[(e / (2 * n)) * ld + (e % (2 * n))] = cur[e];
   }
   det = mk<double>(dre, dim);
 }
