@@ -166,6 +166,28 @@ AFQMC_API afqmc_status afqmc_orthonormalize(afqmc_ctx* ctx, void* phi, void* ovl
 AFQMC_API afqmc_status afqmc_population_control(afqmc_ctx* ctx, void* phi, double* weight, void* ovlp, void* theta, void* fb,
                                       double u, int32_t* parent);
 
+/* Building blocks of the comb over a population SHARDED across ranks (PAPER.md:111
+ * "subsets which are independently propagated and measured on different GPU cards", :121-127): the one exchange step
+ * of the method.  Every rank holds N_w walkers; global slot g = rank * N_w + local index.  Protocol (the collectives
+ * themselves are the caller's: paper_1804_03310_b200/dist.py uses torch.distributed all_gather + all_to_all_single):
+ *   1. all-gather the weights -> weight_all [n_total]; afqmc_comb_map on every rank (same bits everywhere) gives
+ *      parent_all [n_total] (reading R22, as afqmc_population_control) and w_new = { W / n_total, W } (DEVICE [2]).
+ *      cum_scratch: DEVICE double [n_total].
+ *   2. the map is monotone, so the global slots whose parent lives on this rank form ONE contiguous range
+ *      [slot_lo, slot_lo + count): afqmc_comb_pack writes their parents' records, in slot order, into sendbuf
+ *      (count * afqmc_comb_record_bytes; record = [phi | theta | fb | S]); first_local = rank * N_w.
+ *   3. all-to-all with per-rank counts derived from parent_all; the receive buffer then holds this rank's N_w new
+ *      walkers in slot order; afqmc_comb_unpack stores them and sets every weight to w_new[0] (kept if w_new[0] < 0,
+ *      the dead-population case).
+ * All pointers DEVICE; nothing synchronises.  Errors: EINVAL. */
+AFQMC_API size_t afqmc_comb_record_bytes(const afqmc_ctx* ctx);
+AFQMC_API afqmc_status afqmc_comb_map(afqmc_ctx* ctx, const double* weight_all, int64_t n_total, double u, double* cum_scratch,
+                            int32_t* parent_all, double* w_new);
+AFQMC_API afqmc_status afqmc_comb_pack(afqmc_ctx* ctx, const void* phi, const void* ovlp, const void* theta, const void* fb,
+                             const int32_t* parent_all, int64_t slot_lo, int64_t count, int64_t first_local, void* sendbuf);
+AFQMC_API afqmc_status afqmc_comb_unpack(afqmc_ctx* ctx, const void* recvbuf, void* phi, double* weight, void* ovlp, void* theta,
+                               void* fb, const double* w_new);
+
 /* The paper's schedule around the walker step (NEXT-2; hybrid weights "to minimize evaluations of the
  * local energy, which is measured every 0.1 Ha^-1", orthonormalisation every 2 steps, population control every
  * 0.1 Ha^-1).  n_steps steps of [shift -> assemble -> Taylor -> overlap/Theta -> weight -> force bias]; after step n

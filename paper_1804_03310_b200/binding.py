@@ -20,7 +20,8 @@ FLAG_SINGULAR, FLAG_NONFINITE, FLAG_KILLED = 1, 2, 4
 SYMBOLS = ["afqmc_query_bytes", "afqmc_init", "afqmc_destroy", "afqmc_last_error", "afqmc_overlap_green",
            "afqmc_force_bias", "afqmc_propagate", "afqmc_local_energy", "afqmc_step", "afqmc_step_host",
            "afqmc_launch_count", "afqmc_gemm_path", "afqmc_profile_enable", "afqmc_profile_read",
-           "afqmc_orthonormalize", "afqmc_population_control", "afqmc_run"]
+           "afqmc_orthonormalize", "afqmc_population_control", "afqmc_run", "afqmc_comb_record_bytes",
+           "afqmc_comb_map", "afqmc_comb_pack", "afqmc_comb_unpack"]
 
 STAGES = ["shift", "assemble", "taylor", "green", "force_bias", "energy", "symmetrize", "ortho", "popctl"]
 
@@ -67,6 +68,11 @@ def load_library():
     lib.afqmc_orthonormalize.argtypes = [vp, vp, vp, i32p]
     lib.afqmc_population_control.argtypes = [vp, vp, vp, vp, vp, vp, C.c_double, i32p]
     lib.afqmc_run.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp, vp, i32p, i32p]
+    lib.afqmc_comb_record_bytes.argtypes = [vp]
+    lib.afqmc_comb_record_bytes.restype = C.c_size_t
+    lib.afqmc_comb_map.argtypes = [vp, vp, C.c_int64, C.c_double, vp, i32p, vp]
+    lib.afqmc_comb_pack.argtypes = [vp, vp, vp, vp, vp, i32p, C.c_int64, C.c_int64, C.c_int64, vp]
+    lib.afqmc_comb_unpack.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
     lib.afqmc_launch_count.argtypes = [vp]
     lib.afqmc_launch_count.restype = C.c_int64
     lib.afqmc_gemm_path.argtypes = [vp]
@@ -77,7 +83,7 @@ def load_library():
     lib.afqmc_profile_read.restype = C.c_int
     for name in ("afqmc_query_bytes", "afqmc_init", "afqmc_overlap_green", "afqmc_force_bias", "afqmc_propagate",
                  "afqmc_local_energy", "afqmc_step", "afqmc_step_host", "afqmc_orthonormalize", "afqmc_population_control",
-                 "afqmc_run"):
+                 "afqmc_run", "afqmc_comb_map", "afqmc_comb_pack", "afqmc_comb_unpack"):
         getattr(lib, name).restype = C.c_int
     _lib = lib
     return lib
@@ -211,6 +217,22 @@ class AfqmcContext:
         self._chk(self._lib.afqmc_run(self._ctx, _dp(phi), _dp(weight), _dp(ovlp), _dp(theta), _dp(fb), _dp(x),
                                       int(n_steps), int(energy_every), int(ortho_every), int(pc_every), _hp(ua),
                                       _dp(eloc), _dp(w_meas), _dp(parents), _dp(flags)))
+
+    @property
+    def afqmc_comb_record_bytes(self) -> int:
+        return int(self._lib.afqmc_comb_record_bytes(self._ctx))
+
+    def afqmc_comb_map(self, weight_all, u, cum_scratch, parent_all, w_new):
+        self._chk(self._lib.afqmc_comb_map(self._ctx, _dp(weight_all), int(weight_all.numel()), float(u), _dp(cum_scratch),
+                                           _dp(parent_all), _dp(w_new)))
+
+    def afqmc_comb_pack(self, phi, ovlp, theta, fb, parent_all, slot_lo, count, first_local, sendbuf):
+        self._chk(self._lib.afqmc_comb_pack(self._ctx, _dp(phi), _dp(ovlp), _dp(theta), _dp(fb), _dp(parent_all),
+                                            int(slot_lo), int(count), int(first_local), _dp(sendbuf)))
+
+    def afqmc_comb_unpack(self, recvbuf, phi, weight, ovlp, theta, fb, w_new):
+        self._chk(self._lib.afqmc_comb_unpack(self._ctx, _dp(recvbuf), _dp(phi), _dp(weight), _dp(ovlp), _dp(theta),
+                                              _dp(fb), _dp(w_new)))
 
     def afqmc_step_host(self, phi_h, weight_h, ovlp_h, x_h, n_steps, eloc_h, flags_h=None):
         """HOST buffers: numpy arrays or CPU (pinned) torch tensors, updated in place. Returns (h2d, d2h) bytes."""

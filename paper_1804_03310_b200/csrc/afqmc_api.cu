@@ -1117,8 +1117,8 @@ afqmc_status afqmc_step(afqmc_ctx* c, void* phi, double* weight, void* ovlp, voi
 afqmc_status afqmc_orthonormalize(afqmc_ctx* c, void* phi, void* ovlp, int32_t* flags) {
   if (!c) return AFQMC_EINVAL;
   c->err[0] = 0;
-  NEED(c, phi && ovlp, "afqmc_orthonormalize: null pointer");
   if (c->nw == 0) return AFQMC_OK;
+  NEED(c, phi && ovlp, "afqmc_orthonormalize: null pointer");
   return DISPATCH(c, do_ortho, c, phi, ovlp, flags);
 }
 
@@ -1130,6 +1130,57 @@ afqmc_status afqmc_population_control(afqmc_ctx* c, void* phi, double* weight, v
   if (c->nw == 0) return AFQMC_OK;
   NEED(c, phi && weight && ovlp && theta && fb, "afqmc_population_control: null pointer");
   return DISPATCH(c, do_popctl, c, phi, weight, ovlp, theta, fb, u, parent);
+}
+
+size_t afqmc_comb_record_bytes(const afqmc_ctx* c) {
+  if (!c) return 0;
+  return (size_t)(2 * (c->M * c->nt * 2 * c->ts / 8) + c->ng * 2 * c->ts / 8 + 2) * 8;
+}
+
+static CombRecord comb_record(const afqmc_ctx* c, void* phi, void* ovlp, void* theta, void* fb) {
+  CombRecord m;
+  m.phi = (uint2*)phi; m.theta = (uint2*)theta; m.fb = (uint2*)fb; m.ovlp = (zcplx*)ovlp;
+  m.words_phi = c->M * c->nt * 2 * c->ts / 8; m.words_fb = c->ng * 2 * c->ts / 8;
+  m.words_rec = 2 * m.words_phi + m.words_fb + 2;
+  return m;
+}
+
+afqmc_status afqmc_comb_map(afqmc_ctx* c, const double* weight_all, int64_t n_total, double u, double* cum_scratch,
+                            int32_t* parent_all, double* w_new) {
+  if (!c) return AFQMC_EINVAL;
+  c->err[0] = 0;
+  NEED(c, n_total >= 0 && n_total < (int64_t)1 << 31, "afqmc_comb_map: n_total out of range");
+  NEED(c, u >= 0.0 && u < 1.0, "afqmc_comb_map: u must be in [0, 1)");
+  if (n_total == 0) return AFQMC_OK;
+  NEED(c, weight_all && cum_scratch && parent_all && w_new, "afqmc_comb_map: null pointer");
+  StageScope sc(c, AFQMC_STAGE_POPCTL);
+  LAUNCH(c, k_comb_parents, 1, 1024, 0, (int)n_total, weight_all, u, cum_scratch, parent_all, w_new);
+  return AFQMC_OK;
+}
+
+afqmc_status afqmc_comb_pack(afqmc_ctx* c, const void* phi, const void* ovlp, const void* theta, const void* fb,
+                             const int32_t* parent_all, int64_t slot_lo, int64_t count, int64_t first_local, void* sendbuf) {
+  if (!c) return AFQMC_EINVAL;
+  c->err[0] = 0;
+  NEED(c, count >= 0 && slot_lo >= 0 && first_local >= 0, "afqmc_comb_pack: negative index");
+  if (count == 0 || c->nw == 0) return AFQMC_OK;
+  NEED(c, phi && ovlp && theta && fb && parent_all && sendbuf, "afqmc_comb_pack: null pointer");
+  StageScope sc(c, AFQMC_STAGE_POPCTL);
+  CombRecord m = comb_record(c, (void*)phi, (void*)ovlp, (void*)theta, (void*)fb);
+  LAUNCH(c, k_comb_pack_send, (unsigned)count, 256, 0, m, parent_all, (long long)slot_lo, (long long)first_local, (uint2*)sendbuf);
+  return AFQMC_OK;
+}
+
+afqmc_status afqmc_comb_unpack(afqmc_ctx* c, const void* recvbuf, void* phi, double* weight, void* ovlp, void* theta, void* fb,
+                               const double* w_new) {
+  if (!c) return AFQMC_EINVAL;
+  c->err[0] = 0;
+  if (c->nw == 0) return AFQMC_OK;
+  NEED(c, recvbuf && phi && weight && ovlp && theta && fb && w_new, "afqmc_comb_unpack: null pointer");
+  StageScope sc(c, AFQMC_STAGE_POPCTL);
+  CombRecord m = comb_record(c, phi, ovlp, theta, fb);
+  LAUNCH(c, k_comb_unpack_recv, c->nw, 256, 0, m, (const uint2*)recvbuf, weight, w_new);
+  return AFQMC_OK;
 }
 
 afqmc_status afqmc_run(afqmc_ctx* c, void* phi, double* weight, void* ovlp, void* theta, void* fb, const void* x,

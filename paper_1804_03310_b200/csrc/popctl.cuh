@@ -218,4 +218,50 @@ __global__ void __launch_bounds__(256) k_comb_unpack(CombMove m, const int32_t* 
   if (threadIdx.x == 0) m.ovlp[i] = m.s_ovlp[i];
 }
 
+// ------------------------------------------------------------------------------------------------
+// Comb over a population sharded across ranks: every rank runs
+// k_comb_parents on the all-gathered weights (same bits everywhere), packs the records of ITS walkers that the map
+// hands out (to itself or to peers) in global-slot order -- the map is monotone, so these slots are one contiguous
+// range and the all-to-all's receive buffer arrives in slot order -- and unpacks the received records in place.
+// Record = [phi | theta | fb | S] in 8-byte words.
+// ------------------------------------------------------------------------------------------------
+struct CombRecord {
+  uint2 *phi, *theta, *fb;
+  zcplx* ovlp;
+  int words_phi, words_fb, words_rec;   // words_rec = 2 words_phi + words_fb + 2
+};
+
+__global__ void __launch_bounds__(256) k_comb_pack_send(CombRecord m, const int32_t* __restrict__ parent_all, long long slot_lo,
+                                                         long long first_local, uint2* __restrict__ sendbuf) {
+  const long long j = blockIdx.x;
+  const long long p = (long long)parent_all[slot_lo + j] - first_local;   // local index of the parent
+  uint2* dst = sendbuf + j * m.words_rec;
+  const uint2* sp = m.phi + p * m.words_phi;
+  const uint2* st = m.theta + p * m.words_phi;
+  for (int e = threadIdx.x; e < m.words_phi; e += 256) { dst[e] = sp[e]; dst[m.words_phi + e] = st[e]; }
+  const uint2* sf = m.fb + p * m.words_fb;
+  for (int e = threadIdx.x; e < m.words_fb; e += 256) dst[2 * m.words_phi + e] = sf[e];
+  if (threadIdx.x == 0) {   // 8-byte stores: a record is only 8-byte aligned
+    const zcplx sv = m.ovlp[p];
+    double* d = reinterpret_cast<double*>(dst + 2 * m.words_phi + m.words_fb);
+    d[0] = sv.x; d[1] = sv.y;
+  }
+}
+
+__global__ void __launch_bounds__(256) k_comb_unpack_recv(CombRecord m, const uint2* __restrict__ recvbuf, double* __restrict__ weight,
+                                                           const double* __restrict__ wnew) {
+  const long long i = blockIdx.x;
+  const uint2* src = recvbuf + i * m.words_rec;
+  uint2* dp = m.phi + i * m.words_phi;
+  uint2* dt = m.theta + i * m.words_phi;
+  for (int e = threadIdx.x; e < m.words_phi; e += 256) { dp[e] = src[e]; dt[e] = src[m.words_phi + e]; }
+  uint2* df = m.fb + i * m.words_fb;
+  for (int e = threadIdx.x; e < m.words_fb; e += 256) df[e] = src[2 * m.words_phi + e];
+  if (threadIdx.x == 0) {
+    const double* d = reinterpret_cast<const double*>(src + 2 * m.words_phi + m.words_fb);
+    m.ovlp[i] = mk<double>(d[0], d[1]);
+    if (wnew[0] >= 0.0) weight[i] = wnew[0];
+  }
+}
+
 }  // namespace afq

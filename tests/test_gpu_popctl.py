@@ -249,3 +249,109 @@ def test_full_size_schedule_sampled_walkers():
     assert np.array_equal(parent.cpu().numpy(), p)
     assert np.array_equal(o2["phi"], out["phi"][p]) and np.array_equal(o2["S"], out["S"][p])
     assert np.array_equal(o2["w"], np.full(nw, np.cumsum(out["w"])[-1] / nw))
+
+
+def test_run_argument_errors_and_ragged_schedule():
+    """EINVAL before any launch: weight_mode 1, u outside [0, 1), missing u / eloc; an empty batch and n_steps = 0 are
+    no-ops; a step count that is not a multiple of the intervals measures / combs floor(n / every) times."""
+    import torch
+    import paper_1804_03310_b200 as afq
+    wl = make_workload(1, "tame")
+    nw = 8
+    xs = wl.fields(5, nw)
+    ctx = H.make_ctx(wl, nw)
+    st = H.DeviceState(ctx, wl.walkers(nw))
+    st.seed()
+    xd = torch.tensor(np.ascontiguousarray(xs), dtype=ctx.rdtype, device=ctx.device)
+    eloc = torch.full((2, nw), -7.0, dtype=torch.complex128, device=ctx.device)
+    par = torch.full((1, nw), -1, dtype=torch.int32, device=ctx.device)
+    l0 = ctx.launch_count
+    for kw in (dict(u=[1.0]), dict(u=[-0.1]), dict(u=None)):
+        with pytest.raises(afq.AfqmcError) as ei:
+            ctx.afqmc_run(st.phi, st.weight, st.ovlp, st.theta, st.fb, xd, 5, 2, 2, 3, kw["u"], eloc, None, par, st.flags)
+        assert ei.value.status == afq.AFQMC_EINVAL
+    with pytest.raises(afq.AfqmcError):
+        ctx.afqmc_run(st.phi, st.weight, st.ovlp, st.theta, st.fb, xd, 5, 2, 0, 0, None, None, None, None, st.flags)
+    with pytest.raises(afq.AfqmcError):
+        ctx.afqmc_orthonormalize(None, st.ovlp, None)
+    assert ctx.launch_count == l0
+    ctx.afqmc_run(st.phi, st.weight, st.ovlp, st.theta, st.fb, xd, 0, 1, 1, 1, [0.5], eloc, None, par, st.flags)
+    assert ctx.launch_count == l0
+    ctx.afqmc_run(st.phi, st.weight, st.ovlp, st.theta, st.fb, xd, 5, 2, 2, 3, [0.5], eloc, None, par, st.flags)
+    torch.cuda.synchronize()
+    assert torch.all(eloc.real != -7.0) and torch.all(par >= 0)          # 2 measurements, 1 comb
+    ctx1 = H.make_ctx(wl, nw, weight_mode=1)
+    with pytest.raises(afq.AfqmcError):
+        ctx1.afqmc_run(st.phi, st.weight, st.ovlp, st.theta, st.fb, xd, 2, 1, 0, 0, None, eloc, None, None, st.flags)
+    ctx0 = H.make_ctx(wl, 0)
+    e = torch.zeros(0, dtype=ctx0.cdtype, device=ctx0.device)
+    ctx0.afqmc_orthonormalize(e, e, None)
+    ctx0.afqmc_population_control(e, e, e, e, e, 0.5, None)
+    assert ctx0.launch_count == 0
+
+
+@pytest.mark.parametrize("world", [1, 2, 3])
+def test_sharded_comb_emulated_ranks(world):
+    """The comb over a population sharded across `world` ranks (afqmc_comb_map / _pack / _unpack + dist.comb_splits),
+    with the ranks played one after the other on this GPU and the all-to-all replaced by slicing the send buffers the
+    way torch.distributed.all_to_all_single would (no kernel waits on another rank).  Bit-exact against
+    afqmc_population_control on the whole population in one context, and against the oracle's map."""
+    import torch
+    from paper_1804_03310_b200 import dist as D
+    wl = make_workload(2)
+    nl = 50
+    nt = world * nl
+    ctx_all = H.make_ctx(wl, nt)
+    full, w = _random_state(wl, ctx_all, nt, seed=31 + world)
+    w[nl // 2:nl] = 0.0                                   # a dead stretch: its slots are refilled from other ranks
+    full.weight.copy_(torch.tensor(w, dtype=torch.float64))
+    before = full.host()
+    u = 0.613
+    ranks = []
+    for r in range(world):
+        c = H.make_ctx(wl, nl)
+        sl = slice(r * nl, (r + 1) * nl)
+        st = H.DeviceState(c, before["phi"][sl], weight=w[sl], ovlp=before["S"][sl])
+        st.theta.copy_(torch.tensor(before["theta"][sl], dtype=c.cdtype)); st.fb.copy_(torch.tensor(before["f"][sl], dtype=c.cdtype))
+        ranks.append((c, st))
+    w_all = torch.cat([st.weight for _, st in ranks])      # the all-gather
+    sends, plans = [], []
+    for r, (c, st) in enumerate(ranks):
+        cum = torch.empty(nt, dtype=torch.float64, device=c.device)
+        parent_all = torch.empty(nt, dtype=torch.int32, device=c.device)
+        w_new = torch.empty(2, dtype=torch.float64, device=c.device)
+        c.afqmc_comb_map(w_all, u, cum, parent_all, w_new)
+        slot_lo, count, sc, rc = D.comb_splits(parent_all, nl, world, r)
+        rec = c.afqmc_comb_record_bytes
+        sb = torch.zeros(max(count, 1) * rec, dtype=torch.uint8, device=c.device)
+        c.afqmc_comb_pack(st.phi, st.ovlp, st.theta, st.fb, parent_all, slot_lo, count, r * nl, sb)
+        sends.append(sb); plans.append((parent_all, w_new, sc, rc, rec))
+    par_o = orc.o_comb(w, u)
+    for r, (c, st) in enumerate(ranks):
+        parent_all, w_new, sc, rc, rec = plans[r]
+        assert np.array_equal(parent_all.cpu().numpy(), par_o)
+        parts = []
+        for s in range(world):                              # what all_to_all_single delivers to rank r
+            off = sum(plans[s][2][:r]) * rec
+            assert plans[s][2][r] == rc[s]
+            parts.append(sends[s][off:off + plans[s][2][r] * rec])
+        rb = torch.cat(parts)
+        assert rb.numel() == nl * rec
+        c.afqmc_comb_unpack(rb, st.phi, st.weight, st.ovlp, st.theta, st.fb, w_new)
+    ctx_all.afqmc_population_control(full.phi, full.weight, full.ovlp, full.theta, full.fb, u, None)
+    ref = full.host()
+    for r, (c, st) in enumerate(ranks):
+        got = st.host()
+        sl = slice(r * nl, (r + 1) * nl)
+        for k in ("phi", "theta", "f", "S", "w"):
+            assert np.array_equal(got[k], ref[k][sl]), (world, r, k)
+    assert np.array_equal(ref["phi"], before["phi"][par_o])
+    if world == 1:      # the public helper, single rank: no collective
+        c, st = ranks[0]
+        st2 = H.DeviceState(c, before["phi"], weight=w, ovlp=before["S"])
+        st2.theta.copy_(torch.tensor(before["theta"], dtype=c.cdtype)); st2.fb.copy_(torch.tensor(before["f"], dtype=c.cdtype))
+        pm = D.population_control_sharded(c, st2.phi, st2.weight, st2.ovlp, st2.theta, st2.fb, u)
+        g2 = st2.host()
+        assert np.array_equal(pm.cpu().numpy(), par_o)
+        for k in ("phi", "theta", "f", "S", "w"):
+            assert np.array_equal(g2[k], ref[k]), k
