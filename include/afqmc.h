@@ -142,8 +142,10 @@ AFQMC_API afqmc_status afqmc_step(afqmc_ctx* ctx, void* phi, double* weight, voi
 
 /* The same n_steps through HOST buffers (pinned or pageable): copies phi, weight, x to the device,
  * seeds ovlp/theta/fb from phi, runs afqmc_step, copies phi, weight, ovlp, eloc, flags back, and
- * synchronises.  Device staging lives in work_mem (sized by afqmc_query_bytes for one step of fields;
- * x is streamed step by step).  h2d_bytes / d2h_bytes (may be NULL) receive the bytes moved. */
+ * synchronises.  Device staging lives in work_mem (sized by afqmc_query_bytes for two steps of fields;
+ * x is streamed step by step).  The per-step field upload and energy download run on a second, library-owned
+ * non-blocking stream, double-buffered and ordered with events, so that with PINNED host buffers they overlap the
+ * kernels of the neighbouring steps; the walkers go up before and come down after the steps on ctx's stream.  h2d_bytes / d2h_bytes (may be NULL) receive the bytes moved. */
 AFQMC_API afqmc_status afqmc_step_host(afqmc_ctx* ctx, void* phi_h, double* weight_h, void* ovlp_h, const void* x_h,
                              int32_t n_steps, void* eloc_h, int32_t* flags_h, size_t* h2d_bytes,
                              size_t* d2h_bytes);

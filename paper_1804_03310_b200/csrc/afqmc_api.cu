@@ -64,6 +64,8 @@ struct afqmc_ctx {
   zcplx *h_ovlp, *h_eloc;
   double* h_weight;
   int32_t* h_flags;
+  void* h_x2; zcplx* h_eloc2;            // second field / energy staging buffers: copies overlap the previous step
+  cudaStream_t copy_stream; cudaEvent_t ev_x[2], ev_done[2], ev_e[2]; int copy_ready;
   // orthonormalisation / comb population control (popctl.cuh)
   size_t ortho_smem;
   void *pc_phi, *pc_theta, *pc_fb; zcplx* pc_ovlp; double *pc_cum, *pc_wnew; int32_t* pc_parent;
@@ -256,6 +258,8 @@ void carve(const afqmc_params* p, afqmc_ctx* c, char* cbase, char* wbase, size_t
   c->h_eloc = (zcplx*)w.take(nw1 * sizeof(zcplx));
   c->h_weight = (double*)w.take(nw1 * sizeof(double));
   c->h_flags = (int32_t*)w.take(nw1 * sizeof(int32_t));
+  c->h_x2 = w.take(nw1 * ng * ts);
+  c->h_eloc2 = (zcplx*)w.take(nw1 * sizeof(zcplx));
   c->pc_phi = w.take(nw1 * M * nt * 2 * ts);
   c->pc_theta = w.take(nw1 * M * nt * 2 * ts);
   c->pc_fb = w.take(nw1 * ng * 2 * ts);
@@ -1004,6 +1008,10 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
 void afqmc_destroy(afqmc_ctx* ctx) {
   if (!ctx) return;
   afqmc_profile_enable(ctx, 0);
+  if (ctx->copy_ready) {
+    for (int i = 0; i < 2; ++i) { cudaEventDestroy(ctx->ev_x[i]); cudaEventDestroy(ctx->ev_done[i]); cudaEventDestroy(ctx->ev_e[i]); }
+    cudaStreamDestroy(ctx->copy_stream);
+  }
   delete ctx;
 }
 
@@ -1222,13 +1230,50 @@ afqmc_status afqmc_step_host(afqmc_ctx* c, void* phi_h, double* weight_h, void* 
   if (s) return s;
   s = afqmc_force_bias(c, c->h_phi, c->h_theta, c->h_fb);
   if (s) return s;
-  for (int i = 0; i < n_steps; ++i) {
-    CUDA_OK(c, cudaMemcpyAsync(c->h_x, (const char*)x_h + (size_t)i * x_b, x_b, cudaMemcpyHostToDevice, st));
+  // Fields go up and energies come down on a second (non-blocking) stream, double-buffered: the upload of step i+1 and
+  // the download of step i-1 run under the kernels of step i (pinned host buffers; pageable ones serialise).
+  if (!c->copy_ready && n_steps > 0) {
+    CUDA_OK(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+    for (int i = 0; i < 2; ++i) {
+      CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_x[i], cudaEventDisableTiming));
+      CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_done[i], cudaEventDisableTiming));
+      CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_e[i], cudaEventDisableTiming));
+    }
+    c->copy_ready = 1;
+  }
+  cudaStream_t cs = c->copy_stream;
+  void* xb[2] = {c->h_x, c->h_x2};
+  zcplx* eb[2] = {c->h_eloc, c->h_eloc2};
+  if (n_steps > 0) {   // the copy stream starts after everything already queued on the context's stream
+    CUDA_OK(c, cudaEventRecord(c->ev_done[0], st));
+    CUDA_OK(c, cudaStreamWaitEvent(cs, c->ev_done[0], 0));
+  }
+  auto upload = [&](int i) -> cudaError_t {   // fields of step i into buffer i & 1 (free once step i-2 is done)
+    const int b = i & 1;
+    cudaError_t e = cudaSuccess;
+    if (i >= 2) e = cudaStreamWaitEvent(cs, c->ev_done[b], 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(xb[b], (const char*)x_h + (size_t)i * x_b, x_b, cudaMemcpyHostToDevice, cs);
+    if (e == cudaSuccess) e = cudaEventRecord(c->ev_x[b], cs);
     up += x_b;
-    s = afqmc_step(c, c->h_phi, c->h_weight, c->h_ovlp, c->h_theta, c->h_fb, c->h_x, 1, c->h_eloc, c->h_flags);
+    return e;
+  };
+  if (n_steps > 0) CUDA_OK(c, upload(0));
+  for (int i = 0; i < n_steps; ++i) {
+    const int b = i & 1;
+    if (i + 1 < n_steps) CUDA_OK(c, upload(i + 1));                      // queued ahead of step i's download
+    CUDA_OK(c, cudaStreamWaitEvent(st, c->ev_x[b], 0));
+    if (i >= 2) CUDA_OK(c, cudaStreamWaitEvent(st, c->ev_e[b], 0));      // energies of step i-2 have left buffer b
+    s = afqmc_step(c, c->h_phi, c->h_weight, c->h_ovlp, c->h_theta, c->h_fb, xb[b], 1, eb[b], c->h_flags);
     if (s) return s;
-    CUDA_OK(c, cudaMemcpyAsync((char*)eloc_h + (size_t)i * nw * 16, c->h_eloc, nw * 16, cudaMemcpyDeviceToHost, st));
+    CUDA_OK(c, cudaEventRecord(c->ev_done[b], st));
+    CUDA_OK(c, cudaStreamWaitEvent(cs, c->ev_done[b], 0));
+    CUDA_OK(c, cudaMemcpyAsync((char*)eloc_h + (size_t)i * nw * 16, eb[b], nw * 16, cudaMemcpyDeviceToHost, cs));
+    CUDA_OK(c, cudaEventRecord(c->ev_e[b], cs));
     down += nw * 16;
+  }
+  if (n_steps > 0) {   // the context's stream ends after the last download
+    CUDA_OK(c, cudaEventRecord(c->ev_e[0], cs));
+    CUDA_OK(c, cudaStreamWaitEvent(st, c->ev_e[0], 0));
   }
   CUDA_OK(c, cudaMemcpyAsync(phi_h, c->h_phi, phi_b, cudaMemcpyDeviceToHost, st));
   CUDA_OK(c, cudaMemcpyAsync(weight_h, c->h_weight, nw * 8, cudaMemcpyDeviceToHost, st));
