@@ -190,6 +190,12 @@ AFQMC_API afqmc_status afqmc_comb_pack(afqmc_ctx* ctx, const void* phi, const vo
 AFQMC_API afqmc_status afqmc_comb_unpack(afqmc_ctx* ctx, const void* recvbuf, void* phi, double* weight, void* ovlp, void* theta,
                                void* fb, const double* w_new);
 
+/* Sums of the mixed estimator for one measurement: out3 (DEVICE double [3]) =
+ * { sum_w weight[w], Re sum_w weight[w] eloc[w], Im sum_w weight[w] eloc[w] }, FP64, fixed summation tree; walkers with
+ * weight exactly 0 contribute nothing (their E_L may be non-finite).  E_mix = out3[1] / out3[0]; across ranks the three
+ * numbers are what is all-reduced.  An empty batch writes zeros.  All DEVICE. */
+AFQMC_API afqmc_status afqmc_mixed_sums(afqmc_ctx* ctx, const double* weight, const void* eloc, double* out3);
+
 /* The paper's schedule around the walker step (NEXT-2; hybrid weights "to minimize evaluations of the
  * local energy, which is measured every 0.1 Ha^-1", orthonormalisation every 2 steps, population control every
  * 0.1 Ha^-1).  n_steps steps of [shift -> assemble -> Taylor -> overlap/Theta -> weight -> force bias]; after step n

@@ -1191,6 +1191,14 @@ afqmc_status afqmc_comb_unpack(afqmc_ctx* c, const void* recvbuf, void* phi, dou
   return AFQMC_OK;
 }
 
+afqmc_status afqmc_mixed_sums(afqmc_ctx* c, const double* weight, const void* eloc, double* out3) {
+  if (!c) return AFQMC_EINVAL;
+  c->err[0] = 0;
+  NEED(c, out3 && (c->nw == 0 || (weight && eloc)), "afqmc_mixed_sums: null pointer");
+  LAUNCH(c, k_mixed_sums, 1, 1024, 0, c->nw, weight, (const zcplx*)eloc, out3);
+  return AFQMC_OK;
+}
+
 afqmc_status afqmc_run(afqmc_ctx* c, void* phi, double* weight, void* ovlp, void* theta, void* fb, const void* x,
                        int32_t n_steps, int32_t energy_every, int32_t ortho_every, int32_t pc_every, const double* u,
                        void* eloc, double* w_meas, int32_t* parents, int32_t* flags) {

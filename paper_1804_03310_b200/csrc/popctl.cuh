@@ -264,4 +264,29 @@ __global__ void __launch_bounds__(256) k_comb_unpack_recv(CombRecord m, const ui
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Mixed-estimator sums of one measurement ("weighted sum"; the (sum w, sum w E_L) pair that
+// is all-reduced across ranks): out = { sum_w w, Re sum_w w E_L, Im sum_w w E_L }, FP64.  One CTA, fixed-shape tree
+// (thread t sums walkers t, t + 1024, ... in order; then a shared-memory tree): the result does not depend on timing.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(1024) k_mixed_sums(int nw, const double* __restrict__ w, const zcplx* __restrict__ eloc,
+                                                      double* __restrict__ out) {
+  __shared__ double sh[3][1024];
+  const int tid = threadIdx.x;
+  double a = 0.0, b = 0.0, c = 0.0;
+  for (int i = tid; i < nw; i += 1024) {
+    const double wi = w[i];
+    const zcplx e = eloc[i];
+    a += wi;
+    if (wi != 0.0) { b = fma(wi, e.x, b); c = fma(wi, e.y, c); }   // a dead walker's E_L may be Inf/NaN: weight 0 drops it
+  }
+  sh[0][tid] = a; sh[1][tid] = b; sh[2][tid] = c;
+  __syncthreads();
+  for (int o = 512; o > 0; o >>= 1) {
+    if (tid < o) { sh[0][tid] += sh[0][tid + o]; sh[1][tid] += sh[1][tid + o]; sh[2][tid] += sh[2][tid + o]; }
+    __syncthreads();
+  }
+  if (tid < 3) out[tid] = sh[tid][0];
+}
+
 }  // namespace afq

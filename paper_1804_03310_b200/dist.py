@@ -82,3 +82,40 @@ def population_control_sharded(ctx, phi, weight, ovlp, theta, fb, u: float, grou
         recvbuf = sendbuf
     ctx.afqmc_comb_unpack(recvbuf, phi, weight, ovlp, theta, fb, w_new)
     return parent_all
+
+
+def run_sharded(ctx, phi, weight, ovlp, theta, fb, x, n_steps, energy_every=20, ortho_every=2, pc_every=20, us=(),
+                flags=None, group=None):
+    """The paper's schedule (afqmc_run) for a population sharded across the ranks of `group`: every rank
+    steps its own N_w walkers with its own fields x [n_steps][N_w][n_chol]; the comb runs over the WHOLE population
+    (population_control_sharded, same us on every rank) and every measurement all-reduces the three estimator sums of
+    afqmc_mixed_sums.  pc_every must be a multiple of energy_every and of ortho_every (the paper's 20 / 2 / 20), or 0.
+    Returns the list of global mixed-estimator energies (complex) of the measurements, identical on every rank."""
+    import torch
+    import torch.distributed as dist
+    on = dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1
+    nw = int(ctx.params.n_walkers)
+    seg = pc_every if pc_every else n_steps
+    assert seg > 0 and (not energy_every or seg % energy_every == 0) and (not ortho_every or seg % ortho_every == 0)
+    n_meas_seg = seg // energy_every if energy_every else 0
+    eloc = torch.zeros(max(n_meas_seg, 1), nw, dtype=torch.complex128, device=weight.device)
+    wm = torch.zeros(max(n_meas_seg, 1), nw, dtype=torch.float64, device=weight.device)
+    sums = torch.zeros(max(n_meas_seg, 1), 3, dtype=torch.float64, device=weight.device)
+    energies, done, k = [], 0, 0
+    while done < n_steps:
+        n = min(seg, n_steps - done)
+        ctx.afqmc_run(phi, weight, ovlp, theta, fb, x[done:done + n], n, energy_every, ortho_every, 0, None, eloc, wm,
+                      None, flags)
+        m = n // energy_every if energy_every else 0
+        for j in range(m):
+            ctx.afqmc_mixed_sums(wm[j], eloc[j], sums[j])
+        if m:
+            if on:
+                dist.all_reduce(sums[:m], group=group)
+            for row in sums[:m].tolist():
+                energies.append(complex(row[1], row[2]) / row[0] if row[0] else complex("nan"))
+        done += n
+        if pc_every and n == seg:
+            population_control_sharded(ctx, phi, weight, ovlp, theta, fb, us[k], group=group)
+            k += 1
+    return energies

@@ -355,3 +355,41 @@ def test_sharded_comb_emulated_ranks(world):
         assert np.array_equal(pm.cpu().numpy(), par_o)
         for k in ("phi", "theta", "f", "S", "w"):
             assert np.array_equal(g2[k], ref[k]), k
+
+
+def test_mixed_sums_and_sharded_run_single_rank():
+    """afqmc_mixed_sums against the oracle's mixed estimator; dist.run_sharded with one rank (no collective) leaves
+    exactly the state afqmc_run leaves with the same schedule, and its energies are the oracle's mixed estimator of the
+    device's own measurements."""
+    import torch
+    from paper_1804_03310_b200 import dist as D
+    wl = make_workload(2, "tame")
+    nw, steps = 1031, 8
+    ctx = H.make_ctx(wl, nw)
+    rng = np.random.default_rng(3)
+    w = rng.random(nw); w[::7] = 0.0
+    e = rng.standard_normal(nw) + 1j * rng.standard_normal(nw)
+    e[::7] = np.nan                                        # dead walkers may carry garbage energies
+    out3 = torch.zeros(3, dtype=torch.float64, device=ctx.device)
+    ctx.afqmc_mixed_sums(torch.tensor(w, device=ctx.device), torch.tensor(e, device=ctx.device), out3)
+    o = out3.cpu().numpy()
+    alive = w > 0
+    assert abs(o[0] - w.sum()) < 1e-12 * w.sum()
+    assert abs(o[1] / o[0] - orc.o_mixed_energy(w[alive], e[alive])) < 1e-12
+    assert abs(o[2] - np.sum(w[alive] * e[alive].imag)) < 1e-11
+    xs = wl.fields(steps, nw)
+    xd = torch.tensor(np.ascontiguousarray(xs), dtype=ctx.rdtype, device=ctx.device)
+    us = [0.3, 0.85]
+    a = H.DeviceState(ctx, wl.walkers(nw)); a.seed()
+    eloc = torch.zeros(2, nw, dtype=torch.complex128, device=ctx.device)
+    wm = torch.zeros(2, nw, dtype=torch.float64, device=ctx.device)
+    ctx.afqmc_run(a.phi, a.weight, a.ovlp, a.theta, a.fb, xd, steps, 4, 2, 4, us, eloc, wm, None, a.flags)
+    b = H.DeviceState(ctx, wl.walkers(nw)); b.seed()
+    en = D.run_sharded(ctx, b.phi, b.weight, b.ovlp, b.theta, b.fb, xd, steps, 4, 2, 4, us, flags=b.flags)
+    ha, hb = a.host(), b.host()
+    for k in ("phi", "w", "S", "theta", "f"):
+        assert np.array_equal(ha[k], hb[k]), k
+    assert len(en) == 2
+    for j in range(2):
+        ref = orc.o_mixed_energy(wm[j].cpu().numpy(), eloc[j].cpu().numpy())
+        assert abs(en[j].real - ref) < 1e-10 * abs(ref)
