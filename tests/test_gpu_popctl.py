@@ -393,3 +393,49 @@ def test_mixed_sums_and_sharded_run_single_rank():
     for j in range(2):
         ref = orc.o_mixed_energy(wm[j].cpu().numpy(), eloc[j].cpu().numpy())
         assert abs(en[j].real - ref) < 1e-10 * abs(ref)
+
+
+@pytest.mark.parametrize("precision", ["c128", "c64"])
+def test_long_run_on_gpu_vs_fci(precision):
+    """The whole CUDA path end to end against brute-force FCI (the north_star's validation, here on the GPU): cfg 1
+    shapes, `tame_mf` inputs, dt = 0.05, 640 walkers (complex128: FP64 SIMT path; complex64: the FP32 / 3xTF32 tcgen05
+    path, the paper's single-precision claim PAPER.md:135), 700 steps in ONE afqmc_run call with E_L every step,
+    orthonormalisation every 5 and comb every 10 steps (the recipe of the oracle's pin P10b).  The mixed estimator over the
+    last 500 steps must agree with the lowest eigenvalue of the sector Hamiltonian within 3 sigma (reblocked) plus 2 % of
+    the correlation energy (the phaseless bias allowance of P10b)."""
+    import dataclasses
+    import torch
+    from tests.fockspace import sector_one_body_ops
+    from tests.test_oracle_fci import _sector_hamiltonian
+    wl = dataclasses.replace(make_workload(1, "tame_mf"), dt=0.05, precision=precision)
+    fk, idx, E = sector_one_body_ops(wl.M, 2, 2)
+    Hs = _sector_hamiltonian(wl, E) + wl.e_const * np.eye(idx.size)
+    e_fci = np.linalg.eigvalsh(Hs)[0]
+    nw, n_steps, n_eq = 640, 700, 200
+    rng = np.random.default_rng(12345)
+    xs = rng.standard_normal((n_steps, nw, wl.n_chol))
+    us = rng.random(n_steps // 10)
+    ini = orc.o_init(wl.h, wl.L, wl.dt, wl.psi_a, wl.psi_b)
+    e_hf = orc.o_seed_state(ini, wl.walkers(1), 2).eloc[0].real
+    ctx = H.make_ctx(wl, nw, E0=e_hf)
+    st = H.DeviceState(ctx, wl.walkers(nw))
+    st.seed()
+    xd = torch.tensor(xs, dtype=ctx.rdtype, device=ctx.device)
+    eloc = torch.zeros(n_steps, nw, dtype=torch.complex128, device=ctx.device)
+    wm = torch.zeros(n_steps, nw, dtype=torch.float64, device=ctx.device)
+    ctx.afqmc_run(st.phi, st.weight, st.ovlp, st.theta, st.fb, xd, n_steps, 1, 5, 10, us, eloc, wm, None, st.flags)
+    torch.cuda.synchronize()
+    eloc, wm = eloc.cpu().numpy(), wm.cpu().numpy()
+    assert np.all(np.isfinite(wm)) and np.all(wm.sum(axis=1) > 0)
+    num = np.sum(wm * eloc.real, axis=1)[n_eq:]
+    den = wm.sum(axis=1)[n_eq:]
+    e_mix = num.sum() / den.sum() + wl.e_const
+    nb = 20
+    blocks = np.array([b.sum() for b in np.array_split(num, nb)]) / np.array(
+        [b.sum() for b in np.array_split(den, nb)]) + wl.e_const
+    sigma = blocks.std(ddof=1) / np.sqrt(nb)
+    corr = abs(e_hf + wl.e_const - e_fci)
+    print(f"GPU long run ({precision}, gemm_path {ctx.gemm_path}): E_mix {e_mix:.6f} +- {sigma:.6f}, E_FCI {e_fci:.6f}, E_HF {e_hf + wl.e_const:.6f}")
+    assert e_fci < e_hf + wl.e_const
+    assert abs(e_mix - e_fci) <= 3 * sigma + 0.02 * corr, (e_mix, e_fci, sigma)
+    assert abs(e_mix - e_fci) < 0.2 * corr
