@@ -15,7 +15,7 @@ __device__ inline void group_gauss_jordan(zcplx* aug, int n, int ld, zcplx* work
   (void)ctrl;
   zcplx* fac = work;
   zcplx* prow = work + n;
-  const int lane = gtid & 31;
+  const int lane = gtid & 31, gwarp = gtid >> 5;
   double dre = 1.0, dim = 0.0;
   sing = 0;
   double thresh = 0.0;
@@ -63,19 +63,22 @@ __device__ inline void group_gauss_jordan(zcplx* aug, int n, int ld, zcplx* work
     for (int c = gtid; c < 2 * n; c += 128) prow[c] = cmul(cur[piv * lc + c], ip);
     for (int r = gtid; r < n; r += 128) fac[r] = cur[(r == col ? piv : (r == piv ? col : r)) * lc + col];
     asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
-    // new row r <- (row col <-> row piv swapped) - fac[r] * prow ; new row col <- prow
-    for (int e = gtid; e < n * 2 * n; e += 128) {
-      const int r = e / (2 * n), c = e - r * 2 * n;
-      zcplx v;
-      if (r == col) v = prow[c];
-      else {
-        const int src = (r == piv) ? col : r;            // the old row `col` moves to position piv
-        v = cur[src * lc + c];
-        const zcplx f = fac[r], pr = prow[c];
-        v.x = fma(-f.x, pr.x, v.x); v.x = fma(f.y, pr.y, v.x);
-        v.y = fma(-f.x, pr.y, v.y); v.y = fma(-f.y, pr.x, v.y);
+    // new row r <- (row col <-> row piv swapped) - fac[r] * prow ; new row col <- prow.  2-D mapping, no division:
+    // lane = column (the scaled pivot-row entry is loaded once per step), the group's four warps stride over the rows
+    for (int c = lane; c < 2 * n; c += 32) {
+      const zcplx pr = prow[c];
+      for (int r = gwarp; r < n; r += 4) {
+        zcplx v;
+        if (r == col) v = pr;
+        else {
+          const int src = (r == piv) ? col : r;            // the old row `col` moves to position piv
+          v = cur[src * lc + c];
+          const zcplx f = fac[r];
+          v.x = fma(-f.x, pr.x, v.x); v.x = fma(f.y, pr.y, v.x);
+          v.y = fma(-f.x, pr.y, v.y); v.y = fma(-f.y, pr.x, v.y);
+        }
+        nxt[r * ln + c] = v;
       }
-      nxt[r * ln + c] = v;
     }
     asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
     zcplx* t = cur; cur = nxt; nxt = t;
