@@ -121,7 +121,7 @@ class ClockSampler(threading.Thread):
                     samples=len(sm), power_w_max=max(pw) if pw else None)
 
 
-def time_oracle(wl, target_s=12.0):
+def time_oracle(wl, target_s=12.0, one_thread_s=0.0):
     """The FP64 numpy oracle as it stands, on the host cores: walker-steps/s on a bounded sample."""
     from oracle import afqmc_oracle as orc
     from tests import gpu_harness as H
@@ -140,9 +140,29 @@ def time_oracle(wl, target_s=12.0):
             break
         if dt < 1.0 and nw < wl.n_walkers:
             nw = min(wl.n_walkers, nw * 4)
-    return dict(value=done / t_total, unit=UNIT, cores=cores, kind="oracle",
-                sample=f"{nsteps} oracle step(s) over {done} walker-steps of {workload_name(wl)} "
-                       f"({t_total:.1f} s CPU wall, numpy/BLAS threads = all {cores} cores, init excluded)")
+    out = dict(value=done / t_total, unit=UNIT, cores=cores, kind="oracle",
+               sample=f"{nsteps} oracle step(s) over {done} walker-steps of {workload_name(wl)} "
+                      f"({t_total:.1f} s CPU wall, numpy/BLAS threads = all {cores} cores, init excluded)")
+    if one_thread_s > 0:
+        # the paper's comparator is ONE CPU core in double precision: same oracle, BLAS limited to 1 thread
+        try:
+            from threadpoolctl import threadpool_limits
+            n1 = min(wl.n_walkers, 4)
+            ost = orc.o_seed_state(ini, wl.walkers(n1), wl.n_alpha, trial=trial)
+            x = wl.fields(1, n1)[0]
+            d1, t1 = 0, 0.0
+            with threadpool_limits(limits=1):
+                while t1 < one_thread_s:
+                    t0 = time.perf_counter()
+                    orc.o_step(ini, ost, x, wl.n_alpha, K=wl.K, E0=wl.E0, trial=trial)
+                    t1 += time.perf_counter() - t0
+                    d1 += n1
+            out["value_1thread"] = d1 / t1
+            out["sample_1thread"] = f"{d1} walker-steps in {t1:.1f} s with BLAS limited to 1 thread (threadpoolctl)"
+        except Exception as e:          # the baseline is a reported figure only
+            out["value_1thread"] = None
+            out["sample_1thread"] = f"unavailable: {e}"
+    return out
 
 
 def run_reference(args):
@@ -355,7 +375,7 @@ def run_ours(args):
     stage_tflops = {k: (fl[k] * nw / (stage_ms[k] * 1e-3) / 1e12 if stage_ms.get(k) else None) for k in fl}
     base = None
     if not args.no_cpu_baseline:
-        base = time_oracle(wl, target_s=args.cpu_seconds)
+        base = time_oracle(wl, target_s=args.cpu_seconds, one_thread_s=min(6.0, args.cpu_seconds / 2))
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=K, warmup=W, ms_per_step=ms_max / K,
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype=dtype, data="synthetic",
                 config=dict(workload=workload_name(wl), variant=args.variant, global_walkers=world * nw,

@@ -55,7 +55,7 @@ __device__ inline void group_gauss_jordan(zcplx* aug, int n, int ld, zcplx* work
         dim = dre * p.y + dim * p.x;
         dre = nr;
         piv = idx;
-        ip = cinv(p);
+        if (gtid < 2 * n) ip = cinv(p);     // only the threads that scale the pivot row need the FP64 reciprocal
       }
     }
     if (piv < 0) break;                                   // exactly singular: uniform exit (all warps agree)
