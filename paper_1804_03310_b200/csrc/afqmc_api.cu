@@ -544,7 +544,7 @@ template <typename T> afqmc_status run_md_energy(afqmc_ctx* c, const void* theta
   return AFQMC_OK;
 }
 
-template <typename T> afqmc_status run_energy_gemm(afqmc_ctx* c, zcplx* eloc) {
+template <typename T> afqmc_status run_energy_gemm(afqmc_ctx* c, const void* theta, zcplx* eloc) {
   StageScope sc(c, AFQMC_STAGE_ENERGY);
   for (int s = 0; s < 2; ++s) {
     int n = s ? c->nb : c->na, soff = s ? c->KA : 0, Ks = s ? c->KB : c->KA;
@@ -552,7 +552,7 @@ template <typename T> afqmc_status run_energy_gemm(afqmc_ctx* c, zcplx* eloc) {
     if constexpr (sizeof(T) == 4) {
       if (c->path == 2) {
         tc::EpiEnergy e2;
-        e2.thp = (const float*)c->thp; e2.thp_lo = (const float*)c->thp_lo; e2.KT = c->KT; e2.soff = soff;
+        e2.theta = (const float2*)theta; e2.M = c->M; e2.nt = c->nt; e2.off = s ? c->na : 0; e2.n = n;
         e2.hrot = (const float*)c->hrot + soff; e2.eloc = (double*)eloc; e2.m_real = c->M * n; e2.n_real = 2 * c->nw;
         afqmc_status st2 = run_gemm_tc(c, c->map_en[s], c->M * n, 2 * c->nw, Ks, e2, 1);
         if (st2) return st2;
@@ -682,7 +682,7 @@ template <typename T> afqmc_status do_fb_energy_planar(afqmc_ctx* c, const void*
     return run_md_energy<T>(c, theta, eloc);
   }
   LAUNCH(c, k_fb_finish<T>, c->nw, 128, 0, c->ng, c->NGP, c->nw, (const T*)c->fs, (cplx<T>*)fb, eloc);
-  return run_energy_gemm<T>(c, eloc);
+  return run_energy_gemm<T>(c, theta, eloc);
 }
 
 // E_L from an interleaved Theta handed in by the caller

@@ -287,26 +287,33 @@ struct EpiTT {          // H10: row = g*nact + q, col = (w*nt + a)*2 + p -> TT[w
     }
   }
 };
-struct EpiEnergy {      // H9: eloc[w] += sum_rows v[row] (0.5 C[row][w] + hrot[row]), v = Theta plane (hi + lo)
+struct EpiEnergy {      // H9: eloc[w] += sum_rows v[row] (0.5 C[row][w] + hrot[row]), v = Theta of the walker
   static constexpr bool kStaged = false;
-  const float* thp; const float* thp_lo; int KT, soff; const float* hrot; double* eloc; int m_real, n_real;
+  // v is read from the interleaved Theta [N_w][M][N_t] (one 8-byte load per element: Re and Im together) rather than
+  // from the four planar hi/lo operands: the epilogue is bound by the latency of its loads (ncu / tri = 0 experiment:
+  // ~40 us per tile with 64 loads per 32 x 32 block, profiles/r1b_ncu_full.md), and this needs a quarter of them
+  const float2* theta; int M, nt, off, n;      // row r of the spin block = (orbital k = r / n, column off + r % n)
+  const float* hrot; double* eloc; int m_real, n_real;
   __device__ __forceinline__ void operator()(int r, int c0, const float (&v)[32]) const {
     const bool rok = r < m_real;
     const float hr = rok ? hrot[r] : 0.f;
     const int lane = threadIdx.x & 31;
+    const int k = r / n, a = r - k * n;
+    const float2* tp = theta + (size_t)k * nt + off + a;
+    const size_t wstride = (size_t)M * nt;
+    float2 t[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+      const int c = c0 + 2 * j;
+      t[j] = (rok && c < n_real) ? tp[(size_t)(c >> 1) * wstride] : make_float2(0.f, 0.f);
+    }
     float x[32];             // x[2p] / x[2p+1] = this row's contribution to Re / Im of walker (c0/2 + p)
 #pragma unroll
     for (int j = 0; j < 32; j += 2) {
-      const int c = c0 + j;
-      float er = 0.f, ei = 0.f;
-      if (rok && c < n_real) {
-        const size_t o = (size_t)c * KT + soff + r;
-        const float vr = thp[o] + thp_lo[o], vi = thp[o + KT] + thp_lo[o + KT];
-        const float ur = v[j] + hr, ui = v[j + 1];   // v = Y' Theta with Y' = triu(Y), diag / 2: Theta^T Y' Theta = 1/2 Theta^T Y Theta
-        er = vr * ur - vi * ui;
-        ei = vr * ui + vi * ur;
-      }
-      x[j] = er; x[j + 1] = ei;
+      const float vr = t[j >> 1].x, vi = t[j >> 1].y;
+      const float ur = v[j] + hr, ui = v[j + 1];   // v = Y' Theta with Y' = triu(Y), diag / 2: Theta^T Y' Theta = 1/2 Theta^T Y Theta
+      x[j] = vr * ur - vi * ui;
+      x[j + 1] = vr * ui + vi * ur;
     }
     // transpose-reduce over the 32 rows of this warp: 31 shuffles, lane l ends with the sum of x[l]
 #pragma unroll
