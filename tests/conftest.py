@@ -16,3 +16,12 @@ def pytest_configure(config):
 @pytest.fixture(scope="session")
 def repo_root():
     return ROOT
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _library_built():
+    """The in-tree CUDA library is a build artefact (git-ignored): compile it once if it is not there.  A missing
+    nvcc or a compile error fails the session loudly -- there is no CPU fallback to fall back to."""
+    from paper_1804_03310_b200 import build as b
+    if not os.path.exists(b.LIB):
+        b.build()
