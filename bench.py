@@ -336,7 +336,7 @@ def run_ours(args):
         fl["assemble"] = 4.0 * ng_ * M_ * (M_ + 1) / 2
         peak, peak_note = 0.5 * pk["bf16_burst"], (
             f"TF32 dense = {pk['source']} burst BF16 {pk['bf16_burst']} TF/s x nominal TF32/BF16 ratio 0.5 (each kernel runs "
-            f"1-2 ms inside a ~5 ms step, no power-cap reason active; sustained figure would be {0.5 * pk['bf16_sust']:.0f}); "
+            f"0.2-1.6 ms inside a ~3.4 ms step, no power-cap reason active; sustained figure would be {0.5 * pk['bf16_sust']:.0f}); "
             "achieved counts ALGORITHMIC flops and 3xTF32 issues 3x of them, so frac <= 1/3 by construction")
         bound, dtype = "tensor", "tf32x3"
     else:
