@@ -17,6 +17,8 @@ Pins (tests/test_oracle_*.py, all `-m "not gpu"`):
   o_local_energy         P3  Hartree-Fock closed form, Fock space, Y-form == Cholesky form
   o_propagate            P4  Thouless theorem in Fock space, Taylor vs scipy expm bound
   o_step weights         P5  force-bias sign: odd-in-x part of log I cancels
+  o_weight               P15 hand-derived values of the phaseless rule, hybrid and local-energy form (both modes),
+                             kill boundary at arg(rho) = +-pi/2, dead walkers stay dead, no overflow at |rho| = 1e200
   multi-det SMW          P6  Eq. (4) == direct recomputation
   Cholesky <-> V         P7  pivoted Cholesky reproduces V and the energies
   multi-det mixed        P8  Fock-space brute force;  P9 FCI trial => E_L == E_FCI
@@ -182,7 +184,10 @@ def o_weight(S_old, S_new, c, w, dt, E0, mode=0, E_pre=None):
         fac = np.exp(dt * E0) * absI
     else:
         fac = np.exp(-dt * (E_pre.real - E0))
-    killed = (cosd <= 0.0) | (w == 0.0)            # a dead walker stays dead (0 * anything = 0)
+    # max{0, cos dtheta}: cos dtheta = Re(rho)/|rho|, so the walker is killed iff Re(rho) <= 0.  The
+    # decision is taken on Re(rho) itself (reading R6b): cos(atan2(y, x)) in floating point is 6e-17 > 0 at x = 0 and
+    # for tiny negative x, i.e. it misses exactly the boundary the rule is about.
+    killed = (rho.real <= 0.0) | (w == 0.0)        # a dead walker stays dead (0 * anything = 0)
     with np.errstate(invalid="ignore", over="ignore"):
         w_new = np.where(killed, 0.0, w * fac * cosd)
     return w_new, absI, cosd

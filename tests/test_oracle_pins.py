@@ -184,6 +184,89 @@ def test_P5_importance_function(small):
     assert np.abs(odd_with).mean() < 0.1 * np.abs(odd_without).mean()
 
 
+def test_P15_weight_rule_hand_values():
+    """o_weight against values derived by hand from PAPER.md:53 (dtheta = Im ln(S'/S), factor max{0, cos dtheta}),
+    :97 (hybrid: weights from the overlap ratio), :51 (local-energy form e^{-dt E_L}), :34 (projector e^{dt(E_0 - H)}).
+    Every expected number is a literal worked out on paper (30-digit values, rounded), not a re-evaluation of the formula:
+      hybrid  w' = w e^{dt E0} |rho| e^{Re c} cos(arg rho)     (readings R5, R6: the phase is arg(rho), NOT arg(rho e^c))
+      mode 1  w' = w e^{-dt (Re E_pre - E0)} cos(arg rho)
+    A plausible mistake -- arg(rho e^c) instead of arg(rho), Im c leaking into |I|, a missing or mis-signed e^{dt E0},
+    cos < 0 not clamped, <= vs < at the boundary, |rho| formed before the log -- fails at least one line."""
+    z = lambda m, a: m * np.exp(1j * a)
+    one = np.ones(1)
+    # (1) rho = 2 e^{i pi/3}, c = 0.1 + 0.2i, E0 = 0.5, dt = 0.01, w = 3  ->  3 e^{0.005} 2 e^{0.1} (1/2) = 3 e^{0.105}
+    w1, absI, cosd = O.o_weight(np.array([1.0 + 0j]), np.array([z(2.0, np.pi / 3)]), np.array([0.1 + 0.2j]), 3 * one, 0.01, 0.5)
+    assert abs(w1[0] - 3.33213183106711570) < 1e-14
+    assert abs(absI[0] - 2 * 1.10517091807564763) < 1e-14          # |rho| e^{Re c} = 2 e^{0.1}; Im c does not enter
+    assert abs(cosd[0] - 0.5) < 1e-15
+    # with arg(rho e^c) the phase would be pi/3 + 1.2 > pi/2 and the walker would be (wrongly) killed:
+    w1b = O.o_weight(np.array([1.0 + 0j]), np.array([z(2.0, np.pi / 3)]), np.array([0.1 + 1.2j]), 3 * one, 0.01, 0.5)[0]
+    assert abs(w1b[0] - 3.33213183106711570) < 1e-14
+    # (2) the ratio matters, not S' alone: S = 4 e^{i 0.7}, S' = 20 e^{i(0.7 - pi/4)}  ->  rho = 5 e^{-i pi/4};
+    #     c = -1.5 - 2i, E0 = -2, dt = 0.02, w = 1/4  ->  (1/4) e^{-0.04} 5 e^{-1.5} / sqrt(2)
+    w2 = O.o_weight(np.array([z(4.0, 0.7)]), np.array([z(20.0, 0.7 - np.pi / 4)]), np.array([-1.5 - 2.0j]), 0.25 * one, 0.02, -2.0)[0]
+    assert abs(w2[0] - 0.189487913221571439) < 1e-15
+    # (3) the kill boundary: arg(rho) = +-pi/2 exactly (Re rho = 0) and beyond -> weight exactly 0
+    for rho in (1.7j, -1.7j, -0.3 + 2j, -0.3 - 2j, -1.0 + 0j, -1e-300 + 1j):
+        wk, _, _ = O.o_weight(np.array([1.0 + 0j]), np.array([rho]), np.array([0j]), one, 0.01, 0.0)
+        assert wk[0] == 0.0, rho
+    #     just inside: Re rho = +1e-300 survives with a tiny positive weight
+    wk = O.o_weight(np.array([1.0 + 0j]), np.array([1e-300 + 1j]), np.array([0j]), one, 0.01, 0.0)[0]
+    assert wk[0] >= 0.0 and np.isfinite(wk[0])
+    # (4) a dead walker stays dead whatever happens next (both modes)
+    for mode in (0, 1):
+        wd = O.o_weight(np.array([1.0 + 0j]), np.array([z(2.0, 0.1)]), np.array([0.3 + 0j]), 0 * one, 0.01, 0.0, mode=mode,
+                        E_pre=np.array([-5.0 + 0j]))[0]
+        assert wd[0] == 0.0
+    # (5) mode 1 (PAPER.md:51): E_pre = -3.2 + 0.7i, E0 = -3, dt = 0.05, w = 1, rho = 2 e^{i pi/3}, c = 0.4 + 0.9i
+    #     -> e^{-0.05 (-0.2)} cos(pi/3) = e^{0.01} / 2; neither |rho|, nor c, nor Im E_pre enter, and arg(rho e^c) =
+    #     pi/3 + 0.9 > pi/2 would kill it
+    w5, absI5, cos5 = O.o_weight(np.array([1.0 + 0j]), np.array([z(2.0, np.pi / 3)]), np.array([0.4 + 0.9j]), one, 0.05, -3.0,
+                                 mode=1, E_pre=np.array([-3.2 + 0.7j]))
+    assert abs(w5[0] - 0.505025083542084029) < 1e-15
+    assert abs(cos5[0] - 0.5) < 1e-15
+    #     sign of the exponent: lowering the local energy raises the weight, raising E0 raises it too
+    lo = O.o_weight(np.array([1.0 + 0j]), np.array([1.0 + 0j]), np.array([0j]), one, 0.05, 0.0, mode=1, E_pre=np.array([-10.0 + 0j]))[0]
+    hi = O.o_weight(np.array([1.0 + 0j]), np.array([1.0 + 0j]), np.array([0j]), one, 0.05, 0.0, mode=1, E_pre=np.array([+10.0 + 0j]))[0]
+    assert abs(lo[0] - 1.64872127070012815) < 1e-14 and abs(hi[0] - 0.606530659712633424) < 1e-15       # e^{+-1/2}
+    # (6) dynamic range (R17): |rho| = 1e200, c = -455.5 + 3i -> |I| = e^{200 ln 10 - 455.5} = 150.9605582131972579,
+    #     cos(0.3) = 0.955336489125606020
+    w6, absI6, _ = O.o_weight(np.array([1e-100 + 0j]), np.array([z(1e100, 0.3)]), np.array([-455.5 + 3j]), one, 0.01, 0.0)
+    assert abs(absI6[0] / 150.9605582131972579 - 1) < 1e-12
+    assert abs(w6[0] / (150.9605582131972579 * 0.955336489125606020) - 1) < 1e-12
+
+
+def test_P15_weight_modes_agree_to_first_order(small):
+    """Link between the two forms (PAPER.md:51 vs :97): for a walker stepped with x and -x the geometric mean of the
+    hybrid factors |I(x)||I(-x)| equals e^{-2 dt Re E_L} up to O(dt^2), i.e. the hybrid weight is the local-energy weight
+    to first order in dt; and e^{dt E0} multiplies both forms alike."""
+    wl, _, _ = small
+    dt = 2e-4
+    ini = O.o_init(wl.h, wl.L, dt, wl.psi_a, wl.psi_b)
+    phi = random_walkers(wl, 1, seed=31, spread=0.2)
+    n = 4000
+    phi = np.ascontiguousarray(np.broadcast_to(phi[0], (n,) + phi[0].shape))
+    st = O.o_seed_state(ini, phi, wl.n_alpha)
+    x = np.random.default_rng(5).standard_normal((n // 2, wl.n_chol))
+    x = np.concatenate([x, -x])
+    _, rec0 = O.o_step(ini, st, x, wl.n_alpha, K=8, E0=0.0, mode=0)
+    _, rec1 = O.o_step(ini, st, x, wl.n_alpha, K=8, E0=0.0, mode=1)
+    # E_x[log|I|] = -dt Re E_L + O(dt^2) (the O(sqrt dt) term is removed by the force bias, the O(dt) fluctuation by the pairs)
+    mean_log = np.mean(np.log(rec0["absI"]))
+    sem = np.std(0.5 * (np.log(rec0["absI"][: n // 2]) + np.log(rec0["absI"][n // 2:]))) / np.sqrt(n // 2)
+    assert abs(mean_log + dt * st.eloc[0].real) < 5 * sem + 20 * dt * dt * abs(st.eloc[0]) ** 2
+    assert np.allclose(rec1["w"] / rec1["cosd"], np.exp(-dt * st.eloc[0].real), rtol=1e-12)
+    # E0 enters both modes as the same factor e^{dt E0}
+    for mode in (0, 1):
+        _, ra = O.o_step(ini, OracleStateCopy(st, 8), x[:8], wl.n_alpha, K=8, E0=0.0, mode=mode)
+        _, rb = O.o_step(ini, OracleStateCopy(st, 8), x[:8], wl.n_alpha, K=8, E0=7.5, mode=mode)
+        assert np.allclose(rb["w"], ra["w"] * np.exp(dt * 7.5), rtol=1e-12)
+
+
+def OracleStateCopy(st, n):
+    return O.OracleState(st.phi[:n], st.w[:n], st.S[:n], st.theta[:n], st.f_a[:n], st.f_b[:n], st.eloc[:n])
+
+
 def test_P6_smw_identity():
     """Eq. (4) == direct recomputation for rank 0, 1, 2."""
     rng = np.random.default_rng(0)
