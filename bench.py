@@ -124,9 +124,9 @@ class ClockSampler(threading.Thread):
 def time_oracle(wl, target_s=12.0, one_thread_s=0.0):
     """The FP64 numpy oracle as it stands, on the host cores: walker-steps/s on a bounded sample."""
     from oracle import afqmc_oracle as orc
-    from tests import gpu_harness as H
     cores = len(os.sched_getaffinity(0))
-    ini, trial = H.oracle_init(wl)
+    ini = orc.o_init(wl.h, wl.L, wl.dt, wl.psi_a, wl.psi_b)
+    trial = orc.MultiDetTrial(wl.C_act, wl.det_coeff, wl.det_exc, wl.n_alpha, wl.n_beta) if wl.n_det > 1 else None
     nw = min(wl.n_walkers, 8)
     done, t_total, nsteps = 0, 0.0, 0
     while True:
@@ -187,7 +187,7 @@ def run_reference(args):
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from tests import gpu_harness as H
+    from paper_1804_03310_b200.state import WalkerState
     from workloads import make_workload
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -213,7 +213,7 @@ def run_ours(args):
     nfield = min(K, 8)
     x = torch.tensor(rng.standard_normal((nfield, nw, wl.n_chol)), dtype=ctx.rdtype, device=dev)
     phi0 = torch.tensor(wl.walkers(nw), dtype=ctx.cdtype, device=dev)
-    st = H.DeviceState(ctx, wl.walkers(nw))
+    st = WalkerState(ctx, wl.walkers(nw))
     eloc = torch.zeros(1, nw, dtype=torch.complex128, device=dev)
 
     def reseed():

@@ -162,7 +162,9 @@ AFQMC_API afqmc_status afqmc_orthonormalize(afqmc_ctx* ctx, void* phi, void* ovl
 /* "Simple combing" population control (NEXT-1; reading R22): W = sum_w weight, teeth
  * t_i = (i + u) W / N_w, new walker i = copy of the first walker p whose running sum weight[0] + ... + weight[p]
  * (accumulated in index order, FP64) exceeds t_i; every new walker gets weight W / N_w.  phi, ovlp, theta, fb follow
- * their parent (in place; moved through scratch in work_mem).  u in [0, 1) is drawn by the caller (HOST value).
+ * their parent (in place; moved through scratch in work_mem); the caller's flags array is NOT permuted: flags[i] is the
+ * history of SLOT i (every event that happened to a walker while it sat there), not of a lineage.
+ * u in [0, 1) is drawn by the caller (HOST value).
  * parent (DEVICE int32 [N_w], may be NULL) receives the map.  W == 0 or non-finite: nothing moves, weights kept.
  * All other pointers DEVICE.  Errors: EINVAL (null, u outside [0, 1)). */
 AFQMC_API afqmc_status afqmc_population_control(afqmc_ctx* ctx, void* phi, double* weight, void* ovlp, void* theta, void* fb,
@@ -195,6 +197,11 @@ AFQMC_API afqmc_status afqmc_comb_unpack(afqmc_ctx* ctx, const void* recvbuf, vo
  * weight exactly 0 contribute nothing (their E_L may be non-finite).  E_mix = out3[1] / out3[0]; across ranks the three
  * numbers are what is all-reduced.  An empty batch writes zeros.  All DEVICE. */
 AFQMC_API afqmc_status afqmc_mixed_sums(afqmc_ctx* ctx, const double* weight, const void* eloc, double* out3);
+
+/* The mixed estimator itself: e_mix[m] = (sums[m][1] + i sums[m][2]) / sums[m][0] for n measurements, sums
+ * [n][3] as written by afqmc_mixed_sums (and, for a sharded population, all-reduced across ranks first).  A dead
+ * population (sum of weights 0) gives NaN.  sums, e_mix (complex double [n]) DEVICE.  Errors: EINVAL. */
+AFQMC_API afqmc_status afqmc_mixed_energy(afqmc_ctx* ctx, const double* sums, int32_t n, void* e_mix);
 
 /* The paper's schedule around the walker step (NEXT-2; hybrid weights "to minimize evaluations of the
  * local energy, which is measured every 0.1 Ha^-1", orthonormalisation every 2 steps, population control every

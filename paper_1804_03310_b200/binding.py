@@ -21,7 +21,7 @@ SYMBOLS = ["afqmc_query_bytes", "afqmc_init", "afqmc_destroy", "afqmc_last_error
            "afqmc_force_bias", "afqmc_propagate", "afqmc_local_energy", "afqmc_step", "afqmc_step_host",
            "afqmc_launch_count", "afqmc_gemm_path", "afqmc_profile_enable", "afqmc_profile_read",
            "afqmc_orthonormalize", "afqmc_population_control", "afqmc_run", "afqmc_comb_record_bytes",
-           "afqmc_comb_map", "afqmc_comb_pack", "afqmc_comb_unpack", "afqmc_mixed_sums"]
+           "afqmc_comb_map", "afqmc_comb_pack", "afqmc_comb_unpack", "afqmc_mixed_sums", "afqmc_mixed_energy"]
 
 STAGES = ["shift", "assemble", "taylor", "green", "force_bias", "energy", "symmetrize", "ortho", "popctl"]
 
@@ -70,6 +70,8 @@ def load_library():
     lib.afqmc_run.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp, vp, i32p, i32p]
     lib.afqmc_mixed_sums.argtypes = [vp, vp, vp, vp]
     lib.afqmc_mixed_sums.restype = C.c_int
+    lib.afqmc_mixed_energy.argtypes = [vp, vp, C.c_int32, vp]
+    lib.afqmc_mixed_energy.restype = C.c_int
     lib.afqmc_comb_record_bytes.argtypes = [vp]
     lib.afqmc_comb_record_bytes.restype = C.c_size_t
     lib.afqmc_comb_map.argtypes = [vp, vp, C.c_int64, C.c_double, vp, i32p, vp]
@@ -222,6 +224,9 @@ class AfqmcContext:
 
     def afqmc_mixed_sums(self, weight, eloc, out3):
         self._chk(self._lib.afqmc_mixed_sums(self._ctx, _dp(weight), _dp(eloc), _dp(out3)))
+
+    def afqmc_mixed_energy(self, sums, n, e_mix):
+        self._chk(self._lib.afqmc_mixed_energy(self._ctx, _dp(sums), int(n), _dp(e_mix)))
 
     @property
     def afqmc_comb_record_bytes(self) -> int:

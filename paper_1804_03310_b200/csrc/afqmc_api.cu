@@ -51,7 +51,7 @@ struct afqmc_ctx {
   double *psid_ac, *psid_bc;   // FP64 trial orbitals (constants)
   void *thtil, *th_scr; zcplx *ovlp0, *ovlp_scr;
   void *RactT, *RactT_lo, *thT, *thT_lo, *TTg; int MPK; tc::Maps map_tt;
-  size_t mdo_smem, mde_smem;
+  size_t mdo_smem, mde_smem; int mde_attr_done;
   int tay_cw, tay_nch, tay_threads;
   size_t tay_smem, green_smem;
   // constants
@@ -146,6 +146,12 @@ int resolve_path(const afqmc_params* p) {
 }
 // the tcgen05 GEMMs run on CTA pairs unless gemm_path 2 asks for the one-CTA kernels
 int resolve_cta2(const afqmc_params* p) { return resolve_path(p) == 2 && p->gemm_path != 2; }
+// tensor-pipe Taylor kernel (taylor_tc.cuh): complex64 walkers on the tcgen05 path, 96 <= M <= 256, N_t <= 32.  Below
+// M = 96 a 128-row tile is mostly padding and the FP32 SIMT kernel is competitive and free of the tensor pipe's
+// truncation bias
+bool will_tay_tc(const afqmc_params* p) {
+  return resolve_path(p) == 2 && p->M >= 96 && p->M <= 256 && p->n_alpha + p->n_beta <= 32;
+}
 
 afqmc_status check_params(const afqmc_params* p, char* err) {
   if (!p) { snprintf(err, 256, "params is NULL"); return AFQMC_EINVAL; }
@@ -178,10 +184,12 @@ afqmc_status check_params(const afqmc_params* p, char* err) {
     snprintf(err, 256, "gemm_path 2/3 (tcgen05 3xTF32) needs precision 0 (complex64 walkers)");
     return AFQMC_EUNSUPPORTED;
   }
-  int cw, nch;
-  bool ok = p->precision ? taylor_pick<double>(p->M, p->n_alpha + p->n_beta, cw, nch)
-                         : taylor_pick<float>(p->M, p->n_alpha + p->n_beta, cw, nch);
-  if (!ok) { snprintf(err, 256, "M * ceil(N_t / chunk) exceeds one CTA (M too large for the Taylor kernel)"); return AFQMC_EUNSUPPORTED; }
+  if (!will_tay_tc(p)) {   // the one-CTA SIMT Taylor kernel's size limit applies only where the tensor-pipe kernel does not run
+    int cw, nch;
+    bool ok = p->precision ? taylor_pick<double>(p->M, p->n_alpha + p->n_beta, cw, nch)
+                           : taylor_pick<float>(p->M, p->n_alpha + p->n_beta, cw, nch);
+    if (!ok) { snprintf(err, 256, "M * ceil(N_t / chunk) exceeds one CTA (M too large for the SIMT Taylor kernel; the tensor-pipe kernel needs complex64, 96 <= M <= 256, N_t <= 32)"); return AFQMC_EUNSUPPORTED; }
+  }
   size_t gs = p->precision ? green_smem_bytes<double>(p->M, p->n_alpha, p->n_beta)
                            : green_smem_bytes<float>(p->M, p->n_alpha, p->n_beta);
   if (gs > 200 * 1024) { snprintf(err, 256, "walker does not fit one CTA's shared memory"); return AFQMC_EUNSUPPORTED; }
@@ -520,8 +528,9 @@ template <typename T> afqmc_status run_md_energy(afqmc_ctx* c, const void* theta
 #define MDB_LAUNCH(N, D)                                                                                           \
   {                                                                                                                \
     auto kern = k_md_energy_b<T, N, D>;                                                                            \
-    if (smb > 48 * 1024)                                                                                           \
+    if (smb > 48 * 1024 && !c->mde_attr_done)   /* once per context: the first energy call */                      \
       CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb));               \
+    c->mde_attr_done = 1;                                                                                          \
     LAUNCH(c, kern, c->nw, MD_THREADS, smb, a);                                                                    \
   }
 #define MDB_PICK(N)                                                                                                \
@@ -535,8 +544,9 @@ template <typename T> afqmc_status run_md_energy(afqmc_ctx* c, const void* theta
 #define MDE_LAUNCH(D)                                                                                              \
   {                                                                                                                \
     auto kern = k_md_energy<T, D>;                                                                                 \
-    if (c->mde_smem > 48 * 1024)                                                                                   \
+    if (c->mde_smem > 48 * 1024 && !c->mde_attr_done)                                                              \
       CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->mde_smem));       \
+    c->mde_attr_done = 1;                                                                                          \
     LAUNCH(c, kern, c->nw, MD_THREADS, c->mde_smem, a);                                                            \
   }
   if (dpt <= 1) MDE_LAUNCH(1) else if (dpt <= 2) MDE_LAUNCH(2) else if (dpt <= 4) MDE_LAUNCH(4) else MDE_LAUNCH(8)
@@ -587,8 +597,6 @@ template <typename T> afqmc_status run_taylor(afqmc_ctx* c, void* phi) {
     constexpr int MT = sizeof(T) == 4 ? (((CW + 3) & ~3) >= 16 ? 448 : ((CW + 3) & ~3) >= 12 ? 576 : ((CW + 3) & ~3) >= 8 ? 768 : 1024) \
                                       : (((CW + 3) & ~3) >= 8 ? 448 : 768);                                 \
     auto kern = k_taylor<T, CW, MT>;                                                                        \
-    if (c->tay_smem > 48 * 1024)                                                                            \
-      CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tay_smem)); \
     LAUNCH(c, kern, c->nw, c->tay_threads, c->tay_smem, g);                                                 \
   } break;
   switch (c->tay_cw) {
@@ -605,6 +613,28 @@ template <typename T> afqmc_status run_taylor(afqmc_ctx* c, void* phi) {
   }
 #undef TAY_CASE
   return AFQMC_OK;
+}
+
+// dynamic shared-memory opt-in of the SIMT Taylor instantiation that run_taylor will launch (called once, from afqmc_init)
+template <typename T> cudaError_t set_taylor_smem(int cw, size_t smem) {
+#define TAY_SET(CW)                                                                                          \
+  case CW: {                                                                                                \
+    constexpr int MT = sizeof(T) == 4 ? (((CW + 3) & ~3) >= 16 ? 448 : ((CW + 3) & ~3) >= 12 ? 576 : ((CW + 3) & ~3) >= 8 ? 768 : 1024) \
+                                      : (((CW + 3) & ~3) >= 8 ? 448 : 768);                                 \
+    return cudaFuncSetAttribute(k_taylor<T, CW, MT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+  }
+  switch (cw) {
+    TAY_SET(1) TAY_SET(2) TAY_SET(3) TAY_SET(4) TAY_SET(5) TAY_SET(6) TAY_SET(7) TAY_SET(8)
+    default:
+      if constexpr (sizeof(T) == 4) {
+        switch (cw) {
+          TAY_SET(9) TAY_SET(10) TAY_SET(11) TAY_SET(12) TAY_SET(13) TAY_SET(14) TAY_SET(15) TAY_SET(16)
+          default: break;
+        }
+      }
+  }
+#undef TAY_SET
+  return cudaErrorInvalidValue;
 }
 
 template <typename T>
@@ -644,7 +674,7 @@ afqmc_status do_propagate(afqmc_ctx* c, void* phi, const void* x, const void* fb
     if (!st && c->path == 2 && c->M % 4 != 0) {
       StageScope sc(c, AFQMC_STAGE_SYMMETRIZE);
       const int nt32 = (c->M + 31) / 32;
-      dim3 sg(nt32 * (nt32 + 1) / 2, c->nw);
+      dim3 sg(c->nw, nt32 * (nt32 + 1) / 2);   // walkers on grid x (no 65535 cap)
       LAUNCH(c, k_symmetrize<float>, sg, dim3(32, 8), 0, c->M, c->MP, (float*)c->Abuf,
              c->tay_tc ? (float*)c->Abuf_lo : (float*)nullptr);
     }
@@ -871,20 +901,26 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
   }
   size_t cb, wb;
   carve(p, c, (char*)const_mem, (char*)work_mem, &cb, &wb);
-  if (p->precision) {
-    taylor_pick<double>(c->M, c->nt, c->tay_cw, c->tay_nch);
-    c->tay_smem = taylor_smem_bytes<double>(c->M, c->MP, c->tay_nch, (c->tay_cw + 3) & ~3);
-    c->green_smem = green_smem_bytes<double>(c->M, c->na, c->nb);
-  } else {
-    taylor_pick<float>(c->M, c->nt, c->tay_cw, c->tay_nch);
-    c->tay_smem = taylor_smem_bytes<float>(c->M, c->MP, c->tay_nch, (c->tay_cw + 3) & ~3);
-    c->green_smem = green_smem_bytes<float>(c->M, c->na, c->nb);
-  }
-  c->tay_threads = (int)rup((size_t)c->M * c->tay_nch, 32);
-  if (c->tay_smem > 227 * 1024) {
-    s = fail(nullptr, AFQMC_EUNSUPPORTED, "Taylor kernel tile exceeds shared memory");
-    delete c;
-    return s;
+  c->tay_tc = will_tay_tc(p) && c->nw > 0;
+  c->green_smem = p->precision ? green_smem_bytes<double>(c->M, c->na, c->nb) : green_smem_bytes<float>(c->M, c->na, c->nb);
+  if (!will_tay_tc(p)) {
+    if (p->precision) {
+      taylor_pick<double>(c->M, c->nt, c->tay_cw, c->tay_nch);
+      c->tay_smem = taylor_smem_bytes<double>(c->M, c->MP, c->tay_nch, (c->tay_cw + 3) & ~3);
+    } else {
+      taylor_pick<float>(c->M, c->nt, c->tay_cw, c->tay_nch);
+      c->tay_smem = taylor_smem_bytes<float>(c->M, c->MP, c->tay_nch, (c->tay_cw + 3) & ~3);
+    }
+    c->tay_threads = (int)rup((size_t)c->M * c->tay_nch, 32);
+    if (c->tay_smem > 227 * 1024) {
+      s = fail(nullptr, AFQMC_EUNSUPPORTED, "Taylor kernel tile exceeds shared memory");
+      delete c;
+      return s;
+    }
+    if (c->tay_smem > 48 * 1024) {
+      cudaError_t e = p->precision ? set_taylor_smem<double>(c->tay_cw, c->tay_smem) : set_taylor_smem<float>(c->tay_cw, c->tay_smem);
+      if (e != cudaSuccess) { snprintf(g_init_err, 256, "CUDA: %s", cudaGetErrorString(e)); delete c; return AFQMC_ECUDA; }
+    }
   }
   if (c->md) {
     c->mdo_smem = md_overlap_smem(c->M, c->na, c->nb, c->nact, c->ndet, c->ts);
@@ -916,7 +952,6 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
   }
   // tensor-pipe Taylor kernel for 96 <= M <= 256: below that a 128-row tile is mostly padding and the FP32 SIMT
   // kernel is both competitive and free of the tensor pipe's truncation bias
-  c->tay_tc = (c->path == 2 && c->M >= 96 && c->M <= 256 && c->nt <= 32 && c->nw > 0);
   if (c->tay_tc) {
     tt::TaylorTcArgs& a = c->tay_args;
     a.M = c->M; a.MP = c->MP; a.nt = c->nt; a.K = p->taylor_order; a.nw = c->nw;
@@ -1065,7 +1100,7 @@ afqmc_status afqmc_overlap_green(afqmc_ctx* c, const void* phi, void* ovlp, void
   afqmc_status s = DISPATCH(c, run_green, c, phi, ovlp, theta, 0, nullptr, nullptr, flags);
   if (s) return s;
   if (G_or_null) {
-    dim3 grid((c->M * c->M + 255) / 256, c->nw, 2);
+    dim3 grid(c->nw, (c->M * c->M + 255) / 256 < 65535 ? (c->M * c->M + 255) / 256 : 65535, 2);   // walkers on grid x (no 65535 cap)
     if (c->md) {   // mixed G_s^T = Thtil_s C_act^T
       if (c->p.precision)
         LAUNCH(c, k_gfull<double>, grid, 256, 0, c->M, c->nact, c->nact, (const cplx<double>*)c->thtil,
@@ -1196,6 +1231,16 @@ afqmc_status afqmc_mixed_sums(afqmc_ctx* c, const double* weight, const void* el
   c->err[0] = 0;
   NEED(c, out3 && (c->nw == 0 || (weight && eloc)), "afqmc_mixed_sums: null pointer");
   LAUNCH(c, k_mixed_sums, 1, 1024, 0, c->nw, weight, (const zcplx*)eloc, out3);
+  return AFQMC_OK;
+}
+
+afqmc_status afqmc_mixed_energy(afqmc_ctx* c, const double* sums, int32_t n, void* e_mix) {
+  if (!c) return AFQMC_EINVAL;
+  c->err[0] = 0;
+  NEED(c, n >= 0, "afqmc_mixed_energy: n < 0");
+  if (n == 0) return AFQMC_OK;
+  NEED(c, sums && e_mix, "afqmc_mixed_energy: null pointer");
+  LAUNCH(c, k_mixed_ratio, (n + 127) / 128, 128, 0, n, sums, (zcplx*)e_mix);
   return AFQMC_OK;
 }
 

@@ -134,9 +134,12 @@ __device__ inline void weight_update(zcplx S_old, zcplx S_new, zcplx c, double w
   } else {
     fac = exp(-dt * (e_pre_re - E0));
   }
-  bool killed = (cosd <= 0.0) || (w_old == 0.0);
+  // max{0, cos dtheta}: cos dtheta = Re(rho)/|rho|, so the decision is taken on Re(rho) itself (reading R6b): cos(atan2(y, x))
+  // is 6e-17 > 0 at x = 0 and for tiny negative x
+  const bool dead = rho.x <= 0.0;
+  bool killed = dead || (w_old == 0.0);
   w_new = killed ? 0.0 : w_old * fac * cosd;
-  if (cosd <= 0.0) flag |= FLAG_KILLED;
+  if (dead) flag |= FLAG_KILLED;
   if (!isfinite(w_new)) flag |= FLAG_NONFINITE;
 }
 
@@ -312,10 +315,10 @@ __global__ void __launch_bounds__(256) k_green(GreenArgs<T> g) {
 // Full Green's function on request: G_s[i][j] = sum_a Theta_s[j][a] psi_s[i][a]  (R15).
 template <typename T>
 __global__ void k_gfull(int M, int na, int nb, const cplx<T>* theta, const T* psi_a, const T* psi_b, cplx<T>* G) {
-  const int w = blockIdx.y, s = blockIdx.z, nt = na + nb;
+  const int w = blockIdx.x, s = blockIdx.z, nt = na + nb;
   const int n = s ? nb : na, off = s ? na : 0;
   const T* psi = s ? psi_b : psi_a;
-  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < M * M; e += gridDim.x * blockDim.x) {
+  for (int e = blockIdx.y * blockDim.x + threadIdx.x; e < M * M; e += gridDim.y * blockDim.x) {
     int i = e / M, j = e % M;
     T sr = T(0), si = T(0);
     for (int a = 0; a < n; ++a) {

@@ -246,16 +246,16 @@ __global__ void k_pack_Lt(int M, int ng, int NGP, int nblk, const int2* blk, con
 
 
 // A[w][i][p][j] := A[w][j][p][i] for i > j (A_w is symmetric; the assembly GEMM wrote the upper blocks only).
-// grid = (tile pairs TI >= TJ, walkers), block = 32 x 8; each CTA moves one 32 x 32 tile of both planes of both
+// grid = (walkers, tile pairs TI >= TJ), block = 32 x 8; each CTA moves one 32 x 32 tile of both planes of both
 // buffers (hi / lo) through shared memory: 16 independent loads per thread in flight.
 template <typename T>
 __global__ void __launch_bounds__(256) k_symmetrize(int M, int MP, T* A, T* A_lo) {
   __shared__ T tile[4][32][33];
-  int t = blockIdx.x, TI = 0;
+  int t = blockIdx.y, TI = 0;
   while (t > TI) { t -= TI + 1; ++TI; }
   const int TJ = t;                        // TI >= TJ
   const int nbuf = A_lo ? 2 : 1;
-  const size_t woff = ((size_t)blockIdx.y * M) * (2 * MP);
+  const size_t woff = ((size_t)blockIdx.x * M) * (2 * MP);
   const int tx = threadIdx.x, ty = threadIdx.y;
 #pragma unroll
   for (int q = 0; q < 4; ++q) {

@@ -289,4 +289,13 @@ __global__ void __launch_bounds__(1024) k_mixed_sums(int nw, const double* __res
   if (tid < 3) out[tid] = sh[tid][0];
 }
 
+// E_mix[m] = (sums[m][1] + i sums[m][2]) / sums[m][0] for n measurements (the sums are afqmc_mixed_sums' output, possibly
+// all-reduced across ranks in between); a dead population (sum of weights 0) gives NaN.
+__global__ void k_mixed_ratio(int n, const double* __restrict__ sums, zcplx* __restrict__ out) {
+  const int m = blockIdx.x * blockDim.x + threadIdx.x;
+  if (m >= n) return;
+  const double w = sums[3 * m];
+  out[m] = w != 0.0 ? mk<double>(sums[3 * m + 1] / w, sums[3 * m + 2] / w) : mk<double>(nan(""), nan(""));
+}
+
 }  // namespace afq

@@ -56,6 +56,10 @@ def population_control_sharded(ctx, phi, weight, ovlp, theta, fb, u: float, grou
     records; with a single rank (or torch.distributed not initialised) it needs no collective at all."""
     import torch
     import torch.distributed as dist
+    if weight.is_cuda and torch.cuda.current_stream(weight.device) != ctx.stream:
+        # the library enqueues on ctx.stream; torch ops and collectives on torch's current stream: make them the same
+        with torch.cuda.stream(ctx.stream):
+            return population_control_sharded(ctx, phi, weight, ovlp, theta, fb, u, group=group)
     on = dist.is_available() and dist.is_initialized()
     world = dist.get_world_size(group) if on else 1
     rank = dist.get_rank(group) if on else 0
@@ -93,6 +97,10 @@ def run_sharded(ctx, phi, weight, ovlp, theta, fb, x, n_steps, energy_every=20, 
     Returns the list of global mixed-estimator energies (complex) of the measurements, identical on every rank."""
     import torch
     import torch.distributed as dist
+    if weight.is_cuda and torch.cuda.current_stream(weight.device) != ctx.stream:
+        with torch.cuda.stream(ctx.stream):      # one stream for the library's kernels, torch's ops and the collectives
+            return run_sharded(ctx, phi, weight, ovlp, theta, fb, x, n_steps, energy_every, ortho_every, pc_every, us,
+                               flags, group)
     on = dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1
     nw = int(ctx.params.n_walkers)
     seg = pc_every if pc_every else n_steps
@@ -101,6 +109,7 @@ def run_sharded(ctx, phi, weight, ovlp, theta, fb, x, n_steps, energy_every=20, 
     eloc = torch.zeros(max(n_meas_seg, 1), nw, dtype=torch.complex128, device=weight.device)
     wm = torch.zeros(max(n_meas_seg, 1), nw, dtype=torch.float64, device=weight.device)
     sums = torch.zeros(max(n_meas_seg, 1), 3, dtype=torch.float64, device=weight.device)
+    emix = torch.zeros(max(n_meas_seg, 1), dtype=torch.complex128, device=weight.device)
     energies, done, k = [], 0, 0
     while done < n_steps:
         n = min(seg, n_steps - done)
@@ -112,8 +121,8 @@ def run_sharded(ctx, phi, weight, ovlp, theta, fb, x, n_steps, energy_every=20, 
         if m:
             if on:
                 dist.all_reduce(sums[:m], group=group)
-            for row in sums[:m].tolist():
-                energies.append(complex(row[1], row[2]) / row[0] if row[0] else complex("nan"))
+            ctx.afqmc_mixed_energy(sums, m, emix)      # the estimator's division runs in the library too
+            energies.extend(complex(v) for v in emix[:m].tolist())
         done += n
         if pc_every and n == seg:
             population_control_sharded(ctx, phi, weight, ovlp, theta, fb, us[k], group=group)

@@ -48,6 +48,7 @@ def test_stage_overlap_green_forcebias_energy(cfg):
                 G=H.rel_fro(G.cpu().numpy().astype(np.complex128), Gref), f=H.rel_fro(out["f"], fa + fb),
                 E=H.rel_abs(eloc.cpu().numpy(), E))
     print(f"cfg{cfg} stage errors: {errs}")
+    H.record("stage", cfg=cfg, **errs)
     assert np.all(out["flags"] == 0)
     for k, v in errs.items():
         assert v < tol, (k, v)
@@ -153,11 +154,12 @@ def _protocol_A(wl, nw, steps, gemm_path=0):
 
 
 @pytest.mark.parametrize("cfg,variant", [(1, "raw"), (1, "mf"), (2, "raw"), (2, "mf"), (3, "raw"), (3, "mf"), (4, "raw"), (4, "mf"),
-                                         (5, "mf")])
+                                         (5, "raw"), (5, "mf")])
 def test_protocol_A_resync(cfg, variant):
+    """north_star: "per step, over 10 steps" -- 10 steps on every config."""
     wl = _wl(cfg, variant)
-    steps = {4: 4, 5: 3}.get(cfg, 10)
-    _protocol_A(wl, SMALL[cfg], steps)
+    raw = _protocol_A(wl, SMALL[cfg], 10)
+    H.record("protocol_A", cfg=cfg, variant=variant, steps=10, **raw)
 
 
 def _free_run(wl, nw, steps):
@@ -221,6 +223,7 @@ def test_protocol_C_tame(cfg):
     errs = dict(phi=H.rel_fro(out["phi"], ost.phi), S=H.rel_abs(out["S"], ost.S), w=H.rel_abs(out["w"], ost.w),
                 f=H.rel_fro(out["f"], ost.f_a + ost.f_b), E=H.rel_abs(eloc[-1], recs[-1]["eloc"]))
     print(f"cfg{cfg}/tame protocol C after {steps} steps: {errs}")
+    H.record("protocol_C_tame", cfg=cfg, steps=steps, **errs)
     for k, v in errs.items():
         assert v < tol, (k, v)
 
@@ -327,7 +330,8 @@ def test_tcgen05_stage_forcebias_energy_propagate(cfg, path):
 @pytest.mark.parametrize("cfg,variant", [(3, "mf"), (5, "mf")])
 def test_protocol_A_resync_tcgen05(cfg, variant, path):
     wl = _wl(cfg, variant)
-    _protocol_A(wl, SMALL[cfg], {5: 3}.get(cfg, 10), gemm_path=path)
+    raw = _protocol_A(wl, SMALL[cfg], 10, gemm_path=path)
+    H.record("protocol_A_tcgen05", cfg=cfg, variant=variant, path=path, steps=10, **raw)
 
 
 def test_full_size_sampled_walkers():
@@ -351,6 +355,7 @@ def test_full_size_sampled_walkers():
                 w=H.rel_abs(out["w"][idx], ost.w), f=H.rel_fro(out["f"][idx], ost.f_a + ost.f_b),
                 E=H.rel_abs(eloc[-1][idx], rec["eloc"]))
     print(f"cfg5 full size (path {ctx.gemm_path}), sampled walkers: {errs}")
+    H.record("full_size_cfg5", **errs)
     assert np.all(np.isfinite(out["phi"].view(np.float64)))
     for k, v in errs.items():
         assert v < tol, (k, v)
