@@ -334,8 +334,10 @@ template <typename T> afqmc_status init_device(afqmc_ctx* c, const double* h1, c
     double* t = E; E = Tm; Tm = t;
   }
   LAUNCH(c, k_cast2d<T>, (mm + 127) / 128, 128, 0, M, M, E, (size_t)M, (T*)c->Eh, (T*)nullptr, (size_t)MP, 0);
-  if (c->tay_tc)   // TF32 hi / lo planes of E_h for the tensor-pipe Taylor kernel (the SIMT kernel never runs then)
-    LAUNCH(c, k_cast2d<T>, (mm + 127) / 128, 128, 0, M, M, E, (size_t)M, (T*)c->Eh, (T*)c->Eh_lo, (size_t)MP, 1);
+  if (c->tay_tc) {   // TF32 hi / lo planes of D_h = E_h - 1 for the tensor-pipe Taylor kernel (the SIMT kernel never runs then)
+    LAUNCH(c, k_dscale_eye, (mm + 127) / 128, 128, 0, M, 1.0, E, -1.0, Tm);
+    LAUNCH(c, k_cast2d<T>, (mm + 127) / 128, 128, 0, M, M, Tm, (size_t)M, (T*)c->Eh, (T*)c->Eh_lo, (size_t)MP, 1);
+  }
   CUDA_OK(c, cudaMemcpyAsync(c->psid_ac, psid_a, (size_t)M * na * 8, cudaMemcpyDeviceToDevice, st));
   if (nb) CUDA_OK(c, cudaMemcpyAsync(c->psid_bc, psid_b, (size_t)M * nb * 8, cudaMemcpyDeviceToDevice, st));
   // trial orbitals in T

@@ -23,7 +23,7 @@ enum { NST = 3, TILE_BYTES = 128 * 128, STG_BYTES = 2 * TILE_BYTES, PLANE_KB_BYT
 
 struct TaylorMaps {
   CUtensorMap A[2][2];   // [hi/lo][0: 128-row box, 1: last-tile box]  over Abuf viewed as [N_w*M][2*MP]
-  CUtensorMap E[2][2];   // same for E_h [M][MP]
+  CUtensorMap E[2][2];   // same for D_h = E_h - 1 [M][MP]
 };
 
 struct TaylorTcArgs {
@@ -157,7 +157,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
                 for (int k = 0; k < 4; ++k) {
                   const uint64_t adv = (uint64_t)(k * 2);   // 8 tf32 = 32 bytes = 2 x 16 B
                   umma_tf32(d, x_hi + adv, t_all + adv, idesc128, (first && k == 0) ? 0u : 1u);
-                  umma_tf32(d, x_lo + adv, t_all + adv, idesc64, 1u);
+                  // X_lo T_hi joins the other cross term in columns 64-127: the large hi*hi accumulator of columns 0-63 then
+                  // sees half as many (truncating) accumulations, the small cross-term accumulator's truncation is 2^-11 down
+                  umma_tf32(d + 64, x_lo + adv, t_all + adv, idesc64, 1u);
                 }
                 tc_commit(&empty_bar[s]);
               }
@@ -261,14 +263,31 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
                 for (int b = 0; b < 32; ++b) v[b] = half ? v[b] + u0[b] : v[b] - u0[b];
               }
             }
+            const int i = mt * 128 + q * 32 + lane;       // output row = basis index
+            if (ph == 0) {
+              // the streamed operand of the two one-body phases is D_h = E_h - 1 (|D_h| ~ dt |h'| / 2 << 1): E_h T = T + D_h T
+              // with the addition in FP32 round-to-nearest here, so the tensor pipe's truncating accumulation acts on the
+              // small correction only.  T (= Phi_w) is read back from the planes as hi + lo, before this thread overwrites it
+              const int ic = i < M ? i : 0;
+#pragma unroll
+              for (int b = 0; b < 32; ++b)
+                if (b < nt) {
+                  const uint32_t o = plane_off(rb + b, ic);
+                  float th, tl;
+                  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(th) : "r"(pl_hi + o) : "memory");
+                  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(tl) : "r"(pl_lo + o) : "memory");
+                  v[b] += th + tl;
+                }
+            }
 #pragma unroll
             for (int b = 0; b < 32; ++b) {
               float t = v[b] * scale;
-              if (ph == 0) P[mt][b] = t; else P[mt][b] += t;
+              if (last_phase) t += P[mt][b];              // E_h P = P + D_h P
+              else if (ph == 0) P[mt][b] = t;
+              else P[mt][b] += t;
               if (ph == g.K) t = P[mt][b];               // operand of the closing E_h product is the sum
               v[b] = t;
             }
-            const int i = mt * 128 + q * 32 + lane;       // output row = basis index
             if (last_phase) {
               // result rows stay in registers (P is dead) until every MMA has completed, then go to the staging
               // area inside the planes (the non-padding bytes, all rewritten by the next walker's operand)
