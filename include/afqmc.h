@@ -239,6 +239,15 @@ enum {
 AFQMC_API afqmc_status afqmc_profile_enable(afqmc_ctx* ctx, int32_t enable);
 AFQMC_API afqmc_status afqmc_profile_read(afqmc_ctx* ctx, int32_t stage, double* total_ms, int32_t* launches);
 
+/* Peak microbenchmarks behind bench.py --peaks (the TF32 / FP32 / FP64 / L2 denominators are measured, not
+ * assumed).  kind 0: back-to-back tcgen05.mma.kind::tf32 M = 128, N = n, operands from shared memory, one CTA per SM;
+ * 1: the same with the a-operand in TMEM; 2: CTA pairs (cta_group::2, M = 256); 3: FFMA; 4: DFMA; 5: TMA stream of an
+ * n-MiB buffer (L2 resident if n is small) into shared memory.  scratch: DEVICE, >= 1 MiB (kind 5: the streamed buffer).
+ * Synchronises `stream`.  ms = kernel time (CUDA events), units = flops (kinds 0-4) or bytes (kind 5) the kernel did,
+ * clk = clocks per MMA measured inside CTA 0 (kinds 0-2, else 0).  No context needed.  Errors: EINVAL, ECUDA. */
+AFQMC_API afqmc_status afqmc_peak_probe(int32_t kind, int32_t n, int32_t iters, void* scratch, size_t scratch_bytes,
+                                        void* stream, double* ms, double* units, double* clk);
+
 /* Which contraction path the context resolved to: 1 = SIMT, 2 = tcgen05 3xTF32. */
 AFQMC_API int32_t afqmc_gemm_path(const afqmc_ctx* ctx);
 

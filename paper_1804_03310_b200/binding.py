@@ -21,7 +21,7 @@ SYMBOLS = ["afqmc_query_bytes", "afqmc_init", "afqmc_destroy", "afqmc_last_error
            "afqmc_force_bias", "afqmc_propagate", "afqmc_local_energy", "afqmc_step", "afqmc_step_host",
            "afqmc_launch_count", "afqmc_gemm_path", "afqmc_profile_enable", "afqmc_profile_read",
            "afqmc_orthonormalize", "afqmc_population_control", "afqmc_run", "afqmc_comb_record_bytes",
-           "afqmc_comb_map", "afqmc_comb_pack", "afqmc_comb_unpack", "afqmc_mixed_sums", "afqmc_mixed_energy"]
+           "afqmc_comb_map", "afqmc_comb_pack", "afqmc_comb_unpack", "afqmc_mixed_sums", "afqmc_mixed_energy", "afqmc_peak_probe"]
 
 STAGES = ["shift", "assemble", "taylor", "green", "force_bias", "energy", "symmetrize", "ortho", "popctl"]
 
@@ -70,6 +70,9 @@ def load_library():
     lib.afqmc_run.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp, vp, i32p, i32p]
     lib.afqmc_mixed_sums.argtypes = [vp, vp, vp, vp]
     lib.afqmc_mixed_sums.restype = C.c_int
+    dp_ = C.POINTER(C.c_double)
+    lib.afqmc_peak_probe.argtypes = [C.c_int32, C.c_int32, C.c_int32, vp, C.c_size_t, vp, dp_, dp_, dp_]
+    lib.afqmc_peak_probe.restype = C.c_int
     lib.afqmc_mixed_energy.argtypes = [vp, vp, C.c_int32, vp]
     lib.afqmc_mixed_energy.restype = C.c_int
     lib.afqmc_comb_record_bytes.argtypes = [vp]
@@ -107,6 +110,20 @@ def afqmc_query_bytes(params: AfqmcParams):
     if st:
         raise AfqmcError(st, lib.afqmc_last_error(None).decode())
     return cb.value, wb.value
+
+
+def afqmc_peak_probe(kind, n, iters, scratch, stream=None):
+    """(ms, units, clk_per_mma) of one peak microbenchmark; scratch = CUDA uint8 tensor (>= 1 MiB)."""
+    import torch
+    lib = load_library()
+    ms, units, clk = C.c_double(0), C.c_double(0), C.c_double(0)
+    st = stream if stream is not None else torch.cuda.current_stream(scratch.device)
+    with torch.cuda.device(scratch.device):
+        rc = lib.afqmc_peak_probe(int(kind), int(n), int(iters), C.c_void_p(scratch.data_ptr()), scratch.numel(),
+                                  C.c_void_p(st.cuda_stream), C.byref(ms), C.byref(units), C.byref(clk))
+    if rc:
+        raise AfqmcError(rc, "afqmc_peak_probe failed")
+    return ms.value, units.value, clk.value
 
 
 def _f64(a):

@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 #include <new>
 #include <algorithm>
@@ -19,6 +20,7 @@
 #include "taylor.cuh"
 #include "taylor_tc.cuh"
 #include "popctl.cuh"
+#include "peaks.cuh"
 
 using namespace afq;
 
@@ -961,6 +963,7 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
     a.rows_last = (int)rup((size_t)(c->M - 128 * (a.mtiles - 1)), 8);
     a.nkb = (c->M + 31) / 32;
     a.phi = nullptr;
+    { const char* e = getenv("AFQMC_TAYLOR_DBG"); a.dbg = e ? atoi(e) : 0; }
     c->tay_tc_smem = tt::smem_bytes(a.nkb);
     int dev = 0;
     cudaGetDevice(&dev);
@@ -1244,6 +1247,97 @@ afqmc_status afqmc_mixed_energy(afqmc_ctx* c, const double* sums, int32_t n, voi
   NEED(c, sums && e_mix, "afqmc_mixed_energy: null pointer");
   LAUNCH(c, k_mixed_ratio, (n + 127) / 128, 128, 0, n, sums, (zcplx*)e_mix);
   return AFQMC_OK;
+}
+
+// ---- peak microbenchmarks (bench.py --peaks; not on the walker step's path) ----
+afqmc_status afqmc_peak_probe(int32_t kind, int32_t n, int32_t iters, void* scratch, size_t scratch_bytes, void* stream,
+                              double* ms, double* units, double* clk) {
+  if (!ms || !units || !clk || iters < 1 || !scratch || scratch_bytes < (size_t)1 << 20) return AFQMC_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  int dev = 0, n_sm = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+  cudaEvent_t e0, e1;
+  if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return AFQMC_ECUDA;
+  long long* out = (long long*)scratch;
+  *clk = 0.0;
+  cudaError_t err = cudaSuccess;
+  auto finish = [&](double u) -> afqmc_status {
+    cudaEventRecord(e1, st);
+    err = cudaStreamSynchronize(st);
+    float t = 0.f;
+    cudaEventElapsedTime(&t, e0, e1);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    if (err == cudaSuccess) err = cudaGetLastError();
+    *ms = t; *units = u;
+    return err == cudaSuccess ? AFQMC_OK : AFQMC_ECUDA;
+  };
+  if (kind >= 0 && kind <= 2) {          // tcgen05.mma.kind::tf32: SS / TS / SS on CTA pairs; units = flops
+    if (n < 16 || n > 256 || n % 16) return AFQMC_EINVAL;
+    const int grid = kind == 2 ? (n_sm & ~1) : n_sm;
+    const int smem = 16384 + 32768 + 1024;
+    cudaFuncSetAttribute(pk::k_peak_mma<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaFuncSetAttribute(pk::k_peak_mma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaFuncSetAttribute(pk::k_peak_mma<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaMemsetAsync(out, 0, 4096, st);
+    cudaEventRecord(e0, st);
+    if (kind == 0) pk::k_peak_mma<0><<<grid, 128, smem, st>>>(n, iters, out);
+    if (kind == 1) pk::k_peak_mma<1><<<grid, 128, smem, st>>>(n, iters, out);
+    if (kind == 2) {
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3(grid); cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+      cfg.attrs = at; cfg.numAttrs = 1;
+      err = cudaLaunchKernelEx(&cfg, pk::k_peak_mma<2>, (int)n, (int)iters, out);
+    }
+    const double mrows = kind == 2 ? 256.0 : 128.0, ctas = kind == 2 ? grid / 2 : grid;
+    afqmc_status s = finish(ctas * (double)iters * 4.0 * 2.0 * mrows * n * 8.0);
+    if (s == AFQMC_OK) {
+      long long c0 = 0;
+      cudaMemcpy(&c0, out, 8, cudaMemcpyDeviceToHost);
+      *clk = (double)c0 / ((double)iters * 4.0);      // clocks per MMA in CTA 0
+    }
+    return s;
+  }
+  if (kind == 6 || kind == 7) {          // the Taylor kernel's MMA pattern alone (6) and with the other warps loading the smem ports (7)
+    const int smem = 49152 + 3 * 32768 + 16384 + 1024;
+    cudaFuncSetAttribute(pk::k_peak_mma<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaFuncSetAttribute(pk::k_peak_mma<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaMemsetAsync(out, 0, 4096, st);
+    cudaEventRecord(e0, st);
+    if (kind == 6) pk::k_peak_mma<3><<<n_sm, 128, smem, st>>>(128, iters, out);
+    else pk::k_peak_mma<4><<<n_sm, 320, smem, st>>>(128, iters, out);
+    afqmc_status s = finish((double)n_sm * iters * 4.0 * 2.0 * 128.0 * 192.0 * 8.0);
+    if (s == AFQMC_OK) {
+      long long c0 = 0;
+      cudaMemcpy(&c0, out, 8, cudaMemcpyDeviceToHost);
+      *clk = (double)c0 / ((double)iters * 4.0);      // clocks per (N = 128, N = 64) MMA pair
+    }
+    return s;
+  }
+  if (kind == 3 || kind == 4) {          // FFMA / DFMA; units = flops
+    const int grid = n_sm * 4, thr = 512;
+    cudaEventRecord(e0, st);
+    if (kind == 3) pk::k_peak_fma<float><<<grid, thr, 0, st>>>(iters, 1.0f, (float*)scratch);
+    else pk::k_peak_fma<double><<<grid, thr, 0, st>>>(iters, 1.0, (double*)scratch);
+    return finish((double)grid * thr * 8.0 * 2.0 * iters);
+  }
+  if (kind == 5) {                       // L2 -> smem TMA stream; units = bytes; n = MiB of the streamed buffer
+    size_t bytes = (size_t)n << 20;
+    if (bytes > scratch_bytes) bytes = scratch_bytes;
+    const int rows = (int)(bytes / 128) / 128 * 128;
+    CUtensorMap map;
+    if (rows < 128 || !tc::make_map(&map, scratch, 32, (uint64_t)rows, 32, 128)) return AFQMC_EINVAL;
+    const int smem = 4 * 16384 + 1024;
+    cudaFuncSetAttribute(pk::k_peak_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    pk::k_peak_tma<<<n_sm, 64, smem, st>>>(map, rows, 64);      // warm the L2
+    cudaEventRecord(e0, st);
+    pk::k_peak_tma<<<n_sm, 64, smem, st>>>(map, rows, iters);
+    return finish((double)n_sm * iters * 16384.0);
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  return AFQMC_EINVAL;
 }
 
 afqmc_status afqmc_run(afqmc_ctx* c, void* phi, double* weight, void* ovlp, void* theta, void* fb, const void* x,

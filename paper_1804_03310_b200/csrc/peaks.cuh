@@ -1,0 +1,140 @@
+// peaks.cuh -- self-written peak microbenchmarks ("the builder measures them with tiny self-written
+// microbenchmarks ... before quoting any fraction"): back-to-back tcgen05.mma.kind::tf32 (operands from shared memory,
+// the a-operand from TMEM, or on a CTA pair), FFMA and DFMA loops, and an L2 -> shared-memory TMA stream.  bench.py --peaks
+// prints them beside the nominal figures; they are the denominators DESIGN.md 7 argues with.  Not on the walker step's path.
+#pragma once
+#include "gemm_tf32.cuh"
+
+namespace afq {
+namespace pk {
+
+using namespace tc;
+
+__device__ __forceinline__ void umma_tf32_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
+      "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n}"
+      ::"r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(acc)
+      : "memory");
+}
+
+// mode 0: SS (a, b from shared memory), one CTA;  1: TS (a from TMEM);  2: SS on a CTA pair (M = 256)
+// Every CTA issues `iters` k-blocks of 4 MMAs (K = 8 each) into one accumulator; out[blockIdx] = clocks of the issue loop
+// (first MMA issued -> last MMA completed).
+template <int MODE>
+__global__ void __launch_bounds__(320, 1) k_peak_mma(int N, int iters, long long* out) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  __shared__ __align__(8) uint64_t done_bar_s[2];
+  uint64_t& done_bar = done_bar_s[0];
+  __shared__ uint32_t tmem_base_s;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  float* a = reinterpret_cast<float*>(smem);                    // 128 rows x 32 columns, K-major (content irrelevant to timing;
+  float* b = reinterpret_cast<float*>(smem + 16384);            // N rows x 32 columns     small finite numbers, no NaN patterns)
+  for (int e = threadIdx.x; e < (128 + 256) * 32; e += blockDim.x) a[e] = (float)((e * 2654435761u) >> 20) * (1.0f / 4096.0f) - 0.5f;
+  if (threadIdx.x == 0) { mbar_init(&done_bar, 1); mbar_init(&done_bar + 1, 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+  if (warp == 0) {
+    if (MODE == 2) {
+      asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "r"(512u) : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    } else {
+      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "r"(512u) : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+  }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  tc_fence_before();
+  __syncthreads();
+  if (MODE == 2) cluster_sync_all();
+  tc_fence_after();
+  const uint32_t tmem = tmem_base_s;
+  const uint32_t rank = MODE == 2 ? cluster_ctarank() : 0u;
+  if (warp == 1 && lane == 0 && rank == 0) {
+    const uint32_t idesc = make_idesc(MODE == 2 ? 256 : 128, N);
+    const uint64_t ad = make_desc(smem_u32(a)), bd = make_desc(smem_u32(b));
+    const uint32_t a_t = tmem + 256;      // TS: a-operand rows = lanes, K elements = columns 256.. (uninitialised TMEM: timing only)
+    const long long t0 = clock64();
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const uint64_t adv = (uint64_t)(k * 2);
+        const uint32_t acc = (it | k) ? 1u : 0u;
+        if (MODE == 0) umma_tf32(tmem, ad + adv, bd + adv, idesc, acc);
+        if (MODE == 1) umma_tf32_ts(tmem, a_t + k * 8, bd + adv, idesc, acc);
+        if (MODE == 2) umma_tf32_pair(tmem, ad + adv, bd + adv, idesc, acc);
+        if (MODE >= 3) {   // the Taylor kernel's k-step: X_hi [T_hi | T_lo] (N = 128) then X_lo T_hi (N = 64), rotating stage slots
+          const uint64_t as = make_desc(smem_u32(smem + 49152 + (it % 3) * 32768));
+          umma_tf32(tmem, as + adv, bd + adv, make_idesc(128, 128), acc);
+          umma_tf32(tmem + 64, as + 1024 + adv, bd + adv, make_idesc(128, 64), 1u);
+        }
+      }
+      if (MODE >= 3 && (it & 1)) tc_commit(&done_bar + 1);
+    }
+    if (MODE == 2) tc_commit_pair(&done_bar); else tc_commit(&done_bar);
+    mbar_wait(&done_bar, 0);
+    out[blockIdx.x] = clock64() - t0;
+  } else if (MODE == 2 && warp == 1 && lane == 0) {
+    mbar_wait(&done_bar, 0);      // the peer's copy of the barrier receives the multicast commit
+  } else if (MODE == 4 && warp >= 2) {
+    // other warps keep the shared-memory ports busy the way the Taylor epilogue does (scalar stores + loads)
+    volatile float* z = reinterpret_cast<volatile float*>(smem + 49152 + 3 * 32768);
+    float acc2 = 0.f;
+    for (int it = 0; it < iters * 6; ++it) {
+#pragma unroll
+      for (int u = 0; u < 8; ++u) { z[((threadIdx.x - 64) * 33 + u * 67 + it) & 4095] = acc2; acc2 += z[(threadIdx.x * 17 + u * 129 + it) & 4095]; }
+    }
+    if (acc2 == -1.f) out[1] = 0;
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (MODE == 2) cluster_sync_all();
+  if (warp == 0) {
+    if (MODE == 2) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512u) : "memory");
+    else asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512u) : "memory");
+  }
+}
+
+// FFMA / DFMA: 8 independent chains per thread, 8 * 2 * iters flops per thread
+template <typename T> __global__ void __launch_bounds__(512) k_peak_fma(int iters, T seed, T* out) {
+  T v[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) v[i] = seed + (T)(threadIdx.x + i);
+  const T m = (T)0.999, c = (T)1e-3;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = fma(v[i], m, c);
+  }
+  T s = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) s += v[i];
+  if (s == (T)-12345) out[0] = s;     // never true: keeps the chains alive
+}
+
+// L2 -> shared memory: every CTA streams `iters` boxes of 128 rows x 32 floats (16 KB) by TMA through a 4-deep ring from a
+// buffer of `rows` rows (small enough to stay L2 resident), starting at a CTA-dependent row.
+__global__ void __launch_bounds__(64, 1) k_peak_tma(const __grid_constant__ CUtensorMap map, int rows, int iters) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  __shared__ __align__(8) uint64_t full[4];
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < 4; ++s) mbar_init(&full[s], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    const int nbox = rows / 128;
+    int box = (blockIdx.x * 37) % nbox;
+    for (int it = 0; it < iters + 4; ++it) {
+      const int s = it & 3;
+      if (it >= 4) mbar_wait(&full[s], ((it - 4) >> 2) & 1);
+      if (it < iters) {
+        mbar_expect_tx(&full[s], 16384);
+        tma_load_2d(smem + s * 16384, &map, &full[s], 0, box * 128);
+        box = box + 1 == nbox ? 0 : box + 1;
+      }
+    }
+  }
+}
+
+}  // namespace pk
+}  // namespace afq

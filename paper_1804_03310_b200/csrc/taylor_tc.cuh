@@ -30,6 +30,7 @@ struct TaylorTcArgs {
   int M, MP, nt, K, nw;
   int mtiles, rows_last, nkb;   // 128-row tiles, rows of the last one (multiple of 8), 32-column k-blocks
   cplx<float>* phi;             // [nw][M][nt] in/out
+  int dbg;                      // timing experiments only (AFQMC_TAYLOR_DBG): 1 no TMA, 2 no epilogue data movement, 4 no MMA
 };
 
 inline size_t smem_bytes(int nkb) { return (size_t)nkb * PLANE_KB_BYTES + (size_t)NST * STG_BYTES + 1024; }
@@ -102,7 +103,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
   const uint32_t tmem = tmem_base_s;
 
   if (warp == EPW) {
-    if (lane == 0) {   // ===== TMA producer: streams X tiles for every (walker, phase, tile, k-block, plane) =====
+    if (lane == 0 && !(g.dbg & 1)) {   // ===== TMA producer: streams X tiles for every (walker, phase, tile, k-block, plane) =====
       uint32_t it = 0;
       for (int w = blockIdx.x; w < g.nw; w += gridDim.x)
         for (int ph = 0; ph < nphase; ++ph) {
@@ -146,7 +147,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
               for (int p = 0; p < (cx ? 2 : 1); ++p, ++it) {
                 const uint32_t d = tmem + (mt * 2 + p) * 128;
                 const int s = it % NST;
-                mbar_wait(&full_bar[s], (it / NST) & 1);
+                if (!(g.dbg & 1)) mbar_wait(&full_bar[s], (it / NST) & 1);
                 tc_fence_after();
                 const uint32_t sa = smem_u32(stages + (size_t)s * STG_BYTES);
                 const uint64_t x_hi = make_desc(sa), x_lo = make_desc(sa + TILE_BYTES);
@@ -155,6 +156,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
                 const bool first = kb == 0;
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
+                  if (g.dbg & 4) break;
                   const uint64_t adv = (uint64_t)(k * 2);   // 8 tf32 = 32 bytes = 2 x 16 B
                   umma_tf32(d, x_hi + adv, t_all + adv, idesc128, (first && k == 0) ? 0u : 1u);
                   // X_lo T_hi joins the other cross term in columns 64-127: the large hi*hi accumulator of columns 0-63 then
@@ -248,7 +250,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
             float v[32];
             mbar_wait(&tmem_full_bar[mt], gph & 1);
             tc_fence_after();
-            {
+            if (g.dbg & 2) {
+#pragma unroll
+              for (int b = 0; b < 32; ++b) v[b] = 0.f;
+            } else {
               float u0[32], u1[32];
               tmem_ld32x2(tl + (mt * 2 + 0) * 128 + half * 32, tl + (mt * 2 + 0) * 128 + 64 + half * 32, u0, u1);
 #pragma unroll
@@ -312,7 +317,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
               // k-block mt*4+q of T may be overwritten once every MMA that reads it has completed: for the last
               // tile that is tmem_full (above), for tile 0 of two the last tile's pass over that k-block
               if (mt == 0 && mtiles == 2) mbar_wait(&t_free_bar[q], gph & 1);
-              if (i < M) {
+              if (i < M && !(g.dbg & 2)) {
 #pragma unroll
                 for (int b = 0; b < 32; ++b)
                   if (b < nt) {
