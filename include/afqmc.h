@@ -248,6 +248,11 @@ AFQMC_API afqmc_status afqmc_profile_read(afqmc_ctx* ctx, int32_t stage, double*
 AFQMC_API afqmc_status afqmc_peak_probe(int32_t kind, int32_t n, int32_t iters, void* scratch, size_t scratch_bytes,
                                         void* stream, double* ms, double* units, double* clk);
 
+/* Operand-ordering experiment behind DESIGN.md 7 (which tcgen05 operand slices may repeat back to back): issues the
+ * tab[0] MMAs {a byte offset, b byte offset, N, accumulator column} of tab = {n, a[64], b[64], nn[64], d[64]} (HOST int32)
+ * `iters` times on every SM; clk = clocks per MMA in CTA 0.  scratch DEVICE >= 4 KiB.  Synchronises. */
+AFQMC_API afqmc_status afqmc_peak_mma_table(const int32_t* tab, int32_t iters, void* scratch, void* stream, double* clk);
+
 /* Which contraction path the context resolved to: 1 = SIMT, 2 = tcgen05 3xTF32. */
 AFQMC_API int32_t afqmc_gemm_path(const afqmc_ctx* ctx);
 

@@ -21,7 +21,7 @@ SYMBOLS = ["afqmc_query_bytes", "afqmc_init", "afqmc_destroy", "afqmc_last_error
            "afqmc_force_bias", "afqmc_propagate", "afqmc_local_energy", "afqmc_step", "afqmc_step_host",
            "afqmc_launch_count", "afqmc_gemm_path", "afqmc_profile_enable", "afqmc_profile_read",
            "afqmc_orthonormalize", "afqmc_population_control", "afqmc_run", "afqmc_comb_record_bytes",
-           "afqmc_comb_map", "afqmc_comb_pack", "afqmc_comb_unpack", "afqmc_mixed_sums", "afqmc_mixed_energy", "afqmc_peak_probe"]
+           "afqmc_comb_map", "afqmc_comb_pack", "afqmc_comb_unpack", "afqmc_mixed_sums", "afqmc_mixed_energy", "afqmc_peak_probe", "afqmc_peak_mma_table"]
 
 STAGES = ["shift", "assemble", "taylor", "green", "force_bias", "energy", "symmetrize", "ortho", "popctl"]
 
@@ -73,6 +73,8 @@ def load_library():
     dp_ = C.POINTER(C.c_double)
     lib.afqmc_peak_probe.argtypes = [C.c_int32, C.c_int32, C.c_int32, vp, C.c_size_t, vp, dp_, dp_, dp_]
     lib.afqmc_peak_probe.restype = C.c_int
+    lib.afqmc_peak_mma_table.argtypes = [vp, C.c_int32, vp, vp, dp_]
+    lib.afqmc_peak_mma_table.restype = C.c_int
     lib.afqmc_mixed_energy.argtypes = [vp, vp, C.c_int32, vp]
     lib.afqmc_mixed_energy.restype = C.c_int
     lib.afqmc_comb_record_bytes.argtypes = [vp]
@@ -124,6 +126,23 @@ def afqmc_peak_probe(kind, n, iters, scratch, stream=None):
     if rc:
         raise AfqmcError(rc, "afqmc_peak_probe failed")
     return ms.value, units.value, clk.value
+
+
+def afqmc_peak_mma_table(mmas, iters, scratch, stream=None):
+    """mmas: list of (a_offset, b_offset, N, d_column); returns clocks per MMA."""
+    import torch
+    lib = load_library()
+    tab = np.zeros(1 + 4 * 64, dtype=np.int32)
+    tab[0] = len(mmas)
+    for i, (a, b, n, d) in enumerate(mmas):
+        tab[1 + i], tab[65 + i], tab[129 + i], tab[193 + i] = a, b, n, d
+    clk = C.c_double(0)
+    st = stream if stream is not None else torch.cuda.current_stream(scratch.device)
+    rc = lib.afqmc_peak_mma_table(tab.ctypes.data_as(C.c_void_p), int(iters), C.c_void_p(scratch.data_ptr()),
+                                  C.c_void_p(st.cuda_stream), C.byref(clk))
+    if rc:
+        raise AfqmcError(rc, "afqmc_peak_mma_table failed")
+    return clk.value
 
 
 def _f64(a):

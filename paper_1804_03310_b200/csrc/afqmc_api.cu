@@ -77,7 +77,7 @@ struct afqmc_ctx {
   int nblk; int2* blk;   // symmetric block list of the tcgen05 assembly GEMM
   int cta2;   // tcgen05 GEMMs run on CTA pairs (cta_group::2), gemm_path 3
   int ps_ok;  // the persistent pair kernel's shared-memory request was accepted
-  int tay_tc; void *Abuf_lo, *Eh_lo; tt::TaylorMaps map_tay; tt::TaylorTcArgs tay_args; size_t tay_tc_smem; int n_sm;   // TMA descriptors of the tcgen05 path (path == 2)
+  int tay_tc; tt::TaylorMaps map_tay; tt::TaylorTcArgs tay_args; size_t tay_tc_smem; int n_sm;   // TMA descriptors of the tcgen05 path (path == 2)
   char err[256];
   int64_t launches;
   // optional per-stage timing (afqmc_profile_enable)
@@ -216,7 +216,6 @@ void carve(const afqmc_params* p, afqmc_ctx* c, char* cbase, char* wbase, size_t
   c->psid_ac = (double*)cc.take((size_t)M * na * 8);
   c->psid_bc = (double*)cc.take((size_t)M * (nb ? nb : 1) * 8);
   c->Eh = cc.take((size_t)M * MP * ts);
-  c->Eh_lo = split ? cc.take((size_t)M * MP * ts) : nullptr;
   // tcgen05 path: only the 8 x 16 blocks (i-block, j-block) that touch the upper triangle of the symmetric A_w
   c->nblk = 0;
   for (int ib = 0; ib * 8 < M; ++ib)
@@ -247,7 +246,6 @@ void carve(const afqmc_params* p, afqmc_ctx* c, char* cbase, char* wbase, size_t
   c->Z = w.take(2 * nw1 * NGP * ts);
   c->Z_lo = split ? w.take(2 * nw1 * NGP * ts) : nullptr;
   c->Abuf = w.take(nw1 * M * 2 * MP * ts);
-  c->Abuf_lo = split ? w.take(nw1 * M * 2 * MP * ts) : nullptr;
   c->thp = w.take(2 * nw1 * KT * ts);
   c->thp_lo = split ? w.take(2 * nw1 * KT * ts) : nullptr;
   c->fs = w.take(2 * 2 * nw1 * NGP * ts);
@@ -336,9 +334,9 @@ template <typename T> afqmc_status init_device(afqmc_ctx* c, const double* h1, c
     double* t = E; E = Tm; Tm = t;
   }
   LAUNCH(c, k_cast2d<T>, (mm + 127) / 128, 128, 0, M, M, E, (size_t)M, (T*)c->Eh, (T*)nullptr, (size_t)MP, 0);
-  if (c->tay_tc) {   // TF32 hi / lo planes of D_h = E_h - 1 for the tensor-pipe Taylor kernel (the SIMT kernel never runs then)
+  if (c->tay_tc) {   // D_h = E_h - 1 in FP32 for the tensor-pipe Taylor kernel, which splits it on the fly (the SIMT kernel never runs then)
     LAUNCH(c, k_dscale_eye, (mm + 127) / 128, 128, 0, M, 1.0, E, -1.0, Tm);
-    LAUNCH(c, k_cast2d<T>, (mm + 127) / 128, 128, 0, M, M, Tm, (size_t)M, (T*)c->Eh, (T*)c->Eh_lo, (size_t)MP, 1);
+    LAUNCH(c, k_cast2d<T>, (mm + 127) / 128, 128, 0, M, M, Tm, (size_t)M, (T*)c->Eh, (T*)nullptr, (size_t)MP, 0);
   }
   CUDA_OK(c, cudaMemcpyAsync(c->psid_ac, psid_a, (size_t)M * na * 8, cudaMemcpyDeviceToDevice, st));
   if (nb) CUDA_OK(c, cudaMemcpyAsync(c->psid_bc, psid_b, (size_t)M * nb * 8, cudaMemcpyDeviceToDevice, st));
@@ -657,13 +655,14 @@ afqmc_status do_propagate(afqmc_ctx* c, void* phi, const void* x, const void* fb
       if (c->path == 2) {
         if (c->M % 4 == 0) {   // staged epilogue writes both triangles: no symmetrize pass
           tc::EpiAssembleSym e3;
-          e3.out = (float*)c->Abuf; e3.out_lo = c->tay_tc ? (float*)c->Abuf_lo : nullptr; e3.blk = c->blk; e3.M = c->M;
+          e3.out = (float*)c->Abuf; e3.out_lo = nullptr;   // A_w is stored once, in FP32: the Taylor kernel splits it on the fly
+          e3.blk = c->blk; e3.M = c->M;
           e3.MP = c->MP; e3.n_real = 2 * c->nw;
           st = run_gemm_tc(c, c->map_asm, c->nblk * 128, 2 * c->nw, c->NGP, e3);
           done = true;
         }
         tc::EpiAssemble e2;
-        e2.out = (float*)c->Abuf; e2.out_lo = c->tay_tc ? (float*)c->Abuf_lo : nullptr; e2.blk = c->blk; e2.M = c->M; e2.MP = c->MP; e2.m_real = c->nblk * 128; e2.n_real = 2 * c->nw;
+        e2.out = (float*)c->Abuf; e2.out_lo = nullptr; e2.blk = c->blk; e2.M = c->M; e2.MP = c->MP; e2.m_real = c->nblk * 128; e2.n_real = 2 * c->nw;
         if (!done) st = run_gemm_tc(c, c->map_asm, c->nblk * 128, 2 * c->nw, c->NGP, e2);
         done = true;
       }
@@ -679,8 +678,7 @@ afqmc_status do_propagate(afqmc_ctx* c, void* phi, const void* x, const void* fb
       StageScope sc(c, AFQMC_STAGE_SYMMETRIZE);
       const int nt32 = (c->M + 31) / 32;
       dim3 sg(c->nw, nt32 * (nt32 + 1) / 2);   // walkers on grid x (no 65535 cap)
-      LAUNCH(c, k_symmetrize<float>, sg, dim3(32, 8), 0, c->M, c->MP, (float*)c->Abuf,
-             c->tay_tc ? (float*)c->Abuf_lo : (float*)nullptr);
+      LAUNCH(c, k_symmetrize<float>, sg, dim3(32, 8), 0, c->M, c->MP, (float*)c->Abuf, (float*)nullptr);
     }
   }
   if (st) return st;
@@ -963,19 +961,19 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
     a.rows_last = (int)rup((size_t)(c->M - 128 * (a.mtiles - 1)), 8);
     a.nkb = (c->M + 31) / 32;
     a.phi = nullptr;
-    { const char* e = getenv("AFQMC_TAYLOR_DBG"); a.dbg = e ? atoi(e) : 0; }
     c->tay_tc_smem = tt::smem_bytes(a.nkb);
     int dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
     bool ok = true;
-    for (int hl = 0; hl < 2; ++hl)
-      for (int v = 0; v < 2; ++v) {
-        const uint32_t rows = v ? (uint32_t)a.rows_last : 128u;
-        ok &= tc::make_map(&c->map_tay.A[hl][v], hl ? c->Abuf_lo : c->Abuf, 2 * (uint64_t)c->MP, (uint64_t)c->nw * c->M,
-                           2 * (uint64_t)c->MP, rows);
-        ok &= tc::make_map(&c->map_tay.E[hl][v], hl ? c->Eh_lo : c->Eh, (uint64_t)c->MP, (uint64_t)c->M, (uint64_t)c->MP, rows);
-      }
+    a.nf = tt::pick_nf(a.nkb);
+    ok &= a.nf >= 3;
+    for (int v = 0; v < 2; ++v) {
+      const uint32_t rows = v ? (uint32_t)a.rows_last : 128u;
+      ok &= tc::make_map(&c->map_tay.A[v], c->Abuf, 2 * (uint64_t)c->MP, (uint64_t)c->nw * c->M, 2 * (uint64_t)c->MP, rows);
+      ok &= tc::make_map(&c->map_tay.E[v], c->Eh, (uint64_t)c->MP, (uint64_t)c->M, (uint64_t)c->MP, rows);
+    }
+
     cudaError_t e0 = cudaFuncSetAttribute(tt::k_taylor_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tay_tc_smem);
     if (!ok || e0 != cudaSuccess || c->n_sm <= 0) {
       snprintf(g_init_err, 256, "tensor-pipe Taylor kernel: tensor-map / shared-memory set-up failed");
@@ -1249,6 +1247,25 @@ afqmc_status afqmc_mixed_energy(afqmc_ctx* c, const double* sums, int32_t n, voi
   return AFQMC_OK;
 }
 
+// table-driven MMA ordering experiment (peaks.cuh): tab = {n, a[64], b[64], nn[64], d[64]} int32 HOST; clk = clocks per MMA
+afqmc_status afqmc_peak_mma_table(const int32_t* tab, int32_t iters, void* scratch, void* stream, double* clk) {
+  if (!tab || !scratch || !clk || tab[0] < 1 || tab[0] > 64) return AFQMC_EINVAL;
+  pk::MmaTab t;
+  memcpy(&t, tab, sizeof(t));
+  cudaStream_t st = (cudaStream_t)stream;
+  int dev = 0, n_sm = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+  const int smem = 221 * 1024;
+  cudaFuncSetAttribute(pk::k_peak_tab, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  pk::k_peak_tab<<<n_sm, 64, smem, st>>>(t, iters, (long long*)scratch);
+  if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) return AFQMC_ECUDA;
+  long long c0 = 0;
+  cudaMemcpy(&c0, scratch, 8, cudaMemcpyDeviceToHost);
+  *clk = (double)c0 / ((double)iters * t.n);
+  return AFQMC_OK;
+}
+
 // ---- peak microbenchmarks (bench.py --peaks; not on the walker step's path) ----
 afqmc_status afqmc_peak_probe(int32_t kind, int32_t n, int32_t iters, void* scratch, size_t scratch_bytes, void* stream,
                               double* ms, double* units, double* clk) {
@@ -1306,13 +1323,60 @@ afqmc_status afqmc_peak_probe(int32_t kind, int32_t n, int32_t iters, void* scra
     cudaFuncSetAttribute(pk::k_peak_mma<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     cudaMemsetAsync(out, 0, 4096, st);
     cudaEventRecord(e0, st);
-    if (kind == 6) pk::k_peak_mma<3><<<n_sm, 128, smem, st>>>(128, iters, out);
+    if (kind == 6) pk::k_peak_mma<3><<<n_sm, 128, smem, st>>>(n, iters, out);
     else pk::k_peak_mma<4><<<n_sm, 320, smem, st>>>(128, iters, out);
     afqmc_status s = finish((double)n_sm * iters * 4.0 * 2.0 * 128.0 * 192.0 * 8.0);
     if (s == AFQMC_OK) {
       long long c0 = 0;
       cudaMemcpy(&c0, out, 8, cudaMemcpyDeviceToHost);
       *clk = (double)c0 / ((double)iters * 4.0);      // clocks per (N = 128, N = 64) MMA pair
+    }
+    return s;
+  }
+  if (kind == 8) {                       // the Taylor kernel's MMA pattern, uniform issue; n = commits per 8 MMAs (0..2), + 10: 10 more warps poll an mbarrier
+    const int smem = 16384 + 6 * 16384 + 1024;
+    const int nc = n % 10, poll = n >= 10;
+#define PT_LAUNCH(NC, PL)                                                                                         \
+    {                                                                                                              \
+      cudaFuncSetAttribute(pk::k_peak_taylor<NC, PL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);          \
+      cudaMemsetAsync(out, 0, 4096, st);                                                                           \
+      cudaEventRecord(e0, st);                                                                                     \
+      pk::k_peak_taylor<NC, PL><<<n_sm, PL ? 384 : 64, smem, st>>>(iters, out);                                    \
+    }
+    if (nc == 0 && !poll) PT_LAUNCH(0, 0) else if (nc == 1 && !poll) PT_LAUNCH(1, 0) else if (nc == 2 && !poll) PT_LAUNCH(2, 0)
+    else if (nc == 0) PT_LAUNCH(0, 1) else if (nc == 1) PT_LAUNCH(1, 1) else PT_LAUNCH(2, 1)
+#undef PT_LAUNCH
+    afqmc_status s = finish((double)n_sm * iters * 4.0 * 2.0 * 128.0 * 192.0 * 8.0);
+    if (s == AFQMC_OK) {
+      long long c0 = 0;
+      cudaMemcpy(&c0, out, 8, cudaMemcpyDeviceToHost);
+      *clk = (double)c0 / ((double)iters * 4.0);      // clocks per (N = 128, N = 64) MMA pair
+    }
+    return s;
+  }
+  if (kind == 9) {                       // MMA orderings for the Taylor product: n = 10 * pattern + (1: seven T k-blocks cycle, 0: one)
+    const int smem = 225 * 1024;
+#define PP_LAUNCH(PAT, NB, EX)                                                                                    \
+    {                                                                                                              \
+      cudaFuncSetAttribute(pk::k_peak_pat<PAT, NB, EX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);        \
+      cudaMemsetAsync(out, 0, 4096, st);                                                                           \
+      cudaEventRecord(e0, st);                                                                                     \
+      pk::k_peak_pat<PAT, NB, EX><<<n_sm, 64, smem, st>>>(iters, out);                                             \
+    }
+    switch (n) {
+      case 0: PP_LAUNCH(0, 1, 0) break; case 1: PP_LAUNCH(0, 7, 0) break;
+      case 10: PP_LAUNCH(1, 1, 0) break; case 11: PP_LAUNCH(1, 7, 0) break;
+      case 20: PP_LAUNCH(2, 1, 0) break; case 21: PP_LAUNCH(2, 7, 0) break;
+      case 101: PP_LAUNCH(0, 7, 1) break; case 102: PP_LAUNCH(0, 7, 2) break; case 103: PP_LAUNCH(0, 7, 3) break;
+      case 104: PP_LAUNCH(0, 7, 4) break; case 107: PP_LAUNCH(0, 7, 7) break;
+      default: cudaEventDestroy(e0); cudaEventDestroy(e1); return AFQMC_EINVAL;
+    }
+#undef PP_LAUNCH
+    afqmc_status s = finish(0.0);
+    if (s == AFQMC_OK) {
+      long long c0 = 0;
+      cudaMemcpy(&c0, out, 8, cudaMemcpyDeviceToHost);
+      *clk = (double)c0 / (double)iters;      // clocks per (k-block, plane)
     }
     return s;
   }

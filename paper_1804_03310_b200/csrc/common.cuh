@@ -56,6 +56,15 @@ __device__ __forceinline__ void tf32_split(float v, float& hi, float& lo) {
   lo = tf32_rn(v - hi);
 }
 
+// The tensor pipe ignores the low 13 mantissa bits of a kind::tf32 operand, i.e. it consumes raw FP32 v as trunc13(v).  The
+// matching low part, rounded to TF32 (cvt.rna: nearest, ties away), as raw bits.
+__device__ __forceinline__ uint32_t tf32_lo_bits(uint32_t vbits) {
+  const float d = __uint_as_float(vbits) - __uint_as_float(vbits & 0xffffe000u);
+  uint32_t r;
+  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(d));
+  return r;
+}
+
 // cp.async 16-byte global -> shared (LDGSTS)
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
   uint32_t s = (uint32_t)__cvta_generic_to_shared(smem);

@@ -69,6 +69,8 @@ __global__ void __launch_bounds__(320, 1) k_peak_mma(int N, int iters, long long
         }
       }
       if (MODE >= 3 && (it & 1)) tc_commit(&done_bar + 1);
+      if (MODE == 3 && N == 144) { tc_commit(&done_bar + 1); tc_commit(&done_bar + 1); }               // two commits per 8 MMAs
+      if (MODE == 3 && N == 160) { tc_commit(&done_bar + 1); mbar_wait(&done_bar + 1, 0); }             // + an (already complete) wait
     }
     if (MODE == 2) tc_commit_pair(&done_bar); else tc_commit(&done_bar);
     mbar_wait(&done_bar, 0);
@@ -92,6 +94,189 @@ __global__ void __launch_bounds__(320, 1) k_peak_mma(int N, int iters, long long
     if (MODE == 2) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512u) : "memory");
     else asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512u) : "memory");
   }
+}
+
+// The Taylor kernel's issue pattern, warp-uniform issue (elect_one): per iteration 4 k-steps of [N = 128 into d, N = 64 into
+// d + 64] on rotating a-tiles, followed by NC tcgen05.commit (NC = 0: one commit at the very end only).
+template <int NC, int POLL>
+__global__ void __launch_bounds__(384, 1) k_peak_taylor(int iters, long long* out) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  __shared__ __align__(8) uint64_t bars[4];
+  __shared__ uint32_t tmem_base_s;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  float* a = reinterpret_cast<float*>(smem);
+  for (int e = threadIdx.x; e < (16384 + 6 * 16384) / 4; e += blockDim.x) a[e] = (float)((e * 2654435761u) >> 20) * (1.0f / 4096.0f) - 0.5f;
+  if (threadIdx.x == 0) { for (int i = 0; i < 4; ++i) mbar_init(&bars[i], 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "r"(512u) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_base_s;
+  if (warp == 1) {
+    const uint32_t base = smem_u32(smem);
+    const uint64_t bd = make_desc(base);                       // T planes stand-in: 128 rows
+    int s = 0;
+    const long long t0 = clock64();
+    for (int it = 0; it < iters; ++it) {
+      const uint64_t xh = make_desc(base + 16384 + (uint32_t)s * 32768), xl = make_desc(base + 32768 + (uint32_t)s * 32768);
+      const uint32_t d = tmem + (uint32_t)(it & 3) * 128;
+      if (elect_one()) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const uint64_t adv = (uint64_t)(k * 2);
+          umma_tf32(d, xh + adv, bd + adv, make_idesc(128, 128), (it | k) ? 1u : 0u);
+          umma_tf32(d + 64, xl + adv, bd + adv, make_idesc(128, 64), 1u);
+        }
+#pragma unroll
+        for (int c = 0; c < NC; ++c) tc_commit(&bars[1 + c]);
+      }
+      __syncwarp();
+      if (++s == 3) s = 0;
+    }
+    if (elect_one()) tc_commit(&bars[0]);
+    __syncwarp();
+    mbar_wait(&bars[0], 0);
+    if (lane == 0) out[blockIdx.x] = clock64() - t0;
+  } else if (POLL && warp >= 2) {
+    mbar_wait(&bars[0], 0);      // the other warps poll a barrier that completes at the very end, as the epilogue warps do
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512u) : "memory");
+}
+
+// Table-driven MMA pattern: per iteration the warp issues tab.n MMAs {a offset, b offset (bytes from the 1024-aligned base),
+// N, accumulator column}, uniform issue; used to compare operand orderings (which operand slices repeat back to back).
+struct MmaTab { int n; int a[64]; int b[64]; int nn[64]; int d[64]; };
+__global__ void __launch_bounds__(64, 1) k_peak_tab(const __grid_constant__ MmaTab tab, int iters, long long* out) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  __shared__ __align__(8) uint64_t bars[2];
+  __shared__ uint32_t tmem_base_s;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  float* a = reinterpret_cast<float*>(smem);
+  for (int e = threadIdx.x; e < 220 * 1024 / 4; e += blockDim.x) a[e] = (float)((e * 2654435761u) >> 20) * (1.0f / 4096.0f) - 0.5f;
+  if (threadIdx.x == 0) { mbar_init(&bars[0], 1); mbar_init(&bars[1], 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "r"(512u) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_base_s;
+  if (warp == 1) {
+    const uint32_t base = smem_u32(smem);
+    const long long t0 = clock64();
+    for (int it = 0; it < iters; ++it) {
+      for (int m = 0; m < tab.n; ++m) {
+        const uint64_t ad = make_desc(base + (uint32_t)tab.a[m]), bd = make_desc(base + (uint32_t)tab.b[m]);
+        const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(tab.nn[m] >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+        if (elect_one()) umma_tf32(tmem + (uint32_t)tab.d[m], ad, bd, idesc, (it | m) ? 1u : 0u);
+        __syncwarp();
+      }
+    }
+    if (elect_one()) tc_commit(&bars[0]);
+    __syncwarp();
+    mbar_wait(&bars[0], 0);
+    if (lane == 0) out[blockIdx.x] = clock64() - t0;
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512u) : "memory");
+}
+
+// Compile-time MMA orderings for the Taylor product, uniform issue, operands rotating through shared memory the
+// way the real kernel's do: T k-blocks (NB of them, 16 KB apart from offset 0) and X tiles (from 112 KB on).
+//   PAT 0  current:  per (k-block, plane): 4 x [X_hi (N=128, b = T slice) ; X_lo (N=64, same b)]
+//   PAT 1  swapped:  T slice is the a-operand (128 rows), X tiles (208 rows) the b-operand: 4 x [X_hi ; X_lo], N = 208
+//   PAT 2  grouped:  per k-block 4 x [X_r_hi, X_i_hi (N=128), X_r_lo, X_i_lo (N=64)] all on the same T slice
+// out = clocks per k-block-plane equivalent (PAT 2 covers two planes per group: reported per plane).
+template <int PAT, int NB, int EXTRA>
+__global__ void __launch_bounds__(64, 1) k_peak_pat(int iters, long long* out) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  __shared__ __align__(8) uint64_t bars[4];
+  __shared__ uint32_t tmem_base_s;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  float* a = reinterpret_cast<float*>(smem);
+  for (int e = threadIdx.x; e < 224 * 1024 / 4; e += blockDim.x) a[e] = (float)((e * 2654435761u) >> 20) * (1.0f / 4096.0f) - 0.5f;
+  if (threadIdx.x == 0) { for (int i = 0; i < 4; ++i) mbar_init(&bars[i], 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "r"(512u) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_base_s;
+  if (warp == 1) {
+    const uint32_t base = smem_u32(smem), xb = base + 112 * 1024;
+    int kb = 0, s = 0;
+    const long long t0 = clock64();
+    for (int it = 0; it < iters; ++it) {
+      const uint64_t t = make_desc(base + (uint32_t)kb * 16384);
+      if (PAT == 0) {
+        const uint64_t xh = make_desc(xb + (uint32_t)s * 16384), xl = make_desc(xb + (uint32_t)(s + 1) * 16384);
+        const uint32_t d = tmem + (uint32_t)(it & 3) * 128;
+        if (EXTRA & 2) mbar_wait(&bars[1], 1);      // a wait that is already satisfied: its latency only
+        if (EXTRA & 4) tc_fence_after();
+        if (elect_one()) {
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            umma_tf32(d, xh + 2 * k, t + 2 * k, make_idesc(128, 128), (it | k) ? 1u : 0u);
+            umma_tf32(d + 64, xl + 2 * k, t + 2 * k, make_idesc(128, 64), 1u);
+          }
+          if (EXTRA & 1) { tc_commit(&bars[2]); tc_commit(&bars[3]); }
+        }
+        __syncwarp();
+        s += 2; if (s >= 6) s = 0;
+        if (it & 1) { if (++kb == NB) kb = 0; }        // two planes per k-block
+      } else if (PAT == 1) {
+        const uint64_t xh = make_desc(xb + (uint32_t)s * 53248), xl = make_desc(xb + (uint32_t)s * 53248 + 26624);
+        const uint32_t d = tmem + (uint32_t)(it & 1) * 256;
+        if (elect_one()) {
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            umma_tf32(d, t + 2 * k, xh + 2 * k, make_idesc(128, 208), (it | k) ? 1u : 0u);
+            umma_tf32(d, t + 2 * k, xl + 2 * k, make_idesc(128, 208), 1u);
+          }
+        }
+        __syncwarp();
+        s ^= 1;
+        if (it & 1) { if (++kb == NB) kb = 0; }
+      } else {
+        const uint64_t x0 = make_desc(xb + (uint32_t)s * 65536), x1 = make_desc(xb + (uint32_t)s * 65536 + 16384),
+                       x2 = make_desc(xb + (uint32_t)s * 65536 + 32768), x3 = make_desc(xb + (uint32_t)s * 65536 + 49152);
+        if (elect_one()) {
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            umma_tf32(tmem, x0 + 2 * k, t + 2 * k, make_idesc(128, 128), (it | k) ? 1u : 0u);
+            umma_tf32(tmem + 128, x1 + 2 * k, t + 2 * k, make_idesc(128, 128), (it | k) ? 1u : 0u);
+            umma_tf32(tmem + 64, x2 + 2 * k, t + 2 * k, make_idesc(128, 64), 1u);
+            umma_tf32(tmem + 192, x3 + 2 * k, t + 2 * k, make_idesc(128, 64), 1u);
+          }
+        }
+        __syncwarp();
+        s = (s + 1) % 1;      // 4 x 16 KB tiles per group: only one group slot fits beside 112 KB of planes here
+        if (++kb == NB) kb = 0;
+      }
+    }
+    if (elect_one()) tc_commit(&bars[0]);
+    __syncwarp();
+    mbar_wait(&bars[0], 0);
+    if (lane == 0) out[blockIdx.x] = (clock64() - t0) / (PAT == 2 ? 2 : 1);
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512u) : "memory");
 }
 
 // FFMA / DFMA: 8 independent chains per thread, 8 * 2 * iters flops per thread

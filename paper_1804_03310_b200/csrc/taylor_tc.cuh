@@ -1,12 +1,16 @@
 // taylor_tc.cuh -- H7 on the tensor pipe: Phi' = E_h [sum_{k<=K} A^k/k!] E_h Phi  (R3, R9).
-// Persistent CTAs, one walker at a time.  Every product X * T (X = E_h real or A_w complex symmetric, T complex
+// Persistent CTAs, one walker at a time.  Every product X * T (X = D_h = E_h - 1 real, or A_w complex symmetric; T complex
 // M x N_t) is a set of real tcgen05.mma.kind::tf32 products with the 3xTF32 split:
 //     D1 = X_r [T_r | T_i] ,  D2 = X_i [T_r | T_i];  D_re = D1[0:32] - D2[32:64],  D_im = D1[32:64] + D2[0:32]
-//     are combined by the epilogue warps.  Measured: with N this small the kernel is bound by the tensor pipe's
-//     shared-memory operand fetch (~64 B/clk/SM; every MMA re-reads its 4 KB a-operand slice), so the products are
-//     packed into as few, as wide MMAs as possible: X_hi [T_hi | T_lo] is ONE N = 128 MMA (columns 0-63: hi*hi,
-//     64-127: hi*lo) and X_lo T_hi one N = 64 MMA into columns 0-63; the epilogue adds the two column halves.
-// a-operand: 128-row x 32-column tiles of X (hi / lo planes) streamed by TMA through a 3-stage ring;
+//     are combined by the epilogue warps.  X_hi [T_hi | T_lo] is ONE N = 128 MMA (columns 0-63: hi*hi, 64-127: hi*lo) and
+//     X_lo T_hi one N = 64 MMA into columns 64-127 (the cross terms share an accumulator; the epilogue adds the halves).
+// a-operand: X is stored ONCE, in FP32 (A_w as the assembly GEMM wrote it).  128-row x 32-column tiles are streamed by TMA
+//            through a ring of NF stages; the tensor pipe ignores the low 13 mantissa bits of a kind::tf32 operand (measured:
+//            feeding raw FP32 as the hi operand is exact), so the raw tile IS X_hi = trunc(X), and two "splitter" warps
+//            write X_lo = rn_tf32(X - trunc(X)) into one of NL lo buffers (same swizzled offsets, elementwise).  Against
+//            storing hi / lo planes in HBM this halves the bytes A_w costs everywhere: the assembly epilogue's stores, the
+//            Taylor kernel's HBM and L2 reads, and the set of live walkers (148 x 320 KB) now fits the L2, so passes 2-6
+//            over A_w hit it (measured before: the TMA stream alone, MMAs off, took 1.0 ms of the kernel's 1.6).
 // b-operand: T K-major in shared memory, per 32-column k-block 128 rows: [T_r, T_i (hi) | T_r, T_i (lo)],
 //            rewritten by the epilogue warps after every Taylor term (generic -> async proxy fence);
 // accumulators: TMEM, 128 columns per (128-row tile, plane).  The running sum P lives in registers.
@@ -19,21 +23,34 @@ namespace tt {
 
 using namespace tc;
 
-enum { NST = 3, TILE_BYTES = 128 * 128, STG_BYTES = 2 * TILE_BYTES, PLANE_KB_BYTES = 128 * 128, EPW = 8, NTHREADS = (EPW + 2) * 32 };
+enum { NL = 3, TILE_BYTES = 128 * 128, PLANE_KB_BYTES = 128 * 128, EPW = 8, NSPLIT = 3, NTHREADS = 16 * 32 };
+// NSPLIT <= NL <= NF: a parity wait on an mbarrier is only unambiguous within one phase of it.  A splitter that has finished
+// tile it - NSPLIT knows the MMAs of tile it - NSPLIT - NL are done; its wait for the lo buffer of tile `it` needs those of tile
+// it - 2 NL done (a warp that runs two phases ahead sees the parity it waits for as already complete and reads a tile that has
+// not landed -- seen as a hang: the producer's next expect_tx then over-arrives on the full barrier).
+// 16 warps: the two epilogue warpgroups take 200 registers per thread, the producer / MMA / splitter warpgroups 56 (setmaxnreg)
+enum { REGS_EPI = 200, REGS_AUX = 56 };
 
 struct TaylorMaps {
-  CUtensorMap A[2][2];   // [hi/lo][0: 128-row box, 1: last-tile box]  over Abuf viewed as [N_w*M][2*MP]
-  CUtensorMap E[2][2];   // same for D_h = E_h - 1 [M][MP]
+  CUtensorMap A[2];   // [0: 128-row box, 1: last-tile box] over Abuf viewed as [N_w*M][2*MP] FP32
+  CUtensorMap E[2];   // same for D_h = E_h - 1 [M][MP] FP32
 };
 
 struct TaylorTcArgs {
   int M, MP, nt, K, nw;
   int mtiles, rows_last, nkb;   // 128-row tiles, rows of the last one (multiple of 8), 32-column k-blocks
+  int nf;                       // FP32 tile stages in the TMA ring (what shared memory leaves: 5, or 4 at nkb = 8)
   cplx<float>* phi;             // [nw][M][nt] in/out
-  int dbg;                      // timing experiments only (AFQMC_TAYLOR_DBG): 1 no TMA, 2 no epilogue data movement, 4 no MMA
 };
 
-inline size_t smem_bytes(int nkb) { return (size_t)nkb * PLANE_KB_BYTES + (size_t)NST * STG_BYTES + 1024; }
+enum { NF_MAX = 6 };
+static_assert(NSPLIT <= NL, "see above");
+inline int pick_nf(int nkb) {   // >= NL (the splitters' wait order relies on it)
+  const int left = 227 * 1024 - 1024 - 512 - nkb * PLANE_KB_BYTES - NL * TILE_BYTES;
+  const int nf = left / TILE_BYTES;
+  return nf > NF_MAX ? NF_MAX : nf;
+}
+inline size_t smem_bytes(int nkb) { return (size_t)nkb * PLANE_KB_BYTES + (size_t)(pick_nf(nkb) + NL) * TILE_BYTES + 1024; }
 
 // byte offset of element (row b in 0..127, column j) inside the K-major SWIZZLE_128B T operand
 __device__ __forceinline__ uint32_t plane_off(int b, int j) {
@@ -66,27 +83,32 @@ enum { MAXE = 32 };   // complex elements of Phi_w per epilogue thread: M * N_t 
 __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant__ TaylorMaps maps, TaylorTcArgs g) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  __shared__ __align__(8) uint64_t full_bar[NST];
-  __shared__ __align__(8) uint64_t empty_bar[NST];
+  __shared__ __align__(8) uint64_t full_bar[NF_MAX];   // TMA has landed an FP32 tile (= X_hi)
+  __shared__ __align__(8) uint64_t empty_bar[NF_MAX];  // the MMAs that read it have completed
+  __shared__ __align__(8) uint64_t lo_full_bar[NL];    // a splitter warp has written X_lo
+  __shared__ __align__(8) uint64_t lo_empty_bar[NL];   // the MMAs that read it have completed
   __shared__ __align__(8) uint64_t tmem_full_bar[2];   // per 128-row tile: tile 0 is post-processed while tile 1 is issued
-  __shared__ __align__(8) uint64_t b_ready_bar[8];     // per (tile, lane quarter) = 32-column k-block of the T operand
+  __shared__ __align__(8) uint64_t b_ready_bar[2];     // per tile of the PREVIOUS product = 4 k-blocks of the T operand (8 warps arrive)
   __shared__ __align__(8) uint64_t t_free_bar[4];      // last tile has consumed k-block kb < 4 of the current T
   __shared__ uint32_t tmem_base_s;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int M = g.M, nt = g.nt, nkb = g.nkb, mtiles = g.mtiles;
+  const int M = g.M, nt = g.nt, nkb = g.nkb, mtiles = g.mtiles, NF = g.nf;
   const uint32_t plane_bytes = (uint32_t)nkb * PLANE_KB_BYTES;
   uint8_t* planes = smem;                                   // rows 0-31 T_r hi, 32-63 T_i hi, 64-95 T_r lo, 96-127 T_i lo
-  uint8_t* stages = smem + (size_t)plane_bytes;
+  uint8_t* stages = smem + (size_t)plane_bytes;             // NF FP32 tiles, then NL lo tiles
+  uint8_t* lobufs = stages + (size_t)NF * TILE_BYTES;
   const int nphase = g.K + 2;
   const uint32_t tmem_cols = 512u;
 
-  // zero the planes once: rows >= nt and columns >= M must stay 0 for the whole kernel
-  for (uint32_t o = threadIdx.x * 16; o < plane_bytes; o += NTHREADS * 16)
+  // zero the planes once (rows >= nt and columns >= M must stay 0 for the whole kernel) and the tile buffers (rows past a
+  // short last tile are never written by TMA and must not hold NaN patterns)
+  for (uint32_t o = threadIdx.x * 16; o < plane_bytes + (uint32_t)(NF + NL) * TILE_BYTES; o += NTHREADS * 16)
     *reinterpret_cast<uint4*>(planes + o) = make_uint4(0, 0, 0, 0);
   if (warp == EPW && lane == 0) {
-    for (int s = 0; s < NST; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
+    for (int s = 0; s < NF_MAX; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
+    for (int s = 0; s < NL; ++s) { mbar_init(&lo_full_bar[s], 1); mbar_init(&lo_empty_bar[s], 1); }
     mbar_init(&tmem_full_bar[0], 1); mbar_init(&tmem_full_bar[1], 1);
-    for (int x = 0; x < 8; ++x) mbar_init(&b_ready_bar[x], 2);   // the re and the im warp of that quarter
+    mbar_init(&b_ready_bar[0], EPW); mbar_init(&b_ready_bar[1], EPW);
     for (int x = 0; x < 4; ++x) mbar_init(&t_free_bar[x], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -101,80 +123,123 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_base_s;
+  // tiles of this CTA: every (walker, phase, tile, k-block, plane), in this order in all three pipeline roles
+  const int n_mine = blockIdx.x < g.nw ? (g.nw - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
+  const uint32_t tiles_per_walker = (uint32_t)(mtiles * nkb) * (uint32_t)(2 * g.K + 2);
 
   if (warp == EPW) {
-    if (lane == 0 && !(g.dbg & 1)) {   // ===== TMA producer: streams X tiles for every (walker, phase, tile, k-block, plane) =====
-      uint32_t it = 0;
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"((int)REGS_AUX));
+    if (lane == 0) {   // ===== TMA producer: streams FP32 X tiles =====
+      int s = 0;
+      uint32_t par = 1;
       for (int w = blockIdx.x; w < g.nw; w += gridDim.x)
         for (int ph = 0; ph < nphase; ++ph) {
-          const bool cx = ph >= 1 && ph <= g.K;           // complex A_w, else real E_h
+          const bool cx = ph >= 1 && ph <= g.K;           // complex A_w, else real D_h
           for (int mt = 0; mt < mtiles; ++mt) {
             const int last = mt == mtiles - 1;
-            const uint32_t bytes = 2u * (uint32_t)(last ? g.rows_last : 128) * 128u;
+            const uint32_t bytes = (uint32_t)(last ? g.rows_last : 128) * 128u;
             for (int kb = 0; kb < nkb; ++kb)
-              for (int p = 0; p < (cx ? 2 : 1); ++p, ++it) {
-                const int s = it % NST;
-                mbar_wait(&empty_bar[s], ((it / NST) & 1) ^ 1);
-                uint8_t* st = stages + (size_t)s * STG_BYTES;
+              for (int p = 0; p < (cx ? 2 : 1); ++p) {
+                mbar_wait(&empty_bar[s], par);
+                uint8_t* st = stages + (size_t)s * TILE_BYTES;
                 mbar_expect_tx(&full_bar[s], bytes);
-                if (cx) {
-                  tma_load_2d(st, &maps.A[0][last], &full_bar[s], p * g.MP + kb * 32, w * M + mt * 128);
-                  tma_load_2d(st + TILE_BYTES, &maps.A[1][last], &full_bar[s], p * g.MP + kb * 32, w * M + mt * 128);
-                } else {
-                  tma_load_2d(st, &maps.E[0][last], &full_bar[s], kb * 32, mt * 128);
-                  tma_load_2d(st + TILE_BYTES, &maps.E[1][last], &full_bar[s], kb * 32, mt * 128);
-                }
+                if (cx) tma_load_2d(st, &maps.A[last], &full_bar[s], p * g.MP + kb * 32, w * M + mt * 128);
+                else tma_load_2d(st, &maps.E[last], &full_bar[s], kb * 32, mt * 128);
+                if (++s == NF) { s = 0; par ^= 1; }
               }
           }
         }
+    }
+  } else if (warp >= EPW + 2 + NSPLIT) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"((int)REGS_AUX));   // idle warps that complete the last warpgroup
+  } else if (warp >= EPW + 2) {
+    // ===== splitter warps: X_lo = rn_tf32(X - trunc13(X)), elementwise at the same (swizzled) offsets.  The warps take the
+    // tiles round robin, so one tile has NSPLIT stage times to get through its barrier wake-ups, 32 LDS.128 / STS.128 per
+    // lane and the proxy fence =====
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"((int)REGS_AUX));
+    const int sw = warp - (EPW + 2);
+    const uint32_t total = (uint32_t)n_mine * tiles_per_walker;
+    for (uint32_t it = sw; it < total; it += NSPLIT) {
+      const int s = it % NF, sl = it % NL;
+      // order matters: a parity wait is only unambiguous within one phase of the barrier.  Once the MMAs of tile it - NL have
+      // completed (lo buffer free), every tile up to it - NL has been loaded, and NL <= NF: the previous user of stage s is
+      // among them, so full_bar[s] is exactly in the phase this tile completes
+      mbar_wait(&lo_empty_bar[sl], ((it / NL) & 1) ^ 1);
+      mbar_wait(&full_bar[s], (it / NF) & 1);
+      const uint4* src = reinterpret_cast<const uint4*>(stages + (size_t)s * TILE_BYTES);
+      uint4* dst = reinterpret_cast<uint4*>(lobufs + (size_t)sl * TILE_BYTES);
+#pragma unroll
+      for (int u = 0; u < TILE_BYTES / 16 / 32; u += 8) {
+        uint4 v[8];
+#pragma unroll
+        for (int x = 0; x < 8; ++x) v[x] = src[(u + x) * 32 + lane];
+#pragma unroll
+        for (int x = 0; x < 8; ++x) {
+          uint4 r;
+          r.x = tf32_lo_bits(v[x].x); r.y = tf32_lo_bits(v[x].y); r.z = tf32_lo_bits(v[x].z); r.w = tf32_lo_bits(v[x].w);
+          dst[(u + x) * 32 + lane] = r;
+        }
+      }
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      __syncwarp();
+      if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&lo_full_bar[sl])) : "memory");
     }
   } else if (warp == EPW + 1) {
-    if (lane == 0) {   // ===== MMA issuer =====
-      constexpr uint32_t idesc128 = make_idesc(128, 128), idesc64 = make_idesc(128, 64);
-      const uint32_t pl = smem_u32(planes);
-      uint32_t it = 0, gph = 0;
-      for (int w = blockIdx.x; w < g.nw; w += gridDim.x)
-        for (int ph = 0; ph < nphase; ++ph, ++gph) {
-          const bool cx = ph >= 1 && ph <= g.K;
-          for (int mt = 0; mt < mtiles; ++mt) {
-            for (int kb = 0; kb < nkb; ++kb) {
-              if (mt == 0 && (kb & 3) == 0) {
-                // k-blocks kb..kb+3 of this phase's T are in shared memory, and (all 8 epilogue warps arrive on
-                // them after their TMEM loads) the accumulators of tile kb/4 have been read
-                for (int x = 0; x < 4; ++x) mbar_wait(&b_ready_bar[kb + x], gph & 1);
-                tc_fence_after();
-              }
-              for (int p = 0; p < (cx ? 2 : 1); ++p, ++it) {
-                const uint32_t d = tmem + (mt * 2 + p) * 128;
-                const int s = it % NST;
-                if (!(g.dbg & 1)) mbar_wait(&full_bar[s], (it / NST) & 1);
-                tc_fence_after();
-                const uint32_t sa = smem_u32(stages + (size_t)s * STG_BYTES);
-                const uint64_t x_hi = make_desc(sa), x_lo = make_desc(sa + TILE_BYTES);
-                const uint32_t kboff = (uint32_t)kb * PLANE_KB_BYTES;
-                const uint64_t t_all = make_desc(pl + kboff);   // 128 rows: hi then lo; its first 64 rows = T_hi
-                const bool first = kb == 0;
+    // ===== MMA issuer warp.  The whole warp runs the loop (uniform control flow) and ONE elected lane issues: with the
+    // descriptors computed under uniform control flow ptxas keeps them in uniform registers and the 8 MMAs of a tile are 8
+    // back-to-back UTCHMMA.  Inside an `if (lane == 0)` region it wraps every MMA in an ELECT / 5 x R2UR / branch-back
+    // sequence.  What a tile costs beyond its 448 clk of tensor-pipe time is this warp's scalar code between two tiles (the
+    // pipe's queue is short), so that code is kept minimal: incremental descriptors, no divisions, one barrier wait. =====
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"((int)REGS_AUX));
+    constexpr uint32_t idesc128 = make_idesc(128, 128), idesc64 = make_idesc(128, 64);
+    const uint64_t xh0 = make_desc(smem_u32(stages)), xl0 = make_desc(smem_u32(lobufs)), t0 = make_desc(smem_u32(planes));
+    constexpr uint64_t TSTEP = TILE_BYTES >> 4;     // descriptor address field counts 16-byte units
+    uint64_t xh = xh0, xl = xl0;
+    uint32_t gph = 0;
+    int s = 0, sl = 0;
+    uint32_t lpar = 0;
+    for (int w = blockIdx.x; w < g.nw; w += gridDim.x)
+      for (int ph = 0; ph < nphase; ++ph, ++gph) {
+        const int np = (ph >= 1 && ph <= g.K) ? 2 : 1;
+        for (int mt = 0; mt < mtiles; ++mt) {
+          uint64_t t_all = t0;                       // k-block kb of T: 128 rows (hi then lo); its first 64 rows = T_hi
+          for (int kb = 0; kb < nkb; ++kb, t_all += TSTEP) {
+            // k-blocks 4 j .. 4 j + 3 of this phase's T are in shared memory, and (all 8 epilogue warps arrive after their
+            // TMEM loads) the accumulators of tile j have been read
+            if (mt == 0 && (kb & 3) == 0) mbar_wait(&b_ready_bar[kb >> 2], gph & 1);
+            for (int p = 0; p < np; ++p) {
+              const uint32_t d = tmem + (mt * 2 + p) * 128;
+              mbar_wait(&lo_full_bar[sl], lpar);     // the splitter arrives after it has seen the TMA tile: X_hi is in place too
+              tc_fence_after();
+              if (elect_one()) {
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
-                  if (g.dbg & 4) break;
                   const uint64_t adv = (uint64_t)(k * 2);   // 8 tf32 = 32 bytes = 2 x 16 B
-                  umma_tf32(d, x_hi + adv, t_all + adv, idesc128, (first && k == 0) ? 0u : 1u);
+                  umma_tf32(d, xh + adv, t_all + adv, idesc128, (kb == 0 && k == 0) ? 0u : 1u);
                   // X_lo T_hi joins the other cross term in columns 64-127: the large hi*hi accumulator of columns 0-63 then
                   // sees half as many (truncating) accumulations, the small cross-term accumulator's truncation is 2^-11 down
-                  umma_tf32(d + 64, x_lo + adv, t_all + adv, idesc64, 1u);
+                  umma_tf32(d + 64, xl + adv, t_all + adv, idesc64, 1u);
                 }
                 tc_commit(&empty_bar[s]);
+                tc_commit(&lo_empty_bar[sl]);
+                if (p == np - 1) {
+                  if (mtiles == 2 && mt == 1 && kb < 4) tc_commit(&t_free_bar[kb]);
+                  if (kb == nkb - 1) tc_commit(&tmem_full_bar[mt]);
+                }
               }
-              if (mtiles == 2 && mt == 1 && kb < 4) tc_commit(&t_free_bar[kb]);
+              __syncwarp();
+              xh += TSTEP; xl += TSTEP;
+              if (++s == NF) { s = 0; xh = xh0; }
+              if (++sl == NL) { sl = 0; xl = xl0; lpar ^= 1; }
             }
-            tc_commit(&tmem_full_bar[mt]);
           }
         }
-    }
-  } else {   // ===== epilogue warps 0..7: TMEM lane quarter = warp & 3, half = warp >> 2 (0: real part, 1: imaginary) =====
+      }
+  } else if (warp < EPW) {   // ===== epilogue warps 0..7: TMEM lane quarter = warp & 3, half = warp >> 2 (0: real part, 1: imaginary) =====
     // Rows i = mt*128 + q*32 + lane of the product are k-block mt*4+q of the next T operand.  Tile 0 is post-processed
     // and written back while tile 1 is being issued (each k-block as soon as tile 1 has consumed it), and the next
     // phase starts on k-blocks 0-3 while tile 1 is post-processed: the tensor pipe does not wait between phases.
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"((int)REGS_EPI));
     const int q = warp & 3, half = warp >> 2;
     const uint32_t plu = smem_u32(planes);
     const uint32_t pl_hi = plu, pl_lo = plu + 64 * 128;   // lo rows start 64 rows further down inside every k-block
@@ -235,8 +300,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
         tc_fence_before();
         asm volatile("bar.sync 1, 256;" ::: "memory");
         if (lane == 0)
-          for (int mt = 0; mt < mtiles; ++mt)
-            asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&b_ready_bar[mt * 4 + q])) : "memory");
+          for (int mt = 0; mt < 2; ++mt)
+            asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&b_ready_bar[mt])) : "memory");
       }
       for (int ph = 0; ph < nphase; ++ph, ++gph) {
         const bool last_phase = ph == nphase - 1;
@@ -250,10 +315,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
             float v[32];
             mbar_wait(&tmem_full_bar[mt], gph & 1);
             tc_fence_after();
-            if (g.dbg & 2) {
-#pragma unroll
-              for (int b = 0; b < 32; ++b) v[b] = 0.f;
-            } else {
+            {
               float u0[32], u1[32];
               tmem_ld32x2(tl + (mt * 2 + 0) * 128 + half * 32, tl + (mt * 2 + 0) * 128 + 64 + half * 32, u0, u1);
 #pragma unroll
@@ -317,7 +379,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
               // k-block mt*4+q of T may be overwritten once every MMA that reads it has completed: for the last
               // tile that is tmem_full (above), for tile 0 of two the last tile's pass over that k-block
               if (mt == 0 && mtiles == 2) mbar_wait(&t_free_bar[q], gph & 1);
-              if (i < M && !(g.dbg & 2)) {
+              if (i < M) {
 #pragma unroll
                 for (int b = 0; b < 32; ++b)
                   if (b < nt) {
@@ -330,7 +392,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
               tc_fence_before();
               __syncwarp();
               if (lane == 0)
-                asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&b_ready_bar[mt * 4 + q])) : "memory");
+                asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&b_ready_bar[mt])) : "memory");
             }
           }
         }
