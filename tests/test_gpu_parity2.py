@@ -228,6 +228,7 @@ def _run_ortho(wl, nw, steps, idx=None):
     ost = orc.o_seed_state(ini, wl.walkers(nw)[sel], wl.n_alpha)
     s32 = F.seed32(i32, wl.walkers(nw)[sel], wl.n_alpha)
     per_step = []
+    kappa = np.ones(sel.shape[0])
     for n in range(1, steps + 1):
         w_prev = ost.w
         ost, rec = orc.o_step(ini, ost, xs[n - 1][sel], wl.n_alpha, K=wl.K, E0=wl.E0)
@@ -237,14 +238,18 @@ def _run_ortho(wl, nw, steps, idx=None):
         # relative error unbounded for a walker about to be killed)
         den = w_prev * np.exp(wl.dt * wl.E0) * rec["absI"]
         den = np.where(den > 0, den, 1.0)
-        per_step.append(dict(alive=alive,
+        with np.errstate(all="ignore"):
+            kn = H.cond_number(wl, ost.phi)
+        kappa = np.maximum(kappa, np.where(np.isfinite(kn), kn, np.inf))
+        per_step.append(dict(alive=alive & np.isfinite(kappa), kappa=kappa.copy(),
+                             amp_w=np.maximum(1.0, wl.dt * np.sum(np.abs(rec["f_used"]) ** 2, axis=-1)),
                              E_gpu=H.energy_err_w(eloc[n - 1][sel], ost.eloc, rec["f"]), E_32=H.energy_err_w(s32.eloc, ost.eloc, rec["f"]),
                              w_gpu=np.abs(wm[n - 1][sel] - ost.w) / den, w_32=np.abs(s32.w - ost.w) / den))
         if n % 2 == 0:
             q, s = orc.o_orthonormalize(ost.phi, ost.S, wl.n_alpha)
             ost = orc.OracleState(q, ost.w, s, ost.theta, ost.f_a, ost.f_b, ost.eloc)
             s32 = F.ortho32(s32, wl.n_alpha)
-    final = dict(alive=(ost.w > 0) & np.isfinite(ost.S),
+    final = dict(alive=(ost.w > 0) & np.isfinite(ost.S) & np.isfinite(kappa), kappa=kappa,
                  phi_gpu=H.rel_fro_w(out["phi"][sel], ost.phi), phi_32=H.rel_fro_w(s32.phi.astype(np.complex128), ost.phi),
                  S_gpu=H.rel_abs_w(out["S"][sel], ost.S), S_32=H.rel_abs_w(s32.S, ost.S),
                  f_gpu=H.rel_fro_w(out["f"][sel], ost.f_a + ost.f_b, H.fb_floor(ini)),
@@ -279,37 +284,46 @@ def test_free_run_ortho_flat_tolerance(cfg, variant):
 def test_free_run_ortho_vs_fp32_floor(cfg, variant):
     """The same schedule on the literal / mean-field-subtracted configs (violent: ||A||_2 ~ 1.8, walkers die within ~8 steps,
     errors of ANY FP32 pipeline are amplified chaotically once kappa grows -- tests/test_fp32_floor.py).  Graded over the walkers
-    alive in the oracle, per step: the GPU's worst error must stay below max(2e-4, 16 x the worst error of the plain numpy
-    complex64 pipeline over the same walkers at the same step) -- no kappa model, no step accumulation.  Why 16: measured at
-    step 1 (kappa ~ 2, nothing amplified yet) the 3xTF32 tensor-pipe GEMMs leave S at 4e-6 where plain FP32 leaves 4e-7 (the
-    tensor pipe accumulates with truncation; gemm_path 1 reproduces the numpy figures digit for digit), and
-    the later steps amplify both by the same chaotic factors."""
+    alive in the oracle, per step, two ways:
+      * the TYPICAL walker (median, steps with >= 4 alive) against the measured floor, no kappa model: median error <=
+        max(2e-4, 16 x median error of the plain numpy complex64 pipeline on the same walkers).  Why 16: at step 1 (kappa ~ 2,
+        nothing amplified yet) the 3xTF32 tensor-pipe GEMMs leave S at 4e-6 where plain FP32 leaves 4e-7 (the tensor pipe
+        accumulates with truncation, DESIGN.md 7; gemm_path 1 reproduces the numpy figures digit for digit);
+      * the WORST walker against protocol B's budget (per-step tolerance scaled by the largest kappa met, times the steps taken):
+        the maximum over a chaotic ensemble is a single-sample quantity, two FP32 pipelines differ by an order of magnitude on it."""
     wl = make_workload(cfg, variant)
     nw, steps = SMALL[cfg], 10
     tol = H.tol_for(wl)
     per_step, final, out = _run_ortho(wl, nw, steps)
-    worst_ratio, raw, raw32, n_alive = 0.0, {}, {}, []
-    for p in per_step:
+    med_ratio, worst_ratio, raw, raw32, n_alive = 0.0, 0.0, {}, {}, []
+    for n, p in enumerate(per_step):
         a = p["alive"]
         n_alive.append(int(a.sum()))
         if not np.any(a):
             continue
+        tw = (n + 1) * H.walker_tol(wl, p["kappa"])
         for k in ("E", "w"):
-            g, r = float(p[f"{k}_gpu"][a].max()), float(p[f"{k}_32"][a].max())
-            raw[k], raw32[k] = max(raw.get(k, 0.0), g), max(raw32.get(k, 0.0), r)
-            worst_ratio = max(worst_ratio, g / max(tol, 16 * r))
+            g, r = p[f"{k}_gpu"][a], p[f"{k}_32"][a]
+            raw[k], raw32[k] = max(raw.get(k, 0.0), float(g.max())), max(raw32.get(k, 0.0), float(r.max()))
+            # log w' contains c = x.xbar - xbar.xbar/2 of size dt ||f||^2 (protocol A): the weight budget carries that factor,
+            # accumulated like the rest
+            amp = np.maximum.accumulate(np.stack([q["amp_w"] for q in per_step[:n + 1]]), axis=0)[-1][a] if k == "w" else 1.0
+            worst_ratio = max(worst_ratio, float(np.max(g / (tw[a] * amp))))
+            if a.sum() >= 4:
+                med_ratio = max(med_ratio, float(np.median(g)) / max(tol, 16 * float(np.median(r))))
     a = final["alive"]
     if np.any(a):
+        tw = steps * H.walker_tol(wl, final["kappa"])
         for k in ("phi", "S", "f"):
-            g, r = float(final[f"{k}_gpu"][a].max()), float(final[f"{k}_32"][a].max())
-            raw[k], raw32[k] = g, r
-            worst_ratio = max(worst_ratio, g / max(tol, 16 * r))
-    print(f"cfg{cfg}/{variant} afqmc_run E/1 QR/2, 10 free-running steps, alive per step {n_alive}: GPU raw {raw}; "
-          f"plain complex64 numpy {raw32}; worst err / max(2e-4, 16 x numpy) = {worst_ratio:.3f}")
-    H.record("free_run_ortho_vs_floor", cfg=cfg, variant=variant, alive=n_alive, ratio=worst_ratio,
+            g, r = final[f"{k}_gpu"][a], final[f"{k}_32"][a]
+            raw[k], raw32[k] = float(g.max()), float(r.max())
+            worst_ratio = max(worst_ratio, float(np.max(g / tw[a])))
+    print(f"cfg{cfg}/{variant} afqmc_run E/1 QR/2, 10 free-running steps, alive per step {n_alive}: GPU raw max {raw}; "
+          f"plain complex64 numpy max {raw32}; median err / max(2e-4, 16 x numpy median) = {med_ratio:.3f}; worst err / protocol-B budget = {worst_ratio:.3f}")
+    H.record("free_run_ortho_vs_floor", cfg=cfg, variant=variant, alive=n_alive, median_ratio=med_ratio, worst_ratio=worst_ratio,
              **{f"gpu_{k}": v for k, v in raw.items()}, **{f"numpy_c64_{k}": v for k, v in raw32.items()})
     assert n_alive[0] > 0
-    assert worst_ratio < 1.0
+    assert med_ratio < 1.0 and worst_ratio < 1.0
     assert np.all(np.isfinite(out["phi"].view(np.float64)[np.isfinite(out["w"]) & (out["w"] > 0)]))
 
 
