@@ -57,6 +57,35 @@ def peaks():
     return dict(hbm=6650.0, bf16_burst=1590.0, bf16_sust=1400.0, sm_max_mhz=1965.0, source="fallback")
 
 
+def measure_peaks(device):
+    """Self-written microbenchmarks (csrc/peaks.cuh, afqmc_peak_probe): the TF32 / FP32 / FP64 / L2 denominators the fractions are
+    quoted against.  ~50 ms in total."""
+    import torch
+    import paper_1804_03310_b200 as afq
+    scr = torch.zeros(96 << 20, dtype=torch.uint8, device=device)
+
+    def best(kind, n, iters, rep=3):
+        r = [afq.afqmc_peak_probe(kind, n, iters, scr) for _ in range(rep)]
+        return min(r, key=lambda t: t[0])
+    out = {}
+    for key, kind in (("tf32_ss_n256", 0), ("tf32_ts_n256", 1), ("tf32_pair_n256", 2)):
+        ms, fl, clk = best(kind, 256, 8000)
+        out[key] = dict(tflops=fl / ms / 1e9, clk_per_mma=clk)
+    ms, fl, clk = best(0, 128, 8000)
+    out["tf32_ss_n128"] = dict(tflops=fl / ms / 1e9, clk_per_mma=clk)
+    ms, fl, clk = best(0, 64, 8000)
+    out["tf32_ss_n64"] = dict(tflops=fl / ms / 1e9, clk_per_mma=clk)
+    ms, fl, _ = best(3, 0, 100000)
+    out["ffma_tflops"] = fl / ms / 1e9
+    ms, fl, _ = best(4, 0, 100000)
+    out["dfma_tflops"] = fl / ms / 1e9
+    ms, by, _ = best(5, 48, 3000)
+    out["l2_to_smem_tma_gbs"] = by / ms / 1e6
+    out["note"] = ("back-to-back tcgen05.mma.kind::tf32 M=128 (pair: M=256) K=8 from shared memory (ss), with the a-operand in TMEM (ts), "
+                   "on CTA pairs; FFMA / DFMA 8 chains per thread; TMA stream of a 48 MiB (L2-resident) buffer into shared memory")
+    return out
+
+
 class ClockSampler(threading.Thread):
     """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -321,52 +350,113 @@ def run_ours(args):
                                  achieved_gbs=pb / (p_ms * 1e-3) / 1e9 if p_ms else None),
                      note="one afqmc_run call: propagate-only steps (no energy contraction) except the measured one")
 
+    # ---- launch-latency-bound configs (M < 96: cfgs 1-4): the same K steps as ONE CUDA graph replay ----
+    graph = None
+    if wl.M < 96 and not args.no_graph:
+        xg = x[torch.arange(K, device=dev) % nfield].contiguous()
+        elg = torch.zeros(K, nw, dtype=torch.complex128, device=dev)
+        reseed()
+        side = torch.cuda.Stream(device=dev)
+        side.wait_stream(torch.cuda.current_stream(dev))
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(side):
+            ctx.use_stream(side)
+            ctx.afqmc_step(st.phi, st.weight, st.ovlp, st.theta, st.fb, xg, K, elg, st.flags)   # warm on the capture stream
+            side.synchronize()
+            reseed()
+            lg = ctx.launch_count
+            with torch.cuda.graph(g, stream=side):
+                ctx.afqmc_step(st.phi, st.weight, st.ovlp, st.theta, st.fb, xg, K, elg, st.flags)
+            lg = ctx.launch_count - lg
+            g.replay(); side.synchronize()
+            reseed(); side.synchronize()
+            eg0, eg1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            eg0.record(side)
+            g.replay()
+            eg1.record(side)
+            side.synchronize()
+            ms_g = eg0.elapsed_time(eg1)
+            # empty-launch floor: the library's smallest kernel (k_mixed_ratio, one thread of work), launched back to back
+            o3 = torch.ones(3, dtype=torch.float64, device=dev)
+            o1 = torch.zeros(1, dtype=torch.complex128, device=dev)
+            for _ in range(20):
+                ctx.afqmc_mixed_energy(o3, 1, o1)
+            side.synchronize()
+            eg0.record(side)
+            for _ in range(200):
+                ctx.afqmc_mixed_energy(o3, 1, o1)
+            eg1.record(side)
+            side.synchronize()
+            floor_us = eg0.elapsed_time(eg1) * 1e3 / 200
+        ctx.use_stream(torch.cuda.current_stream(dev))
+        ms_g = D.max_over_ranks(ms_g, dev)
+        graph = dict(value=world * nw * K / (ms_g * 1e-3), unit=UNIT, us_per_step=ms_g * 1e3 / K, kernels_in_graph=lg,
+                     eager_us_per_step=ms_max * 1e3 / K, launch_floor_us_per_kernel=floor_us,
+                     floor_us_per_step=floor_us * lg / K,
+                     note="one afqmc_step(n_steps) call captured into a CUDA graph and replayed; the floor is the measured "
+                          "back-to-back launch rate of a one-CTA kernel times the kernels per step")
+
+    mp = measure_peaks(dev)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
     pk = peaks()
     fl = flops_per_walker_step(wl)
-    value = D.whole_job_rate(nw * K, world, ms_max * 1e-3)
-    # roofline of the dominant kernel = the stage with the largest device time (CUDA events on the launching
-    # stream, afqmc_profile_*); the H6 assembly GEMM is always reported beside it as `roofline_h6`
-    M_, ng_ = wl.M, wl.n_chol
-    if ctx.gemm_path >= 2:
-        # the tcgen05 assembly GEMM exploits A = A^T: its algorithmic work is the upper triangle only
-        fl["assemble"] = 4.0 * ng_ * M_ * (M_ + 1) / 2
-        peak, peak_note = 0.5 * pk["bf16_burst"], (
-            f"TF32 dense = {pk['source']} burst BF16 {pk['bf16_burst']} TF/s x nominal TF32/BF16 ratio 0.5 (each kernel runs "
-            f"0.2-1.6 ms inside a ~3.4 ms step, no power-cap reason active; sustained figure would be {0.5 * pk['bf16_sust']:.0f}); "
-            "achieved counts ALGORITHMIC flops and 3xTF32 issues 3x of them, so frac <= 1/3 by construction")
-        bound, dtype = "tensor", "tf32x3"
-    else:
-        fp32_peak = 148 * 128 * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
-        bound, peak, peak_note = "alu", fp32_peak, "FP32 FMA: 148 SMs x 128 lanes x 2 flop x clocks.max.sm (DESIGN.md)"
-        dtype = "f32" if wl.precision == "c64" else "f64"
-        if wl.precision == "c128":
-            peak, peak_note = fp32_peak / 2, "FP64 FMA: 148 SMs x 64 lanes x 2 flop x clocks.max.sm (DESIGN.md)"
-    names = dict(assemble="H6 assembly GEMM A_w = sum_g z_g L_g (tc::k_gemm_tf32_pair<EpiAssembleSym> / k_gemm_tf32 / k_gemm_nt)",
-                 taylor="H7 Taylor propagator (tt::k_taylor_tc / k_taylor)",
-                 energy="H9 energy GEMMs + fused dot (or H10 multi-det energy)", force_bias="H4 force-bias GEMMs",
-                 green="H1-H3/H8 overlap, LU, Theta, weights (k_green)")
-    traffic_ncu = {"assemble": 2.227e9, "taylor": 2.131e9} if (ctx.gemm_path >= 2 and args.cfg == 5) else {}
+    headline_ms = ms_max
+    if graph is not None:          # latency-bound configs: the graph replay is the library's fast path and the headline
+        headline_ms = graph["us_per_step"] * K * 1e-3
+    value = D.whole_job_rate(nw * K, world, headline_ms * 1e-3)
+    M_, ng_, nt_ = wl.M, wl.n_chol, wl.n_t
+    tensor_path = ctx.gemm_path >= 2
+    tay_tc = tensor_path and 96 <= M_ <= 256 and nt_ <= 32
+    if tensor_path:
+        fl["assemble"] = 4.0 * ng_ * M_ * (M_ + 1) / 2       # the tcgen05 assembly GEMM exploits A = A^T: upper triangle only
+    if wl.n_det > 1:
+        # H10: TT = C_act^T X Theta_0 for all X (one GEMM), W / WT per operator, E x E work per determinant
+        nact, nd = wl.n_act, wl.n_det
+        fl["energy"] = (4.0 * (ng_ + 1) * nact * M_ * nt_ + sum(16.0 * (nact - n) * n * n for n in (wl.n_alpha, wl.n_beta)) * (ng_ + 1)
+                        + 120.0 * nd * (ng_ + 1))
+    tf32_peak = max(mp["tf32_ss_n256"]["tflops"], mp["tf32_pair_n256"]["tflops"])
+    tensor_note = (f"TF32 dense MEASURED by back-to-back tcgen05.mma.kind::tf32 N=256 on every SM (afqmc_peak_probe): {tf32_peak:.0f} TFLOP/s "
+                   f"(nominal-ratio estimate 0.5 x BF16 {pk['bf16_burst']:.0f} = {0.5 * pk['bf16_burst']:.0f}); achieved counts ALGORITHMIC flops and "
+                   "3xTF32 issues 3x of them, so frac <= 1/3 by construction")
+    fp32_note = f"FP32 FMA MEASURED (8 chains per thread, afqmc_peak_probe): {mp['ffma_tflops']:.1f} TFLOP/s (nominal 148 x 128 x 2 x {pk['sm_max_mhz']:.0f} MHz = {148 * 128 * 2 * pk['sm_max_mhz'] * 1e-6:.1f})"
+    fp64_note = f"FP64 FMA MEASURED (afqmc_peak_probe): {mp['dfma_tflops']:.1f} TFLOP/s"
+    alu_peak, alu_note = (mp["dfma_tflops"], fp64_note) if wl.precision == "c128" else (mp["ffma_tflops"], fp32_note)
+    kind = dict(assemble="tensor" if tensor_path else "alu", force_bias="tensor" if tensor_path else "alu",
+                taylor="tensor" if tay_tc else "alu", energy="alu" if wl.n_det > 1 else ("tensor" if tensor_path else "alu"), green="hbm")
+    names = dict(assemble="H6 assembly GEMM A_w = sum_g z_g L_g (" + ("tc::k_gemm_tf32_pair_ps<EpiAssembleSym>" if tensor_path else "k_gemm_nt") + ")",
+                 taylor="H7 Taylor propagator (" + ("tt::k_taylor_tc" if tay_tc else "k_taylor, FP32/FP64 SIMT") + ")",
+                 energy=("H10 multi-determinant energy (TT GEMM + k_md_energy_b, FP32 SIMT)" if wl.n_det > 1 else
+                         "H9 energy GEMMs + fused dot (" + ("tc::k_gemm_tf32_pair<EpiEnergy>" if tensor_path else "k_gemm_nt") + ")"),
+                 force_bias="H4 force-bias GEMMs", green="H1-H3/H8 overlap, LU, Theta, weights (k_green)")
+    dtype = "tf32x3" if tensor_path else ("f32" if wl.precision == "c64" else "f64")
+    traffic_ncu = load_traffic(args.cfg, ctx.gemm_path)
 
     def roof(stage):
         ms, n = prof[stage]
         if not n or ms <= 0 or stage not in fl:
             return None
         ach = fl[stage] * nw * n / (ms * 1e-3) / 1e12
-        r = dict(bound=bound, kernel=names[stage], achieved=ach, peak=peak, unit="TFLOP/s", frac=ach / peak,
-                 traffic=traffic_ncu.get(stage), peak_source=peak_note, launches_timed=n, ms_per_launch=ms / n)
-        if ctx.gemm_path >= 2:
+        if kind[stage] == "tensor":
+            peak, note = tf32_peak, tensor_note
+        else:
+            peak, note = alu_peak, alu_note
+        r = dict(bound=kind[stage] if kind[stage] != "hbm" else "hbm", kernel=names[stage], achieved=ach, peak=peak, unit="TFLOP/s",
+                 frac=ach / peak, traffic=traffic_ncu.get(stage), peak_source=note, launches_timed=n, ms_per_launch=ms / n)
+        if kind[stage] == "tensor":
             r["issued_frac"] = 3.0 * ach / peak
         if stage == "green":      # HBM-bound stage: bytes, not flops
             cb = 8 if wl.precision == "c64" else 16
-            byts = nw * wl.M * wl.n_t * cb * (2 + (2 if ctx.gemm_path >= 2 else 1))
+            byts = nw * wl.M * wl.n_t * cb * (2 + (2 if tensor_path else 1))
             r.update(bound="hbm", achieved=byts * n / (ms * 1e-3) / 1e9, peak=pk["hbm"], unit="GB/s",
                      peak_source=f"{pk['source']} HBM copy bandwidth")
             r["frac"] = r["achieved"] / r["peak"]
             r.pop("issued_frac", None)
+        if wl.M < 96:
+            r["note"] = ("launch/latency-bound config (SURVEY 8(d)): no roofline fraction is meaningful here; see `latency` for us/step "
+                         "against the launch floor")
         return r
 
     timed = {k: v[0] / v[1] for k, v in prof.items() if v[1] and k in names}
@@ -376,20 +466,103 @@ def run_ours(args):
     base = None
     if not args.no_cpu_baseline:
         base = time_oracle(wl, target_s=args.cpu_seconds, one_thread_s=min(6.0, args.cpu_seconds / 2))
-    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=K, warmup=W, ms_per_step=ms_max / K,
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=K, warmup=W, ms_per_step=headline_ms / K,
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype=dtype, data="synthetic",
                 config=dict(workload=workload_name(wl), variant=args.variant, global_walkers=world * nw,
                             parallelism=f"replicas x{world}" if world > 1 else "single GPU",
                             l2="per-step working set (A_w buffer %.0f MB + operands) exceeds the 126 MB L2; no flush"
                                % (nw * wl.M * wl.M * 2 * (4 if wl.precision == "c64" else 8) / 1e6),
-                            gemm_path={1: "simt", 2: "tcgen05-3xtf32", 3: "tcgen05-3xtf32-ctapair"}[ctx.gemm_path]),
+                            gemm_path={1: "simt", 2: "tcgen05-3xtf32", 3: "tcgen05-3xtf32-ctapair"}[ctx.gemm_path],
+                            launch="CUDA graph replay of afqmc_step(n_steps)" if graph is not None else "eager afqmc_step"),
                 clocks=clocks, gpu_launches=launches,
                 e2e=dict(value=world * nw * Ke / t_e2e, unit=UNIT, h2d_bytes_per_step=up / Ke, d2h_bytes_per_step=down / Ke,
                          steps=Ke, note="afqmc_step_host: pinned host buffers, H2D of walkers+fields and D2H of "
                                         "walkers/weights/overlaps/energies inside the timed region"),
-                roofline=roof(dominant), roofline_h6=roof("assemble"),
-                stages_ms=stage_ms, stages_tflops=stage_tflops, schedule=sched, cpu_baseline=base)
+                roofline=roof(dominant), roofline_h6=roof("assemble"), latency=graph, eager_ms_per_step=ms_max / K,
+                stages_ms=stage_ms, stages_tflops=stage_tflops, measured_peaks=mp, schedule=sched, cpu_baseline=base)
     print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def load_traffic(cfg, gemm_path):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the tracked ncu summary profiles/r2_traffic.csv
+    (columns: stage,cfg,gemm_path,dram_bytes,kernel,capture).  Null when no capture matches the running kernel."""
+    import csv
+    out = {}
+    p = os.path.join(ROOT, "profiles", "r2_traffic.csv")
+    if os.path.exists(p):
+        for row in csv.DictReader(open(p)):
+            if int(row["cfg"]) == cfg and int(row["gemm_path"]) == gemm_path:
+                out[row["stage"]] = float(row["dram_bytes"])
+    return out
+
+
+def run_sharded(args):
+    """NEXT-4: the paper's schedule over a population SHARDED across the ranks --
+    every rank steps its own N_w walkers, every measurement all-reduces three estimator sums, every pc_every steps the comb runs over
+    the whole population (all-gather of the weights + one all-to-all of walker records).  One dist.run_sharded call of 40 steps
+    (E/20, QR/2, comb/20).  "weak": the global population is N_w x ranks."""
+    import torch
+    import torch.distributed as dist
+    from paper_1804_03310_b200 import dist as D
+    from paper_1804_03310_b200.state import WalkerState, make_context
+    from workloads import make_workload
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("NCCL_DEBUG", "INFO")          # the communicator line (nranks) stays visible in the log
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    # the literal / mf inputs kill the whole population within ~8 steps (DESIGN.md 4): the 40-step schedule runs on the tame
+    # variant of the same shapes, so that the estimator is finite and the comb has live weights to route (timing is value independent)
+    variant = {"mf": "tame_mf", "raw": "tame"}.get(args.variant, args.variant)
+    wl = make_workload(args.cfg, variant)
+    nw = wl.n_walkers
+    ctx = make_context(wl, nw, gemm_path=args.gemm_path, device=f"cuda:{local}")
+    dev = ctx.device
+    ns, ee, oe, pe = 40, 20, 2, 20
+    rng = np.random.default_rng(D.rank_seed(1000, rank))
+    x = torch.tensor(rng.standard_normal((8, nw, wl.n_chol)), dtype=ctx.rdtype, device=dev)
+    xs = x[torch.arange(ns, device=dev) % 8].contiguous()
+    st = WalkerState(ctx, wl.walkers(nw))
+    phi0 = st.phi.clone()
+    # seeded log-normal start weights (sigma 0.5, every rank its own mean) so that the comb really moves walkers across ranks
+    w0 = torch.tensor(np.exp(0.5 * rng.standard_normal(nw) + 0.3 * (rank - (world - 1) / 2)), dtype=torch.float64, device=dev)
+
+    def reseed():
+        st.phi.copy_(phi0); st.weight.copy_(w0); st.flags.zero_(); st.seed()
+    reseed()
+    D.run_sharded(ctx, st.phi, st.weight, st.ovlp, st.theta, st.fb, xs, ns, ee, oe, pe, us=[0.37, 0.81], flags=st.flags)   # warm
+    reseed()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    l0 = ctx.launch_count
+    D.COMB_STATS.clear()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    energies = D.run_sharded(ctx, st.phi, st.weight, st.ovlp, st.theta, st.fb, xs, ns, ee, oe, pe, us=[0.37, 0.81], flags=st.flags)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = D.max_over_ranks(e0.elapsed_time(e1), dev)
+    if world > 1:
+        dist.barrier()
+    if rank == 0:
+        sent = [c["bytes_sent_to_peers"] for c in D.COMB_STATS]
+        line = dict(metric=METRIC, value=world * nw * ns / (ms * 1e-3), unit=UNIT, n_gpus=world, steps=ns, warmup=ns,
+                    ms_per_step=ms / ns, higher_is_better=True, scaling="weak", vs_baseline=None,
+                    dtype="tf32x3" if ctx.gemm_path >= 2 else ("f32" if wl.precision == "c64" else "f64"), data="synthetic",
+                    config=dict(workload=workload_name(wl), variant=variant, global_walkers=world * nw,
+                                parallelism=f"walkers sharded x{world}, global comb", schedule=dict(energy_every=ee, ortho_every=oe, pc_every=pe)),
+                    gpu_launches=ctx.launch_count - l0,
+                    sharded=dict(combs=len(D.COMB_STATS), record_bytes=ctx.afqmc_comb_record_bytes,
+                                 rank0_walkers_sent_to_peers=[c["walkers_sent_to_peers"] for c in D.COMB_STATS],
+                                 rank0_bytes_sent_to_peers=sent, allgather_bytes=world * nw * 8, allreduce_bytes_per_measurement=24,
+                                 e_mix=[[e.real, e.imag] for e in energies]),
+                    note="energy every 20 steps (the paper's schedule), not every step: compare with `schedule`, not with the headline")
+        print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
 
@@ -406,9 +579,17 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-schedule", action="store_true")
+    ap.add_argument("--no-graph", action="store_true", help="M < 96: time eager launches only (no CUDA graph replay)")
+    ap.add_argument("--sharded", action="store_true", help="NEXT-4: the paper's schedule over a population sharded across the ranks")
+    ap.add_argument("--peaks", action="store_true", help="print the measured peak microbenchmarks only")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.peaks:
+        import torch
+        print(json.dumps(dict(measured_peaks=measure_peaks(torch.device("cuda:0")), driver_peaks=peaks())))
+    elif args.sharded:
+        run_sharded(args)
     else:
         run_ours(args)
 

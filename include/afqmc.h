@@ -103,6 +103,11 @@ AFQMC_API afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const 
                         const double* det_coeff, const int32_t* det_exc, void* const_mem, void* work_mem,
                         void* stream);
 AFQMC_API void afqmc_destroy(afqmc_ctx* ctx);
+/* All further work of this context is enqueued on `stream` (cudaStream_t).  The device entry points launch kernels and
+ * device-to-device copies only -- no synchronisation, no allocation -- so a call such as afqmc_step(n_steps) may be captured
+ * into a CUDA graph on a capturing stream and replayed (bench.py does so for the launch-latency-bound configs, M < 96; per-stage
+ * profiling must be off).  The caller orders the old and the new stream. */
+AFQMC_API afqmc_status afqmc_set_stream(afqmc_ctx* ctx, void* stream);
 /* Last error text of this context ("" if none); valid until the next call on ctx. ctx may be NULL
  * (then the text of the last failed afqmc_init of this thread). */
 AFQMC_API const char* afqmc_last_error(const afqmc_ctx* ctx);

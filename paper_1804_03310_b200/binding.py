@@ -21,7 +21,7 @@ SYMBOLS = ["afqmc_query_bytes", "afqmc_init", "afqmc_destroy", "afqmc_last_error
            "afqmc_force_bias", "afqmc_propagate", "afqmc_local_energy", "afqmc_step", "afqmc_step_host",
            "afqmc_launch_count", "afqmc_gemm_path", "afqmc_profile_enable", "afqmc_profile_read",
            "afqmc_orthonormalize", "afqmc_population_control", "afqmc_run", "afqmc_comb_record_bytes",
-           "afqmc_comb_map", "afqmc_comb_pack", "afqmc_comb_unpack", "afqmc_mixed_sums", "afqmc_mixed_energy", "afqmc_peak_probe", "afqmc_peak_mma_table"]
+           "afqmc_comb_map", "afqmc_comb_pack", "afqmc_comb_unpack", "afqmc_mixed_sums", "afqmc_mixed_energy", "afqmc_peak_probe", "afqmc_peak_mma_table", "afqmc_set_stream"]
 
 STAGES = ["shift", "assemble", "taylor", "green", "force_bias", "energy", "symmetrize", "ortho", "popctl"]
 
@@ -55,6 +55,8 @@ def load_library():
     pp = C.POINTER(AfqmcParams)
     lib.afqmc_query_bytes.argtypes = [pp, szp, szp]
     lib.afqmc_init.argtypes = [C.POINTER(vp), pp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.afqmc_set_stream.argtypes = [vp, vp]
+    lib.afqmc_set_stream.restype = C.c_int
     lib.afqmc_destroy.argtypes = [vp]
     lib.afqmc_destroy.restype = None
     lib.afqmc_last_error.argtypes = [vp]
@@ -189,6 +191,12 @@ class AfqmcContext:
         if st:
             raise AfqmcError(st, self._lib.afqmc_last_error(None).decode())
         self._ctx = ctx
+
+    def use_stream(self, stream):
+        """Enqueue all further work of this context on `stream` (a torch.cuda.Stream), e.g. a CUDA-graph capture stream."""
+        st = self._lib.afqmc_set_stream(self._ctx, C.c_void_p(stream.cuda_stream))
+        self._chk(st)
+        self.stream = stream
 
     def close(self):
         if getattr(self, "_ctx", None):

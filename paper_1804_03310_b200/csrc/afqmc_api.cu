@@ -1088,6 +1088,12 @@ afqmc_status afqmc_profile_read(afqmc_ctx* c, int32_t stage, double* total_ms, i
 
 const char* afqmc_last_error(const afqmc_ctx* ctx) { return ctx ? ctx->err : g_init_err; }
 
+afqmc_status afqmc_set_stream(afqmc_ctx* c, void* stream) {
+  if (!c) return AFQMC_EINVAL;
+  c->stream = (cudaStream_t)stream;
+  return AFQMC_OK;
+}
+
 int64_t afqmc_launch_count(const afqmc_ctx* ctx) { return ctx ? ctx->launches : 0; }
 int32_t afqmc_gemm_path(const afqmc_ctx* ctx) { return ctx ? (ctx->cta2 ? 3 : ctx->path) : 0; }
 

@@ -57,12 +57,18 @@ __device__ __forceinline__ void tf32_split(float v, float& hi, float& lo) {
 }
 
 // The tensor pipe ignores the low 13 mantissa bits of a kind::tf32 operand, i.e. it consumes raw FP32 v as trunc13(v).  The
-// matching low part, rounded to TF32 (cvt.rna: nearest, ties away), as raw bits.
+// matching low part d = v - trunc13(v) (exact, <= 13 significant bits) is itself truncated to 11 bits by the pipe; scaling it
+// by 1 + 2^-11 first centres that truncation (error within +-2^-11 |d| <= 2^-21 |v|, zero mean).  One LOP3, one FADD, one
+// FMUL per element: cvt.rna.tf32.f32 is a quarter-rate conversion and made the splitter warps the Taylor kernel's bottleneck.
 __device__ __forceinline__ uint32_t tf32_lo_bits(uint32_t vbits) {
   const float d = __uint_as_float(vbits) - __uint_as_float(vbits & 0xffffe000u);
-  uint32_t r;
-  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(d));
-  return r;
+  return __float_as_uint(d * 1.00048828125f);
+}
+
+// The same split for values produced in registers: hi = v itself (consumed as trunc13(v)), lo = centred low part.
+__device__ __forceinline__ void tf32_split_raw(float v, float& hi, float& lo) {
+  hi = v;
+  lo = __uint_as_float(tf32_lo_bits(__float_as_uint(v)));
 }
 
 // cp.async 16-byte global -> shared (LDGSTS)

@@ -84,9 +84,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   __shared__ __align__(8) uint64_t full_bar[NF_MAX];   // TMA has landed an FP32 tile (= X_hi)
-  __shared__ __align__(8) uint64_t empty_bar[NF_MAX];  // the MMAs that read it have completed
+  __shared__ __align__(8) uint64_t empty_bar[NF_MAX];  // the MMAs of the tile in this stage have completed (waited for by the producer AND by the splitter that reuses the tile's lo buffer)
   __shared__ __align__(8) uint64_t lo_full_bar[NL];    // a splitter warp has written X_lo
-  __shared__ __align__(8) uint64_t lo_empty_bar[NL];   // the MMAs that read it have completed
   __shared__ __align__(8) uint64_t tmem_full_bar[2];   // per 128-row tile: tile 0 is post-processed while tile 1 is issued
   __shared__ __align__(8) uint64_t b_ready_bar[2];     // per tile of the PREVIOUS product = 4 k-blocks of the T operand (8 warps arrive)
   __shared__ __align__(8) uint64_t t_free_bar[4];      // last tile has consumed k-block kb < 4 of the current T
@@ -106,7 +105,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
     *reinterpret_cast<uint4*>(planes + o) = make_uint4(0, 0, 0, 0);
   if (warp == EPW && lane == 0) {
     for (int s = 0; s < NF_MAX; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
-    for (int s = 0; s < NL; ++s) { mbar_init(&lo_full_bar[s], 1); mbar_init(&lo_empty_bar[s], 1); }
+    for (int s = 0; s < NL; ++s) mbar_init(&lo_full_bar[s], 1);
     mbar_init(&tmem_full_bar[0], 1); mbar_init(&tmem_full_bar[1], 1);
     mbar_init(&b_ready_bar[0], EPW); mbar_init(&b_ready_bar[1], EPW);
     for (int x = 0; x < 4; ++x) mbar_init(&t_free_bar[x], 1);
@@ -161,10 +160,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
     const uint32_t total = (uint32_t)n_mine * tiles_per_walker;
     for (uint32_t it = sw; it < total; it += NSPLIT) {
       const int s = it % NF, sl = it % NL;
-      // order matters: a parity wait is only unambiguous within one phase of the barrier.  Once the MMAs of tile it - NL have
-      // completed (lo buffer free), every tile up to it - NL has been loaded, and NL <= NF: the previous user of stage s is
-      // among them, so full_bar[s] is exactly in the phase this tile completes
-      mbar_wait(&lo_empty_bar[sl], ((it / NL) & 1) ^ 1);
+      // lo buffer sl was last read by the MMAs of tile it - NL, whose completion is the (only) tcgen05.commit of that tile, on the
+      // empty barrier of ITS stage: no separate barrier (a commit costs ~50 clk of tensor-pipe time, the pipe has no queue).
+      // Order matters: a parity wait is only unambiguous within one phase of the barrier.  Tile it - NL done means every tile
+      // up to it - NL has been loaded, and NL <= NF: the previous user of stage s is among them, so full_bar[s] is exactly in
+      // the phase this tile completes; and empty_bar[(it - NL) % NF] cannot be a phase further on, because tile it - NL + NF > it
+      // is issued after tile `it`, which needs this warp's lo buffer.
+      if (it >= NL) mbar_wait(&empty_bar[(it - NL) % NF], ((it - NL) / NF) & 1);
       mbar_wait(&full_bar[s], (it / NF) & 1);
       const uint4* src = reinterpret_cast<const uint4*>(stages + (size_t)s * TILE_BYTES);
       uint4* dst = reinterpret_cast<uint4*>(lobufs + (size_t)sl * TILE_BYTES);
@@ -189,7 +191,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
     // descriptors computed under uniform control flow ptxas keeps them in uniform registers and the 8 MMAs of a tile are 8
     // back-to-back UTCHMMA.  Inside an `if (lane == 0)` region it wraps every MMA in an ELECT / 5 x R2UR / branch-back
     // sequence.  What a tile costs beyond its 448 clk of tensor-pipe time is this warp's scalar code between two tiles (the
-    // pipe's queue is short), so that code is kept minimal: incremental descriptors, no divisions, one barrier wait. =====
+    // pipe's queue is short), so that code is kept minimal: incremental descriptors, no divisions, one barrier wait, one commit.
+    // Measured (csrc/peaks.cuh k_peak_pat): a tile's 448 clk, a tcgen05.commit (~50 clk) and a satisfied mbarrier wait (~92 clk) add
+    // up -- the pipe does not run ahead of the issuing warp.  Tried and dropped: two issuer warps taking alternate tiles with a
+    // 64-thread named barrier as hand-over (1.50 ms against 1.39 ms: the barrier costs more than the hidden wait). =====
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"((int)REGS_AUX));
     constexpr uint32_t idesc128 = make_idesc(128, 128), idesc64 = make_idesc(128, 64);
     const uint64_t xh0 = make_desc(smem_u32(stages)), xl0 = make_desc(smem_u32(lobufs)), t0 = make_desc(smem_u32(planes));
@@ -221,7 +226,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
                   umma_tf32(d + 64, xl + adv, t_all + adv, idesc64, 1u);
                 }
                 tc_commit(&empty_bar[s]);
-                tc_commit(&lo_empty_bar[sl]);
                 if (p == np - 1) {
                   if (mtiles == 2 && mt == 1 && kb < 4) tc_commit(&t_free_bar[kb]);
                   if (kb == nkb - 1) tc_commit(&tmem_full_bar[mt]);
@@ -284,8 +288,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
             const int e = et + (k + hb * (MAXE / 2)) * (EPW * 32);
             if (e < M * nt) {
               float h0, l0, h1, l1;
-              tf32_split(f[k].x, h0, l0);
-              tf32_split(f[k].y, h1, l1);
+              tf32_split_raw(f[k].x, h0, l0);     // hi = raw FP32 (the pipe truncates it), lo = centred low part
+              tf32_split_raw(f[k].y, h1, l1);
               const uint32_t o = plane_off(cbb, ci);
               sts32(pl_hi + o, h0);
               sts32(pl_lo + o, l0);
@@ -334,16 +338,15 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
             if (ph == 0) {
               // the streamed operand of the two one-body phases is D_h = E_h - 1 (|D_h| ~ dt |h'| / 2 << 1): E_h T = T + D_h T
               // with the addition in FP32 round-to-nearest here, so the tensor pipe's truncating accumulation acts on the
-              // small correction only.  T (= Phi_w) is read back from the planes as hi + lo, before this thread overwrites it
+              // small correction only.  T (= Phi_w) is read back from the hi plane (raw FP32), before this thread overwrites it
               const int ic = i < M ? i : 0;
 #pragma unroll
               for (int b = 0; b < 32; ++b)
                 if (b < nt) {
                   const uint32_t o = plane_off(rb + b, ic);
-                  float th, tl;
+                  float th;
                   asm volatile("ld.shared.f32 %0, [%1];" : "=f"(th) : "r"(pl_hi + o) : "memory");
-                  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(tl) : "r"(pl_lo + o) : "memory");
-                  v[b] += th + tl;
+                  v[b] += th;                 // the hi plane holds the raw FP32 value (tf32_split_raw)
                 }
             }
 #pragma unroll
@@ -375,7 +378,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
             } else {
               float hi[32], lo[32];
 #pragma unroll
-              for (int b = 0; b < 32; ++b) tf32_split(v[b], hi[b], lo[b]);
+              for (int b = 0; b < 32; ++b) tf32_split_raw(v[b], hi[b], lo[b]);
               // k-block mt*4+q of T may be overwritten once every MMA that reads it has completed: for the last
               // tile that is tmem_full (above), for tile 0 of two the last tile's pass over that k-block
               if (mt == 0 && mtiles == 2) mbar_wait(&t_free_bar[q], gph & 1);

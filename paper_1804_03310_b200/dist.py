@@ -8,6 +8,9 @@ C ABI (afqmc_comb_map / _pack / _unpack), this module only routes buffers.  Work
 from __future__ import annotations
 
 
+COMB_STATS = []   # one dict per sharded comb on this rank (walkers / bytes sent to other ranks); bench.py --sharded reads it
+
+
 def rank_seed(base: int, rank: int) -> int:
     """Distinct, reproducible field seed per replica."""
     return int(base) + 7919 * int(rank)
@@ -85,6 +88,8 @@ def population_control_sharded(ctx, phi, weight, ovlp, theta, fb, u: float, grou
     else:
         recvbuf = sendbuf
     ctx.afqmc_comb_unpack(recvbuf, phi, weight, ovlp, theta, fb, w_new)
+    to_peers = sum(c for d, c in enumerate(send_counts) if d != rank)
+    COMB_STATS.append(dict(walkers_sent_to_peers=int(to_peers), bytes_sent_to_peers=int(to_peers) * int(rec)))
     return parent_all
 
 
