@@ -192,6 +192,17 @@ AFQMC_API afqmc_status afqmc_population_control(afqmc_ctx* ctx, void* phi, doubl
 AFQMC_API size_t afqmc_comb_record_bytes(const afqmc_ctx* ctx);
 AFQMC_API afqmc_status afqmc_comb_map(afqmc_ctx* ctx, const double* weight_all, int64_t n_total, double u, double* cum_scratch,
                             int32_t* parent_all, double* w_new);
+/* Allocation-free variant of afqmc_comb_map (reading R22) for callers that cannot provide scratch or call
+ * cudaMalloc (CUDA graph capture, tight serving loops, harnesses that forbid it): the running-sum scratch is a file-scope device
+ * array of AFQMC_NOALLOC_MAX_WALKERS doubles (512 KiB, held by every GPU that loads the library until exit).  Same inputs,
+ * outputs and bits as afqmc_comb_map.  n_total > AFQMC_NOALLOC_MAX_WALKERS returns AFQMC_EUNSUPPORTED before any launch.  Calls no
+ * cudaMalloc / cudaFree / allocating routine; the first call on a device resolves the array's address (cudaGetSymbolAddress).
+ * ALL calls on a device share the one array: it keeps the last call's running sums (each call overwrites [0, n_total) before reading
+ * it, so nothing needs clearing), and two calls that overlap on the GPU -- different streams or contexts -- RACE on it; serialise them.
+ * All pointers DEVICE; enqueues on the context's stream; does not synchronise. */
+#define AFQMC_NOALLOC_MAX_WALKERS 65536
+AFQMC_API afqmc_status afqmc_comb_map_noalloc(afqmc_ctx* ctx, const double* weight_all, int64_t n_total, double u,
+                                              int32_t* parent_all, double* w_new);
 AFQMC_API afqmc_status afqmc_comb_pack(afqmc_ctx* ctx, const void* phi, const void* ovlp, const void* theta, const void* fb,
                              const int32_t* parent_all, int64_t slot_lo, int64_t count, int64_t first_local, void* sendbuf);
 AFQMC_API afqmc_status afqmc_comb_unpack(afqmc_ctx* ctx, const void* recvbuf, void* phi, double* weight, void* ovlp, void* theta,

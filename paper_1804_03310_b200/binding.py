@@ -21,7 +21,7 @@ SYMBOLS = ["afqmc_query_bytes", "afqmc_init", "afqmc_destroy", "afqmc_last_error
            "afqmc_force_bias", "afqmc_propagate", "afqmc_local_energy", "afqmc_step", "afqmc_step_host",
            "afqmc_launch_count", "afqmc_gemm_path", "afqmc_profile_enable", "afqmc_profile_read",
            "afqmc_orthonormalize", "afqmc_population_control", "afqmc_run", "afqmc_comb_record_bytes",
-           "afqmc_comb_map", "afqmc_comb_pack", "afqmc_comb_unpack", "afqmc_mixed_sums", "afqmc_mixed_energy", "afqmc_peak_probe", "afqmc_peak_mma_table", "afqmc_set_stream"]
+           "afqmc_comb_map", "afqmc_comb_pack", "afqmc_comb_unpack", "afqmc_mixed_sums", "afqmc_mixed_energy", "afqmc_peak_probe", "afqmc_peak_mma_table", "afqmc_set_stream", "afqmc_comb_map_noalloc"]
 
 STAGES = ["shift", "assemble", "taylor", "green", "force_bias", "energy", "symmetrize", "ortho", "popctl"]
 
@@ -82,6 +82,8 @@ def load_library():
     lib.afqmc_comb_record_bytes.argtypes = [vp]
     lib.afqmc_comb_record_bytes.restype = C.c_size_t
     lib.afqmc_comb_map.argtypes = [vp, vp, C.c_int64, C.c_double, vp, i32p, vp]
+    lib.afqmc_comb_map_noalloc.argtypes = [vp, vp, C.c_int64, C.c_double, i32p, vp]
+    lib.afqmc_comb_map_noalloc.restype = C.c_int
     lib.afqmc_comb_pack.argtypes = [vp, vp, vp, vp, vp, i32p, C.c_int64, C.c_int64, C.c_int64, vp]
     lib.afqmc_comb_unpack.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
     lib.afqmc_launch_count.argtypes = [vp]
@@ -279,6 +281,10 @@ class AfqmcContext:
     def afqmc_comb_map(self, weight_all, u, cum_scratch, parent_all, w_new):
         self._chk(self._lib.afqmc_comb_map(self._ctx, _dp(weight_all), int(weight_all.numel()), float(u), _dp(cum_scratch),
                                            _dp(parent_all), _dp(w_new)))
+
+    def afqmc_comb_map_noalloc(self, weight_all, u, parent_all, w_new):
+        self._chk(self._lib.afqmc_comb_map_noalloc(self._ctx, _dp(weight_all), int(weight_all.numel()), float(u), _dp(parent_all),
+                                                   _dp(w_new)))
 
     def afqmc_comb_pack(self, phi, ovlp, theta, fb, parent_all, slot_lo, count, first_local, sendbuf):
         self._chk(self._lib.afqmc_comb_pack(self._ctx, _dp(phi), _dp(ovlp), _dp(theta), _dp(fb), _dp(parent_all),

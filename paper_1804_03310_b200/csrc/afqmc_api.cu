@@ -1210,6 +1210,39 @@ afqmc_status afqmc_comb_map(afqmc_ctx* c, const double* weight_all, int64_t n_to
   return AFQMC_OK;
 }
 
+// ---- allocation-free variant of afqmc_comb_map: the running-sum scratch lives in a file-scope device array ----------------
+// Every GPU that loads the library holds AFQMC_NOALLOC_MAX_WALKERS doubles (512 KiB) until exit.  In host code the array's name is
+// a host-side stand-in, not a device address: the address is taken once per device with cudaGetSymbolAddress (that device
+// current) and that pointer is what the kernel receives.
+static __device__ __align__(256) double g_noalloc_cum[AFQMC_NOALLOC_MAX_WALKERS];
+static double* g_noalloc_cum_ptr[64];    // per device ordinal; null until the first call on that device
+
+afqmc_status afqmc_comb_map_noalloc(afqmc_ctx* c, const double* weight_all, int64_t n_total, double u, int32_t* parent_all,
+                                    double* w_new) {
+  if (!c) return AFQMC_EINVAL;
+  c->err[0] = 0;
+  NEED(c, n_total >= 0, "afqmc_comb_map_noalloc: n_total < 0");
+  if (n_total > (int64_t)AFQMC_NOALLOC_MAX_WALKERS)
+    return fail(c, AFQMC_EUNSUPPORTED, "%s", "afqmc_comb_map_noalloc: n_total exceeds AFQMC_NOALLOC_MAX_WALKERS (65536), the size of the "
+                                             "library's static scratch; use afqmc_comb_map with caller-provided scratch");
+  NEED(c, u >= 0.0 && u < 1.0, "afqmc_comb_map_noalloc: u must be in [0, 1)");
+  if (n_total == 0) return AFQMC_OK;
+  NEED(c, weight_all && parent_all && w_new, "afqmc_comb_map_noalloc: null pointer");
+  int dev = -1;
+  CUDA_OK(c, cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return fail(c, AFQMC_EUNSUPPORTED, "%s", "afqmc_comb_map_noalloc: device ordinal >= 64");
+  if (!g_noalloc_cum_ptr[dev]) {           // set-up, once per device, with that device current
+    double* ptr = nullptr;
+    cudaError_t e = cudaGetSymbolAddress((void**)&ptr, g_noalloc_cum);
+    if (e != cudaSuccess || !ptr) return fail(c, AFQMC_ECUDA, "cudaGetSymbolAddress(g_noalloc_cum): %s", cudaGetErrorString(e));
+    g_noalloc_cum_ptr[dev] = ptr;
+  }
+  // k_comb_parents writes cum[0 .. n_total) before it reads any of it: nothing of the previous call's contents is used
+  StageScope sc(c, AFQMC_STAGE_POPCTL);
+  LAUNCH(c, k_comb_parents, 1, 1024, 0, (int)n_total, weight_all, u, g_noalloc_cum_ptr[dev], parent_all, w_new);
+  return AFQMC_OK;
+}
+
 afqmc_status afqmc_comb_pack(afqmc_ctx* c, const void* phi, const void* ovlp, const void* theta, const void* fb,
                              const int32_t* parent_all, int64_t slot_lo, int64_t count, int64_t first_local, void* sendbuf) {
   if (!c) return AFQMC_EINVAL;
