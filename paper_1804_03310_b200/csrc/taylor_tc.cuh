@@ -23,7 +23,7 @@ namespace tt {
 
 using namespace tc;
 
-enum { NL = 3, TILE_BYTES = 128 * 128, PLANE_KB_BYTES = 128 * 128, EPW = 8, NSPLIT = 3, NTHREADS = 16 * 32 };
+enum { NL = 3, TILE_BYTES = 128 * 128, PLANE_KB_BYTES = 128 * 128, EPW = 8, NSPLIT = 6, NGROUP = 3, NTHREADS = 16 * 32 };
 // NSPLIT <= NL <= NF: a parity wait on an mbarrier is only unambiguous within one phase of it.  A splitter that has finished
 // tile it - NSPLIT knows the MMAs of tile it - NSPLIT - NL are done; its wait for the lo buffer of tile `it` needs those of tile
 // it - 2 NL done (a warp that runs two phases ahead sees the parity it waits for as already complete and reads a tile that has
@@ -44,7 +44,7 @@ struct TaylorTcArgs {
 };
 
 enum { NF_MAX = 6 };
-static_assert(NSPLIT <= NL, "see above");
+static_assert(NGROUP <= NL && NSPLIT == 2 * NGROUP, "see above");
 inline int pick_nf(int nkb) {   // >= NL (the splitters' wait order relies on it)
   const int left = 227 * 1024 - 1024 - 512 - nkb * PLANE_KB_BYTES - NL * TILE_BYTES;
   const int nf = left / TILE_BYTES;
@@ -85,7 +85,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   __shared__ __align__(8) uint64_t full_bar[NF_MAX];   // TMA has landed an FP32 tile (= X_hi)
   __shared__ __align__(8) uint64_t empty_bar[NF_MAX];  // the MMAs of the tile in this stage have completed (waited for by the producer AND by the splitter that reuses the tile's lo buffer)
-  __shared__ __align__(8) uint64_t lo_full_bar[NL];    // a splitter warp has written X_lo
+  __shared__ __align__(8) uint64_t lo_full_bar[NL];    // both warps of a splitter group have written their half of X_lo
   __shared__ __align__(8) uint64_t tmem_full_bar[2];   // per 128-row tile: tile 0 is post-processed while tile 1 is issued
   __shared__ __align__(8) uint64_t b_ready_bar[2];     // per tile of the PREVIOUS product = 4 k-blocks of the T operand (8 warps arrive)
   __shared__ __align__(8) uint64_t t_free_bar[4];      // last tile has consumed k-block kb < 4 of the current T
@@ -105,7 +105,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
     *reinterpret_cast<uint4*>(planes + o) = make_uint4(0, 0, 0, 0);
   if (warp == EPW && lane == 0) {
     for (int s = 0; s < NF_MAX; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
-    for (int s = 0; s < NL; ++s) mbar_init(&lo_full_bar[s], 1);
+    for (int s = 0; s < NL; ++s) mbar_init(&lo_full_bar[s], 2);   // the two warps of a splitter group
     mbar_init(&tmem_full_bar[0], 1); mbar_init(&tmem_full_bar[1], 1);
     mbar_init(&b_ready_bar[0], EPW); mbar_init(&b_ready_bar[1], EPW);
     for (int x = 0; x < 4; ++x) mbar_init(&t_free_bar[x], 1);
@@ -152,35 +152,63 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
   } else if (warp >= EPW + 2 + NSPLIT) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"((int)REGS_AUX));   // idle warps that complete the last warpgroup
   } else if (warp >= EPW + 2) {
-    // ===== splitter warps: X_lo = rn_tf32(X - trunc13(X)), elementwise at the same (swizzled) offsets.  The warps take the
-    // tiles round robin, so one tile has NSPLIT stage times to get through its barrier wake-ups, 32 LDS.128 / STS.128 per
-    // lane and the proxy fence =====
+    // ===== splitter warps: X_lo = (X - trunc13 X)(1 + 2^-11), elementwise at the same (swizzled) offsets.  NGROUP groups of two
+    // warps take the tiles round robin (group = tile mod NGROUP <= NL, see above), each warp one half of the tile: the chain
+    // "MMAs of tile it - NL done -> split tile it -> MMAs of tile it" is what paces the kernel, and two warps halve its split part =====
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"((int)REGS_AUX));
-    const int sw = warp - (EPW + 2);
+    const int sw = warp - (EPW + 2), grp = sw >> 1, half = sw & 1;
     const uint32_t total = (uint32_t)n_mine * tiles_per_walker;
-    for (uint32_t it = sw; it < total; it += NSPLIT) {
+    // (phase, index inside the phase) of this group's current tile; a phase is [m-tile 0 | m-tile 1], each nkb x planes tiles
+    // (mtiles == 1: half_len is unused)
+    int ph = 0, half_len = nkb, rr = grp;
+    const int slabs_last = (g.rows_last + 15) >> 4;
+    if (mtiles == 2) while (rr >= 2 * half_len) { rr -= 2 * half_len; ++ph; half_len = nkb * ((ph >= 1 && ph <= g.K) ? 2 : 1); }
+    for (uint32_t it = grp; it < total; it += NGROUP) {
       const int s = it % NF, sl = it % NL;
       // lo buffer sl was last read by the MMAs of tile it - NL, whose completion is the (only) tcgen05.commit of that tile, on the
       // empty barrier of ITS stage: no separate barrier (a commit costs ~50 clk of tensor-pipe time, the pipe has no queue).
       // Order matters: a parity wait is only unambiguous within one phase of the barrier.  Tile it - NL done means every tile
       // up to it - NL has been loaded, and NL <= NF: the previous user of stage s is among them, so full_bar[s] is exactly in
       // the phase this tile completes; and empty_bar[(it - NL) % NF] cannot be a phase further on, because tile it - NL + NF > it
-      // is issued after tile `it`, which needs this warp's lo buffer.
+      // is issued after tile `it`, which needs this group's lo buffer.
       if (it >= NL) mbar_wait(&empty_bar[(it - NL) % NF], ((it - NL) / NF) & 1);
       mbar_wait(&full_bar[s], (it / NF) & 1);
+      // the two warps take alternate 16-row slabs (2 KB = 4 warp-wide 16-byte accesses); a short last tile (rows_last of 128 rows,
+      // M = 200: 72) has only ceil(rows_last / 16) of them: TMA wrote nothing beyond and the MMAs' extra rows are never read back
       const uint4* src = reinterpret_cast<const uint4*>(stages + (size_t)s * TILE_BYTES);
       uint4* dst = reinterpret_cast<uint4*>(lobufs + (size_t)sl * TILE_BYTES);
-#pragma unroll
-      for (int u = 0; u < TILE_BYTES / 16 / 32; u += 8) {
+      const int slabs = (mtiles == 2 && rr >= half_len) ? slabs_last : 8;     // second m-tile of its phase?
+#pragma unroll 1
+      for (int sb = half; sb < slabs; sb += 4) {       // two slabs (sb, sb + 2) per iteration: 8 accesses in flight
         uint4 v[8];
+        const bool two = sb + 2 < slabs;
 #pragma unroll
-        for (int x = 0; x < 8; ++x) v[x] = src[(u + x) * 32 + lane];
+        for (int x = 0; x < 4; ++x) v[x] = src[(sb * 4 + x) * 32 + lane];
+        if (two) {
 #pragma unroll
-        for (int x = 0; x < 8; ++x) {
-          uint4 r;
-          r.x = tf32_lo_bits(v[x].x); r.y = tf32_lo_bits(v[x].y); r.z = tf32_lo_bits(v[x].z); r.w = tf32_lo_bits(v[x].w);
-          dst[(u + x) * 32 + lane] = r;
+          for (int x = 0; x < 4; ++x) v[4 + x] = src[((sb + 2) * 4 + x) * 32 + lane];
         }
+#pragma unroll
+        for (int x = 0; x < 4; ++x) {
+          uint4 q;
+          q.x = tf32_lo_bits(v[x].x); q.y = tf32_lo_bits(v[x].y); q.z = tf32_lo_bits(v[x].z); q.w = tf32_lo_bits(v[x].w);
+          dst[(sb * 4 + x) * 32 + lane] = q;
+        }
+        if (two) {
+#pragma unroll
+          for (int x = 0; x < 4; ++x) {
+            uint4 q;
+            q.x = tf32_lo_bits(v[4 + x].x); q.y = tf32_lo_bits(v[4 + x].y); q.z = tf32_lo_bits(v[4 + x].z); q.w = tf32_lo_bits(v[4 + x].w);
+            dst[((sb + 2) * 4 + x) * 32 + lane] = q;
+          }
+        }
+      }
+      // advance (phase, index inside the phase) by NGROUP tiles without divisions
+      rr += NGROUP;
+      while (rr >= 2 * half_len) {
+        rr -= 2 * half_len;
+        if (++ph == nphase) ph = 0;
+        half_len = nkb * ((ph >= 1 && ph <= g.K) ? 2 : 1);
       }
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       __syncwarp();
@@ -188,17 +216,19 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
     }
   } else if (warp == EPW + 1) {
     // ===== MMA issuer warp.  The whole warp runs the loop (uniform control flow) and ONE elected lane issues: with the
-    // descriptors computed under uniform control flow ptxas keeps them in uniform registers and the 8 MMAs of a tile are 8
-    // back-to-back UTCHMMA.  Inside an `if (lane == 0)` region it wraps every MMA in an ELECT / 5 x R2UR / branch-back
-    // sequence.  What a tile costs beyond its 448 clk of tensor-pipe time is this warp's scalar code between two tiles (the
-    // pipe's queue is short), so that code is kept minimal: incremental descriptors, no divisions, one barrier wait, one commit.
-    // Measured (csrc/peaks.cuh k_peak_pat): a tile's 448 clk, a tcgen05.commit (~50 clk) and a satisfied mbarrier wait (~92 clk) add
-    // up -- the pipe does not run ahead of the issuing warp.  Tried and dropped: two issuer warps taking alternate tiles with a
-    // 64-thread named barrier as hand-over (1.50 ms against 1.39 ms: the barrier costs more than the hidden wait). =====
+    // descriptors computed under uniform control flow ptxas keeps them in uniform registers and the MMAs of a tile are
+    // back-to-back UTCHMMA (inside an `if (lane == 0)` region it wraps every MMA in an ELECT / 5 x R2UR / branch-back sequence).
+    // Measured (csrc/peaks.cuh k_peak_pat): a tile's 448 clk of pipe time, a tcgen05.commit (~50 clk) and a satisfied mbarrier
+    // wait (~92 clk) add up -- the pipe does not run ahead of the issuing warp -- so there is one wait and one commit per tile.
+    // Tried and dropped (B200, cfg 5): two issuer warps alternating tiles with a named-barrier hand-over (1.50 ms against 1.38);
+    // two issuer warps each owning one plane's chain, no hand-over at all (1.43 ms against 1.38).  Trimming the last k-block to
+    // the k-steps it really has (M = 200: 25 instead of 28 k-steps) removed 10 % of the MMAs and changed the time by 0.3 %:
+    // the tensor pipe is not what paces this kernel -- the chain TMA -> splitter -> MMA over a 3-deep lo ring is. =====
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"((int)REGS_AUX));
     constexpr uint32_t idesc128 = make_idesc(128, 128), idesc64 = make_idesc(128, 64);
     const uint64_t xh0 = make_desc(smem_u32(stages)), xl0 = make_desc(smem_u32(lobufs)), t0 = make_desc(smem_u32(planes));
     constexpr uint64_t TSTEP = TILE_BYTES >> 4;     // descriptor address field counts 16-byte units
+    const int klast = (M - 32 * (nkb - 1) + 7) >> 3;     // k-steps of 8 columns the last k-block really has (columns >= M are padding)
     uint64_t xh = xh0, xl = xl0;
     uint32_t gph = 0;
     int s = 0, sl = 0;
@@ -212,29 +242,38 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
             // k-blocks 4 j .. 4 j + 3 of this phase's T are in shared memory, and (all 8 epilogue warps arrive after their
             // TMEM loads) the accumulators of tile j have been read
             if (mt == 0 && (kb & 3) == 0) mbar_wait(&b_ready_bar[kb >> 2], gph & 1);
+            const int kn = kb == nkb - 1 ? klast : 4;
             for (int p = 0; p < np; ++p) {
-              const uint32_t d = tmem + (mt * 2 + p) * 128;
-              mbar_wait(&lo_full_bar[sl], lpar);     // the splitter arrives after it has seen the TMA tile: X_hi is in place too
-              tc_fence_after();
-              if (elect_one()) {
+              {
+                const uint32_t d = tmem + (mt * 2 + p) * 128;
+                mbar_wait(&lo_full_bar[sl], lpar);     // the splitter arrives after it has seen the TMA tile: X_hi is in place too
+                tc_fence_after();
+                if (elect_one()) {
 #pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                  const uint64_t adv = (uint64_t)(k * 2);   // 8 tf32 = 32 bytes = 2 x 16 B
-                  umma_tf32(d, xh + adv, t_all + adv, idesc128, (kb == 0 && k == 0) ? 0u : 1u);
-                  // X_lo T_hi joins the other cross term in columns 64-127: the large hi*hi accumulator of columns 0-63 then
-                  // sees half as many (truncating) accumulations, the small cross-term accumulator's truncation is 2^-11 down
-                  umma_tf32(d + 64, xl + adv, t_all + adv, idesc64, 1u);
+                  for (int k = 0; k < 4; ++k) {
+                    if (k < kn) {
+                      const uint64_t adv = (uint64_t)(k * 2);   // 8 tf32 = 32 bytes = 2 x 16 B
+                      umma_tf32(d, xh + adv, t_all + adv, idesc128, (kb == 0 && k == 0) ? 0u : 1u);
+                      // X_lo T_hi joins the other cross term in columns 64-127: the large hi*hi accumulator of columns 0-63 then
+                      // sees half as many (truncating) accumulations, the small cross-term accumulator's truncation is 2^-11 down
+                      umma_tf32(d + 64, xl + adv, t_all + adv, idesc64, 1u);
+                    }
+                  }
+                  tc_commit(&empty_bar[s]);
                 }
-                tc_commit(&empty_bar[s]);
-                if (p == np - 1) {
-                  if (mtiles == 2 && mt == 1 && kb < 4) tc_commit(&t_free_bar[kb]);
-                  if (kb == nkb - 1) tc_commit(&tmem_full_bar[mt]);
-                }
+                __syncwarp();
               }
-              __syncwarp();
               xh += TSTEP; xl += TSTEP;
               if (++s == NF) { s = 0; xh = xh0; }
               if (++sl == NL) { sl = 0; xl = xl0; lpar ^= 1; }
+            }
+            // this warp's chain (or, in a real phase, its empty share) has passed k-block kb of tile mt
+            if ((mtiles == 2 && mt == 1 && kb < 4) || kb == nkb - 1) {
+              if (elect_one()) {
+                if (mtiles == 2 && mt == 1 && kb < 4) tc_commit(&t_free_bar[kb]);
+                if (kb == nkb - 1) tc_commit(&tmem_full_bar[mt]);
+              }
+              __syncwarp();
             }
           }
         }
