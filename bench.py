@@ -498,6 +498,52 @@ def load_traffic(cfg, gemm_path):
     return out
 
 
+def run_ndet_scan(args):
+    """cfg 4 (multi-determinant trial) at N_det = 10 / 100 / 1000: ms per walker step and the ratio to N_det = 10, beside the paper's
+    "10 -> 1200 determinants multiplies the propagation time by 3.9" (Fig. 1 :74; other hardware, other workload,
+    energy every 20 steps there, every step here: context, not a target)."""
+    import torch
+    from paper_1804_03310_b200.state import WalkerState, make_context
+    from workloads import make_workload, random_walkers
+    rows = []
+    for nd in (10, 100, 1000):
+        wl = make_workload(4, args.variant, overrides=dict(n_det=nd))
+        nw, K = wl.n_walkers, args.steps
+        ctx = make_context(wl, nw, gemm_path=args.gemm_path)
+        dev = ctx.device
+        x = torch.tensor(np.random.default_rng(1000).standard_normal((4, nw, wl.n_chol)), dtype=ctx.rdtype, device=dev)
+        phi0 = random_walkers(wl, nw, seed=21, spread=0.05)
+        st = WalkerState(ctx, phi0)
+        p0 = st.phi.clone()
+        eloc = torch.zeros(1, nw, dtype=torch.complex128, device=dev)
+
+        def reseed():
+            st.phi.copy_(p0); st.weight.fill_(1.0); st.flags.zero_(); st.seed()
+        out = {}
+        for mode, ee in (("energy_every_step", 1), ("energy_every_20", 20)):
+            reseed()
+            xs = x[torch.arange(20, device=dev) % 4].contiguous()
+            e20 = torch.zeros(20, nw, dtype=torch.complex128, device=dev)
+            ctx.afqmc_run(st.phi, st.weight, st.ovlp, st.theta, st.fb, xs, 20, ee, 2, 0, None, e20, None, None, st.flags)   # warm
+            reseed()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            ctx.afqmc_run(st.phi, st.weight, st.ovlp, st.theta, st.fb, xs, 20, ee, 2, 0, None, e20, None, None, st.flags)
+            e1.record()
+            torch.cuda.synchronize()
+            out[mode] = e0.elapsed_time(e1) / 20
+        rows.append(dict(n_det=nd, ms_per_step=out["energy_every_step"], ms_per_step_paper_schedule=out["energy_every_20"]))
+        ctx.close()
+    r0 = rows[0]
+    for r in rows:
+        r["ratio_to_10"] = r["ms_per_step"] / r0["ms_per_step"]
+        r["ratio_to_10_paper_schedule"] = r["ms_per_step_paper_schedule"] / r0["ms_per_step_paper_schedule"]
+    print(json.dumps(dict(metric="ms per walker step vs N_det (cfg 4 shapes, 512 walkers)", rows=rows,
+                          paper="x3.9 for 10 -> 1200 determinants (Mn QZ, 20 walkers, GTX 1080, energy every 20 steps; PAPER.md:68, :74)",
+                          note="20 steps per afqmc_run call, orthonormalisation every 2; energy_every_20 is the paper's schedule")))
+
+
 def run_sharded(args):
     """NEXT-4: the paper's schedule over a population SHARDED across the ranks --
     every rank steps its own N_w walkers, every measurement all-reduces three estimator sums, every pc_every steps the comb runs over
@@ -581,6 +627,7 @@ def main():
     ap.add_argument("--no-schedule", action="store_true")
     ap.add_argument("--no-graph", action="store_true", help="M < 96: time eager launches only (no CUDA graph replay)")
     ap.add_argument("--sharded", action="store_true", help="NEXT-4: the paper's schedule over a population sharded across the ranks")
+    ap.add_argument("--ndet-scan", action="store_true", help="cfg 4 at N_det = 10 / 100 / 1000 (PAPER.md Fig. 1)")
     ap.add_argument("--peaks", action="store_true", help="print the measured peak microbenchmarks only")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -588,6 +635,8 @@ def main():
     elif args.peaks:
         import torch
         print(json.dumps(dict(measured_peaks=measure_peaks(torch.device("cuda:0")), driver_peaks=peaks())))
+    elif args.ndet_scan:
+        run_ndet_scan(args)
     elif args.sharded:
         run_sharded(args)
     else:

@@ -255,7 +255,7 @@ inline size_t md_energy_smem(int M, int na, int nb, int nact, int ndet, int ts) 
   const size_t nw_ = (size_t)(nact - na) * na + (size_t)(nact - nb) * nb;
   // TT, W, WT, Q_virt copy, Z copy, 4 scalars: complex T (the bulk arithmetic follows the walker precision;
   // per-determinant energies and the final mixture are accumulated in FP64)
-  b += ((size_t)2 * nact * (na + nb) + 3 * nw_ + (size_t)ndet * 8 + 4) * 2 * ts + 16;   // TT is double buffered
+  b += ((size_t)2 * nact * (na + nb) + 3 * nw_ + 4) * 2 * ts + 16;   // TT is double buffered; Z is read from md_prepare's FP64 copy
   return b;
 }
 
@@ -278,13 +278,11 @@ __global__ void __launch_bounds__(MD_THREADS) k_md_energy(MdEnergyArgs<T> g) {
   Wm[0] = TT0 + 2 * nact * nt; Wm[1] = Wm[0] + nwa;
   WTm[0] = Wm[1] + nwb; WTm[1] = WTm[0] + nwa;
   Qc[0] = WTm[1] + nwb; Qc[1] = Qc[0] + nwa;
-  C* Zc = Qc[1] + nwb;                 // [ndet][2][4]
-  C* scal = Zc + (size_t)m.ndet * 8;   // f0[2], X0[2]
+  C* scal = Qc[1] + nwb;               // f0[2], X0[2]   (Z_i is read from s.Z, FP64: a second copy in T would not fit 1000 determinants)
   for (int e = tid; e < M * nt; e += nthr) th0[e] = g.theta0[(size_t)w * M * nt + e];
   __syncthreads();
   md_prepare<T>(m, th0, s);
   for (int e = tid; e < nwa + nwb; e += nthr) Qc[0][e] = mk<T>((T)s.Qv[0][e].x, (T)s.Qv[0][e].y);
-  for (int e = tid; e < m.ndet * 8; e += nthr) Zc[e] = mk<T>((T)s.Z[e].x, (T)s.Z[e].y);
 
   zcplx Eacc[MD_DPT];
 #pragma unroll
@@ -372,7 +370,10 @@ __global__ void __launch_bounds__(MD_THREADS) k_md_energy(MdEnergyArgs<T> g) {
         const int rk = (rks[j] >> (2 * sp)) & 3;
         const uint32_t pt = pat[j][sp];
         const int h0 = pt & 255, p0 = (pt >> 8) & 255, h1 = (pt >> 16) & 255, p1 = (pt >> 24) & 255;
-        const C* Zi = Zc + ((size_t)i * 2 + sp) * 4;
+        const zcplx* Zd = s.Z + ((size_t)i * 2 + sp) * 4;
+        C Zi[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) Zi[u] = mk<T>((T)Zd[u].x, (T)Zd[u].y);
         C t = scal[sp], xch = scal[2 + sp];
         if (rk == 1) {
           C zw = cmul(Zi[0], Wm[sp][p0 * n + h0]);

@@ -371,3 +371,27 @@ def test_large_M_accepted_on_tensor_path_only():
             with pytest.raises(afq.AfqmcError) as ei:
                 afq.afqmc_query_bytes(p)
             assert ei.value.status == afq.AFQMC_EUNSUPPORTED
+
+
+def test_multidet_large_expansion():
+    """N_det = 1000 (the paper's expansions reach 1266 determinants, Fig. 1 :68): S, mixed f and mixed E_L on
+    random walkers against the oracle's definition path.  Runs the general multi-determinant energy kernel (8 determinants
+    per thread) with Z read from its FP64 copy -- a second copy does not fit one CTA's shared memory at this size."""
+    import torch
+    wl = make_workload(4, "raw", overrides=dict(n_det=1000))
+    nw = 4
+    tol = H.tol_for(wl)
+    ini, trial = H.oracle_init(wl)
+    phi = random_walkers(wl, nw, seed=11, spread=0.2)
+    ctx = H.make_ctx(wl, nw)
+    st = H.DeviceState(ctx, phi)
+    st.seed()
+    eloc = torch.zeros(nw, dtype=torch.complex128, device=ctx.device)
+    ctx.afqmc_local_energy(st.phi, st.theta, eloc)
+    out = st.host()
+    S, f, E = orc.o_multidet_definition(ini, trial, phi, wl.n_alpha)
+    errs = dict(S=H.rel_abs(out["S"], S), f=H.rel_fro(out["f"], f), E=H.rel_abs(eloc.cpu().numpy(), E))
+    print(f"cfg4 shapes, 1000 determinants: {errs}")
+    H.record("multidet_1000", **errs)
+    for k, v in errs.items():
+        assert v < tol, (k, v)
