@@ -23,13 +23,23 @@ namespace tt {
 
 using namespace tc;
 
-enum { NL = 3, TILE_BYTES = 128 * 128, PLANE_KB_BYTES = 128 * 128, EPW = 8, NSPLIT = 6, NGROUP = 3, NTHREADS = 16 * 32 };
+#ifndef TAYLOR_NL
+#define TAYLOR_NL 3
+#endif
+#ifndef TAYLOR_NGROUP
+#define TAYLOR_NGROUP 3
+#endif
+enum { NL = TAYLOR_NL, TILE_BYTES = 128 * 128, PLANE_KB_BYTES = 128 * 128, EPW = 8, NSPLIT = 6, NGROUP = TAYLOR_NGROUP, WPG = NSPLIT / NGROUP, NTHREADS = 16 * 32 };
 // NSPLIT <= NL <= NF: a parity wait on an mbarrier is only unambiguous within one phase of it.  A splitter that has finished
 // tile it - NSPLIT knows the MMAs of tile it - NSPLIT - NL are done; its wait for the lo buffer of tile `it` needs those of tile
 // it - 2 NL done (a warp that runs two phases ahead sees the parity it waits for as already complete and reads a tile that has
 // not landed -- seen as a hang: the producer's next expect_tx then over-arrives on the full barrier).
 // 16 warps: the two epilogue warpgroups take 200 registers per thread, the producer / MMA / splitter warpgroups 56 (setmaxnreg)
 enum { REGS_EPI = 200, REGS_AUX = 56 };
+// warp roles: 0..EPW-1 epilogue, then the splitters, then the TMA producer, and the MMA issuer LAST: the warp scheduler favours the
+// highest warp id of a sub-partition, and the MMA warp's few instructions between two tiles are the kernel's critical path
+enum { W_SPLIT0 = EPW, W_PROD = EPW + NSPLIT, W_MMA = EPW + NSPLIT + 1 };
+static_assert(W_MMA == 15, "16 warps");
 
 struct TaylorMaps {
   CUtensorMap A[2];   // [0: 128-row box, 1: last-tile box] over Abuf viewed as [N_w*M][2*MP] FP32
@@ -44,7 +54,7 @@ struct TaylorTcArgs {
 };
 
 enum { NF_MAX = 6 };
-static_assert(NGROUP <= NL && NSPLIT == 2 * NGROUP, "see above");
+static_assert(NGROUP <= NL && NSPLIT == WPG * NGROUP, "see above");
 inline int pick_nf(int nkb) {   // >= NL (the splitters' wait order relies on it)
   const int left = 227 * 1024 - 1024 - 512 - nkb * PLANE_KB_BYTES - NL * TILE_BYTES;
   const int nf = left / TILE_BYTES;
@@ -103,15 +113,15 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
   // short last tile are never written by TMA and must not hold NaN patterns)
   for (uint32_t o = threadIdx.x * 16; o < plane_bytes + (uint32_t)(NF + NL) * TILE_BYTES; o += NTHREADS * 16)
     *reinterpret_cast<uint4*>(planes + o) = make_uint4(0, 0, 0, 0);
-  if (warp == EPW && lane == 0) {
+  if (warp == W_PROD && lane == 0) {
     for (int s = 0; s < NF_MAX; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
-    for (int s = 0; s < NL; ++s) mbar_init(&lo_full_bar[s], 2);   // the two warps of a splitter group
+    for (int s = 0; s < NL; ++s) mbar_init(&lo_full_bar[s], WPG);   // the warps of a splitter group
     mbar_init(&tmem_full_bar[0], 1); mbar_init(&tmem_full_bar[1], 1);
     mbar_init(&b_ready_bar[0], EPW); mbar_init(&b_ready_bar[1], EPW);
     for (int x = 0; x < 4; ++x) mbar_init(&t_free_bar[x], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == EPW + 1) {
+  if (warp == W_MMA) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)),
                  "r"(tmem_cols)
                  : "memory");
@@ -126,7 +136,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
   const int n_mine = blockIdx.x < g.nw ? (g.nw - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
   const uint32_t tiles_per_walker = (uint32_t)(mtiles * nkb) * (uint32_t)(2 * g.K + 2);
 
-  if (warp == EPW) {
+  if (warp == W_PROD) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"((int)REGS_AUX));
     if (lane == 0) {   // ===== TMA producer: streams FP32 X tiles =====
       int s = 0;
@@ -149,14 +159,12 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
           }
         }
     }
-  } else if (warp >= EPW + 2 + NSPLIT) {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"((int)REGS_AUX));   // idle warps that complete the last warpgroup
-  } else if (warp >= EPW + 2) {
+  } else if (warp >= W_SPLIT0 && warp < W_PROD) {
     // ===== splitter warps: X_lo = (X - trunc13 X)(1 + 2^-11), elementwise at the same (swizzled) offsets.  NGROUP groups of two
     // warps take the tiles round robin (group = tile mod NGROUP <= NL, see above), each warp one half of the tile: the chain
     // "MMAs of tile it - NL done -> split tile it -> MMAs of tile it" is what paces the kernel, and two warps halve its split part =====
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"((int)REGS_AUX));
-    const int sw = warp - (EPW + 2), grp = sw >> 1, half = sw & 1;
+    const int sw = warp - W_SPLIT0, grp = sw / WPG, half = sw % WPG;
     const uint32_t total = (uint32_t)n_mine * tiles_per_walker;
     // (phase, index inside the phase) of this group's current tile; a phase is [m-tile 0 | m-tile 1], each nkb x planes tiles
     // (mtiles == 1: half_len is unused)
@@ -179,14 +187,14 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
       uint4* dst = reinterpret_cast<uint4*>(lobufs + (size_t)sl * TILE_BYTES);
       const int slabs = (mtiles == 2 && rr >= half_len) ? slabs_last : 8;     // second m-tile of its phase?
 #pragma unroll 1
-      for (int sb = half; sb < slabs; sb += 4) {       // two slabs (sb, sb + 2) per iteration: 8 accesses in flight
+      for (int sb = half; sb < slabs; sb += 2 * WPG) {       // two slabs (sb, sb + WPG) per iteration: 8 accesses in flight
         uint4 v[8];
-        const bool two = sb + 2 < slabs;
+        const bool two = sb + WPG < slabs;
 #pragma unroll
         for (int x = 0; x < 4; ++x) v[x] = src[(sb * 4 + x) * 32 + lane];
         if (two) {
 #pragma unroll
-          for (int x = 0; x < 4; ++x) v[4 + x] = src[((sb + 2) * 4 + x) * 32 + lane];
+          for (int x = 0; x < 4; ++x) v[4 + x] = src[((sb + WPG) * 4 + x) * 32 + lane];
         }
 #pragma unroll
         for (int x = 0; x < 4; ++x) {
@@ -199,7 +207,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
           for (int x = 0; x < 4; ++x) {
             uint4 q;
             q.x = tf32_lo_bits(v[4 + x].x); q.y = tf32_lo_bits(v[4 + x].y); q.z = tf32_lo_bits(v[4 + x].z); q.w = tf32_lo_bits(v[4 + x].w);
-            dst[((sb + 2) * 4 + x) * 32 + lane] = q;
+            dst[((sb + WPG) * 4 + x) * 32 + lane] = q;
           }
         }
       }
@@ -214,7 +222,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
       __syncwarp();
       if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&lo_full_bar[sl])) : "memory");
     }
-  } else if (warp == EPW + 1) {
+  } else if (warp == W_MMA) {
     // ===== MMA issuer warp.  The whole warp runs the loop (uniform control flow) and ONE elected lane issues: with the
     // descriptors computed under uniform control flow ptxas keeps them in uniform registers and the MMAs of a tile are
     // back-to-back UTCHMMA (inside an `if (lane == 0)` region it wraps every MMA in an ELECT / 5 x R2UR / branch-back sequence).
@@ -297,12 +305,18 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
       // consecutive complex numbers (coalesced, all loads in flight at once); every MMA of the previous walker has
       // completed (each warp has observed tmem_full of its last tile)
       {
+        // The next walker of this CTA is pulled into L2 now, a whole walker ahead: its first touch would otherwise be a DRAM round trip on
+        // the critical path (nothing else runs on this SM between two walkers).
         float2 f[MAXE / 2];
         const float2* src = reinterpret_cast<const float2*>(phi_w);
 #pragma unroll
         for (int k = 0; k < MAXE / 2; ++k) {
           const int e = et + k * (EPW * 32);
           if (e < M * nt) f[k] = src[e];
+        }
+        if (w + (int)gridDim.x < g.nw) {
+          const char* nxt = reinterpret_cast<const char*>(g.phi + (size_t)(w + gridDim.x) * M * nt);
+          for (int o = et * 128; o < M * nt * 8; o += EPW * 32 * 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(nxt + o));
         }
         if (w != (int)blockIdx.x) {
           // the previous walker's result is staged in the planes: write it out before they are overwritten
@@ -326,9 +340,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
           for (int k = 0; k < MAXE / 2; ++k) {
             const int e = et + (k + hb * (MAXE / 2)) * (EPW * 32);
             if (e < M * nt) {
+              const float2 fv = f[k];
               float h0, l0, h1, l1;
-              tf32_split_raw(f[k].x, h0, l0);     // hi = raw FP32 (the pipe truncates it), lo = centred low part
-              tf32_split_raw(f[k].y, h1, l1);
+              tf32_split_raw(fv.x, h0, l0);     // hi = raw FP32 (the pipe truncates it), lo = centred low part
+              tf32_split_raw(fv.y, h1, l1);
               const uint32_t o = plane_off(cbb, ci);
               sts32(pl_hi + o, h0);
               sts32(pl_lo + o, l0);
@@ -338,13 +353,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
             ci += di; cbb += db;
             if (cbb >= nt) { cbb -= nt; ++ci; }
           }
+          // the first half holds the elements e < 4096, i.e. basis indices i < 4096 / N_t >= 128 (N_t <= 32): k-blocks 0-3 are
+          // complete and the MMA warp can start on the first m-tile while the rest is being written
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          tc_fence_before();
+          asm volatile("bar.sync 1, 256;" ::: "memory");
+          if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&b_ready_bar[hb])) : "memory");
         }
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        tc_fence_before();
-        asm volatile("bar.sync 1, 256;" ::: "memory");
-        if (lane == 0)
-          for (int mt = 0; mt < 2; ++mt)
-            asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&b_ready_bar[mt])) : "memory");
       }
       for (int ph = 0; ph < nphase; ++ph, ++gph) {
         const bool last_phase = ph == nphase - 1;
@@ -449,7 +464,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == EPW + 1) {
+  if (warp == W_MMA) {
     __syncwarp();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(tmem_cols) : "memory");
   }
