@@ -73,6 +73,14 @@ __device__ __forceinline__ uint32_t plane_off(int b, int j) {
 // never touched.  Needs ceil(M / 16) <= 4 * floor(M / 32) (true for M >= 64).
 __device__ __forceinline__ uint32_t stage_chunk(int c) { return (uint32_t)((c >> 2) * PLANE_KB_BYTES + (c & 3) * (32 * 128)); }
 __device__ __forceinline__ uint32_t stage_row(int i, int nt) { return stage_chunk(i >> 4) + (uint32_t)((i & 15) * nt * 8); }
+__device__ __forceinline__ uint4 lds128(uint32_t a) {
+  uint4 v;
+  asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a) : "memory");
+  return v;
+}
+__device__ __forceinline__ void sts128(uint32_t a, uint4 v) {
+  asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
 __device__ __forceinline__ void sts32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
 __device__ __forceinline__ float2 lds64(uint32_t a) {
   float2 v;
@@ -183,31 +191,32 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_taylor_tc(const __grid_constant
       mbar_wait(&full_bar[s], (it / NF) & 1);
       // the two warps take alternate 16-row slabs (2 KB = 4 warp-wide 16-byte accesses); a short last tile (rows_last of 128 rows,
       // M = 200: 72) has only ceil(rows_last / 16) of them: TMA wrote nothing beyond and the MMAs' extra rows are never read back
-      const uint4* src = reinterpret_cast<const uint4*>(stages + (size_t)s * TILE_BYTES);
-      uint4* dst = reinterpret_cast<uint4*>(lobufs + (size_t)sl * TILE_BYTES);
+      // explicit shared-space accesses (LDS.128 / STS.128): through generic pointers ptxas emitted LD.E.128 / ST.E.128
+      const uint32_t src = smem_u32(stages + (size_t)s * TILE_BYTES) + lane * 16;
+      const uint32_t dst = smem_u32(lobufs + (size_t)sl * TILE_BYTES) + lane * 16;
       const int slabs = (mtiles == 2 && rr >= half_len) ? slabs_last : 8;     // second m-tile of its phase?
 #pragma unroll 1
       for (int sb = half; sb < slabs; sb += 2 * WPG) {       // two slabs (sb, sb + WPG) per iteration: 8 accesses in flight
         uint4 v[8];
         const bool two = sb + WPG < slabs;
 #pragma unroll
-        for (int x = 0; x < 4; ++x) v[x] = src[(sb * 4 + x) * 32 + lane];
+        for (int x = 0; x < 4; ++x) v[x] = lds128(src + (sb * 4 + x) * 512);
         if (two) {
 #pragma unroll
-          for (int x = 0; x < 4; ++x) v[4 + x] = src[((sb + WPG) * 4 + x) * 32 + lane];
+          for (int x = 0; x < 4; ++x) v[4 + x] = lds128(src + ((sb + WPG) * 4 + x) * 512);
         }
 #pragma unroll
         for (int x = 0; x < 4; ++x) {
           uint4 q;
           q.x = tf32_lo_bits(v[x].x); q.y = tf32_lo_bits(v[x].y); q.z = tf32_lo_bits(v[x].z); q.w = tf32_lo_bits(v[x].w);
-          dst[(sb * 4 + x) * 32 + lane] = q;
+          sts128(dst + (sb * 4 + x) * 512, q);
         }
         if (two) {
 #pragma unroll
           for (int x = 0; x < 4; ++x) {
             uint4 q;
             q.x = tf32_lo_bits(v[4 + x].x); q.y = tf32_lo_bits(v[4 + x].y); q.z = tf32_lo_bits(v[4 + x].z); q.w = tf32_lo_bits(v[4 + x].w);
-            dst[((sb + WPG) * 4 + x) * 32 + lane] = q;
+            sts128(dst + ((sb + WPG) * 4 + x) * 512, q);
           }
         }
       }
