@@ -258,7 +258,9 @@ AFQMC_API afqmc_status afqmc_profile_read(afqmc_ctx* ctx, int32_t stage, double*
 /* Peak microbenchmarks behind bench.py --peaks (the TF32 / FP32 / FP64 / L2 denominators are measured, not
  * assumed).  kind 0: back-to-back tcgen05.mma.kind::tf32 M = 128, N = n, operands from shared memory, one CTA per SM;
  * 1: the same with the a-operand in TMEM; 2: CTA pairs (cta_group::2, M = 256); 3: FFMA; 4: DFMA; 5: TMA stream of an
- * n-MiB buffer (L2 resident if n is small) into shared memory.  scratch: DEVICE, >= 1 MiB (kind 5: the streamed buffer).
+ * n-MiB buffer (L2 resident if n is small) into shared memory; 6-9: MMA issue patterns of the Taylor kernel (csrc/peaks.cuh);
+ * 10: correctness probe of a TS-mode MMA (a-operand written to TMEM by tcgen05.st; n = N + 1000 r0; scratch receives D[128][N]).
+ * scratch: DEVICE, >= 1 MiB (kind 5: the streamed buffer).
  * Synchronises `stream`.  ms = kernel time (CUDA events), units = flops (kinds 0-4) or bytes (kind 5) the kernel did,
  * clk = clocks per MMA measured inside CTA 0 (kinds 0-2, else 0).  No context needed.  Errors: EINVAL, ECUDA. */
 AFQMC_API afqmc_status afqmc_peak_probe(int32_t kind, int32_t n, int32_t iters, void* scratch, size_t scratch_bytes,

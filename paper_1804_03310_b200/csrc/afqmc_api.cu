@@ -1419,6 +1419,14 @@ afqmc_status afqmc_peak_probe(int32_t kind, int32_t n, int32_t iters, void* scra
     }
     return s;
   }
+  if (kind == 10) {                      // TS-mode correctness probe: n = N + 1000 * r0; scratch receives D[128][N] floats
+    const int N = n % 1000, r0 = n / 1000;
+    if (N < 16 || N > 128 || N % 16 || r0 + N > 128) { cudaEventDestroy(e0); cudaEventDestroy(e1); return AFQMC_EINVAL; }
+    cudaFuncSetAttribute(pk::k_probe_ts, cudaFuncAttributeMaxDynamicSharedMemorySize, 32768);
+    cudaEventRecord(e0, st);
+    pk::k_probe_ts<<<1, 128, 32768, st>>>(N, r0, (float*)scratch);
+    return finish(0.0);
+  }
   if (kind == 3 || kind == 4) {          // FFMA / DFMA; units = flops
     const int grid = n_sm * 4, thr = 512;
     cudaEventRecord(e0, st);

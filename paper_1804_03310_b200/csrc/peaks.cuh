@@ -10,14 +10,6 @@ namespace pk {
 
 using namespace tc;
 
-__device__ __forceinline__ void umma_tf32_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
-  asm volatile(
-      "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
-      "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n}"
-      ::"r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(acc)
-      : "memory");
-}
-
 // mode 0: SS (a, b from shared memory), one CTA;  1: TS (a from TMEM);  2: SS on a CTA pair (M = 256)
 // Every CTA issues `iters` k-blocks of 4 MMAs (K = 8 each) into one accumulator; out[blockIdx] = clocks of the issue loop
 // (first MMA issued -> last MMA completed).
@@ -273,6 +265,72 @@ __global__ void __launch_bounds__(64, 1) k_peak_pat(int iters, long long* out) {
     __syncwarp();
     mbar_wait(&bars[0], 0);
     if (lane == 0) out[blockIdx.x] = (clock64() - t0) / (PAT == 2 ? 2 : 1);
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512u) : "memory");
+}
+
+// Correctness probe for the TS-mode Taylor design: A (128 x 32 tf32) is written to TMEM by tcgen05.st (thread = row, 32 columns),
+// B is N rows of a K-major SWIZZLE_128B tile starting r0 rows into the tile; D[128][N] is read back.  a[r][c] = ((r * 3 + c * 5) % 17) - 8,
+// b[n][c] = ((n * 7 + c * 11) % 13) - 6 (small integers: exact in TF32), out[r * N + n] = sum_c a[r][c] b[r0 + n][c].
+__global__ void __launch_bounds__(128, 1) k_probe_ts(int N, int r0, float* out) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  __shared__ __align__(8) uint64_t bar;
+  __shared__ uint32_t tmem_base_s;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  for (int e = threadIdx.x; e < 128 * 32; e += blockDim.x) {
+    const int n = e >> 5, c = e & 31;
+    const float v = (float)(((n * 7 + c * 11) % 13) - 6);
+    *reinterpret_cast<float*>(smem + n * 128 + ((((c >> 2) ^ (n & 7)) << 4) | ((c & 3) << 2))) = v;
+  }
+  if (threadIdx.x == 0) { mbar_init(&bar, 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "r"(512u) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_base_s;
+  {
+    const int r = warp * 32 + lane;
+    uint32_t a[32];
+#pragma unroll
+    for (int c = 0; c < 32; ++c) a[c] = __float_as_uint((float)(((r * 3 + c * 5) % 17) - 8));
+    const uint32_t taddr = tmem + ((uint32_t)(warp * 32) << 16) + 256;
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+        "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};"
+        ::"r"(taddr), "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(a[4]), "r"(a[5]), "r"(a[6]), "r"(a[7]), "r"(a[8]), "r"(a[9]),
+          "r"(a[10]), "r"(a[11]), "r"(a[12]), "r"(a[13]), "r"(a[14]), "r"(a[15]), "r"(a[16]), "r"(a[17]), "r"(a[18]), "r"(a[19]),
+          "r"(a[20]), "r"(a[21]), "r"(a[22]), "r"(a[23]), "r"(a[24]), "r"(a[25]), "r"(a[26]), "r"(a[27]), "r"(a[28]), "r"(a[29]),
+          "r"(a[30]), "r"(a[31])
+        : "memory");
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  if (warp == 1) {
+    const uint64_t bd = make_desc(smem_u32(smem) + (uint32_t)r0 * 128);
+    const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+    if (elect_one()) {
+#pragma unroll
+      for (int k = 0; k < 4; ++k) umma_tf32_ts(tmem, tmem + 256 + k * 8, bd + 2 * k, idesc, k ? 1u : 0u);
+      tc_commit(&bar);
+    }
+    __syncwarp();
+  }
+  mbar_wait(&bar, 0);
+  tc_fence_after();
+  for (int c0 = 0; c0 < N; c0 += 28) {        // 28-column steps on purpose: the design reads at offsets that are multiples of 28
+    float v[32];
+    tmem_ld32(tmem + ((uint32_t)(warp * 32) << 16) + c0, v);
+    const int r = warp * 32 + lane;
+    for (int j = 0; j < 28 && c0 + j < N; ++j) out[r * N + c0 + j] = v[j];
   }
   tc_fence_before();
   __syncthreads();
