@@ -69,7 +69,8 @@ typedef struct {
   int32_t weight_mode;  /* 0: hybrid; 1: local-energy form */
   int32_t n_det;        /* determinants in the trial, 1 = single determinant */
   int32_t n_act;        /* active orbitals spanning all determinants (0 if n_det == 1) */
-  int32_t max_exc;      /* slots per spin in det_exc; excitation rank per spin <= 2 */
+  int32_t max_exc;      /* slots per spin in det_exc = largest excitation rank per spin, 1..4 (<= 2: closed-form 2 x 2 inverses and the
+                           batched energy kernel; 3, 4: general small elimination, one-operator-at-a-time energy kernel) */
   int32_t gemm_path;    /* 0: auto (3 for precision 0, else 1); 1: SIMT FP32/FP64 everywhere; 2: tcgen05 3xTF32
                            GEMMs, one CTA per 128x256 tile; 3: the same on CTA pairs (cta_group::2, 256x256
                            tiles).  2 and 3 need precision 0.  DESIGN.md "Precision split". */

@@ -48,7 +48,7 @@ struct afqmc_ctx {
   int M, MP, na, nb, nt, ng, NGP, nw, KA, KB, KT, ts;  // ts = sizeof(T)
   int split, path;
   // multi-determinant trial (md != 0): ca/cb = columns per spin of the generalised Theta (n_act), else n_alpha/n_beta
-  int md, nact, ndet, ca, cb;
+  int md, nact, ndet, ca, cb, emax;   // emax: slots per spin of the normalised excitation list (2, or 4 when max_exc > 2)
   void* Cact; double* coeff; int32_t* exc;
   double *psid_ac, *psid_bc;   // FP64 trial orbitals (constants)
   void *thtil, *th_scr; zcplx *ovlp0, *ovlp_scr;
@@ -173,12 +173,12 @@ afqmc_status check_params(const afqmc_params* p, char* err) {
     if (p->n_act < p->n_alpha || p->n_act < p->n_beta || p->n_act > p->M || p->n_beta < 1) {
       snprintf(err, 256, "multi-det: need max(n_alpha, n_beta) <= n_act <= M and n_beta >= 1"); return AFQMC_EINVAL;
     }
-    if (p->max_exc < 1 || p->max_exc > 2) { snprintf(err, 256, "max_exc must be 1 or 2"); return AFQMC_EUNSUPPORTED; }
+    if (p->max_exc < 1 || p->max_exc > 4) { snprintf(err, 256, "max_exc (excitation rank per spin) must be 1..4"); return AFQMC_EUNSUPPORTED; }
     if (p->n_det > 1024) { snprintf(err, 256, "n_det <= 1024 supported"); return AFQMC_EUNSUPPORTED; }
     if (p->n_act * (p->n_alpha + p->n_beta) > 1024) { snprintf(err, 256, "n_act * N_t <= 1024 supported"); return AFQMC_EUNSUPPORTED; }
-    const int ts_ = p->precision ? 8 : 4;
-    if (md_energy_smem(p->M, p->n_alpha, p->n_beta, p->n_act, p->n_det, ts_) > 200 * 1024 ||
-        md_overlap_smem(p->M, p->n_alpha, p->n_beta, p->n_act, p->n_det, ts_) > 200 * 1024) {
+    const int ts_ = p->precision ? 8 : 4, emax_ = p->max_exc > 2 ? 4 : 2;
+    if (md_energy_smem(p->M, p->n_alpha, p->n_beta, p->n_act, p->n_det, ts_, emax_) > 200 * 1024 ||
+        md_overlap_smem(p->M, p->n_alpha, p->n_beta, p->n_act, p->n_det, ts_, emax_) > 200 * 1024) {
       snprintf(err, 256, "multi-det working set exceeds one CTA's shared memory"); return AFQMC_EUNSUPPORTED;
     }
   }
@@ -235,7 +235,7 @@ void carve(const afqmc_params* p, afqmc_ctx* c, char* cbase, char* wbase, size_t
   c->hrot = cc.take((size_t)KT * ts);
   c->Cact = cc.take((size_t)M * (md ? p->n_act : 1) * ts);
   c->coeff = (double*)cc.take((size_t)p->n_det * 8);
-  c->exc = (int32_t*)cc.take((size_t)p->n_det * 8 * 4);
+  c->exc = (int32_t*)cc.take((size_t)p->n_det * 16 * 4);      // [n_det][2][emax <= 4][2]
   c->MPK = (int)rup(M, 32);   // K of the TT GEMM, padded to the tcgen05 k-block
   c->RactT = cc.take(md ? (size_t)(ng + 1) * p->n_act * c->MPK * ts : 256);
   c->RactT_lo = (md && split) ? cc.take((size_t)(ng + 1) * p->n_act * c->MPK * ts) : nullptr;
@@ -348,7 +348,7 @@ template <typename T> afqmc_status init_device(afqmc_ctx* c, const double* h1, c
     const int nact = c->nact;
     CUDA_OK(c, cudaMemcpyAsync(Cact_d, Cact_h, (size_t)M * nact * 8, cudaMemcpyHostToDevice, st));
     CUDA_OK(c, cudaMemcpyAsync(c->coeff, coeff_h, (size_t)c->ndet * 8, cudaMemcpyHostToDevice, st));
-    CUDA_OK(c, cudaMemcpyAsync(c->exc, exc_h, (size_t)c->ndet * 8 * 4, cudaMemcpyHostToDevice, st));
+    CUDA_OK(c, cudaMemcpyAsync(c->exc, exc_h, (size_t)c->ndet * 4 * c->emax * 4, cudaMemcpyHostToDevice, st));
     LAUNCH(c, k_cast2d<T>, (M * nact + 127) / 128, 128, 0, M, nact, Cact_d, (size_t)nact, (T*)c->Cact, (T*)nullptr,
            (size_t)nact, 0);
   }
@@ -421,7 +421,7 @@ afqmc_status run_green(afqmc_ctx* c, const void* phi, void* ovlp, void* theta, i
     LAUNCH(c, k_green<T>, c->nw, 256, c->green_smem, g);
     MdOverlapArgs<T> a;
     a.m.M = c->M; a.m.na = c->na; a.m.nb = c->nb; a.m.nact = c->nact; a.m.ndet = c->ndet;
-    a.m.C = c->Cact; a.m.coeff = c->coeff; a.m.exc = c->exc;
+    a.m.C = c->Cact; a.m.coeff = c->coeff; a.m.exc = c->exc; a.m.emax = c->emax;
     a.theta0 = (const cplx<T>*)theta; a.ovlp0 = c->ovlp0; a.thtil = (cplx<T>*)c->thtil; a.ovlp = (zcplx*)ovlp;
     a.do_weight = do_weight; a.cshift = c->cshift; a.weight = weight; a.eloc_pre = (const zcplx*)eloc_pre;
     a.weight_mode = c->p.weight_mode; a.dt = c->p.dt; a.E0 = c->p.E0; a.flags = flags;
@@ -496,7 +496,7 @@ template <typename T> afqmc_status run_md_energy(afqmc_ctx* c, const void* theta
   StageScope sc(c, AFQMC_STAGE_ENERGY);
   MdEnergyArgs<T> a;
   a.m.M = c->M; a.m.na = c->na; a.m.nb = c->nb; a.m.nact = c->nact; a.m.ndet = c->ndet;
-  a.m.C = c->Cact; a.m.coeff = c->coeff; a.m.exc = c->exc;
+  a.m.C = c->Cact; a.m.coeff = c->coeff; a.m.exc = c->exc; a.m.emax = c->emax;
   a.ng = c->ng; a.ldr = c->KT; a.theta0 = (const cplx<T>*)theta; a.TTg = (const cplx<T>*)c->TTg;
   a.eloc = eloc;
   // TT[w][g][q][a] = sum_k (C_act^T X_g)[q][k] Theta_0[w][k][a] for every g (and h) in one GEMM over all walkers
@@ -526,7 +526,7 @@ template <typename T> afqmc_status run_md_energy(afqmc_ctx* c, const void* theta
     // registers), tiles that are 16-byte multiples, shared memory that fits
     const int nmax = c->na > c->nb ? c->na : c->nb;
     const size_t smb = md_energy_b_smem(c->M, c->na, c->nb, c->nact, c->ndet, c->ts);
-    if (c->path == 2 && nmax <= 16 && dpt <= 2 && ((size_t)c->nact * c->nt * 2 * c->ts) % 16 == 0 && smb <= 200 * 1024) {
+    if (c->path == 2 && c->emax == 2 && nmax <= 16 && dpt <= 2 && ((size_t)c->nact * c->nt * 2 * c->ts) % 16 == 0 && smb <= 200 * 1024) {
 #define MDB_LAUNCH(N, D)                                                                                           \
   {                                                                                                                \
     auto kern = k_md_energy_b<T, N, D>;                                                                            \
@@ -834,7 +834,8 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
   }
   // multi-det: reference orbitals = first n_sigma columns of C_act; excitation list normalised to 2 slots
   std::vector<double> pa_md, pb_md;
-  std::vector<int32_t> exc2((size_t)p->n_det * 8, -1);
+  const int emax = p->max_exc > 2 ? 4 : 2;
+  std::vector<int32_t> exc2((size_t)p->n_det * 4 * emax, -1);
   if (md) {
     const int nact = p->n_act;
     pa_md.resize((size_t)p->M * p->n_alpha); pb_md.resize((size_t)p->M * p->n_beta);
@@ -846,19 +847,21 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
     for (int i = 0; i < p->n_det; ++i)
       for (int sp = 0; sp < 2; ++sp) {
         const int n = sp ? p->n_beta : p->n_alpha;
-        int cnt = 0, hs[2] = {-1, -1}, ps[2] = {-1, -1};
+        int cnt = 0, hs[4] = {-1, -1, -1, -1}, ps[4] = {-1, -1, -1, -1};
         for (int e = 0; e < p->max_exc; ++e) {
           const int32_t* ex = det_exc + (((size_t)i * 2 + sp) * p->max_exc + e) * 2;
           if (ex[0] < 0) continue;
-          if (ex[0] >= n || ex[1] < n || ex[1] >= nact || (cnt == 1 && (ex[0] == hs[0] || ex[1] == ps[0]))) {
+          bool dup = false;
+          for (int q = 0; q < cnt; ++q) dup |= ex[0] == hs[q] || ex[1] == ps[q];
+          if (ex[0] >= n || ex[1] < n || ex[1] >= nact || dup) {
             snprintf(g_init_err, 256, "det_exc: need hole < n_sigma <= particle < n_act, distinct within a determinant");
             return AFQMC_EINVAL;
           }
           hs[cnt] = ex[0]; ps[cnt] = ex[1]; ++cnt;
         }
         for (int e = 0; e < cnt; ++e) {
-          exc2[((size_t)i * 2 + sp) * 4 + 2 * e] = hs[e];
-          exc2[((size_t)i * 2 + sp) * 4 + 2 * e + 1] = ps[e];
+          exc2[((size_t)i * 2 + sp) * 2 * emax + 2 * e] = hs[e];
+          exc2[((size_t)i * 2 + sp) * 2 * emax + 2 * e + 1] = ps[e];
         }
       }
   }
@@ -896,6 +899,7 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
   c->path = resolve_path(p);
   c->split = c->path == 2;
   c->cta2 = resolve_cta2(p);
+  c->emax = emax;
   {
     int dev = 0;
     cudaGetDevice(&dev);
@@ -925,8 +929,8 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
     }
   }
   if (c->md) {
-    c->mdo_smem = md_overlap_smem(c->M, c->na, c->nb, c->nact, c->ndet, c->ts);
-    c->mde_smem = md_energy_smem(c->M, c->na, c->nb, c->nact, c->ndet, c->ts);
+    c->mdo_smem = md_overlap_smem(c->M, c->na, c->nb, c->nact, c->ndet, c->ts, c->emax);
+    c->mde_smem = md_energy_smem(c->M, c->na, c->nb, c->nact, c->ndet, c->ts, c->emax);
     cudaError_t e1, e2;
     if (p->precision) {
       e1 = cudaFuncSetAttribute(k_md_overlap<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->mdo_smem);

@@ -17,24 +17,25 @@ __device__ __forceinline__ zcplx zscale(zcplx a, double s) { return mk<double>(a
 
 struct MdConst {
   int M, na, nb, nact, ndet;
+  int emax;                // slots per spin in exc: 2 (excitation rank <= 2, closed forms) or 4 (rank <= 4, general small elimination)
   const void* C;           // [M][nact]  (T)
   const double* coeff;     // [ndet]
-  const int32_t* exc;      // [ndet][2][2][2] (hole, particle) or -1
+  const int32_t* exc;      // [ndet][2][emax][2] (hole, particle) or -1
 };
 
 // Shared-memory view used by both multi-det kernels.
 struct MdSmem {
   zcplx* Qv[2];    // [nvirt_s][n_s]     Q_virt = C_virt^T Theta_0
-  zcplx* Z;        // [ndet][2][4]       Z_i^s[f][e] (row = hole slot f, col = particle slot e)
+  zcplx* Z;        // [ndet][2][emax^2]  Z_i^s[f][e] (row = hole slot f, col = particle slot e), index md_zidx(rank, f, e)
   zcplx* omega;    // [ndet]             c_i S_i / S
   int8_t* rank;    // [ndet][2]          excitation rank per spin
   zcplx* red;      // [64] reduction scratch
   int* flag;       // bit 0: a determinant has exactly zero overlap with the walker (its Z is undefined)
 };
 
-inline size_t md_smem_bytes(int na, int nb, int nact, int ndet) {
+inline size_t md_smem_bytes(int na, int nb, int nact, int ndet, int emax = 2) {
   size_t b = (size_t)((nact - na) * na + (nact - nb) * nb) * sizeof(zcplx);
-  b += (size_t)ndet * 8 * sizeof(zcplx) + (size_t)ndet * sizeof(zcplx) + 64 * sizeof(zcplx);
+  b += (size_t)ndet * 2 * emax * emax * sizeof(zcplx) + (size_t)ndet * sizeof(zcplx) + 64 * sizeof(zcplx);
   b += ((size_t)ndet * 2 + 15) & ~size_t(15);
   b += 16;
   return b;
@@ -43,7 +44,7 @@ inline size_t md_smem_bytes(int na, int nb, int nact, int ndet) {
 __device__ inline unsigned char* md_carve(unsigned char* p, const MdConst& m, MdSmem& s) {
   s.Qv[0] = reinterpret_cast<zcplx*>(p); p += (size_t)(m.nact - m.na) * m.na * sizeof(zcplx);
   s.Qv[1] = reinterpret_cast<zcplx*>(p); p += (size_t)(m.nact - m.nb) * m.nb * sizeof(zcplx);
-  s.Z = reinterpret_cast<zcplx*>(p); p += (size_t)m.ndet * 8 * sizeof(zcplx);
+  s.Z = reinterpret_cast<zcplx*>(p); p += (size_t)m.ndet * 2 * m.emax * m.emax * sizeof(zcplx);
   s.omega = reinterpret_cast<zcplx*>(p); p += (size_t)m.ndet * sizeof(zcplx);
   s.red = reinterpret_cast<zcplx*>(p); p += 64 * sizeof(zcplx);
   s.rank = reinterpret_cast<int8_t*>(p); p += ((size_t)m.ndet * 2 + 15) & ~size_t(15);
@@ -62,6 +63,55 @@ __device__ inline zcplx block_sum(zcplx v, zcplx* red) {
   for (int i = 0; i < nwarp; ++i) t = zadd(t, red[i]);
   __syncthreads();
   return t;
+}
+
+// canonical (hole, particle) slots of determinant i, spin sp (valid pairs first, in list order); returns the rank
+__device__ __forceinline__ int md_exc(const MdConst& m, int i, int sp, int (&h)[4], int (&p)[4]) {
+  const int32_t* ex = m.exc + ((size_t)i * 2 + sp) * 2 * m.emax;
+  int rk = 0;
+#pragma unroll
+  for (int e = 0; e < 4; ++e) { h[e] = -1; p[e] = -1; }
+  for (int e = 0; e < m.emax; ++e)
+    if (ex[2 * e] >= 0) { h[rk] = ex[2 * e]; p[rk] = ex[2 * e + 1]; ++rk; }
+  return rk;
+}
+
+// index of Z[f][e] inside a determinant's block: rank 1 and 2 keep the layout of the closed forms, rank 3 and 4 use rows of 4
+__device__ __forceinline__ int md_zidx(int rk, int f, int e) { return rk == 1 ? 0 : (rk == 2 ? f * 2 + e : f * 4 + e); }
+
+// determinant and inverse of the rk x rk matrix A (rk <= 4, row-major, stride 4) by Gauss-Jordan with partial pivoting; inv row-major
+// stride 4.  An exactly singular matrix returns det = 0 and leaves inv zero (the caller flags the walker).  FP64.
+__device__ inline zcplx md_small_inverse(int rk, zcplx (&A)[16], zcplx (&inv)[16]) {
+  for (int e = 0; e < 16; ++e) inv[e] = mk<double>(((e >> 2) == (e & 3)) ? 1.0 : 0.0, 0.0);
+  zcplx det = mk<double>(1.0, 0.0);
+  for (int c = 0; c < rk; ++c) {
+    int piv = c; double best = cabs2(A[c * 4 + c]);
+    for (int r = c + 1; r < rk; ++r) { const double m2 = cabs2(A[r * 4 + c]); if (m2 > best) { best = m2; piv = r; } }
+    if (!(best > 0.0)) {
+      for (int e = 0; e < 16; ++e) inv[e] = mk<double>(0.0, 0.0);
+      return mk<double>(0.0, 0.0);
+    }
+    if (piv != c) {
+      for (int k = 0; k < rk; ++k) {
+        zcplx t = A[c * 4 + k]; A[c * 4 + k] = A[piv * 4 + k]; A[piv * 4 + k] = t;
+        t = inv[c * 4 + k]; inv[c * 4 + k] = inv[piv * 4 + k]; inv[piv * 4 + k] = t;
+      }
+      det = mk<double>(-det.x, -det.y);
+    }
+    const zcplx pv = A[c * 4 + c];
+    det = zmul(det, pv);
+    const zcplx ip = zdiv(mk<double>(1.0, 0.0), pv);
+    for (int k = 0; k < rk; ++k) { A[c * 4 + k] = zmul(A[c * 4 + k], ip); inv[c * 4 + k] = zmul(inv[c * 4 + k], ip); }
+    for (int r = 0; r < rk; ++r) {
+      if (r == c) continue;
+      const zcplx f = A[r * 4 + c];
+      for (int k = 0; k < rk; ++k) {
+        A[r * 4 + k] = zsub(A[r * 4 + k], zmul(f, A[c * 4 + k]));
+        inv[r * 4 + k] = zsub(inv[r * 4 + k], zmul(f, inv[c * 4 + k]));
+      }
+    }
+  }
+  return det;
 }
 
 // From Theta_0 (shared, [M][nt] complex T): Q_virt, per-determinant ratios r_i, Z_i, mixing weights
@@ -91,12 +141,11 @@ __device__ zcplx md_prepare(const MdConst& m, const cplx<T>* th0, MdSmem& s) {
     zcplx ratio = mk<double>(1.0, 0.0);
     for (int sp = 0; sp < 2; ++sp) {
       const int n = sp ? m.nb : m.na;
-      const int32_t* ex = m.exc + ((size_t)i * 2 + sp) * 4;
-      int h0 = ex[0], p0 = ex[1], h1 = ex[2], p1 = ex[3];
-      int rk = (h0 >= 0) + (h1 >= 0);
-      if (h0 < 0 && h1 >= 0) { h0 = h1; p0 = p1; }
+      int hs[4], ps[4];
+      const int rk = md_exc(m, i, sp, hs, ps);
+      const int h0 = hs[0], p0 = ps[0], h1 = hs[1], p1 = ps[1];
       s.rank[i * 2 + sp] = (int8_t)rk;
-      zcplx* Zi = s.Z + ((size_t)i * 2 + sp) * 4;
+      zcplx* Zi = s.Z + ((size_t)i * 2 + sp) * m.emax * m.emax;
       const zcplx* Q = s.Qv[sp];
       if (rk == 1) {
         zcplx q = Q[(p0 - n) * n + h0];
@@ -116,6 +165,16 @@ __device__ zcplx md_prepare(const MdConst& m, const cplx<T>* th0, MdSmem& s) {
         Zi[1] = zmul(mk<double>(-b.x, -b.y), id);
         Zi[2] = zmul(mk<double>(-c.x, -c.y), id);
         Zi[3] = zmul(a, id);
+      } else if (rk >= 3) {
+        // Q_i[e][f] = Q[p_e][h_f] (rows = particle slot, columns = hole slot); Z = Q_i^-1, Z[f][e]
+        zcplx A[16], inv[16];
+        for (int e = 0; e < rk; ++e)
+          for (int f = 0; f < rk; ++f) A[e * 4 + f] = Q[(ps[e] - n) * n + hs[f]];
+        const zcplx det = md_small_inverse(rk, A, inv);
+        if (det.x == 0.0 && det.y == 0.0) atomicOr(s.flag, 1);
+        ratio = zmul(ratio, det);
+        for (int f = 0; f < rk; ++f)
+          for (int e = 0; e < rk; ++e) Zi[f * 4 + e] = inv[f * 4 + e];
       }
     }
     zcplx cr = zscale(ratio, m.coeff[i]);
@@ -129,15 +188,6 @@ __device__ zcplx md_prepare(const MdConst& m, const cplx<T>* th0, MdSmem& s) {
 }
 
 
-// canonical (hole, particle) slots of determinant i, spin sp; returns the rank
-__device__ __forceinline__ int md_exc(const MdConst& m, int i, int sp, int (&h)[2], int (&p)[2]) {
-  const int32_t* ex = m.exc + ((size_t)i * 2 + sp) * 4;
-  h[0] = ex[0]; p[0] = ex[1]; h[1] = ex[2]; p[1] = ex[3];
-  int rk = (h[0] >= 0) + (h[1] >= 0);
-  if (h[0] < 0 && h[1] >= 0) { h[0] = h[1]; p[0] = p[1]; }
-  return rk;
-}
-
 template <typename T> struct MdOverlapArgs {
   MdConst m;
   const cplx<T>* theta0;   // [nw][M][nt]   reference Theta_0 (from k_green)
@@ -150,8 +200,8 @@ template <typename T> struct MdOverlapArgs {
   int* flags;
 };
 
-inline size_t md_overlap_smem(int M, int na, int nb, int nact, int ndet, int ts) {
-  size_t b = md_smem_bytes(na, nb, nact, ndet);
+inline size_t md_overlap_smem(int M, int na, int nb, int nact, int ndet, int ts, int emax = 2) {
+  size_t b = md_smem_bytes(na, nb, nact, ndet, emax);
   b += ((size_t)M * (na + nb) * 2 * ts + 15) & ~size_t(15);
   b += (size_t)(na * (nact - na) + nb * (nact - nb)) * sizeof(zcplx);   // Btil
   b += (size_t)(na * na + nb * nb) * sizeof(zcplx);                     // Btil Q_virt
@@ -179,13 +229,13 @@ __global__ void __launch_bounds__(256) k_md_overlap(MdOverlapArgs<T> g) {
   for (int i = tid; i < m.ndet; i += nthr) {
     zcplx om = s.omega[i];
     for (int sp = 0; sp < 2; ++sp) {
-      int h[2], pp[2];
+      int h[4], pp[4];
       int rk = md_exc(m, i, sp, h, pp);
       const int n = sp ? m.nb : m.na, nv = m.nact - n;
-      const zcplx* Zi = s.Z + ((size_t)i * 2 + sp) * 4;
+      const zcplx* Zi = s.Z + ((size_t)i * 2 + sp) * m.emax * m.emax;
       for (int f = 0; f < rk; ++f)
         for (int e = 0; e < rk; ++e) {
-          zcplx v = zmul(om, Zi[rk == 1 ? 0 : f * 2 + e]);
+          zcplx v = zmul(om, Zi[md_zidx(rk, f, e)]);
           double* dst = reinterpret_cast<double*>(&Bt[sp][h[f] * nv + (pp[e] - n)]);
           atomicAdd(dst, v.x); atomicAdd(dst + 1, v.y);
         }
@@ -249,8 +299,8 @@ template <typename T> struct MdEnergyArgs {
   zcplx* eloc;             // [nw]
 };
 
-inline size_t md_energy_smem(int M, int na, int nb, int nact, int ndet, int ts) {
-  size_t b = md_smem_bytes(na, nb, nact, ndet);
+inline size_t md_energy_smem(int M, int na, int nb, int nact, int ndet, int ts, int emax = 2) {
+  size_t b = md_smem_bytes(na, nb, nact, ndet, emax);
   b += ((size_t)M * (na + nb) * 2 * ts + 15) & ~size_t(15);
   const size_t nw_ = (size_t)(nact - na) * na + (size_t)(nact - nb) * nb;
   // TT, W, WT, Q_virt copy, Z copy, 4 scalars: complex T (the bulk arithmetic follows the walker precision;
@@ -295,10 +345,10 @@ __global__ void __launch_bounds__(MD_THREADS) k_md_energy(MdEnergyArgs<T> g) {
     rks[j] = 0; pat[j][0] = pat[j][1] = 0;
     if (i < m.ndet)
       for (int sp = 0; sp < 2; ++sp) {
-        int h[2], pp[2];
+        int h[4], pp[4];
         const int rk = md_exc(m, i, sp, h, pp);
         const int n = sp ? m.nb : m.na;
-        rks[j] |= rk << (2 * sp);
+        rks[j] |= rk << (4 * sp);
         pat[j][sp] = (uint32_t)(h[0] & 255) | ((uint32_t)((pp[0] - n) & 255) << 8) | ((uint32_t)(h[1] & 255) << 16) |
                      ((uint32_t)((pp[1] - n) & 255) << 24);
       }
@@ -367,15 +417,41 @@ __global__ void __launch_bounds__(MD_THREADS) k_md_energy(MdEnergyArgs<T> g) {
 #pragma unroll
       for (int sp = 0; sp < 2; ++sp) {
         const int n = sp ? m.nb : m.na;
-        const int rk = (rks[j] >> (2 * sp)) & 3;
+        const int rk = (rks[j] >> (4 * sp)) & 15;
         const uint32_t pt = pat[j][sp];
         const int h0 = pt & 255, p0 = (pt >> 8) & 255, h1 = (pt >> 16) & 255, p1 = (pt >> 24) & 255;
-        const zcplx* Zd = s.Z + ((size_t)i * 2 + sp) * 4;
+        const zcplx* Zd = s.Z + ((size_t)i * 2 + sp) * m.emax * m.emax;
         C Zi[4];
 #pragma unroll
         for (int u = 0; u < 4; ++u) Zi[u] = mk<T>((T)Zd[u].x, (T)Zd[u].y);
         C t = scal[sp], xch = scal[2 + sp];
-        if (rk == 1) {
+        if (rk >= 3) {
+          // general rank (3, 4): A = Z W[P,H] (rk x rk), t += Tr A, xch += 2 Tr(Z WT[P,H]) + Tr(A A)
+          int hh[4], pq[4];
+          md_exc(m, i, sp, hh, pq);
+          C A[16];
+          for (int f = 0; f < rk; ++f)
+            for (int f2 = 0; f2 < rk; ++f2) {
+              C acc = mk<T>(T(0), T(0));
+              for (int e = 0; e < rk; ++e) {
+                const zcplx zd = Zd[f * 4 + e];
+                cfma(acc, mk<T>((T)zd.x, (T)zd.y), Wm[sp][(pq[e] - n) * n + hh[f2]]);
+              }
+              A[f * 4 + f2] = acc;
+            }
+          for (int f = 0; f < rk; ++f) t = cadd(t, A[f * 4 + f]);
+          if (!is_h) {
+            C tr2 = mk<T>(T(0), T(0));
+            for (int f = 0; f < rk; ++f)
+              for (int e = 0; e < rk; ++e) {
+                const zcplx zd = Zd[f * 4 + e];
+                cfma(tr2, mk<T>((T)zd.x, (T)zd.y), WTm[sp][(pq[e] - n) * n + hh[f]]);
+              }
+            xch = cadd(xch, mk<T>(2 * tr2.x, 2 * tr2.y));
+            for (int f = 0; f < rk; ++f)
+              for (int f2 = 0; f2 < rk; ++f2) cfma(xch, A[f * 4 + f2], A[f2 * 4 + f]);
+          }
+        } else if (rk == 1) {
           C zw = cmul(Zi[0], Wm[sp][p0 * n + h0]);
           t = cadd(t, zw);
           if (!is_h) {
@@ -503,7 +579,7 @@ __global__ void __launch_bounds__(MD_THREADS) k_md_energy_b(MdEnergyArgs<T> g) {
     rks[j] = 0; pat[j][0] = pat[j][1] = 0;
     if (i < m.ndet)
       for (int sp = 0; sp < 2; ++sp) {
-        int h[2], pp[2];
+        int h[4], pp[4];
         const int rk = md_exc(m, i, sp, h, pp);
         const int n = sp ? m.nb : m.na;
         rks[j] |= rk << (2 * sp);

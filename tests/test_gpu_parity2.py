@@ -395,3 +395,74 @@ def test_multidet_large_expansion():
     H.record("multidet_1000", **errs)
     for k, v in errs.items():
         assert v < tol, (k, v)
+
+
+def _high_rank_trial(wl, n_det, seed=5):
+    """Determinants with excitation rank 0..4 per spin (in-place column replacement, distinct holes / particles per spin)."""
+    rng = np.random.default_rng(seed)
+    exc = -np.ones((n_det, 2, 4, 2), dtype=np.int32)
+    seen = {()}
+    i = 1
+    while i < n_det:
+        key = []
+        for s, n in enumerate((wl.n_alpha, wl.n_beta)):
+            rk = int(rng.integers(0, 5)) if i > 4 else (i if s == 0 else 4 - (i - 1))      # dets 1-4 force ranks (1,4) (2,3) (3,2) (4,1)
+            rk = min(rk, n, wl.n_act - n)
+            holes = rng.permutation(n)[:rk]
+            parts = n + rng.permutation(wl.n_act - n)[:rk]
+            key += [(s, int(h), int(p)) for h, p in zip(holes, parts)]
+        if not key or tuple(sorted(key)) in seen:
+            continue
+        seen.add(tuple(sorted(key)))
+        cnt = [0, 0]
+        for s, h, p in key:
+            exc[i, s, cnt[s]] = (h, p)
+            cnt[s] += 1
+        i += 1
+    c = rng.standard_normal(n_det)
+    c[0] = 3.0
+    return c / np.linalg.norm(c), exc
+
+
+@pytest.mark.parametrize("path", [0, 1])
+def test_multidet_excitation_rank_up_to_4(path):
+    """excitation rank > 2.  Eq. (4) holds for any rank E_i; the GPU inverts the E x E matrices
+    Q[P_i, H_i] by a small pivoted elimination for E = 3, 4 (closed forms for E <= 2).  S, mixed G, mixed f, mixed E_L and one full
+    step against the oracle's definition path (every determinant recomputed directly)."""
+    import torch
+    wl = make_workload(4, "raw", overrides=dict(M=26, n_alpha=6, n_beta=5, n_chol=22, n_act=12, n_det=2, n_walkers=8))
+    wl.n_det = 24
+    wl.det_coeff, wl.det_exc = _high_rank_trial(wl, wl.n_det)
+    ranks = {(int((wl.det_exc[i, 0, :, 0] >= 0).sum()), int((wl.det_exc[i, 1, :, 0] >= 0).sum())) for i in range(wl.n_det)}
+    assert {(1, 4), (2, 3), (3, 2), (4, 1)} <= ranks
+    nw = 8
+    tol = H.tol_for(wl)
+    ini, trial = H.oracle_init(wl)
+    phi = random_walkers(wl, nw, seed=11, spread=0.25)
+    ctx = H.make_ctx(wl, nw, gemm_path=path)
+    st = H.DeviceState(ctx, phi)
+    G = torch.zeros(nw, 2, wl.M, wl.M, dtype=ctx.cdtype, device=ctx.device)
+    ctx.afqmc_overlap_green(st.phi, st.ovlp, st.theta, G, st.flags)
+    ctx.afqmc_force_bias(st.phi, st.theta, st.fb)
+    eloc = torch.zeros(nw, dtype=torch.complex128, device=ctx.device)
+    ctx.afqmc_local_energy(st.phi, st.theta, eloc)
+    out = st.host()
+    S, f, E, Gref = orc.o_multidet_definition(ini, trial, phi, wl.n_alpha, want_G=True)
+    errs = dict(S=H.rel_abs(out["S"], S), G=H.rel_fro(G.cpu().numpy().astype(np.complex128), Gref),
+                f=H.rel_fro(out["f"], f), E=H.rel_abs(eloc.cpu().numpy(), E))
+    x = wl.fields(1, nw)
+    e1 = st.step(x)
+    o1 = st.host()
+    ost = orc.o_seed_state(ini, phi, wl.n_alpha, trial=trial)
+    new, rec = orc.o_step(ini, ost, x[0], wl.n_alpha, K=wl.K, E0=wl.E0, trial=trial)
+    kappa = np.maximum(H.cond_number(wl, phi), H.cond_number(wl, rec["phi"]))
+    tw = H.walker_tol(wl, kappa)
+    step = dict(phi=H.rel_fro_w(o1["phi"], rec["phi"]), S1=H.rel_abs_w(o1["S"], rec["S"]),
+                E1=H.energy_err_w(e1[0], rec["eloc"], rec["f"]))
+    print(f"rank <= 4 trial ({wl.n_det} determinants, gemm_path {ctx.gemm_path}): stage {errs}; step {({k: float(v.max()) for k, v in step.items()})}")
+    H.record("multidet_rank4", path=path, **errs, **{k: float(v.max()) for k, v in step.items()})
+    assert np.all(out["flags"] == 0)
+    for k, v in errs.items():
+        assert v < tol, (k, v)
+    for k, v in step.items():
+        assert np.all(v < tw), (k, float(v.max()))
