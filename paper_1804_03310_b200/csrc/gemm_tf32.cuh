@@ -112,10 +112,12 @@ __device__ __forceinline__ void tc_commit_pair(uint64_t* bar) {
                ::"r"(smem_u32(bar)), "h"((uint16_t)3)
                : "memory");
 }
-// arrive on the leader CTA's copy of a barrier
+// arrive on the leader CTA's copy of a barrier.  Default semantics (release at CTA scope): the arrive only hands a drained
+// TMEM buffer back (ordered by tcgen05.fence::before_thread_sync), no generic-memory data travels with it; the
+// .release.cluster form costs a MEMBAR.ALL.GPU + ERRBAR per arrive (measured: 1650 clk each, 18 % of the epilogue warps' time).
 __device__ __forceinline__ void mbar_arrive_leader(uint64_t* bar) {
   asm volatile(
-      "{\n.reg .b32 ra;\nmapa.shared::cluster.u32 ra, %0, 0;\nmbarrier.arrive.release.cluster.shared::cluster.b64 _, [ra];\n}"
+      "{\n.reg .b32 ra;\nmapa.shared::cluster.u32 ra, %0, 0;\nmbarrier.arrive.shared::cluster.b64 _, [ra];\n}"
       ::"r"(smem_u32(bar))
       : "memory");
 }
@@ -179,6 +181,20 @@ struct Maps {
 
 
 // ---- epilogues: called per epilogue thread with its accumulator row and 32 consecutive columns -------------
+// explicit shared-space accesses for the staging area (generic LD / ST cost an address-space check and a uniform
+// descriptor each)
+__device__ __forceinline__ float4 ld_s128(uint32_t a) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ float ld_s32(uint32_t a) {
+  float v;
+  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ void st_s32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
+
 struct EpiStoreT {      // H4: out[col][row]
   static constexpr bool kStaged = false;
   float* out; int ldo, m_real, n_real;
@@ -262,26 +278,54 @@ struct EpiAssembleSym {
       put4((size_t)(col >> 1) * M * (2 * MP) + (col & 1) * MP + (size_t)j * (2 * MP) + i, x);
     }
   }
-  // Quarter r of the tile (persistent kernel): staged column sc = half * 32 + j  <->  tile column half * 128 + r * 32 + j
-  __device__ __forceinline__ void flush_part(const float* S, int m0, int n0, int t, int r) const {
-    const int2 b = blk[m0 >> 7];
-    const int i0 = b.x * 8, j0 = b.y * 16;
-    for (int u = t; u < 64 * 32; u += 256) {           // direct
-      const int sc = u >> 5, ii = (u >> 2) & 7, v = u & 3;
-      const int col = n0 + (sc >> 5) * 128 + r * 32 + (sc & 31), i = i0 + ii, j = j0 + 4 * v;
-      if (col >= n_real || i >= M || j >= M) continue;
-      const float4 x = *reinterpret_cast<const float4*>(S + sc * 128 + ii * 16 + 4 * v);
-      put4((size_t)(col >> 1) * M * (2 * MP) + (col & 1) * MP + (size_t)i * (2 * MP) + j, x);
+  // Quarter r of the tile (persistent kernel) from the staging area at shared address sS: staged column
+  // sc = half * 32 + j  <->  tile column half * 128 + r * 32 + j.  Thread t of 256 owns a fixed (row, vector) of the
+  // 8 x 16 block in either orientation and the staged columns (t >> 5) + 8 k, k = 0..7; its eight stores differ by
+  // compile-time multiples of the stride of four walkers.  With two warps per scheduler this phase runs at the latency
+  // of its instruction stream, so it is written for few instructions: no 64-bit index products, predicated stores,
+  // loads issued four at a time (A_w has a single FP32 plane; out_lo is not used here).
+  __device__ __forceinline__ void flush_part(uint32_t sS, int2 b, int n0, int t, int r) const {
+    const int wp = t >> 5, c0 = n0 + wp;
+    const uint32_t WS4B = (uint32_t)M * (uint32_t)(2 * MP) * 16u;      // bytes per four walkers
+    const int lim = n_real - c0;                                        // staged column k is real iff its tile offset < lim
+    char* wb = reinterpret_cast<char*>(out) + ((size_t)(c0 >> 1) * M * (2 * MP) + (size_t)(c0 & 1) * MP) * 4;
+    {                                                                   // direct: row ii, vector v of 4 jj
+      const int ii = (t >> 2) & 7, v = t & 3, i = b.x * 8 + ii, j = b.y * 16 + 4 * v;
+      const uint32_t a = sS + (uint32_t)(wp * 128 + ii * 16 + 4 * v) * 4;
+      const int limd = (i < M && j < M) ? lim : 0;
+      char* pd = wb + ((size_t)i * (2 * MP) + j) * 4;
+#pragma unroll
+      for (int kb = 0; kb < 8; kb += 4) {
+        float4 x[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) x[k] = ld_s128(a + (kb + k) * 4096);
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+          if (r * 32 + (kb >> 2) * 128 + k * 8 < limd)
+            *reinterpret_cast<float4*>(pd + (size_t)(4 * r + k + 4 * kb) * WS4B) = x[k];
+      }
     }
-    for (int u = t; u < 64 * 32; u += 256) {           // mirrored
-      const int sc = u >> 5, jj = (u >> 1) & 15, v = u & 1;
-      const int col = n0 + (sc >> 5) * 128 + r * 32 + (sc & 31), j = j0 + jj, i = i0 + 4 * v;
-      if (col >= n_real || i >= M || j >= M) continue;
-      const float* p = S + sc * 128 + (4 * v) * 16 + jj;
-      const float4 x = make_float4(p[0], p[16], p[32], p[48]);
-      put4((size_t)(col >> 1) * M * (2 * MP) + (col & 1) * MP + (size_t)j * (2 * MP) + i, x);
+    {                                                                   // mirrored: row jj, vector v of 4 ii
+      const int jj = (t >> 1) & 15, v = t & 1, j = b.y * 16 + jj, i = b.x * 8 + 4 * v;
+      const uint32_t a = sS + (uint32_t)(wp * 128 + (4 * v) * 16 + jj) * 4;
+      const int limm = (i < M && j < M) ? lim : 0;
+      char* pm = wb + ((size_t)j * (2 * MP) + i) * 4;
+#pragma unroll
+      for (int kb = 0; kb < 8; kb += 4) {
+        float4 x[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const uint32_t ak = a + (kb + k) * 4096;
+          x[k] = make_float4(ld_s32(ak), ld_s32(ak + 64), ld_s32(ak + 128), ld_s32(ak + 192));
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+          if (r * 32 + (kb >> 2) * 128 + k * 8 < limm)
+            *reinterpret_cast<float4*>(pm + (size_t)(4 * r + k + 4 * kb) * WS4B) = x[k];
+      }
     }
   }
+  __device__ __forceinline__ int2 block_of(int m0) const { return blk[m0 >> 7]; }
 };
 
 struct EpiTT {          // H10: row = g*nact + q, col = (w*nt + a)*2 + p -> TT[w][g][q][a] (interleaved complex)
@@ -640,6 +684,10 @@ k_gemm_tf32_pair(const __grid_constant__ Maps maps, int K, int tri, int m_tiles,
 // push the finished tile out in four rounds, the TMA producer and the MMA issuer are already two accumulation chunks
 // into the next tile (the two TMEM buffers are free as soon as the last chunk sits in registers).  Barrier phases run
 // on across tiles (global k-block / chunk counters).
+#ifndef AFQMC_PS_CHUNK_KB
+#define AFQMC_PS_CHUNK_KB 4
+#endif
+enum { PS_CHUNK_KB = AFQMC_PS_CHUNK_KB };
 enum { STG_COLS = 64, STG_BYTES = BM * STG_COLS * 4, SMEM_PS_BYTES = STAGES2 * STAGE2_BYTES + STG_BYTES + 1024 };
 
 template <class Epi>
@@ -658,7 +706,7 @@ k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps, int K, int m_tiles, int n
   const uint32_t rank = cluster_ctarank();
   const int cid = blockIdx.x >> 1, ncl = gridDim.x >> 1;
   const int nkb = K / BK;
-  const int nchunk = (nkb + CHUNK_KB - 1) / CHUNK_KB;
+  const int nchunk = (nkb + PS_CHUNK_KB - 1) / PS_CHUNK_KB;
 
   if (warp == EPI_WARPS && lane == 0) {
 #pragma unroll
@@ -709,7 +757,7 @@ k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps, int K, int m_tiles, int n
         for (int kb = 0; kb < nkb; ++kb, ++it) {
           const int s = it % STAGES2;
           const int buf = cg & 1;
-          const bool chunk_start = (kb % CHUNK_KB) == 0;
+          const bool chunk_start = (kb % PS_CHUNK_KB) == 0;
           if (chunk_start) {   // both CTAs' epilogue warps have drained this TMEM buffer (two chunks ago)
             mbar_wait(&tmem_empty_bar[buf], ((cg >> 1) & 1) ^ 1);
             tc_fence_after();
@@ -728,7 +776,7 @@ k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps, int K, int m_tiles, int n
             umma_tf32_pair(d, a_hi + adv, b_hi + adv, idesc, 1u);
           }
           tc_commit_pair(&empty_bar[s]);
-          if ((kb % CHUNK_KB) == CHUNK_KB - 1 || kb == nkb - 1) { tc_commit_pair(&tmem_full_bar[buf]); ++cg; }
+          if ((kb % PS_CHUNK_KB) == PS_CHUNK_KB - 1 || kb == nkb - 1) { tc_commit_pair(&tmem_full_bar[buf]); ++cg; }
         }
       }
     }
@@ -737,6 +785,7 @@ k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps, int K, int m_tiles, int n
     uint32_t cg = 0;
     for (int tp = cid; tp < n_pairs; tp += ncl) {
       const int mt = (tp / n_tiles) * 2 + (int)rank, m0 = mt * BM, n0 = (tp % n_tiles) * BN;
+      const int2 bij = mt < m_tiles ? epi.block_of(m0) : make_int2(0, 0);   // asked for now, used after the chunk loop
       float acc[COLS_PER_WARP];
 #pragma unroll
       for (int i = 0; i < COLS_PER_WARP; ++i) acc[i] = 0.f;
@@ -758,15 +807,16 @@ k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps, int K, int m_tiles, int n
       }
       // the tile sits in registers and both TMEM buffers are released: the next tile's MMAs run while it is written out
       const bool valid = mt < m_tiles;
+      const uint32_t sS = smem_u32(S), sW = sS + (uint32_t)((half * 32) * BM + q * 32 + lane) * 4;
 #pragma unroll
       for (int r = 0; r < COLS_PER_WARP / 32; ++r) {
         asm volatile("bar.sync 1, 256;" ::: "memory");      // the previous round has left the staging area
         if (valid) {
 #pragma unroll
-          for (int j = 0; j < 32; ++j) S[(half * 32 + j) * BM + q * 32 + lane] = acc[r * 32 + j];
+          for (int j = 0; j < 32; ++j) st_s32(sW + j * (BM * 4), acc[r * 32 + j]);
         }
         asm volatile("bar.sync 1, 256;" ::: "memory");
-        if (valid) epi.flush_part(S, m0, n0, (int)threadIdx.x, r);
+        if (valid) epi.flush_part(sS, bij, n0, (int)threadIdx.x, r);
       }
     }
   }
