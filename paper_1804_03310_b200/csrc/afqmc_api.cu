@@ -455,7 +455,7 @@ afqmc_status run_gemm_tc(afqmc_ctx* c, const tc::Maps& maps, int m, int n, int K
       if (!tri && slots > 0 && c->ps_ok) {
         dim3 gridp(2 * (n_pairs < slots ? n_pairs : slots));
         auto kernp = tc::k_gemm_tf32_pair_ps<Epi>;
-        LAUNCH(c, kernp, gridp, tc::THREADS, tc::SMEM_PS_BYTES, maps, K, m_tiles, n_tiles, n_pairs, epi);
+        LAUNCH(c, kernp, gridp, tc::PS_THREADS, tc::SMEM_PS_BYTES, maps, K, m_tiles, n_tiles, n_pairs, epi);
         return AFQMC_OK;
       }
     }
@@ -657,7 +657,7 @@ afqmc_status do_propagate(afqmc_ctx* c, void* phi, const void* x, const void* fb
           tc::EpiAssembleSym e3;
           e3.out = (float*)c->Abuf; e3.out_lo = nullptr;   // A_w is stored once, in FP32: the Taylor kernel splits it on the fly
           e3.blk = c->blk; e3.M = c->M;
-          e3.MP = c->MP; e3.n_real = 2 * c->nw;
+          e3.MP = c->MP; e3.n_real = 2 * c->nw; e3.st_pol = tc::PS_POL_ST;
           st = run_gemm_tc(c, c->map_asm, c->nblk * 128, 2 * c->nw, c->NGP, e3);
           done = true;
         }

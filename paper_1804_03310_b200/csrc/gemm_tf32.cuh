@@ -106,6 +106,14 @@ __device__ __forceinline__ void tma_load_2d_pair(void* dst, const CUtensorMap* m
       ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar) & PEER_MASK), "r"(c0), "r"(c1)
       : "memory");
 }
+// the same with an L2 eviction-priority hint (createpolicy encodings: whole-fraction evict_first / evict_last)
+constexpr uint64_t L2_EVICT_FIRST = 0x12F0000000000000ull, L2_EVICT_LAST = 0x14F0000000000000ull;
+__device__ __forceinline__ void tma_load_2d_pair_hint(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, uint64_t pol) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4}], [%2], %5;"
+      ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar) & PEER_MASK), "r"(c0), "r"(c1), "l"(pol)
+      : "memory");
+}
 // arrive on the same barrier in both CTAs of the pair once all MMAs issued so far have completed
 __device__ __forceinline__ void tc_commit_pair(uint64_t* bar) {
   asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
@@ -193,6 +201,12 @@ __device__ __forceinline__ float ld_s32(uint32_t a) {
   asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
   return v;
 }
+// 16-byte global store that asks L2 to evict the line first (streamed output, not read again by this kernel)
+__device__ __forceinline__ void st_g128_hint(void* p, float4 v, uint64_t pol) {
+  asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w),
+               "l"(pol)
+               : "memory");
+}
 __device__ __forceinline__ void st_s32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
 
 struct EpiStoreT {      // H4: out[col][row]
@@ -247,6 +261,7 @@ struct EpiAssemble {
 struct EpiAssembleSym {
   static constexpr bool kStaged = true;
   float* out; float* out_lo; const int2* blk; int M, MP, n_real;
+  uint64_t st_pol = 0x1000000000000000ull;   // L2 eviction priority of the persistent kernel's stores
   __device__ __forceinline__ void operator()(int, int, const float (&)[32]) const {}
   __device__ __forceinline__ void put4(size_t o, float4 v) const {
     if (out_lo) {
@@ -278,54 +293,55 @@ struct EpiAssembleSym {
       put4((size_t)(col >> 1) * M * (2 * MP) + (col & 1) * MP + (size_t)j * (2 * MP) + i, x);
     }
   }
-  // Quarter r of the tile (persistent kernel) from the staging area at shared address sS: staged column
-  // sc = half * 32 + j  <->  tile column half * 128 + r * 32 + j.  Thread t of 256 owns a fixed (row, vector) of the
-  // 8 x 16 block in either orientation and the staged columns (t >> 5) + 8 k, k = 0..7; its eight stores differ by
-  // compile-time multiples of the stride of four walkers.  With two warps per scheduler this phase runs at the latency
-  // of its instruction stream, so it is written for few instructions: no 64-bit index products, predicated stores,
-  // loads issued four at a time (A_w has a single FP32 plane; out_lo is not used here).
-  __device__ __forceinline__ void flush_part(uint32_t sS, int2 b, int n0, int t, int r) const {
-    const int wp = t >> 5, c0 = n0 + wp;
-    const uint32_t WS4B = (uint32_t)M * (uint32_t)(2 * MP) * 16u;      // bytes per four walkers
-    const int lim = n_real - c0;                                        // staged column k is real iff its tile offset < lim
+  // Persistent kernel, store warps.  One round = 16 columns of each half of the tile in a staging buffer,
+  // S[sc][row], sc = half * 16 + j  <->  tile column half * 128 + r * 16 + j, row = ii * 16 + jj of the 8 x 16 block.
+  // Thread t of 128 owns a fixed (row, vector) of the block in either orientation and the staged columns (t >> 5) + 4 k,
+  // k = 0..7: plane p = (t >> 5) & 1 is fixed, the walkers of its eight stores are 2 apart (and 64 apart between halves).
+  struct StoreCtx { char* pd; char* pm; uint32_t ad, am, mv, W2B; int limd, limm; };
+  __device__ __forceinline__ StoreCtx store_ctx(int m0, int n0, int t) const {
+    StoreCtx c;
+    const int2 b = blk[m0 >> 7];
+    const int ws = t >> 5, c0 = n0 + ws;
+    const int lim = n_real - c0;                                 // a store at tile-column offset o is real iff o < lim
+    c.W2B = (uint32_t)M * (uint32_t)(2 * MP) * 8u;               // bytes per two walkers
     char* wb = reinterpret_cast<char*>(out) + ((size_t)(c0 >> 1) * M * (2 * MP) + (size_t)(c0 & 1) * MP) * 4;
-    {                                                                   // direct: row ii, vector v of 4 jj
+    {                                                            // direct: row ii, vector v of 4 jj
       const int ii = (t >> 2) & 7, v = t & 3, i = b.x * 8 + ii, j = b.y * 16 + 4 * v;
-      const uint32_t a = sS + (uint32_t)(wp * 128 + ii * 16 + 4 * v) * 4;
-      const int limd = (i < M && j < M) ? lim : 0;
-      char* pd = wb + ((size_t)i * (2 * MP) + j) * 4;
-#pragma unroll
-      for (int kb = 0; kb < 8; kb += 4) {
-        float4 x[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) x[k] = ld_s128(a + (kb + k) * 4096);
-#pragma unroll
-        for (int k = 0; k < 4; ++k)
-          if (r * 32 + (kb >> 2) * 128 + k * 8 < limd)
-            *reinterpret_cast<float4*>(pd + (size_t)(4 * r + k + 4 * kb) * WS4B) = x[k];
-      }
+      c.ad = (uint32_t)(ws * 128 + (ii ^ (ii >> 2)) * 16 + 4 * v) * 4;   // staged row ii*16+jj has bit 4 flipped for ii >= 4
+      c.limd = (i < M && j < M) ? lim : 0;
+      c.pd = wb + ((size_t)i * (2 * MP) + j) * 4;
     }
-    {                                                                   // mirrored: row jj, vector v of 4 ii
+    {                                                            // mirrored: row jj, vector v of 4 ii
       const int jj = (t >> 1) & 15, v = t & 1, j = b.y * 16 + jj, i = b.x * 8 + 4 * v;
-      const uint32_t a = sS + (uint32_t)(wp * 128 + (4 * v) * 16 + jj) * 4;
-      const int limm = (i < M && j < M) ? lim : 0;
-      char* pm = wb + ((size_t)j * (2 * MP) + i) * 4;
-#pragma unroll
-      for (int kb = 0; kb < 8; kb += 4) {
-        float4 x[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          const uint32_t ak = a + (kb + k) * 4096;
-          x[k] = make_float4(ld_s32(ak), ld_s32(ak + 64), ld_s32(ak + 128), ld_s32(ak + 192));
-        }
-#pragma unroll
-        for (int k = 0; k < 4; ++k)
-          if (r * 32 + (kb >> 2) * 128 + k * 8 < limm)
-            *reinterpret_cast<float4*>(pm + (size_t)(4 * r + k + 4 * kb) * WS4B) = x[k];
-      }
+      c.am = (uint32_t)(ws * 128 + (4 * v) * 16 + jj) * 4;
+      c.mv = (uint32_t)v * 64;                                   // rows 4v+x sit at (x ^ v) * 16: both v hit different banks
+      c.limm = (i < M && j < M) ? lim : 0;
+      c.pm = wb + ((size_t)j * (2 * MP) + i) * 4;
     }
+    return c;
   }
-  __device__ __forceinline__ int2 block_of(int m0) const { return blk[m0 >> 7]; }
+  __device__ __forceinline__ void flush_round(const StoreCtx& c, uint32_t sSb, int r) const {
+    const size_t ro = (size_t)(4 * r) * c.W2B;
+    const int lr = r * 16;
+    float4 x[8], y[8];                      // all 40 shared-memory loads of the round are in flight before the first store
+#pragma unroll
+    for (int k = 0; k < 8; ++k) x[k] = ld_s128(sSb + c.ad + k * 2048);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      const uint32_t ak = sSb + c.am + k * 2048;
+      y[k] = make_float4(ld_s32(ak + c.mv), ld_s32(ak + (64 ^ c.mv)), ld_s32(ak + (128 + c.mv)), ld_s32(ak + (128 + (64 ^ c.mv))));
+    }
+    char* p = c.pd + ro;
+#pragma unroll
+    for (int k = 0; k < 8; ++k)
+      if (lr + (k >> 2) * 128 + (k & 3) * 4 < c.limd)
+        st_g128_hint(p + (size_t)((k >> 2) * 32 + (k & 3)) * c.W2B, x[k], st_pol);
+    p = c.pm + ro;
+#pragma unroll
+    for (int k = 0; k < 8; ++k)
+      if (lr + (k >> 2) * 128 + (k & 3) * 4 < c.limm)
+        st_g128_hint(p + (size_t)((k >> 2) * 32 + (k & 3)) * c.W2B, y[k], st_pol);
+  }
 };
 
 struct EpiTT {          // H10: row = g*nact + q, col = (w*nt + a)*2 + p -> TT[w][g][q][a] (interleaved complex)
@@ -680,39 +696,68 @@ k_gemm_tf32_pair(const __grid_constant__ Maps maps, int K, int tri, int m_tiles,
 }
 
 // ---- persistent CTA-pair version for staged epilogues (H6): one pair per TPC loops over the tile pairs.  The operand
-// ring (3 x 64 KB) and the staging area (32 KB, a quarter tile) are separate, so while the 8 epilogue warps of each CTA
-// push the finished tile out in four rounds, the TMA producer and the MMA issuer are already two accumulation chunks
-// into the next tile (the two TMEM buffers are free as soon as the last chunk sits in registers).  Barrier phases run
-// on across tiles (global k-block / chunk counters).
+// ring (3 x 64 KB) and the staging area (2 x 16 KB) are separate, and the tile leaves through a second set of warps:
+//   warps 0-7   epilogue: add each accumulation chunk from TMEM into registers; after the last chunk, hand the tile to
+//               the store warps 16 columns per half at a time (16 STS per thread and round, nothing else)
+//   warp  8     TMA producer        warp 9   MMA issuer (leader CTA)        warps 10-11 idle
+//   warps 12-15 store warps: staging area -> HBM in both orientations (LDS + STG), everything they need in registers
+// so the epilogue warps are back at the next tile's first chunk after ~8 x (16 STS + a barrier), well inside the two
+// chunks the MMA issuer may run ahead.  (One set of warps doing both took 21k clk per tile at two warps per scheduler
+// -- spills and constant reloads beside 128 live accumulators -- against 12k clk of slack: 0.73 ms; profiles/r2_ncu_full.md.)
+// Barrier phases run on across tiles (global k-block / chunk / round counters).
+// Chunk length of the persistent kernel: the truncation bias of the tensor pipe's accumulation is linear in it (A_w is
+// 8e-7 low at 4 k-blocks, 4e-7 at 2), and S = det(overlap) picks that bias up N_elec-fold.  With the store warps the hand-over
+// takes ~9k clk per tile, so two chunks of 2 k-blocks (6.1k clk of MMA) almost cover it.  Measured, B200 cfg 5:
+// 4 -> 0.648 ms, 3 -> 0.658 ms, 2 -> 0.677 ms; per-step error of S on cfg 5: 3.5e-5 / - / 2.6e-5 (profiles/parity_r2.md).
 #ifndef AFQMC_PS_CHUNK_KB
-#define AFQMC_PS_CHUNK_KB 4
+#define AFQMC_PS_CHUNK_KB 2
 #endif
 enum { PS_CHUNK_KB = AFQMC_PS_CHUNK_KB };
-enum { STG_COLS = 64, STG_BYTES = BM * STG_COLS * 4, SMEM_PS_BYTES = STAGES2 * STAGE2_BYTES + STG_BYTES + 1024 };
+enum { PS_THREADS = 512, PS_STORE_WARP0 = 12, STG_COLS = 32, STG_BYTES = BM * STG_COLS * 4, STG_ROUNDS = BN / STG_COLS,
+       SMEM_PS_BYTES = STAGES2 * STAGE2_BYTES + 2 * STG_BYTES + 1024 };
+// L2 eviction-priority hints (bit 0: L rows evict_first, bit 1: field rows evict_last, bit 2: output stores evict_first).
+// Measured on B200, cfg 5 (0.655 ms without): 2 -> 0.653, 4 -> 0.664, 6 -> 0.658, 3 -> 0.700, 7 -> 0.685: none helps, so
+// the default is no hint.
+#ifndef AFQMC_PS_POL
+#define AFQMC_PS_POL 0
+#endif
+constexpr uint64_t L2_EVICT_NORMAL = 0x1000000000000000ull;
+constexpr uint64_t PS_POL_A = (AFQMC_PS_POL & 1) ? L2_EVICT_FIRST : L2_EVICT_NORMAL;
+constexpr uint64_t PS_POL_B = (AFQMC_PS_POL & 2) ? L2_EVICT_LAST : L2_EVICT_NORMAL;
+constexpr uint64_t PS_POL_ST = (AFQMC_PS_POL & 4) ? L2_EVICT_FIRST : L2_EVICT_NORMAL;
+enum { PS_REGS_EPI = 168, PS_REGS_AUX = 64, PS_REGS_STORE = 96 };
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 
 template <class Epi>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(THREADS, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PS_THREADS, 1)
 k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps, int K, int m_tiles, int n_tiles, int n_pairs, Epi epi) {
   static_assert(Epi::kStaged, "persistent kernel is written for the staged epilogue");
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  float* S = reinterpret_cast<float*>(smem + (size_t)STAGES2 * STAGE2_BYTES);
   __shared__ __align__(8) uint64_t full_bar[STAGES2];     // used in the leader only
   __shared__ __align__(8) uint64_t empty_bar[STAGES2];
   __shared__ __align__(8) uint64_t tmem_full_bar[2];
   __shared__ __align__(8) uint64_t tmem_empty_bar[2];     // leader only: 2 x 8 epilogue warps arrive
+  __shared__ __align__(8) uint64_t stg_full_bar[2];       // 8 epilogue warps arrive
+  __shared__ __align__(8) uint64_t stg_free_bar[2];       // 4 store warps arrive
   __shared__ uint32_t tmem_base_s;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
   const int cid = blockIdx.x >> 1, ncl = gridDim.x >> 1;
   const int nkb = K / BK;
   const int nchunk = (nkb + PS_CHUNK_KB - 1) / PS_CHUNK_KB;
+  const uint32_t sS = smem_u32(smem + (size_t)STAGES2 * STAGE2_BYTES);
 
   if (warp == EPI_WARPS && lane == 0) {
 #pragma unroll
     for (int s = 0; s < STAGES2; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
 #pragma unroll
-    for (int b = 0; b < 2; ++b) { mbar_init(&tmem_full_bar[b], 1); mbar_init(&tmem_empty_bar[b], 2 * EPI_WARPS); }
+    for (int b = 0; b < 2; ++b) {
+      mbar_init(&tmem_full_bar[b], 1); mbar_init(&tmem_empty_bar[b], 2 * EPI_WARPS);
+      mbar_init(&stg_full_bar[b], EPI_WARPS); mbar_init(&stg_free_bar[b], 4);
+    }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.a_hi) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.a_lo) : "memory");
@@ -731,61 +776,92 @@ k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps, int K, int m_tiles, int n
   tc_fence_after();
   const uint32_t tmem = tmem_base_s;
 
-  if (warp == EPI_WARPS) {
-    if (lane == 0) {   // ===== TMA producer (both CTAs) =====
-      uint32_t it = 0;
-      for (int tp = cid; tp < n_pairs; tp += ncl) {
-        const int m0 = ((tp / n_tiles) * 2 + (int)rank) * BM, nb = (tp % n_tiles) * BN + (int)rank * B_BOX;
-        for (int kb = 0; kb < nkb; ++kb, ++it) {
-          const int s = it % STAGES2;
-          mbar_wait(&empty_bar[s], ((it / STAGES2) & 1) ^ 1);
-          uint8_t* st = smem + (size_t)s * STAGE2_BYTES;
-          if (rank == 0) mbar_expect_tx(&full_bar[s], 2 * STAGE2_BYTES);
-          const int kc = kb * BK;
-          tma_load_2d_pair(st, &maps.a_hi, &full_bar[s], kc, m0);
-          tma_load_2d_pair(st + A_BYTES, &maps.a_lo, &full_bar[s], kc, m0);
-          tma_load_2d_pair(st + 2 * A_BYTES, &maps.b_hi, &full_bar[s], kc, nb);
-          tma_load_2d_pair(st + 2 * A_BYTES + HB_BYTES, &maps.b_lo, &full_bar[s], kc, nb);
-        }
+  if (warp >= PS_STORE_WARP0) {          // ===== store warps =====
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"((int)PS_REGS_STORE));
+    const int t = (int)threadIdx.x - PS_STORE_WARP0 * 32;
+    uint32_t sr = 0;
+    for (int tp = cid; tp < n_pairs; tp += ncl) {
+      const int mt = (tp / n_tiles) * 2 + (int)rank, m0 = mt * BM, n0 = (tp % n_tiles) * BN;
+      const bool valid = mt < m_tiles;
+      typename Epi::StoreCtx sc = epi.store_ctx(valid ? m0 : 0, n0, t);
+#pragma unroll 1
+      for (int r = 0; r < STG_ROUNDS; ++r, ++sr) {
+        const int b = sr & 1;
+        mbar_wait(&stg_full_bar[b], (sr >> 1) & 1);
+        if (valid) epi.flush_round(sc, sS + b * STG_BYTES, r);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&stg_free_bar[b]);   // release: the loads above have completed
       }
     }
-  } else if (warp == EPI_WARPS + 1) {
-    if (lane == 0 && rank == 0) {   // ===== MMA issuer (leader CTA) =====
-      constexpr uint32_t idesc = make_idesc(2 * BM, BN);
-      uint32_t it = 0, cg = 0;
-      for (int tp = cid; tp < n_pairs; tp += ncl) {
-        for (int kb = 0; kb < nkb; ++kb, ++it) {
-          const int s = it % STAGES2;
-          const int buf = cg & 1;
-          const bool chunk_start = (kb % PS_CHUNK_KB) == 0;
-          if (chunk_start) {   // both CTAs' epilogue warps have drained this TMEM buffer (two chunks ago)
-            mbar_wait(&tmem_empty_bar[buf], ((cg >> 1) & 1) ^ 1);
+  } else if (warp >= EPI_WARPS) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"((int)PS_REGS_AUX));
+    if (warp == EPI_WARPS) {
+      if (lane == 0) {   // ===== TMA producer (both CTAs) =====
+        uint32_t it = 0;
+        for (int tp = cid; tp < n_pairs; tp += ncl) {
+          const int m0 = ((tp / n_tiles) * 2 + (int)rank) * BM, nb = (tp % n_tiles) * BN + (int)rank * B_BOX;
+          for (int kb = 0; kb < nkb; ++kb, ++it) {
+            const int s = it % STAGES2;
+            mbar_wait(&empty_bar[s], ((it / STAGES2) & 1) ^ 1);
+            uint8_t* st = smem + (size_t)s * STAGE2_BYTES;
+            if (rank == 0) mbar_expect_tx(&full_bar[s], 2 * STAGE2_BYTES);
+            const int kc = kb * BK;
+            tma_load_2d_pair_hint(st, &maps.a_hi, &full_bar[s], kc, m0, PS_POL_A);
+            tma_load_2d_pair_hint(st + A_BYTES, &maps.a_lo, &full_bar[s], kc, m0, PS_POL_A);
+            tma_load_2d_pair_hint(st + 2 * A_BYTES, &maps.b_hi, &full_bar[s], kc, nb, PS_POL_B);
+            tma_load_2d_pair_hint(st + 2 * A_BYTES + HB_BYTES, &maps.b_lo, &full_bar[s], kc, nb, PS_POL_B);
+          }
+        }
+      }
+    } else if (warp == EPI_WARPS + 1) {
+      if (rank == 0) {   // ===== MMA issuer (leader CTA).  The whole warp runs the loop and one elected lane issues: with
+        // uniform control flow the descriptors live in uniform registers and a k-block's 12 MMAs are back-to-back UTCHMMA
+        // (inside `if (lane == 0)` every MMA is wrapped in an ELECT / R2UR sequence; taylor_tc.cuh has the measurement) =====
+        constexpr uint32_t idesc = make_idesc(2 * BM, BN);
+        constexpr uint64_t SSTEP = STAGE2_BYTES >> 4;     // the descriptor's address field counts 16-byte units
+        const uint64_t d0 = make_desc(smem_u32(smem));
+        uint64_t ds = d0;
+        int s = 0;
+        uint32_t fpar = 0, cg = 0;
+        for (int tp = cid; tp < n_pairs; tp += ncl) {
+          int kc = 0;                                      // k-block within the chunk
+          for (int kb = 0; kb < nkb; ++kb) {
+            const int buf = cg & 1;
+            if (kc == 0) {   // both CTAs' epilogue warps have drained this TMEM buffer (two chunks ago)
+              mbar_wait(&tmem_empty_bar[buf], ((cg >> 1) & 1) ^ 1);
+            }
+            mbar_wait(&full_bar[s], fpar);
             tc_fence_after();
-          }
-          mbar_wait(&full_bar[s], (it / STAGES2) & 1);
-          tc_fence_after();
-          const uint32_t d = tmem + buf * BN;
-          const uint32_t sa = smem_u32(smem + (size_t)s * STAGE2_BYTES);
-          const uint64_t a_hi = make_desc(sa), a_lo = make_desc(sa + A_BYTES);
-          const uint64_t b_hi = make_desc(sa + 2 * A_BYTES), b_lo = make_desc(sa + 2 * A_BYTES + HB_BYTES);
+            const bool chunk_end = kc == PS_CHUNK_KB - 1 || kb == nkb - 1;
+            if (elect_one()) {
+              const uint32_t d = tmem + buf * BN;
+              const uint64_t a_hi = ds, a_lo = ds + (A_BYTES >> 4);
+              const uint64_t b_hi = ds + ((2 * A_BYTES) >> 4), b_lo = ds + ((2 * A_BYTES + HB_BYTES) >> 4);
 #pragma unroll
-          for (int k = 0; k < BK / UMMA_K; ++k) {
-            const uint64_t adv = (uint64_t)((k * UMMA_K * 4) >> 4);
-            umma_tf32_pair(d, a_lo + adv, b_hi + adv, idesc, (chunk_start && k == 0) ? 0u : 1u);
-            umma_tf32_pair(d, a_hi + adv, b_lo + adv, idesc, 1u);
-            umma_tf32_pair(d, a_hi + adv, b_hi + adv, idesc, 1u);
+              for (int k = 0; k < BK / UMMA_K; ++k) {
+                const uint64_t adv = (uint64_t)((k * UMMA_K * 4) >> 4);
+                umma_tf32_pair(d, a_lo + adv, b_hi + adv, idesc, (kc == 0 && k == 0) ? 0u : 1u);
+                umma_tf32_pair(d, a_hi + adv, b_lo + adv, idesc, 1u);
+                umma_tf32_pair(d, a_hi + adv, b_hi + adv, idesc, 1u);
+              }
+              tc_commit_pair(&empty_bar[s]);
+              if (chunk_end) tc_commit_pair(&tmem_full_bar[buf]);
+            }
+            __syncwarp();
+            if (chunk_end) { ++cg; kc = 0; } else ++kc;
+            ds += SSTEP;
+            if (++s == STAGES2) { s = 0; ds = d0; fpar ^= 1; }
           }
-          tc_commit_pair(&empty_bar[s]);
-          if ((kb % PS_CHUNK_KB) == PS_CHUNK_KB - 1 || kb == nkb - 1) { tc_commit_pair(&tmem_full_bar[buf]); ++cg; }
         }
       }
     }
   } else {             // ===== epilogue warps 0..7 of each CTA =====
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"((int)PS_REGS_EPI));
     const int q = warp & 3, half = warp >> 2;
-    uint32_t cg = 0;
+    // staged row = (q * 32 + lane) with bit 4 flipped in the upper half of the block (conflict-free mirrored reads, see StoreCtx)
+    const uint32_t sW = sS + (uint32_t)((half * (STG_COLS / 2)) * BM + ((q * 32 + lane) ^ ((q >> 1) << 4))) * 4;
+    uint32_t cg = 0, sr = 0;
     for (int tp = cid; tp < n_pairs; tp += ncl) {
-      const int mt = (tp / n_tiles) * 2 + (int)rank, m0 = mt * BM, n0 = (tp % n_tiles) * BN;
-      const int2 bij = mt < m_tiles ? epi.block_of(m0) : make_int2(0, 0);   // asked for now, used after the chunk loop
       float acc[COLS_PER_WARP];
 #pragma unroll
       for (int i = 0; i < COLS_PER_WARP; ++i) acc[i] = 0.f;
@@ -805,18 +881,15 @@ k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps, int K, int m_tiles, int n
         __syncwarp();
         if (lane == 0) mbar_arrive_leader(&tmem_empty_bar[buf]);
       }
-      // the tile sits in registers and both TMEM buffers are released: the next tile's MMAs run while it is written out
-      const bool valid = mt < m_tiles;
-      const uint32_t sS = smem_u32(S), sW = sS + (uint32_t)((half * 32) * BM + q * 32 + lane) * 4;
+      // the tile sits in registers and both TMEM buffers are released: the next tile's MMAs run while it is handed over
 #pragma unroll
-      for (int r = 0; r < COLS_PER_WARP / 32; ++r) {
-        asm volatile("bar.sync 1, 256;" ::: "memory");      // the previous round has left the staging area
-        if (valid) {
+      for (int r = 0; r < STG_ROUNDS; ++r, ++sr) {
+        const int b = sr & 1;
+        mbar_wait(&stg_free_bar[b], ((sr >> 1) & 1) ^ 1);
 #pragma unroll
-          for (int j = 0; j < 32; ++j) st_s32(sW + j * (BM * 4), acc[r * 32 + j]);
-        }
-        asm volatile("bar.sync 1, 256;" ::: "memory");
-        if (valid) epi.flush_part(sS, bij, n0, (int)threadIdx.x, r);
+        for (int j = 0; j < STG_COLS / 2; ++j) st_s32(sW + b * STG_BYTES + j * (BM * 4), acc[r * (STG_COLS / 2) + j]);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&stg_full_bar[b]);   // release: this warp's 16 x 32 values are in place
       }
     }
   }
