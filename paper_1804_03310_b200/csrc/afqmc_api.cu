@@ -68,6 +68,7 @@ struct afqmc_ctx {
   int32_t* h_flags;
   void* h_x2; zcplx* h_eloc2;            // second field / energy staging buffers: copies overlap the previous step
   cudaStream_t copy_stream; cudaEvent_t ev_x[2], ev_done[2], ev_e[2]; int copy_ready;
+  cudaEvent_t ev_phi; int ev_phi_armed;   // afqmc_step_host: recorded once the walker of the call's last step is final (after H7)
   // orthonormalisation / comb population control (popctl.cuh)
   size_t ortho_smem;
   void *pc_phi, *pc_theta, *pc_fb; zcplx* pc_ovlp; double *pc_cum, *pc_wnew; int32_t* pc_parent;
@@ -684,6 +685,10 @@ afqmc_status do_propagate(afqmc_ctx* c, void* phi, const void* x, const void* fb
   if (st) return st;
   st = run_taylor<T>(c, phi);
   if (st) return st;
+  if (c->ev_phi_armed) {   // the walker is final: afqmc_step_host starts its download under the rest of the step
+    c->ev_phi_armed = 0;
+    CUDA_OK(c, cudaEventRecord(c->ev_phi, c->stream));
+  }
   return run_green<T>(c, phi, ovlp, theta, 1, weight, eloc_pre, flags);
 }
 
@@ -1052,6 +1057,7 @@ void afqmc_destroy(afqmc_ctx* ctx) {
   afqmc_profile_enable(ctx, 0);
   if (ctx->copy_ready) {
     for (int i = 0; i < 2; ++i) { cudaEventDestroy(ctx->ev_x[i]); cudaEventDestroy(ctx->ev_done[i]); cudaEventDestroy(ctx->ev_e[i]); }
+    cudaEventDestroy(ctx->ev_phi);
     cudaStreamDestroy(ctx->copy_stream);
   }
   delete ctx;
@@ -1503,6 +1509,7 @@ afqmc_status afqmc_step_host(afqmc_ctx* c, void* phi_h, double* weight_h, void* 
       CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_done[i], cudaEventDisableTiming));
       CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_e[i], cudaEventDisableTiming));
     }
+    CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_phi, cudaEventDisableTiming));
     c->copy_ready = 1;
   }
   cudaStream_t cs = c->copy_stream;
@@ -1527,8 +1534,15 @@ afqmc_status afqmc_step_host(afqmc_ctx* c, void* phi_h, double* weight_h, void* 
     if (i + 1 < n_steps) CUDA_OK(c, upload(i + 1));                      // queued ahead of step i's download
     CUDA_OK(c, cudaStreamWaitEvent(st, c->ev_x[b], 0));
     if (i >= 2) CUDA_OK(c, cudaStreamWaitEvent(st, c->ev_e[b], 0));      // energies of step i-2 have left buffer b
+    const bool last = i == n_steps - 1;
+    c->ev_phi_armed = last;
     s = afqmc_step(c, c->h_phi, c->h_weight, c->h_ovlp, c->h_theta, c->h_fb, xb[b], 1, eb[b], c->h_flags);
+    c->ev_phi_armed = 0;
     if (s) return s;
+    if (last) {   // the walker is final after H7: it goes down while overlap / force bias / energy of this step still run
+      CUDA_OK(c, cudaStreamWaitEvent(cs, c->ev_phi, 0));
+      CUDA_OK(c, cudaMemcpyAsync(phi_h, c->h_phi, phi_b, cudaMemcpyDeviceToHost, cs));
+    }
     CUDA_OK(c, cudaEventRecord(c->ev_done[b], st));
     CUDA_OK(c, cudaStreamWaitEvent(cs, c->ev_done[b], 0));
     CUDA_OK(c, cudaMemcpyAsync((char*)eloc_h + (size_t)i * nw * 16, eb[b], nw * 16, cudaMemcpyDeviceToHost, cs));
@@ -1539,7 +1553,7 @@ afqmc_status afqmc_step_host(afqmc_ctx* c, void* phi_h, double* weight_h, void* 
     CUDA_OK(c, cudaEventRecord(c->ev_e[0], cs));
     CUDA_OK(c, cudaStreamWaitEvent(st, c->ev_e[0], 0));
   }
-  CUDA_OK(c, cudaMemcpyAsync(phi_h, c->h_phi, phi_b, cudaMemcpyDeviceToHost, st));
+  if (n_steps == 0) CUDA_OK(c, cudaMemcpyAsync(phi_h, c->h_phi, phi_b, cudaMemcpyDeviceToHost, st));
   CUDA_OK(c, cudaMemcpyAsync(weight_h, c->h_weight, nw * 8, cudaMemcpyDeviceToHost, st));
   CUDA_OK(c, cudaMemcpyAsync(ovlp_h, c->h_ovlp, nw * 16, cudaMemcpyDeviceToHost, st));
   down += phi_b + nw * 8 + nw * 16;
