@@ -28,6 +28,11 @@ namespace {
 
 inline size_t rup(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+#ifndef AFQMC_EN_CHUNK
+#define AFQMC_EN_CHUNK 4
+#endif
+enum { EN_SCHED_INTS = 16384, EN_CHUNK = AFQMC_EN_CHUNK };   // room for the persistent energy GEMM's tile lists
+
 struct Carver {
   size_t off = 0;
   char* base = nullptr;
@@ -78,6 +83,7 @@ struct afqmc_ctx {
   int nblk; int2* blk;   // symmetric block list of the tcgen05 assembly GEMM
   int cta2;   // tcgen05 GEMMs run on CTA pairs (cta_group::2), gemm_path 3
   int ps_ok;  // the persistent pair kernel's shared-memory request was accepted
+  int* en_sched; int en_stride, en_ok;   // H9: tile lists of the persistent energy GEMM (both spins in one launch), [n_sm/2][en_stride]
   int tay_tc; tt::TaylorMaps map_tay; tt::TaylorTcArgs tay_args; size_t tay_tc_smem; int n_sm;   // TMA descriptors of the tcgen05 path (path == 2)
   char err[256];
   int64_t launches;
@@ -226,6 +232,7 @@ void carve(const afqmc_params* p, afqmc_ctx* c, char* cbase, char* wbase, size_t
   c->Lt = cc.take(lt_rows * NGP * ts);
   c->Lt_lo = split ? cc.take(lt_rows * NGP * ts) : nullptr;
   c->blk = (int2*)cc.take((size_t)(c->nblk ? c->nblk : 1) * sizeof(int2));
+  c->en_sched = (int*)cc.take(EN_SCHED_INTS * sizeof(int));
   c->Rall = cc.take((size_t)rup(ng, 128) * KT * ts);
   c->Rall_lo = split ? cc.take((size_t)rup(ng, 128) * KT * ts) : nullptr;
   const size_t ya = md ? 32 : KA, yb = (md || !KB) ? 32 : KB;   // Y is not used by the multi-det energy
@@ -455,8 +462,10 @@ afqmc_status run_gemm_tc(afqmc_ctx* c, const tc::Maps& maps, int m, int n, int K
       const int n_pairs = (m_tiles + 1) / 2 * n_tiles, slots = c->n_sm / 2;
       if (!tri && slots > 0 && c->ps_ok) {
         dim3 gridp(2 * (n_pairs < slots ? n_pairs : slots));
+        tc::PsWork wk{};
+        wk.K[0] = K; wk.m_tiles[0] = m_tiles; wk.n_tiles = n_tiles; wk.n_pairs = n_pairs;
         auto kernp = tc::k_gemm_tf32_pair_ps<Epi>;
-        LAUNCH(c, kernp, gridp, tc::PS_THREADS, tc::SMEM_PS_BYTES, maps, K, m_tiles, n_tiles, n_pairs, epi);
+        LAUNCH(c, kernp, gridp, tc::PS_THREADS, tc::SMEM_PS_BYTES, maps, maps, wk, epi, epi);
         return AFQMC_OK;
       }
     }
@@ -557,8 +566,59 @@ template <typename T> afqmc_status run_md_energy(afqmc_ctx* c, const void* theta
   return AFQMC_OK;
 }
 
+// H9 tile lists: every (spin, row pair, column tile) of the triangular energy GEMM with its cost (k-blocks from the
+// pair's diagonal block on + the fused dot epilogue), longest first onto the least loaded CTA pair (LPT).  Tiles of one
+// row pair cost the same, sit next to each other in the order and so start at about the same time on different pairs:
+// they share their rows of Y in L2.
+static bool build_energy_schedule(afqmc_ctx* c, std::vector<int>& out, int& stride) {
+  const int slots = c->n_sm / 2, n_tiles = (2 * c->nw + tc::BN - 1) / tc::BN;
+  if (slots <= 0) return false;
+  struct Item { int cost, entry; };
+  std::vector<Item> items;
+  for (int sp = 0; sp < 2; ++sp) {
+    const int n = sp ? c->nb : c->na, Ks = sp ? c->KB : c->KA;
+    if (!n) continue;
+    const int m_tiles = (c->M * n + tc::BM - 1) / tc::BM;
+    for (int mp = 0; mp < (m_tiles + 1) / 2; ++mp) {
+      const int nkb = Ks / tc::BK - (mp * 2 * tc::BM) / tc::BK;
+      for (int nt = 0; nt < n_tiles; ++nt) items.push_back({nkb + 6, (sp << 24) | (mp * n_tiles + nt)});
+    }
+  }
+  std::stable_sort(items.begin(), items.end(), [](const Item& a, const Item& b) { return a.cost > b.cost; });
+  std::vector<std::vector<int>> lists(slots);
+  std::vector<long> load(slots, 0);
+  for (const Item& it : items) {
+    int best = 0;
+    for (int k = 1; k < slots; ++k) if (load[k] < load[best]) best = k;
+    lists[best].push_back(it.entry); load[best] += it.cost;
+  }
+  size_t longest = 0;
+  for (auto& l : lists) longest = l.size() > longest ? l.size() : longest;
+  stride = (int)longest + 1;
+  if ((size_t)stride * slots > EN_SCHED_INTS) return false;
+  out.assign((size_t)stride * slots, -1);
+  for (int k = 0; k < slots; ++k) for (size_t j = 0; j < lists[k].size(); ++j) out[(size_t)k * stride + j] = lists[k][j];
+  return true;
+}
+
 template <typename T> afqmc_status run_energy_gemm(afqmc_ctx* c, const void* theta, zcplx* eloc) {
   StageScope sc(c, AFQMC_STAGE_ENERGY);
+  if constexpr (sizeof(T) == 4) {
+    if (c->path == 2 && c->cta2 && c->en_ok) {   // both spins, one persistent launch
+      tc::EpiEnergy e[2];
+      tc::PsWork wk{};
+      for (int s = 0; s < 2; ++s) {
+        const int n = s ? c->nb : c->na, soff = s ? c->KA : 0;
+        e[s].theta = (const float2*)theta; e[s].M = c->M; e[s].nt = c->nt; e[s].off = s ? c->na : 0; e[s].n = n ? n : 1;
+        e[s].hrot = (const float*)c->hrot + soff; e[s].eloc = (double*)eloc; e[s].m_real = c->M * n; e[s].n_real = 2 * c->nw;
+        wk.K[s] = s ? c->KB : c->KA; wk.m_tiles[s] = (c->M * n + tc::BM - 1) / tc::BM;
+      }
+      wk.n_tiles = (2 * c->nw + tc::BN - 1) / tc::BN; wk.tri = 1; wk.sched = c->en_sched; wk.sched_stride = c->en_stride;
+      auto kernp = tc::k_gemm_tf32_pair_ps<tc::EpiEnergy, EN_CHUNK, true>;
+      LAUNCH(c, kernp, dim3(2 * (c->n_sm / 2)), tc::PS_THREADS, tc::SMEM_PS_BYTES, c->map_en[0], c->map_en[c->nb ? 1 : 0], wk, e[0], e[1]);
+      return AFQMC_OK;
+    }
+  }
   for (int s = 0; s < 2; ++s) {
     int n = s ? c->nb : c->na, soff = s ? c->KA : 0, Ks = s ? c->KB : c->KA;
     if (!n) continue;
@@ -1033,6 +1093,8 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
     if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(k_gemm_tf32_pair<tc::EpiTT>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(k_gemm_tf32_pair<tc::EpiAssembleSym>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     c->ps_ok = cudaFuncSetAttribute(k_gemm_tf32_pair_ps<tc::EpiAssembleSym>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_PS_BYTES) == cudaSuccess;
+    c->en_ok = c->cta2 && !c->md &&
+               cudaFuncSetAttribute(k_gemm_tf32_pair_ps<tc::EpiEnergy, EN_CHUNK, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_PS_BYTES) == cudaSuccess;
     (void)cudaGetLastError();
     if (!ok || e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) {
       snprintf(g_init_err, 256, "tcgen05 path: tensor-map / shared-memory set-up failed");
@@ -1046,6 +1108,12 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
     memcpy(g_init_err, c->err, 256);
     delete c;
     return s;
+  }
+  if (c->en_ok) {   // after init_device: it clears the constant region the lists live in
+    std::vector<int> sched;
+    c->en_ok = build_energy_schedule(c, sched, c->en_stride) &&
+               cudaMemcpyAsync(c->en_sched, sched.data(), sched.size() * sizeof(int), cudaMemcpyHostToDevice, c->stream) == cudaSuccess &&
+               cudaStreamSynchronize(c->stream) == cudaSuccess;
   }
   c->launches = 0;
   *out = c;

@@ -730,10 +730,40 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
-template <class Epi>
+// Work description of the persistent kernel.  Up to two problems (same column count; H9: the two spins) share one launch;
+// `sched` (device, may be null) holds for every CTA pair its tile list, `sched_stride` entries per pair, -1 terminated,
+// entry = problem << 24 | tile pair index (row-pair major, column tile fastest); used by the LIST instantiation only.
+// tri: the a-operand is upper triangular in 128 x 128 blocks, a row pair starts at its leader's diagonal k-block.
+struct PsWork {
+  int K[2], m_tiles[2], n_tiles, n_pairs, tri, sched_stride;
+  const int* sched;
+};
+struct PsTile { int prob, mt, m0, n0, kb0, nkb; bool valid; };
+// LIST = false: one problem, full K range, pairs dealt round-robin (everything about a tile but its origin is loop-invariant)
+template <bool LIST>
+__device__ __forceinline__ bool ps_tile(const PsWork& wk, int cid, int ncl, int rank, int k, PsTile& t) {
+  int e;
+  if (LIST) {
+    if (k >= wk.sched_stride) return false;
+    e = wk.sched[(size_t)cid * wk.sched_stride + k];
+    if (e < 0) return false;
+  } else {
+    e = cid + k * ncl;
+    if (e >= wk.n_pairs) return false;
+  }
+  t.prob = LIST ? e >> 24 : 0;
+  const int tp = LIST ? (e & 0xFFFFFF) : e, mp = tp / wk.n_tiles;
+  t.mt = mp * 2 + rank; t.m0 = t.mt * BM; t.n0 = (tp - mp * wk.n_tiles) * BN;
+  t.kb0 = (LIST && wk.tri) ? (mp * 2 * BM) / BK : 0;
+  t.nkb = wk.K[t.prob] / BK - t.kb0;
+  t.valid = t.mt < wk.m_tiles[t.prob];
+  return true;
+}
+
+template <class Epi, int CHUNK = PS_CHUNK_KB, bool LIST = false>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PS_THREADS, 1)
-k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps, int K, int m_tiles, int n_tiles, int n_pairs, Epi epi) {
-  static_assert(Epi::kStaged, "persistent kernel is written for the staged epilogue");
+k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps0, const __grid_constant__ Maps maps1, const __grid_constant__ PsWork wk,
+                    const __grid_constant__ Epi epi0, const __grid_constant__ Epi epi1) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   __shared__ __align__(8) uint64_t full_bar[STAGES2];     // used in the leader only
@@ -746,8 +776,6 @@ k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps, int K, int m_tiles, int n
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
   const int cid = blockIdx.x >> 1, ncl = gridDim.x >> 1;
-  const int nkb = K / BK;
-  const int nchunk = (nkb + PS_CHUNK_KB - 1) / PS_CHUNK_KB;
   const uint32_t sS = smem_u32(smem + (size_t)STAGES2 * STAGE2_BYTES);
 
   if (warp == EPI_WARPS && lane == 0) {
@@ -759,10 +787,10 @@ k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps, int K, int m_tiles, int n
       mbar_init(&stg_full_bar[b], EPI_WARPS); mbar_init(&stg_free_bar[b], 4);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.a_hi) : "memory");
-    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.a_lo) : "memory");
-    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.b_hi) : "memory");
-    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.b_lo) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps0.a_hi) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps0.a_lo) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps0.b_hi) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps0.b_lo) : "memory");
   }
   if (warp == EPI_WARPS + 1) {
     asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)),
@@ -775,22 +803,24 @@ k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps, int K, int m_tiles, int n
   cluster_sync_all();
   tc_fence_after();
   const uint32_t tmem = tmem_base_s;
+  PsTile tl;
 
-  if (warp >= PS_STORE_WARP0) {          // ===== store warps =====
+  if (warp >= PS_STORE_WARP0) {          // ===== store warps (staged epilogues only) =====
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"((int)PS_REGS_STORE));
-    const int t = (int)threadIdx.x - PS_STORE_WARP0 * 32;
-    uint32_t sr = 0;
-    for (int tp = cid; tp < n_pairs; tp += ncl) {
-      const int mt = (tp / n_tiles) * 2 + (int)rank, m0 = mt * BM, n0 = (tp % n_tiles) * BN;
-      const bool valid = mt < m_tiles;
-      typename Epi::StoreCtx sc = epi.store_ctx(valid ? m0 : 0, n0, t);
+    if constexpr (Epi::kStaged) {
+      const int t = (int)threadIdx.x - PS_STORE_WARP0 * 32;
+      uint32_t sr = 0;
+      for (int ti = 0; ps_tile<LIST>(wk, cid, ncl, (int)rank, ti, tl); ++ti) {
+        const Epi epi = (LIST && tl.prob) ? epi1 : epi0;
+        typename Epi::StoreCtx sc = epi.store_ctx(tl.valid ? tl.m0 : 0, tl.n0, t);
 #pragma unroll 1
-      for (int r = 0; r < STG_ROUNDS; ++r, ++sr) {
-        const int b = sr & 1;
-        mbar_wait(&stg_full_bar[b], (sr >> 1) & 1);
-        if (valid) epi.flush_round(sc, sS + b * STG_BYTES, r);
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&stg_free_bar[b]);   // release: the loads above have completed
+        for (int r = 0; r < STG_ROUNDS; ++r, ++sr) {
+          const int b = sr & 1;
+          mbar_wait(&stg_full_bar[b], (sr >> 1) & 1);
+          if (tl.valid) epi.flush_round(sc, sS + b * STG_BYTES, r);
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&stg_free_bar[b]);   // release: the loads above have completed
+        }
       }
     }
   } else if (warp >= EPI_WARPS) {
@@ -798,18 +828,19 @@ k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps, int K, int m_tiles, int n
     if (warp == EPI_WARPS) {
       if (lane == 0) {   // ===== TMA producer (both CTAs) =====
         uint32_t it = 0;
-        for (int tp = cid; tp < n_pairs; tp += ncl) {
-          const int m0 = ((tp / n_tiles) * 2 + (int)rank) * BM, nb = (tp % n_tiles) * BN + (int)rank * B_BOX;
-          for (int kb = 0; kb < nkb; ++kb, ++it) {
+        for (int ti = 0; ps_tile<LIST>(wk, cid, ncl, (int)rank, ti, tl); ++ti) {
+          const Maps* mp = (LIST && tl.prob) ? &maps1 : &maps0;
+          const int nb = tl.n0 + (int)rank * B_BOX;
+          for (int kb = 0; kb < tl.nkb; ++kb, ++it) {
             const int s = it % STAGES2;
             mbar_wait(&empty_bar[s], ((it / STAGES2) & 1) ^ 1);
             uint8_t* st = smem + (size_t)s * STAGE2_BYTES;
             if (rank == 0) mbar_expect_tx(&full_bar[s], 2 * STAGE2_BYTES);
-            const int kc = kb * BK;
-            tma_load_2d_pair_hint(st, &maps.a_hi, &full_bar[s], kc, m0, PS_POL_A);
-            tma_load_2d_pair_hint(st + A_BYTES, &maps.a_lo, &full_bar[s], kc, m0, PS_POL_A);
-            tma_load_2d_pair_hint(st + 2 * A_BYTES, &maps.b_hi, &full_bar[s], kc, nb, PS_POL_B);
-            tma_load_2d_pair_hint(st + 2 * A_BYTES + HB_BYTES, &maps.b_lo, &full_bar[s], kc, nb, PS_POL_B);
+            const int kc = (tl.kb0 + kb) * BK;
+            tma_load_2d_pair_hint(st, &mp->a_hi, &full_bar[s], kc, tl.m0, PS_POL_A);
+            tma_load_2d_pair_hint(st + A_BYTES, &mp->a_lo, &full_bar[s], kc, tl.m0, PS_POL_A);
+            tma_load_2d_pair_hint(st + 2 * A_BYTES, &mp->b_hi, &full_bar[s], kc, nb, PS_POL_B);
+            tma_load_2d_pair_hint(st + 2 * A_BYTES + HB_BYTES, &mp->b_lo, &full_bar[s], kc, nb, PS_POL_B);
           }
         }
       }
@@ -823,16 +854,16 @@ k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps, int K, int m_tiles, int n
         uint64_t ds = d0;
         int s = 0;
         uint32_t fpar = 0, cg = 0;
-        for (int tp = cid; tp < n_pairs; tp += ncl) {
+        for (int ti = 0; ps_tile<LIST>(wk, cid, ncl, 0, ti, tl); ++ti) {
           int kc = 0;                                      // k-block within the chunk
-          for (int kb = 0; kb < nkb; ++kb) {
+          for (int kb = 0; kb < tl.nkb; ++kb) {
             const int buf = cg & 1;
             if (kc == 0) {   // both CTAs' epilogue warps have drained this TMEM buffer (two chunks ago)
               mbar_wait(&tmem_empty_bar[buf], ((cg >> 1) & 1) ^ 1);
             }
             mbar_wait(&full_bar[s], fpar);
             tc_fence_after();
-            const bool chunk_end = kc == PS_CHUNK_KB - 1 || kb == nkb - 1;
+            const bool chunk_end = kc == CHUNK - 1 || kb == tl.nkb - 1;
             if (elect_one()) {
               const uint32_t d = tmem + buf * BN;
               const uint64_t a_hi = ds, a_lo = ds + (A_BYTES >> 4);
@@ -861,7 +892,13 @@ k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps, int K, int m_tiles, int n
     // staged row = (q * 32 + lane) with bit 4 flipped in the upper half of the block (conflict-free mirrored reads, see StoreCtx)
     const uint32_t sW = sS + (uint32_t)((half * (STG_COLS / 2)) * BM + ((q * 32 + lane) ^ ((q >> 1) << 4))) * 4;
     uint32_t cg = 0, sr = 0;
-    for (int tp = cid; tp < n_pairs; tp += ncl) {
+    for (int ti = 0;; ++ti) {
+      int nchunk;
+      {   // only the chunk count stays live beside the 128 accumulators; the tile is looked up again after the loop
+        PsTile t0;
+        if (!ps_tile<LIST>(wk, cid, ncl, (int)rank, ti, t0)) break;
+        nchunk = (t0.nkb + CHUNK - 1) / CHUNK;
+      }
       float acc[COLS_PER_WARP];
 #pragma unroll
       for (int i = 0; i < COLS_PER_WARP; ++i) acc[i] = 0.f;
@@ -881,15 +918,29 @@ k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps, int K, int m_tiles, int n
         __syncwarp();
         if (lane == 0) mbar_arrive_leader(&tmem_empty_bar[buf]);
       }
-      // the tile sits in registers and both TMEM buffers are released: the next tile's MMAs run while it is handed over
+      // the tile sits in registers and both TMEM buffers are released: the next tile's MMAs run while it leaves
+      if constexpr (Epi::kStaged) {
 #pragma unroll
-      for (int r = 0; r < STG_ROUNDS; ++r, ++sr) {
-        const int b = sr & 1;
-        mbar_wait(&stg_free_bar[b], ((sr >> 1) & 1) ^ 1);
+        for (int r = 0; r < STG_ROUNDS; ++r, ++sr) {
+          const int b = sr & 1;
+          mbar_wait(&stg_free_bar[b], ((sr >> 1) & 1) ^ 1);
 #pragma unroll
-        for (int j = 0; j < STG_COLS / 2; ++j) st_s32(sW + b * STG_BYTES + j * (BM * 4), acc[r * (STG_COLS / 2) + j]);
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&stg_full_bar[b]);   // release: this warp's 16 x 32 values are in place
+          for (int j = 0; j < STG_COLS / 2; ++j) st_s32(sW + b * STG_BYTES + j * (BM * 4), acc[r * (STG_COLS / 2) + j]);
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&stg_full_bar[b]);   // release: this warp's 16 x 32 values are in place
+        }
+      } else {
+        ps_tile<LIST>(wk, cid, ncl, (int)rank, ti, tl);
+        if (tl.valid) {
+          const Epi epi = (LIST && tl.prob) ? epi1 : epi0;
+#pragma unroll
+          for (int cb = 0; cb < COLS_PER_WARP / 32; ++cb) {
+            float v[32];
+#pragma unroll
+            for (int j = 0; j < 32; ++j) v[j] = acc[cb * 32 + j];
+            epi(tl.m0 + q * 32 + lane, tl.n0 + half * COLS_PER_WARP + cb * 32, v);
+          }
+        }
       }
     }
   }
