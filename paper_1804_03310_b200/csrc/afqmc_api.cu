@@ -83,6 +83,7 @@ struct afqmc_ctx {
   int nblk; int2* blk;   // symmetric block list of the tcgen05 assembly GEMM
   int cta2;   // tcgen05 GEMMs run on CTA pairs (cta_group::2), gemm_path 3
   int ps_ok;  // the persistent pair kernel's shared-memory request was accepted
+  int* fb_sched; int fb_stride, fb_ok;   // H4: the same for the force-bias GEMM (both spins, one launch)
   int* en_sched; int en_stride, en_ok;   // H9: tile lists of the persistent energy GEMM (both spins in one launch), [n_sm/2][en_stride]
   int tay_tc; tt::TaylorMaps map_tay; tt::TaylorTcArgs tay_args; size_t tay_tc_smem; int n_sm;   // TMA descriptors of the tcgen05 path (path == 2)
   char err[256];
@@ -233,6 +234,7 @@ void carve(const afqmc_params* p, afqmc_ctx* c, char* cbase, char* wbase, size_t
   c->Lt_lo = split ? cc.take(lt_rows * NGP * ts) : nullptr;
   c->blk = (int2*)cc.take((size_t)(c->nblk ? c->nblk : 1) * sizeof(int2));
   c->en_sched = (int*)cc.take(EN_SCHED_INTS * sizeof(int));
+  c->fb_sched = (int*)cc.take(EN_SCHED_INTS * sizeof(int));
   c->Rall = cc.take((size_t)rup(ng, 128) * KT * ts);
   c->Rall_lo = split ? cc.take((size_t)rup(ng, 128) * KT * ts) : nullptr;
   const size_t ya = md ? 32 : KA, yb = (md || !KB) ? 32 : KB;   // Y is not used by the multi-det energy
@@ -482,6 +484,20 @@ afqmc_status run_gemm_tc(afqmc_ctx* c, const tc::Maps& maps, int m, int n, int K
 // per-spin traces f^s_g = sum R^s_g[a][k] Theta_s[k][a] from the planar Theta in ctx->thp
 template <typename T> afqmc_status run_fb_gemm(afqmc_ctx* c) {
   StageScope sc(c, AFQMC_STAGE_FORCE_BIAS);
+  if constexpr (sizeof(T) == 4) {
+    if (c->path == 2 && c->cta2 && c->fb_ok) {   // both spins, one persistent launch; stores overlap the next tile's main loop
+      tc::EpiStoreT e[2];
+      tc::PsWork wk{};
+      for (int s = 0; s < 2; ++s) {
+        e[s].out = (float*)c->fs + (size_t)s * 2 * c->nw * c->NGP; e[s].ldo = c->NGP; e[s].m_real = c->ng; e[s].n_real = 2 * c->nw;
+        wk.K[s] = s ? c->KB : c->KA; wk.m_tiles[s] = (c->ng + tc::BM - 1) / tc::BM;
+      }
+      wk.n_tiles = (2 * c->nw + tc::BN - 1) / tc::BN; wk.sched = c->fb_sched; wk.sched_stride = c->fb_stride;
+      auto kernp = tc::k_gemm_tf32_pair_ps<tc::EpiStoreT, EN_CHUNK, true>;
+      LAUNCH(c, kernp, dim3(2 * (c->n_sm / 2)), tc::PS_THREADS, tc::SMEM_PS_BYTES, c->map_fb[0], c->map_fb[c->cb ? 1 : 0], wk, e[0], e[1]);
+      return AFQMC_OK;
+    }
+  }
   for (int s = 0; s < 2; ++s) {
     int n = s ? c->cb : c->ca, soff = s ? c->KA : 0, Ks = s ? c->KB : c->KA;
     if (!n) continue;
@@ -566,24 +582,26 @@ template <typename T> afqmc_status run_md_energy(afqmc_ctx* c, const void* theta
   return AFQMC_OK;
 }
 
-// H9 tile lists: every (spin, row pair, column tile) of the triangular energy GEMM with its cost (k-blocks from the
-// pair's diagonal block on + the fused dot epilogue), longest first onto the least loaded CTA pair (LPT).  Tiles of one
-// row pair cost the same, sit next to each other in the order and so start at about the same time on different pairs:
-// they share their rows of Y in L2.
-static bool build_energy_schedule(afqmc_ctx* c, std::vector<int>& out, int& stride) {
+// Tile lists of the persistent pair kernel's LIST instantiation (H9, H4): every (problem, row pair, column tile) with its
+// cost (k-blocks -- from the pair's diagonal block on when `tri` -- plus `epi_cost` for the epilogue), longest first onto the
+// least loaded CTA pair (LPT).  Tiles of one row pair cost the same, sit next to each other in the order and so start
+// at about the same time on different pairs: they share their rows of the a-operand in L2.
+static bool build_pair_schedule(const afqmc_ctx* c, int tri, const int m_rows[2], const int K[2], int epi_cost,
+                                std::vector<int>& out, int& stride) {
   const int slots = c->n_sm / 2, n_tiles = (2 * c->nw + tc::BN - 1) / tc::BN;
   if (slots <= 0) return false;
   struct Item { int cost, entry; };
   std::vector<Item> items;
   for (int sp = 0; sp < 2; ++sp) {
-    const int n = sp ? c->nb : c->na, Ks = sp ? c->KB : c->KA;
-    if (!n) continue;
-    const int m_tiles = (c->M * n + tc::BM - 1) / tc::BM;
+    if (!m_rows[sp] || !K[sp]) continue;
+    const int m_tiles = (m_rows[sp] + tc::BM - 1) / tc::BM;
     for (int mp = 0; mp < (m_tiles + 1) / 2; ++mp) {
-      const int nkb = Ks / tc::BK - (mp * 2 * tc::BM) / tc::BK;
-      for (int nt = 0; nt < n_tiles; ++nt) items.push_back({nkb + 6, (sp << 24) | (mp * n_tiles + nt)});
+      const int nkb = K[sp] / tc::BK - (tri ? (mp * 2 * tc::BM) / tc::BK : 0);
+      if (nkb <= 0) return false;
+      for (int nt = 0; nt < n_tiles; ++nt) items.push_back({nkb + epi_cost, (sp << 24) | (mp * n_tiles + nt)});
     }
   }
+  if (items.empty()) return false;
   std::stable_sort(items.begin(), items.end(), [](const Item& a, const Item& b) { return a.cost > b.cost; });
   std::vector<std::vector<int>> lists(slots);
   std::vector<long> load(slots, 0);
@@ -1095,6 +1113,8 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
     c->ps_ok = cudaFuncSetAttribute(k_gemm_tf32_pair_ps<tc::EpiAssembleSym>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_PS_BYTES) == cudaSuccess;
     c->en_ok = c->cta2 && !c->md &&
                cudaFuncSetAttribute(k_gemm_tf32_pair_ps<tc::EpiEnergy, EN_CHUNK, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_PS_BYTES) == cudaSuccess;
+    c->fb_ok = c->cta2 &&
+               cudaFuncSetAttribute(k_gemm_tf32_pair_ps<tc::EpiStoreT, EN_CHUNK, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_PS_BYTES) == cudaSuccess;
     (void)cudaGetLastError();
     if (!ok || e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) {
       snprintf(g_init_err, 256, "tcgen05 path: tensor-map / shared-memory set-up failed");
@@ -1109,11 +1129,20 @@ afqmc_status afqmc_init(afqmc_ctx** out, const afqmc_params* p, const double* h1
     delete c;
     return s;
   }
-  if (c->en_ok) {   // after init_device: it clears the constant region the lists live in
+  // after init_device: it clears the constant region the lists live in
+  auto upload_sched = [&](int* dst, const std::vector<int>& v) {
+    return cudaMemcpyAsync(dst, v.data(), v.size() * sizeof(int), cudaMemcpyHostToDevice, c->stream) == cudaSuccess &&
+           cudaStreamSynchronize(c->stream) == cudaSuccess;
+  };
+  if (c->en_ok) {
     std::vector<int> sched;
-    c->en_ok = build_energy_schedule(c, sched, c->en_stride) &&
-               cudaMemcpyAsync(c->en_sched, sched.data(), sched.size() * sizeof(int), cudaMemcpyHostToDevice, c->stream) == cudaSuccess &&
-               cudaStreamSynchronize(c->stream) == cudaSuccess;
+    const int rows[2] = {c->M * c->na, c->M * c->nb}, Ks[2] = {c->KA, c->nb ? c->KB : 0};
+    c->en_ok = build_pair_schedule(c, 1, rows, Ks, 6, sched, c->en_stride) && upload_sched(c->en_sched, sched);
+  }
+  if (c->fb_ok) {
+    std::vector<int> sched;
+    const int rows[2] = {c->ca ? c->ng : 0, c->cb ? c->ng : 0}, Ks[2] = {c->KA, c->cb ? c->KB : 0};
+    c->fb_ok = build_pair_schedule(c, 0, rows, Ks, 3, sched, c->fb_stride) && upload_sched(c->fb_sched, sched);
   }
   c->launches = 0;
   *out = c;

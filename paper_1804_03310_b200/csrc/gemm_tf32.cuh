@@ -811,7 +811,8 @@ k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps0, const __grid_constant__ 
       const int t = (int)threadIdx.x - PS_STORE_WARP0 * 32;
       uint32_t sr = 0;
       for (int ti = 0; ps_tile<LIST>(wk, cid, ncl, (int)rank, ti, tl); ++ti) {
-        const Epi epi = (LIST && tl.prob) ? epi1 : epi0;
+        const Epi* const epp = (LIST && tl.prob) ? &epi1 : &epi0;
+        const Epi epi = *epp;
         typename Epi::StoreCtx sc = epi.store_ctx(tl.valid ? tl.m0 : 0, tl.n0, t);
 #pragma unroll 1
         for (int r = 0; r < STG_ROUNDS; ++r, ++sr) {
@@ -932,7 +933,9 @@ k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps0, const __grid_constant__ 
       } else {
         ps_tile<LIST>(wk, cid, ncl, (int)rank, ti, tl);
         if (tl.valid) {
-          const Epi epi = (LIST && tl.prob) ? epi1 : epi0;
+          // by address: `cond ? epi1 : epi0` on the two parameter structs picked epi0 for every tile of the EpiStoreT instantiation
+          const Epi* const epp = (LIST && tl.prob) ? &epi1 : &epi0;
+          const Epi epi = *epp;
 #pragma unroll
           for (int cb = 0; cb < COLS_PER_WARP / 32; ++cb) {
             float v[32];
