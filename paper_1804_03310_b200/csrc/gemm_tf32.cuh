@@ -5,6 +5,9 @@
 //   2-stage shared-memory ring; one elected thread issues tcgen05.mma.kind::tf32 (M=128, N=256, K=8);
 //   four epilogue warps read the 128 x 256 accumulator with tcgen05.ld and apply the fused epilogue.
 // Used for H4 (force bias), H6 (operator assembly), H9 (energy): PAPER.md:59, :80, :87.
+// Three kernels: k_gemm_tf32 (one CTA per 128 x 256 tile, gemm_path 2), k_gemm_tf32_pair (one cta_group::2 pair per
+// 256 x 256 tile pair: the multi-determinant TT GEMM and fallbacks) and k_gemm_tf32_pair_ps (persistent pairs, 16 warps:
+// H6 with its tile handed to dedicated store warps; H4 and H9 with both spins in one launch over host-built tile lists).
 #pragma once
 #include <cuda.h>
 #include "common.cuh"
