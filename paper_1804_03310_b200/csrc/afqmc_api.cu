@@ -736,7 +736,9 @@ afqmc_status do_propagate(afqmc_ctx* c, void* phi, const void* x, const void* fb
           tc::EpiAssembleSym e3;
           e3.out = (float*)c->Abuf; e3.out_lo = nullptr;   // A_w is stored once, in FP32: the Taylor kernel splits it on the fly
           e3.blk = c->blk; e3.M = c->M;
-          e3.MP = c->MP; e3.n_real = 2 * c->nw; e3.st_pol = tc::PS_POL_ST;
+          e3.MP = c->MP; e3.n_real = 2 * c->nw;
+          // A_w beyond the L2 (126 MB) is streamed: its lines are asked to leave first, the field planes stay (gemm_tf32.cuh)
+          e3.st_pol = ((size_t)c->nw * c->M * 2 * c->MP * 4 > ((size_t)96 << 20) || (AFQMC_PS_POL & 4)) ? tc::L2_EVICT_FIRST : tc::L2_EVICT_NORMAL;
           st = run_gemm_tc(c, c->map_asm, c->nblk * 128, 2 * c->nw, c->NGP, e3);
           done = true;
         }

@@ -719,10 +719,12 @@ enum { PS_CHUNK_KB = AFQMC_PS_CHUNK_KB };
 enum { PS_THREADS = 512, PS_STORE_WARP0 = 12, STG_COLS = 32, STG_BYTES = BM * STG_COLS * 4, STG_ROUNDS = BN / STG_COLS,
        SMEM_PS_BYTES = STAGES2 * STAGE2_BYTES + 2 * STG_BYTES + 1024 };
 // L2 eviction-priority hints (bit 0: L rows evict_first, bit 1: field rows evict_last, bit 2: output stores evict_first).
-// Measured on B200, cfg 5 (0.655 ms without): 2 -> 0.653, 4 -> 0.664, 6 -> 0.658, 3 -> 0.700, 7 -> 0.685: none helps, so
-// the default is no hint.
+// Measured on B200, cfg 5, H6: none changes the time (0.653-0.664 ms against 0.655; bit 0 costs 0.03-0.05 ms), but the
+// DRAM reads go from 836 MB (no hint) to 675 MB (bit 1: the 33 MB of field planes, re-read by every row pair, stay in L2
+// under the 650 MB output stream) and 569 MB (bits 1 + 2).  Default: bit 1 here; the stores' hint is chosen at run time
+// (EpiAssembleSym::st_pol: evict_first only when A_w is larger than the L2, so that a small A_w stays there for H7).
 #ifndef AFQMC_PS_POL
-#define AFQMC_PS_POL 0
+#define AFQMC_PS_POL 2
 #endif
 constexpr uint64_t L2_EVICT_NORMAL = 0x1000000000000000ull;
 constexpr uint64_t PS_POL_A = (AFQMC_PS_POL & 1) ? L2_EVICT_FIRST : L2_EVICT_NORMAL;
@@ -843,8 +845,10 @@ k_gemm_tf32_pair_ps(const __grid_constant__ Maps maps0, const __grid_constant__ 
             const int kc = (tl.kb0 + kb) * BK;
             tma_load_2d_pair_hint(st, &mp->a_hi, &full_bar[s], kc, tl.m0, PS_POL_A);
             tma_load_2d_pair_hint(st + A_BYTES, &mp->a_lo, &full_bar[s], kc, tl.m0, PS_POL_A);
-            tma_load_2d_pair_hint(st + 2 * A_BYTES, &mp->b_hi, &full_bar[s], kc, nb, PS_POL_B);
-            tma_load_2d_pair_hint(st + 2 * A_BYTES + HB_BYTES, &mp->b_lo, &full_bar[s], kc, nb, PS_POL_B);
+            // the b-operand hint is for H6's field planes only (33 MB, read by every row pair); H4 / H9 stream 165 MB of Theta planes
+            constexpr uint64_t polb = LIST ? L2_EVICT_NORMAL : PS_POL_B;
+            tma_load_2d_pair_hint(st + 2 * A_BYTES, &mp->b_hi, &full_bar[s], kc, nb, polb);
+            tma_load_2d_pair_hint(st + 2 * A_BYTES + HB_BYTES, &mp->b_lo, &full_bar[s], kc, nb, polb);
           }
         }
       }
