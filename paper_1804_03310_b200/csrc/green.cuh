@@ -6,38 +6,37 @@
 
 namespace afq {
 
-// The same elimination executed by a GROUP of 128 threads (4 warps, named barrier `bar_id`): the serial
-// one-warp version left 6 of the CTA's 8 warps idle and dominated the kernel (ncu: most stall samples at the CTA
-// barrier behind it).  work = [fac (n) | prow (2n) | staging copy (2n^2) | 1] scratch.  det / sing are identical in
-// all threads of the group.
-__device__ inline void group_gauss_jordan(zcplx* aug, int n, int ld, zcplx* work, int* ctrl, int gtid, int bar_id,
-                                          zcplx& det, int& sing, double eps) {
-  (void)ctrl;
-  zcplx* fac = work;
-  zcplx* prow = work + n;
+// In-place Gauss-Jordan inverse with partial (row) pivoting, executed by a GROUP of 128 threads (4 warps, named barrier
+// `bar_id`).  The n x n matrix ping-pongs between two dense buffers (row stride n): every pivot step reads one and writes
+// the other, so a step costs two group barriers (factors ready; update done).  No augmentation with the identity: the
+// column of the pivot is overwritten with the column the identity would have produced (-f / p, and 1 / p in the pivot
+// row), which halves the update work and the shared memory of the augmented form.  Row interchanges of A are column
+// interchanges of the inverse, applied at the end in reverse order -- here composed into cperm[]: inverse[a][b] =
+// result[a * n + cperm[b]].  The pivot search is done by every warp of the group redundantly (same shuffles, same
+// result): no barrier between the search and the factor computation.  det / sing are identical in all threads.
+// Returns the buffer that holds the result.
+__device__ inline zcplx* group_gauss_jordan(zcplx* bufA, zcplx* bufB, int n, zcplx* fac, zcplx* prow, int* ipiv, int* cperm, int gtid,
+                                            int bar_id, zcplx& det, int& sing, double eps) {
   const int lane = gtid & 31, gwarp = gtid >> 5;
   double dre = 1.0, dim = 0.0;
   sing = 0;
   double thresh = 0.0;
   {
     double amax = 0.0;
-    for (int e = lane; e < n * n; e += 32) amax = fmax(amax, cabs2(aug[(e / n) * ld + (e % n)]));
+    for (int e = lane; e < n * n; e += 32) amax = fmax(amax, cabs2(bufA[e]));
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) amax = fmax(amax, __shfl_xor_sync(0xffffffffu, amax, o));
     thresh = amax * eps * eps;
   }
-  // The matrix ping-pongs between `aug` (row stride ld) and a dense staging copy (row stride 2n): every pivot step reads
-  // one and writes the other, so a step costs two group barriers (factors ready; update done) instead of four, and
-  // there is no copy-back pass.  The pivot search is done by every warp of the group redundantly (same shuffles, same
-  // result): no barrier between the search and the factor computation.
-  zcplx* cur = aug; int lc = ld;
-  zcplx* nxt = prow + 2 * n; int ln = 2 * n;
+  zcplx* cur = bufA;
+  zcplx* nxt = bufB;
+  int done = 0;
   for (int col = 0; col < n; ++col) {
     int piv;
     zcplx ip = mk<double>(0.0, 0.0);
     {
       int r = col + lane;
-      double mag = (r < n) ? cabs2(cur[r * lc + col]) : -1.0;
+      double mag = (r < n) ? cabs2(cur[r * n + col]) : -1.0;
       int idx = r;
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) {
@@ -50,44 +49,51 @@ __device__ inline void group_gauss_jordan(zcplx* aug, int n, int ld, zcplx* work
       else {
         if (mag < thresh) sing = 1;
         if (idx != col) { dre = -dre; dim = -dim; }
-        const zcplx p = cur[idx * lc + col];
+        const zcplx p = cur[idx * n + col];
         double nr = dre * p.x - dim * p.y;
         dim = dre * p.y + dim * p.x;
         dre = nr;
         piv = idx;
-        if (gtid < 2 * n) ip = cinv(p);     // only the threads that scale the pivot row need the FP64 reciprocal
+        if (gtid < n) ip = cinv(p);     // only the threads that scale the pivot row need the FP64 reciprocal
       }
     }
     if (piv < 0) break;                                   // exactly singular: uniform exit (all warps agree)
-    // factors (column col, rows permuted) and the scaled pivot row, both out of place
-    for (int c = gtid; c < 2 * n; c += 128) prow[c] = cmul(cur[piv * lc + c], ip);
-    for (int r = gtid; r < n; r += 128) fac[r] = cur[(r == col ? piv : (r == piv ? col : r)) * lc + col];
+    // scaled pivot row (its pivot-column entry is the reciprocal itself) and the factors (column col, rows permuted)
+    if (gtid < n) prow[gtid] = gtid == col ? ip : cmul(cur[piv * n + gtid], ip);
+    for (int r = gtid; r < n; r += 128) fac[r] = cur[(r == col ? piv : (r == piv ? col : r)) * n + col];
+    if (gtid == 0) ipiv[col] = piv;
     asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
-    // new row r <- (row col <-> row piv swapped) - fac[r] * prow ; new row col <- prow.  2-D mapping, no division:
-    // lane = column (the scaled pivot-row entry is loaded once per step), the group's four warps stride over the rows
-    for (int c = lane; c < 2 * n; c += 32) {
+    // new row r <- (rows col, piv swapped) - fac[r] * prow, with 0 in place of the old pivot-column entry; new row col <- prow
+    if (lane < n) {
+      const int c = lane;
       const zcplx pr = prow[c];
       for (int r = gwarp; r < n; r += 4) {
         zcplx v;
         if (r == col) v = pr;
         else {
           const int src = (r == piv) ? col : r;            // the old row `col` moves to position piv
-          v = cur[src * lc + c];
+          v = c == col ? mk<double>(0.0, 0.0) : cur[src * n + c];
           const zcplx f = fac[r];
           v.x = fma(-f.x, pr.x, v.x); v.x = fma(f.y, pr.y, v.x);
           v.y = fma(-f.x, pr.y, v.y); v.y = fma(-f.y, pr.x, v.y);
         }
-        nxt[r * ln + c] = v;
+        nxt[r * n + c] = v;
       }
     }
     asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
     zcplx* t = cur; cur = nxt; nxt = t;
-    const int tl = lc; lc = ln; ln = tl;
+    ++done;
   }
-  if (cur != aug) {   // odd number of completed steps: the result is in the staging copy
-    for (int e = gtid; e < n * 2 * n; e += 128) aug[(e / (2 * n)) * ld + (e % (2 * n))] = cur[e];
+  if (gtid == 0) {   // column order of the inverse: undo the row interchanges, last one first
+    for (int c = 0; c < n; ++c) cperm[c] = c;
+    for (int col = done - 1; col >= 0; --col) {
+      const int q = ipiv[col];
+      if (q != col) { const int t = cperm[col]; cperm[col] = cperm[q]; cperm[q] = t; }
+    }
   }
+  asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
   det = mk<double>(dre, dim);
+  return cur;
 }
 
 template <typename T> struct GreenArgs {
@@ -115,9 +121,9 @@ template <typename T> struct GreenArgs {
 template <typename T> inline size_t green_smem_bytes(int M, int na, int nb) {
   int nt = na + nb, ns = na > nb ? na : nb;
   size_t b = ((size_t)M * nt * sizeof(cplx<T>) + 15) & ~size_t(15);   // phi_s
-  b += (size_t)2 * ns * (2 * ns + 1) * sizeof(zcplx);   // aug per spin (FP64 on both precision paths)
-  b += (size_t)2 * (3 * ns + 2 * ns * ns + 1) * sizeof(zcplx);   // per spin: fac, scaled pivot row, staged update, 1/pivot
-  b += 2 * sizeof(zcplx) + 8 * sizeof(int);
+  b += (size_t)4 * ns * ns * sizeof(zcplx);             // per spin: two ping-pong n x n buffers (FP64 on both precision paths)
+  b += (size_t)4 * ns * sizeof(zcplx);                  // per spin: factors, scaled pivot row
+  b += 2 * sizeof(zcplx) + (8 + 4 * ns) * sizeof(int);  // dets; sing, result buffer, ipiv, cperm
   return (b + 15) & ~size_t(15);
 }
 
@@ -144,28 +150,29 @@ __device__ inline void weight_update(zcplx S_old, zcplx S_new, zcplx c, double w
 }
 
 template <typename T>
-__global__ void __launch_bounds__(256) k_green(GreenArgs<T> g) {
+__global__ void __launch_bounds__(256, 4) k_green(GreenArgs<T> g) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nthr = blockDim.x;
   const int M = g.M, na = g.na, nb = g.nb, nt = na + nb, ns = na > nb ? na : nb;
-  const int ld = 2 * ns + 1;
   cplx<T>* phi_s = reinterpret_cast<cplx<T>*>(smem_raw);
-  // the small N x N work (overlap matrix, LU, inverse) is FP64 on both precision paths: it is
+  // the small N x N work (overlap matrix, inverse) is FP64 on both precision paths: it is
   // 0.3 % of the flops and keeps S, Theta accurate to cond(A) * eps of the FP32 walker itself
-  zcplx* aug = reinterpret_cast<zcplx*>(smem_raw + (((size_t)M * nt * sizeof(cplx<T>) + 15) & ~size_t(15)));
-  zcplx* fac = aug + 2 * ns * ld;
-  zcplx* dets = fac + 2 * (3 * ns + 2 * ns * ns + 1);
+  zcplx* mats = reinterpret_cast<zcplx*>(smem_raw + (((size_t)M * nt * sizeof(cplx<T>) + 15) & ~size_t(15)));   // [spin][2][ns*ns]
+  zcplx* fac = mats + 4 * ns * ns;           // [spin][ns] factors, then [spin][ns] scaled pivot rows
+  zcplx* dets = fac + 4 * ns;
   int* sing = reinterpret_cast<int*>(dets + 2);
-  int* ctrl = sing + 2;
+  int* resb = sing + 2;                      // which ping-pong buffer holds the inverse of spin s
+  int* ipiv = sing + 8;                      // [spin][ns]
+  int* cperm = ipiv + 2 * ns;                // [spin][ns]
 
   const cplx<T>* phi_w = g.phi + (size_t)w * M * nt;
   for (int e = tid; e < M * nt; e += nthr) phi_s[e] = phi_w[e];
   __syncthreads();
 
-  // A_s[a][b] = sum_k psi_s[k][a] phi[k][off+b]  (real x complex, FP64), augmented with the identity.
+  // A_s[a][b] = sum_k psi_s[k][a] phi[k][off+b]  (real x complex, FP64), dense n x n in the first ping-pong buffer of spin s.
   // FP64 issue slots are the scarce resource here (conversions included), so one work item = (spin, column b, group
   // of 4 rows a, half of the k range): phi[k][b] is converted once and reused for 4 rows; halves meet in shared atomics.
-  for (int e = tid; e < 2 * ns * ld; e += nthr) aug[e] = mk<double>(0.0, 0.0);
+  for (int e = tid; e < 4 * ns * ns; e += nthr) mats[e] = mk<double>(0.0, 0.0);
   __syncthreads();
   {
     const int ga = (na + 3) >> 2, gb = (nb + 3) >> 2;
@@ -189,17 +196,13 @@ __global__ void __launch_bounds__(256) k_green(GreenArgs<T> g) {
           si[u] = fma(pu, vi, si[u]);
         }
       }
-      zcplx* A = aug + s * ns * ld;
+      zcplx* A = mats + s * 2 * ns * ns;     // dense n x n, row stride n
 #pragma unroll
       for (int u = 0; u < 4; ++u)
         if (a0 + u < n) {
-          double* dst = reinterpret_cast<double*>(&A[(a0 + u) * ld + b]);
+          double* dst = reinterpret_cast<double*>(&A[(a0 + u) * n + b]);
           atomicAdd(dst, sr[u]); atomicAdd(dst + 1, si[u]);
         }
-    }
-    for (int e = tid; e < na + nb; e += nthr) {
-      const int s = e >= na, a = s ? e - na : e, n = s ? nb : na;
-      aug[s * ns * ld + a * ld + n + a] = mk<double>(1.0, 0.0);
     }
   }
   __syncthreads();
@@ -208,23 +211,27 @@ __global__ void __launch_bounds__(256) k_green(GreenArgs<T> g) {
     const int grp = warp >> 2, n = grp ? nb : na;
     zcplx det = mk<double>(1.0, 0.0);
     int sg = 0;
+    zcplx* res = mats + grp * 2 * ns * ns;
     if (n > 0)
-      group_gauss_jordan(aug + grp * ns * ld, n, ld, fac + grp * (3 * ns + 2 * ns * ns + 1), ctrl + grp, tid & 127, 1 + grp, det, sg,
-                         sizeof(T) == 4 ? 1e-6 : 1e-13);
-    if ((tid & 127) == 0) { dets[grp] = det; sing[grp] = sg; }
+      res = group_gauss_jordan(mats + grp * 2 * ns * ns, mats + grp * 2 * ns * ns + ns * ns, n, fac + grp * ns, fac + 2 * ns + grp * ns,
+                               ipiv + grp * ns, cperm + grp * ns, tid & 127, 1 + grp, det, sg, sizeof(T) == 4 ? 1e-6 : 1e-13);
+    if ((tid & 127) == 0) { dets[grp] = det; sing[grp] = sg; resb[grp] = res != mats + grp * 2 * ns * ns; }
   }
   __syncthreads();
 
   // Theta_s = Phi_s A_s^-1.  FP32 path: the FP64 inverse is split into FP32 hi + lo parts and the product runs on the
   // FP32 pipe (the walker itself is FP32, so FP64 products bought nothing but FP64 issue slots); FP64 path unchanged.
-  cplx<float>* invf = reinterpret_cast<cplx<float>*>(fac);   // [2 spins][ns*ns][hi, lo] (LU scratch, now free)
+  // inverse of spin s: res_s[a * n + cperm_s[b]]; its FP32 hi / lo split goes into the OTHER ping-pong buffer of that spin
+  // ([n*n][hi, lo] complex64 = the same bytes as n*n complex128)
   if constexpr (sizeof(T) == 4) {
     for (int e = tid; e < na * na + nb * nb; e += nthr) {
       const int s = e >= na * na, ee = s ? e - na * na : e, n = s ? nb : na;
-      const zcplx v = aug[s * ns * ld + (ee / n) * ld + n + (ee % n)];
+      const zcplx* res = mats + (s * 2 + resb[s]) * ns * ns;
+      cplx<float>* invf = reinterpret_cast<cplx<float>*>(mats + (s * 2 + (resb[s] ^ 1)) * ns * ns);
+      const zcplx v = res[(ee / n) * n + cperm[s * ns + (ee % n)]];
       const float hr = (float)v.x, hi = (float)v.y;
-      invf[(s * ns * ns + ee) * 2 + 0] = mk<float>(hr, hi);
-      invf[(s * ns * ns + ee) * 2 + 1] = mk<float>((float)(v.x - (double)hr), (float)(v.y - (double)hi));
+      invf[ee * 2 + 0] = mk<float>(hr, hi);
+      invf[ee * 2 + 1] = mk<float>((float)(v.x - (double)hr), (float)(v.y - (double)hi));
     }
     __syncthreads();
   }
@@ -235,7 +242,7 @@ __global__ void __launch_bounds__(256) k_green(GreenArgs<T> g) {
     const int Mq = (M + 3) >> 2;
     for (int s = 0; s < 2; ++s) {
       const int n = s ? nb : na, off = s ? na : 0, soff = s ? g.KA : 0;
-      const float4* iv = reinterpret_cast<const float4*>(invf) + s * ns * ns;
+      const float4* iv = reinterpret_cast<const float4*>(mats + (s * 2 + (resb[s] ^ 1)) * ns * ns);
       for (int e = tid; e < Mq * n; e += nthr) {
         const int kg = e / n, b = e - kg * n;
         cplx<float> ah[4], al[4];
@@ -281,11 +288,12 @@ __global__ void __launch_bounds__(256) k_green(GreenArgs<T> g) {
   } else {
     for (int s = 0; s < 2; ++s) {
       int n = s ? nb : na, off = s ? na : 0, soff = s ? g.KA : 0;
-      const zcplx* inv = aug + s * ns * ld + n;
+      const zcplx* inv = mats + (s * 2 + resb[s]) * ns * ns;
+      const int* cp = cperm + s * ns;
       for (int e = tid; e < M * n; e += nthr) {
         int k = e / n, b = e % n;
         zcplx accd = mk<double>(0.0, 0.0);
-        for (int a = 0; a < n; ++a) cfma(accd, to_z(phi_s[k * nt + off + a]), inv[a * ld + b]);
+        for (int a = 0; a < n; ++a) cfma(accd, to_z(phi_s[k * nt + off + a]), inv[a * n + cp[b]]);
         cplx<T> acc = mk<T>((T)accd.x, (T)accd.y);
         if (g.theta) g.theta[(size_t)w * M * nt + k * nt + off + b] = acc;
         if (g.thp) {
